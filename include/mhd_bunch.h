@@ -1,0 +1,149 @@
+/* include/mhd_bunch.h -- C ABI of the B200-native bunch MHD update.
+ *
+ * One call advances a whole *bunch* -- many small Cartesian patches with guard zones
+ * -- by one step of the MUSCL predictor + HLLD + HLLD-2D +
+ * constrained-transport scheme of PAPER.md section 2.1 (L47-116).  The bunch stays
+ * resident in HBM; there is no host<->device state traffic (the paper's largest cost,
+ * L218, L243) and the number of kernel launches per step does not depend on the bunch
+ * size (the launch overhead the paper attacks, L11, L178).
+ *
+ * Conventions
+ *   - Every pointer argument says HOST or DEVICE.  Device memory (both state buffers and
+ *     the workspace) is OWNED BY THE CALLER and borrowed for the lifetime of the handle.
+ *   - State layout: structure of arrays  state[field][patch][k][j][i]  with the element
+ *     strides and origin returned by mhd_bunch_query (x rows are padded so that interior
+ *     cell 0 sits on a 16-byte boundary).  Indices (i,j,k) are guard-inclusive:
+ *     0 <= i < m_x, m_d = n_d + 2*ng in an active dimension, m_d = 1 in a collapsed one
+ *     (n_d == 1, "collapsed dimension").  Element (f,p,k,j,i) lives at
+ *         origin + f*stride[0] + p*stride[1] + k*stride[2] + j*stride[3] + i*stride[4].
+ *   - Field order is Eq. 6's: rho, rho*u, rho*v, rho*w, E, Bx, By, Bz.
+ *     B components are LOWER-face values (Eq. 10-12); face n of a
+ *     patch (the closing face) is stored in the first high-side guard slot.
+ *   - All functions return MHD_OK (0) or a negative error code; they never throw or
+ *     abort.  Unless stated otherwise a call only enqueues work on desc.stream.
+ *   - No CPU fallback: without a CUDA device every compute call returns MHD_ECUDA.
+ */
+#ifndef MHD_BUNCH_H
+#define MHD_BUNCH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MHD_OK       0
+#define MHD_EINVAL  -1   /* bad argument / unsupported configuration            */
+#define MHD_ENOMEM  -2   /* workspace too small                                 */
+#define MHD_ECUDA   -3   /* CUDA runtime error (mhd_bunch_last_cuda_error)      */
+#define MHD_ESTATE  -4   /* call sequence error (e.g. destroyed handle)         */
+
+#define MHD_F32 0
+#define MHD_F64 1
+
+typedef struct mhd_bunch mhd_bunch; /* opaque, owned by the library */
+
+/* Statement of the problem (PAPER.md: patch dimensions and guard width L212, gamma L68,
+ * bunch size L162).                                                                    */
+typedef struct {
+  int32_t n[3];        /* interior cells per patch (x,y,z); n[d]==1 => collapsed        */
+  int32_t ng;          /* guard width in active dimensions; must be 3   */
+  int32_t npatch;      /* bunch size                                                    */
+  int32_t dtype;       /* MHD_F32 or MHD_F64: storage AND arithmetic type               */
+  int32_t limiter;     /* 1 = minmod (default), 2 = monotonised central */
+  int32_t emf_solver;  /* 0 = HLLD-2D (default), 1 = HLL-2D          */
+  int32_t device;      /* CUDA ordinal                                                  */
+  int32_t reserved;
+  double  gamma;       /* adiabatic index                                               */
+  double  dx[3];       /* cell sizes, uniform over the bunch                            */
+  void   *stream;      /* cudaStream_t supplied by the caller (0 = default stream)      */
+} mhd_bunch_desc;
+
+typedef struct {
+  int64_t stride[5];       /* element strides of state[field][patch][k][j][i]           */
+  int64_t origin;          /* elements from the buffer start to (0,0,0,0,0)             */
+  int64_t state_elems;     /* elements per state buffer                                 */
+  size_t  state_bytes;     /* bytes per state buffer (allocate two)                     */
+  size_t  workspace_min;   /* bytes: smallest workspace mhd_bunch_create accepts        */
+  size_t  workspace_best;  /* bytes: workspace that avoids sub-bunch chunking overhead  */
+  int32_t m[3];            /* guard-inclusive extents                                   */
+  int32_t reserved;
+} mhd_bunch_layout;
+
+/* HOST only.  Fills *layout for the given description.  MHD_EINVAL if the description is
+ * not supported (ng != 3, an active dimension with n_d < ng, npatch < 1, ...).          */
+int mhd_bunch_query(const mhd_bunch_desc *desc, mhd_bunch_layout *layout);
+
+/* Creates a handle.
+ *   nbr        HOST, int32 [npatch][27]; entry (oz+1)*9+(oy+1)*3+(ox+1) is the patch whose
+ *              interior supplies the guard cells on that side, or -1 for zero-gradient
+ *              outflow (the framework supplies neighbours).  Copied.
+ *   state_a/b  DEVICE, state_bytes each, 16-byte aligned.  state_a holds time level n.
+ *   workspace  DEVICE, workspace_bytes >= layout.workspace_min, 16-byte aligned.  Nothing
+ *              is allocated or freed after create (static work arrays).
+ * Synchronises desc.stream once (table upload).                                          */
+int mhd_bunch_create(const mhd_bunch_desc *desc, const int32_t *nbr, void *state_a, void *state_b,
+                     void *workspace, size_t workspace_bytes, mhd_bunch **out);
+
+/* Guard fill of the current level: same-time, same-resolution copy of neighbour
+ * interiors into the 3-deep guard shell, edges and corners included; -1 neighbours give
+ * zero-gradient values and leave the closing face untouched (
+ * DESIGN.md O1).  Must precede mhd_bunch_step.                                        */
+int mhd_bunch_fill_guards(mhd_bunch *b);
+
+/* CFL time step of the current level: courant / max over interior cells of
+ * sum_d (|u_d| + c_fast,d)/dx_d over active d (O9).
+ *   dt_host          HOST, nullable.  If given, the stream is synchronised and *dt_host set.
+ *   dt_dev           DEVICE double*, nullable: receives dt without any synchronisation.
+ *   dt_per_patch_dev DEVICE double[npatch], nullable: per-patch steps.  */
+int mhd_bunch_cfl_dt(mhd_bunch *b, double courant, double *dt_host, void *dt_dev, void *dt_per_patch_dev);
+
+/* One step: current level n -> other buffer (interior cells and closing faces), which
+ * becomes the current level.  Guards of the new level are stale until the next
+ * mhd_bunch_fill_guards.  dt <= 0 or non-finite -> MHD_EINVAL.                         */
+int mhd_bunch_step(mhd_bunch *b, double dt);
+
+/* Same, with dt read on the device (DEVICE const double*), optionally clipped to
+ * dt_max > 0 (pass 0 for no clip): no host round trip between cfl_dt and step.          */
+int mhd_bunch_step_dev(mhd_bunch *b, const void *dt_dev, double dt_max);
+
+/* Host-buffer path (the paper's per-bunch offload): copy a whole
+ * state buffer between HOST memory (same layout as the device buffer, state_bytes long;
+ * pinned memory makes the copy asynchronous) and the current level.  Enqueued on the
+ * stream; mhd_bunch_download synchronises the stream before returning.                   */
+int mhd_bunch_upload(mhd_bunch *b, const void *host_state);
+int mhd_bunch_download(mhd_bunch *b, void *host_state);
+
+/* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
+ * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
+ * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to
+ * `cap` entries (name: HOST const char* owned by the library; ms: total device time;
+ * count: launches) accumulated since timing was enabled, and returns the number of
+ * classes through *n.                                                                    */
+int mhd_bunch_set_timing(mhd_bunch *b, int32_t enable);
+int mhd_bunch_kernel_times(mhd_bunch *b, int32_t cap, const char **names, double *ms, int64_t *count, int32_t *n);
+
+/* HOST out: which of state_a/state_b holds the current level.                           */
+int mhd_bunch_current(mhd_bunch *b, void **state);
+
+/* Synchronises.  *bad_cells = number of interior cells met so far whose density or
+ * pressure was not positive and finite (the scheme has no floors: DESIGN.md Q19).       */
+int mhd_bunch_status(mhd_bunch *b, int64_t *bad_cells);
+
+/* Number of kernel launches issued so far through this handle (for bench.py).           */
+int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
+
+/* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
+ * patches) the workspace allows.                                                        */
+int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);
+
+int mhd_bunch_destroy(mhd_bunch *b);
+
+const char *mhd_bunch_strerror(int code);
+const char *mhd_bunch_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_BUNCH_H */

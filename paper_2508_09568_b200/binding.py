@@ -1,0 +1,221 @@
+"""Thin ctypes binding of include/mhd_bunch.h -- argument marshalling only.
+
+Every step of the path runs in the hand-written sm_100a kernels of libmhd_bunch.so.
+PyTorch is used for device memory and streams only.  There is no CPU fallback: if the
+library cannot be loaded or no CUDA device is present, construction raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MHD_F32, MHD_F64 = 0, 1
+_ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
+
+ABI_SYMBOLS = [
+    "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
+    "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
+    "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
+    "mhd_bunch_chunk", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+]
+
+
+class Desc(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("ng", C.c_int32), ("npatch", C.c_int32), ("dtype", C.c_int32),
+                ("limiter", C.c_int32), ("emf_solver", C.c_int32), ("device", C.c_int32), ("reserved", C.c_int32),
+                ("gamma", C.c_double), ("dx", C.c_double * 3), ("stream", C.c_void_p)]
+
+
+class Layout(C.Structure):
+    _fields_ = [("stride", C.c_int64 * 5), ("origin", C.c_int64), ("state_elems", C.c_int64),
+                ("state_bytes", C.c_size_t), ("workspace_min", C.c_size_t), ("workspace_best", C.c_size_t),
+                ("m", C.c_int32 * 3), ("reserved", C.c_int32)]
+
+
+_lib = None
+
+
+def load_library(build_if_missing=True):
+    """Load libmhd_bunch.so (building it with nvcc if absent or stale).  Raises on failure."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.TARGET
+    if build_if_missing and _build.stale():
+        _build.build()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: the CUDA extension must be built (no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.mhd_bunch_query.argtypes = [C.POINTER(Desc), C.POINTER(Layout)]
+    lib.mhd_bunch_create.argtypes = [C.POINTER(Desc), vp, vp, vp, vp, C.c_size_t, C.POINTER(vp)]
+    lib.mhd_bunch_fill_guards.argtypes = [vp]
+    lib.mhd_bunch_cfl_dt.argtypes = [vp, dbl, C.POINTER(dbl), vp, vp]
+    lib.mhd_bunch_step.argtypes = [vp, dbl]
+    lib.mhd_bunch_step_dev.argtypes = [vp, vp, dbl]
+    lib.mhd_bunch_upload.argtypes = [vp, vp]
+    lib.mhd_bunch_download.argtypes = [vp, vp]
+    lib.mhd_bunch_set_timing.argtypes = [vp, i32]
+    lib.mhd_bunch_kernel_times.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(dbl), C.POINTER(i64), C.POINTER(i32)]
+    lib.mhd_bunch_current.argtypes = [vp, C.POINTER(vp)]
+    lib.mhd_bunch_status.argtypes = [vp, C.POINTER(i64)]
+    lib.mhd_bunch_launch_count.argtypes = [vp, C.POINTER(i64)]
+    lib.mhd_bunch_chunk.argtypes = [vp, C.POINTER(i32)]
+    lib.mhd_bunch_destroy.argtypes = [vp]
+    lib.mhd_bunch_strerror.argtypes = [C.c_int]
+    lib.mhd_bunch_strerror.restype = C.c_char_p
+    lib.mhd_bunch_last_cuda_error.restype = C.c_char_p
+    for name in ABI_SYMBOLS:
+        getattr(lib, name)
+    _lib = lib
+    return lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        lib = load_library()
+        msg = lib.mhd_bunch_strerror(rc).decode()
+        cu = lib.mhd_bunch_last_cuda_error().decode()
+        raise RuntimeError(f"{what}: {_ERR.get(rc, rc)} ({msg}) {cu}")
+
+
+def make_desc(n, npatch, gamma, dx, dtype=MHD_F32, limiter=1, emf_solver=0, device=0, stream=0, ng=3):
+    d = Desc()
+    d.n[:] = list(n)
+    d.ng, d.npatch, d.dtype, d.limiter, d.emf_solver, d.device = ng, npatch, dtype, limiter, emf_solver, device
+    d.gamma = gamma
+    d.dx[:] = list(dx)
+    d.stream = stream
+    return d
+
+
+def query(desc):
+    lay = Layout()
+    _check(load_library().mhd_bunch_query(C.byref(desc), C.byref(lay)), "mhd_bunch_query")
+    return lay
+
+
+class MhdBunch:
+    """A bunch of patches resident in HBM.
+
+        b = MhdBunch(n=(32,32,32), npatch=512, nbr=nbr, gamma=5/3, dx=(h,h,h), dtype="f32")
+        b.load(U_dense_numpy); b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+    """
+
+    def __init__(self, n, npatch, nbr, gamma, dx, dtype="f32", limiter=1, emf_solver=0, device=0,
+                 workspace_bytes=None, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("MhdBunch needs a CUDA device: there is no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        self.tdtype = torch.float32 if dtype == "f32" else torch.float64
+        self.npdtype = np.float32 if dtype == "f32" else np.float64
+        self.n, self.npatch = tuple(n), npatch
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.desc = make_desc(n, npatch, gamma, dx, MHD_F32 if dtype == "f32" else MHD_F64, limiter, emf_solver,
+                              device, self.stream.cuda_stream)
+        self.lay = query(self.desc)
+        self.m = tuple(self.lay.m)
+        ws = self.lay.workspace_best if workspace_bytes is None else max(int(workspace_bytes), self.lay.workspace_min)
+        self.state = [torch.zeros(self.lay.state_elems, dtype=self.tdtype, device=self.device) for _ in range(2)]
+        self.workspace = torch.empty(ws, dtype=torch.uint8, device=self.device)
+        self.dt_dev = torch.zeros(1, dtype=torch.float64, device=self.device)
+        self.dt_patch = torch.zeros(npatch, dtype=torch.float64, device=self.device)
+        nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+        assert nbr.shape == (npatch, 27)
+        h = C.c_void_p()
+        _check(self.lib.mhd_bunch_create(C.byref(self.desc), nbr.ctypes.data_as(C.c_void_p), self.state[0].data_ptr(),
+                                         self.state[1].data_ptr(), self.workspace.data_ptr(), ws, C.byref(h)),
+               "mhd_bunch_create")
+        self.h = h
+
+    # ---- plumbing -----------------------------------------------------------------
+    def _cur_index(self):
+        p = C.c_void_p()
+        _check(self.lib.mhd_bunch_current(self.h, C.byref(p)), "mhd_bunch_current")
+        return 0 if p.value == self.state[0].data_ptr() else 1
+
+    def view(self, which=None):
+        """Strided torch view [8, npatch, mz, my, mx] of the current (or given) buffer."""
+        idx = self._cur_index() if which is None else which
+        shape = (8, self.npatch, self.m[2], self.m[1], self.m[0])
+        return self.state[idx].as_strided(shape, tuple(self.lay.stride), int(self.lay.origin))
+
+    def load(self, U):
+        """Dense numpy [8, npatch, mz, my, mx] -> current buffer."""
+        t = self.torch.from_numpy(np.ascontiguousarray(U, dtype=self.npdtype))
+        with self.torch.cuda.stream(self.stream):
+            self.view().copy_(t.to(self.device, non_blocking=False))
+        self.stream.synchronize()
+
+    def download(self):
+        with self.torch.cuda.stream(self.stream):
+            out = self.view().contiguous().cpu().numpy()
+        return out
+
+    # ---- the path -------------------------------------------------------------------
+    def fill_guards(self):
+        _check(self.lib.mhd_bunch_fill_guards(self.h), "mhd_bunch_fill_guards")
+
+    def cfl_dt(self, courant, sync=True, per_patch=False):
+        dt = C.c_double(0.0)
+        _check(self.lib.mhd_bunch_cfl_dt(self.h, courant, C.byref(dt) if sync else None, self.dt_dev.data_ptr(),
+                                         self.dt_patch.data_ptr() if per_patch else None), "mhd_bunch_cfl_dt")
+        return dt.value if sync else None
+
+    def step(self, dt):
+        _check(self.lib.mhd_bunch_step(self.h, dt), "mhd_bunch_step")
+
+    def step_dev(self, dt_max=0.0):
+        _check(self.lib.mhd_bunch_step_dev(self.h, self.dt_dev.data_ptr(), dt_max), "mhd_bunch_step_dev")
+
+    def upload_host(self, host_tensor):
+        _check(self.lib.mhd_bunch_upload(self.h, host_tensor.data_ptr()), "mhd_bunch_upload")
+
+    def download_host(self, host_tensor):
+        _check(self.lib.mhd_bunch_download(self.h, host_tensor.data_ptr()), "mhd_bunch_download")
+
+    def status(self):
+        v = C.c_int64(0)
+        _check(self.lib.mhd_bunch_status(self.h, C.byref(v)), "mhd_bunch_status")
+        return v.value
+
+    @property
+    def launches(self):
+        v = C.c_int64(0)
+        _check(self.lib.mhd_bunch_launch_count(self.h, C.byref(v)), "mhd_bunch_launch_count")
+        return v.value
+
+    @property
+    def chunk(self):
+        v = C.c_int32(0)
+        _check(self.lib.mhd_bunch_chunk(self.h, C.byref(v)), "mhd_bunch_chunk")
+        return v.value
+
+    def set_timing(self, on):
+        _check(self.lib.mhd_bunch_set_timing(self.h, 1 if on else 0), "mhd_bunch_set_timing")
+
+    def kernel_times(self):
+        cap = 16
+        names = (C.c_char_p * cap)()
+        ms = (C.c_double * cap)()
+        cnt = (C.c_int64 * cap)()
+        n = C.c_int32(0)
+        _check(self.lib.mhd_bunch_kernel_times(self.h, cap, names, ms, cnt, C.byref(n)), "mhd_bunch_kernel_times")
+        return {names[i].decode(): (ms[i], cnt[i]) for i in range(n.value)}
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            self.lib.mhd_bunch_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

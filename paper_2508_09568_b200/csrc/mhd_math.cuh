@@ -1,0 +1,225 @@
+// mhd_math.cuh -- pointwise device arithmetic of the bunch MHD update (sm_100a).
+//
+// Limiter, fast speed, HLLD flux (Miyoshi & Kusano 2005)
+// and the two-dimensional Riemann problem for the edge EMF (
+// DESIGN.md reading O7).  Everything is branch-light: wave-pattern choices are selects,
+// so a warp never serialises over the six HLLD regions.
+#pragma once
+#include <cuda_runtime.h>
+#include <float.h>
+
+namespace mhd {
+
+template <typename T> struct num;
+template <> struct num<float> {
+  static __device__ __forceinline__ float eps() { return FLT_EPSILON; }
+  static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+  static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
+  static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
+  static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
+  static __device__ __forceinline__ float rcp(float x) { return 1.0f / x; }
+};
+template <> struct num<double> {
+  static __device__ __forceinline__ double eps() { return DBL_EPSILON; }
+  static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+  static __device__ __forceinline__ double abs(double x) { return fabs(x); }
+  static __device__ __forceinline__ double min(double a, double b) { return fmin(a, b); }
+  static __device__ __forceinline__ double max(double a, double b) { return fmax(a, b); }
+  static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+};
+
+// ---- slope limiter: 0 at extrema; minmod (1) or monotonised central (2) -------------
+template <typename T>
+__device__ __forceinline__ T limited_slope(int kind, T a, T b) {
+  using N = num<T>;
+  const T fa = N::abs(a), fb = N::abs(b);
+  T m = N::min(fa, fb);
+  if (kind == 2) m = N::min(T(2) * m, T(0.5) * N::abs(a + b));
+  m = (a * b > T(0)) ? m : T(0);
+  return a < T(0) ? -m : m;
+}
+
+// ---- fast magnetosonic speed along a direction with normal field bn ---------------
+// gp = gamma*p, b2 = |B|^2, bn2 = bn^2, irho = 1/rho
+template <typename T>
+__device__ __forceinline__ T fast_speed(T gp, T b2, T bn2, T irho) {
+  using N = num<T>;
+  const T s = gp + b2;
+  const T disc = N::max(s * s - T(4) * gp * bn2, T(0));
+  return N::sqrt(T(0.5) * (s + N::sqrt(disc)) * irho);
+}
+
+// primitive state seen by a 1D Riemann problem: normal velocity u, transverse (v,w),
+// transverse field (by,bz)
+template <typename T> struct State1D { T rho, u, v, w, p, by, bz; };
+template <typename T> struct Flux5 { T d, mu, mv, mw, e; };
+
+// ---- HLLD flux of (rho, rho u, rho v, rho w, E) ------------------------------------
+// The side that contains the interface (left if S_L>0 or S*_L>0 or S_M>=0) is selected
+// first; only that side's star and double-star states are formed.
+template <typename T>
+__device__ __forceinline__ Flux5<T> hlld_flux(T gamma, const State1D<T>& L, const State1D<T>& R, T bn) {
+  using N = num<T>;
+  const T half = T(0.5);
+  const T bn2 = bn * bn;
+  const T igm1 = N::rcp(gamma - T(1));
+
+  const T b2L = bn2 + L.by * L.by + L.bz * L.bz, b2R = bn2 + R.by * R.by + R.bz * R.bz;
+  const T pTL = L.p + half * b2L, pTR = R.p + half * b2R;
+  const T cfL = fast_speed(gamma * L.p, b2L, bn2, N::rcp(L.rho));
+  const T cfR = fast_speed(gamma * R.p, b2R, bn2, N::rcp(R.rho));
+  const T cmax = N::max(cfL, cfR);
+  const T SL = N::min(L.u, R.u) - cmax, SR = N::max(L.u, R.u) + cmax;
+
+  const T sdL = SL - L.u, sdR = SR - R.u;
+  const T mL = L.rho * sdL, mR = R.rho * sdR;
+  const T SM = (mR * R.u - mL * L.u - pTR + pTL) / (mR - mL);
+  const T pTs = pTL + mL * (SM - L.u);
+
+  // star densities and transverse star values of BOTH sides (the double-star state mixes them)
+  const T rsL = mL / (SL - SM), rsR = mR / (SR - SM);
+  const T DL = mL * (SL - SM) - bn2, DR = mR * (SR - SM) - bn2;
+  const T refL = mL * sdL, refR = mR * sdR;
+  const bool degL = N::abs(DL) <= T(16) * N::eps() * refL;
+  const bool degR = N::abs(DR) <= T(16) * N::eps() * refR;
+  const T iDL = degL ? T(0) : N::rcp(DL), iDR = degR ? T(0) : N::rcp(DR);
+  const T kvL = bn * (SM - L.u) * iDL, kvR = bn * (SM - R.u) * iDR;       // v* = v - kv*by
+  const T kbL = degL ? T(1) : (refL - bn2) * iDL, kbR = degR ? T(1) : (refR - bn2) * iDR;
+  const T vsL = L.v - kvL * L.by, wsL = L.w - kvL * L.bz, bysL = L.by * kbL, bzsL = L.bz * kbL;
+  const T vsR = R.v - kvR * R.by, wsR = R.w - kvR * R.bz, bysR = R.by * kbR, bzsR = R.bz * kbR;
+
+  const T rL = N::sqrt(rsL), rR = N::sqrt(rsR);
+  const T abn = N::abs(bn);
+  const T SsL = SM - abn / rL, SsR = SM + abn / rR;
+  const T sg = bn > T(0) ? T(1) : (bn < T(0) ? T(-1) : T(0));
+
+  // which side holds the interface, and how deep into the fan it sits
+  const bool left = (SL > T(0)) || (SsL > T(0)) || (SM >= T(0));
+  const bool star = left ? !(SL > T(0)) : (SsR >= T(0) || SR >= T(0));
+  const bool dstar = left ? !(SL > T(0) || SsL > T(0)) : (SsR >= T(0));
+
+  // own side = the selected one
+  const T rho = left ? L.rho : R.rho, u = left ? L.u : R.u, v = left ? L.v : R.v, w = left ? L.w : R.w;
+  const T p = left ? L.p : R.p, by = left ? L.by : R.by, bz = left ? L.bz : R.bz;
+  const T b2 = left ? b2L : b2R, pT = left ? pTL : pTR;
+  const T S = left ? SL : SR, sd = left ? sdL : sdR, Ss = left ? SsL : SsR;
+  const T rs = left ? rsL : rsR, ro = left ? rL : rR, rx = left ? rR : rL;
+  const T vs = left ? vsL : vsR, ws = left ? wsL : wsR, bys = left ? bysL : bysR, bzs = left ? bzsL : bzsR;
+  const T vx = left ? vsR : vsL, wx = left ? wsR : wsL, byx = left ? bysR : bysL, bzx = left ? bzsR : bzsL;
+  const T tau = left ? sg : -sg;          // sign(bn) seen from the own side
+
+  const T E = p * igm1 + half * rho * (u * u + v * v + w * w) + half * b2;
+  const T ub = u * bn + v * by + w * bz;
+  // physical flux, Eq. 6
+  Flux5<T> F;
+  F.d = rho * u;
+  F.mu = rho * u * u + pT - bn2;
+  F.mv = rho * v * u - by * bn;
+  F.mw = rho * w * u - bz * bn;
+  F.e = u * (E + pT) - bn * ub;
+
+  // star state
+  const T ubs = SM * bn + vs * bys + ws * bzs;
+  const T Es = (sd * E - pT * u + pTs * SM + bn * (ub - ubs)) / (S - SM);
+  // double-star state
+  const T irs = N::rcp(ro + rx);
+  const T vss = (ro * vs + rx * vx + tau * (byx - bys)) * irs;
+  const T wss = (ro * ws + rx * wx + tau * (bzx - bzs)) * irs;
+  const T byss = (ro * byx + rx * bys + ro * rx * tau * (vx - vs)) * irs;
+  const T bzss = (ro * bzx + rx * bzs + ro * rx * tau * (wx - ws)) * irs;
+  const T ubss = SM * bn + vss * byss + wss * bzss;
+  const T Ess = Es - tau * ro * (ubs - ubss);
+
+  const T c1 = star ? S : T(0), c2 = dstar ? Ss : T(0);
+  F.d += c1 * (rs - rho);
+  F.mu += c1 * (rs * SM - rho * u);
+  F.mv += c1 * (rs * vs - rho * v) + c2 * rs * (vss - vs);
+  F.mw += c1 * (rs * ws - rho * w) + c2 * rs * (wss - ws);
+  F.e += c1 * (Es - E) + c2 * (Ess - Es);
+  return F;
+}
+
+// ---- two-dimensional Riemann problem at an edge -------------------------------------
+// Corner states (rho, ua, ub, p, be) with be the out-of-plane field; in-plane fields are
+// single-valued per side: A (component a) south/north, B (component b) west/east.
+template <typename T> struct Corner { T rho, ua, ub, p, be; };
+
+template <typename T> struct Sub1D { T bsL, bsR, lo, hi; };
+
+// star transverse field and Alfven-type bounds of a 1D sub-problem with given outer speeds
+template <typename T>
+__device__ __forceinline__ Sub1D<T> sub_star(T rhoL, T unL, T pTL, T btL, T rhoR, T unR, T pTR, T btR,
+                                             T bn, T SL, T SR) {
+  using N = num<T>;
+  const T bn2 = bn * bn;
+  const T sdL = SL - unL, sdR = SR - unR;
+  const T mL = rhoL * sdL, mR = rhoR * sdR;
+  const T SM = (mR * unR - mL * unL - pTR + pTL) / (mR - mL);
+  const T dL = SL - SM, dR = SR - SM;
+  const T DL = mL * dL - bn2, DR = mR * dR - bn2;
+  const T refL = mL * sdL, refR = mR * sdR;
+  Sub1D<T> s;
+  s.bsL = (N::abs(DL) <= T(16) * N::eps() * refL) ? btL : btL * (refL - bn2) / DL;
+  s.bsR = (N::abs(DR) <= T(16) * N::eps() * refR) ? btR : btR * (refR - bn2) / DR;
+  const T abn = N::abs(bn);
+  // rho*_K = m_K / d_K  =>  |bn| / sqrt(rho*_K) = |bn| * sqrt(d_K / m_K)
+  s.lo = SM - abn * N::sqrt(dL / mL);
+  s.hi = SM + abn * N::sqrt(dR / mR);
+  return s;
+}
+
+template <typename T>
+__device__ __forceinline__ T emf_2d(T gamma, int solver, const Corner<T>& sw, const Corner<T>& se,
+                                    const Corner<T>& nw, const Corner<T>& ne, T AS, T AN, T BW, T BE) {
+  using N = num<T>;
+  const T half = T(0.5), zero = T(0);
+  const T eSW = sw.ua * BW - sw.ub * AS, eSE = se.ua * BE - se.ub * AS;
+  const T eNW = nw.ua * BW - nw.ub * AN, eNE = ne.ua * BE - ne.ub * AN;
+  const T AS2 = AS * AS, AN2 = AN * AN, BW2 = BW * BW, BE2 = BE * BE;
+  const T b2SW = AS2 + BW2 + sw.be * sw.be, b2SE = AS2 + BE2 + se.be * se.be;
+  const T b2NW = AN2 + BW2 + nw.be * nw.be, b2NE = AN2 + BE2 + ne.be * ne.be;
+  const T iSW = N::rcp(sw.rho), iSE = N::rcp(se.rho), iNW = N::rcp(nw.rho), iNE = N::rcp(ne.rho);
+  const T gSW = gamma * sw.p, gSE = gamma * se.p, gNW = gamma * nw.p, gNE = gamma * ne.p;
+  const T ca = N::max(N::max(fast_speed(gSW, b2SW, AS2, iSW), fast_speed(gSE, b2SE, AS2, iSE)),
+                      N::max(fast_speed(gNW, b2NW, AN2, iNW), fast_speed(gNE, b2NE, AN2, iNE)));
+  const T cb = N::max(N::max(fast_speed(gSW, b2SW, BW2, iSW), fast_speed(gSE, b2SE, BE2, iSE)),
+                      N::max(fast_speed(gNW, b2NW, BW2, iNW), fast_speed(gNE, b2NE, BE2, iNE)));
+  const T tW = N::min(N::min(sw.ua, se.ua), N::min(nw.ua, ne.ua)) - ca;
+  const T tE = N::max(N::max(sw.ua, se.ua), N::max(nw.ua, ne.ua)) + ca;
+  const T tS = N::min(N::min(sw.ub, se.ub), N::min(nw.ub, ne.ub)) - cb;
+  const T tN = N::max(N::max(sw.ub, se.ub), N::max(nw.ub, ne.ub)) + cb;
+
+  T SW_, SE_, SS_, SN_, e0 = eSW, e1 = eSE, e2 = eNW, e3 = eNE;
+  T BsSW = BW, BsSE = BE, BsNW = BW, BsNE = BE, AsSW = AS, AsSE = AS, AsNW = AN, AsNE = AN;
+  if (solver == 1) {
+    SW_ = N::min(zero, tW); SE_ = N::max(zero, tE); SS_ = N::min(zero, tS); SN_ = N::max(zero, tN);
+  } else {
+    const T pSW = sw.p + half * b2SW, pSE = se.p + half * b2SE, pNW = nw.p + half * b2NW, pNE = ne.p + half * b2NE;
+    const Sub1D<T> xS = sub_star(sw.rho, sw.ua, pSW, BW, se.rho, se.ua, pSE, BE, AS, tW, tE);
+    const Sub1D<T> xN = sub_star(nw.rho, nw.ua, pNW, BW, ne.rho, ne.ua, pNE, BE, AN, tW, tE);
+    const Sub1D<T> yW = sub_star(sw.rho, sw.ub, pSW, AS, nw.rho, nw.ub, pNW, AN, BW, tS, tN);
+    const Sub1D<T> yE = sub_star(se.rho, se.ub, pSE, AS, ne.rho, ne.ub, pNE, AN, BE, tS, tN);
+    SW_ = tW >= zero ? zero : N::min(zero, N::min(xS.lo, xN.lo));
+    SE_ = tE <= zero ? zero : N::max(zero, N::max(xS.hi, xN.hi));
+    SS_ = tS >= zero ? zero : N::min(zero, N::min(yW.lo, yE.lo));
+    SN_ = tN <= zero ? zero : N::max(zero, N::max(yW.hi, yE.hi));
+    BsSW = xS.bsL; BsSE = xS.bsR; BsNW = xN.bsL; BsNE = xN.bsR;
+    AsSW = yW.bsL; AsNW = yW.bsR; AsSE = yE.bsL; AsNE = yE.bsR;
+    const T SxW = N::min(tW, zero), SxE = N::max(tE, zero), SyS = N::min(tS, zero), SyN = N::max(tN, zero);
+    e0 += SxW * (BsSW - BW) - SyS * (AsSW - AS);
+    e1 += SxE * (BsSE - BE) - SyS * (AsSE - AS);
+    e2 += SxW * (BsNW - BW) - SyN * (AsNW - AN);
+    e3 += SxE * (BsNE - BE) - SyN * (AsNE - AN);
+  }
+  const T dxs = SE_ - SW_, dys = SN_ - SS_;
+  const bool zx = dxs == zero, zy = dys == zero;
+  const T idx = zx ? zero : N::rcp(dxs), idy = zy ? zero : N::rcp(dys);
+  const T aE = zx ? half : SE_ * idx, aW = zx ? half : -SW_ * idx;
+  const T bN = zy ? half : SN_ * idy, bS = zy ? half : -SS_ * idy;
+  const T BsW = bN * BsSW + bS * BsNW, BsE = bN * BsSE + bS * BsNE;
+  const T AsS = aE * AsSW + aW * AsSE, AsN = aE * AsNW + aW * AsNE;
+  return aE * (bN * e0 + bS * e2) + aW * (bN * e1 + bS * e3)
+       + (SW_ * SE_ * idx) * (BsE - BsW) - (SS_ * SN_ * idy) * (AsN - AsS);
+}
+
+}  // namespace mhd

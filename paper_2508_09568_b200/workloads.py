@@ -226,6 +226,9 @@ def _band_limited(rng, N, power, kmin=1, kmax=8, base=32):
     amp = np.where((kk >= kmin) & (kk <= kmax), np.maximum(kk, 1e-30) ** (-power), 0.0)
     spec = spec * amp
     Nz, Ny, Nx = (N, N, N) if np.isscalar(N) else N
+    kmax = max(1, min(kmax, min(Nz, Ny, Nx) // 2 - 1))        # tiny test grids: stay below Nyquist
+    amp = np.where(kk <= kmax, amp, 0.0)
+    spec = spec * (amp > 0)
     big = np.zeros((Nz, Ny, Nx // 2 + 1), dtype=np.complex128)
     h = kmax + 1
     for sz, dz_ in ((slice(0, h), slice(0, h)), (slice(base - h + 1, base), slice(Nz - h + 1, Nz))):

@@ -1,0 +1,319 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's: one step <= 1e-12
+(fp64) / 2e-5 (fp32) per cell; N steps: totals 1e-12 (fp64), L1 norms 1e-4 (fp32).
+fp32 runs are compared with the fp64 oracle on the same fp32-representable inputs."""
+import numpy as np
+import pytest
+
+import exact_riemann
+from parity_util import (TOL_L1_F32, TOL_STEP, TOL_TOTALS_F64, make_gpu, make_oracle, masked, rel_err)
+from paper_2508_09568_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+NPD = {"f32": np.float32, "f64": np.float64}
+
+
+def small_workloads(dtype):
+    t = NPD[dtype]
+    return {
+        "sod_x": W.sod(256, 8, dtype=t),
+        "sod_y": W.sod(96, 3, dtype=t, axis=1),
+        "tube_z": W.mhd_tube((1.0, 0.2, 0.3, -0.1, 1.0, 1.0, 0.4), (0.125, -0.1, -0.2, 0.25, 0.1, -1.0, 0.2), 0.75, 2.0,
+                             ncell=120, npatch=3, axis=2, dtype=t),
+        "ot64": W.orszag_tang(64, 32, dtype=t),
+        "ot_ragged": W.orszag_tang(60, 20, dtype=t),
+        "turb16": W.turbulence(N=32, n=16, dtype=t),
+        "turb_ragged": W.turbulence(N=(24, 20, 36), n=(12, 10, 9), dtype=t),
+        "turb_self": W.turbulence(N=16, n=16, dtype=t),          # one patch, its own neighbour
+    }
+
+
+# ---------------------------------------------------------------- guard fill -------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["sod_x", "sod_y", "tube_z", "ot64", "ot_ragged", "turb16", "turb_ragged", "turb_self"])
+def test_fill_guards_bit_exact(name, dtype):
+    w = small_workloads(dtype)[name]
+    rng = np.random.default_rng(5)
+    U = rng.normal(size=w.U.shape).astype(NPD[dtype])            # every slot distinct, guards included
+    w.U = U
+    o = make_oracle(w)
+    ref = o.fill_guards(U.astype(np.float64).copy(), w.nbr)
+    b = make_gpu(w, dtype)
+    b.fill_guards()
+    got = b.download()
+    assert np.array_equal(got.astype(np.float64), ref)
+    b.close()
+
+
+def test_fill_guards_mixed_outflow_periodic_3d():
+    P = (2, 1, 3)
+    n = (4, 5, 6)
+    nbr = W.neighbour_table(P, (False, True, False))
+    w = W.Workload("mix", n, P, 5 / 3, (1, 1, 1), (False, True, False),
+                   np.random.default_rng(6).normal(size=(8, 6) + tuple(reversed(W.padded(n)))), nbr)
+    ref = make_oracle(w).fill_guards(w.U.copy(), nbr)
+    b = make_gpu(w, "f64")
+    b.fill_guards()
+    assert np.array_equal(b.download(), ref)
+    b.close()
+
+
+# ------------------------------------------------------------------------ CFL -------
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-13), ("f32", 2e-6)])
+@pytest.mark.parametrize("name", ["sod_x", "tube_z", "ot_ragged", "turb_ragged"])
+def test_cfl_dt_matches_oracle(name, dtype, tol):
+    w = small_workloads(dtype)[name]
+    o = make_oracle(w)
+    U = o.fill_guards(w.U.astype(np.float64), w.nbr)
+    dt_ref, pp_ref = o.cfl_dt(U, 0.4, per_patch=True)
+    b = make_gpu(w, dtype)
+    b.fill_guards()
+    dt = b.cfl_dt(0.4, sync=True, per_patch=True)
+    assert abs(dt - dt_ref) <= tol * dt_ref
+    assert np.allclose(b.dt_patch.cpu().numpy(), pp_ref, rtol=tol, atol=0)
+    assert abs(b.dt_dev.item() - dt) == 0
+    b.close()
+
+
+# ------------------------------------------------------------------- one step -------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("limiter,emf_solver", [(1, 0), (2, 0), (1, 1)])
+@pytest.mark.parametrize("name", ["sod_x", "sod_y", "tube_z", "ot64", "ot_ragged", "turb16", "turb_ragged", "turb_self"])
+def test_one_step_matches_oracle(name, dtype, limiter, emf_solver):
+    w = small_workloads(dtype)[name]
+    o = make_oracle(w, limiter, emf_solver)
+    U = o.fill_guards(w.U.astype(np.float64), w.nbr)
+    dt = o.cfl_dt(U, 0.4)
+    ref = o.step(U, dt)
+    b = make_gpu(w, dtype, limiter, emf_solver)
+    b.fill_guards()
+    b.step(dt)
+    got = b.download()
+    err = rel_err(masked(got, w.n), masked(ref, w.n))
+    assert err <= TOL_STEP[dtype], (name, dtype, err)
+    assert b.status() == 0
+    b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_sub_bunch_chunking_is_bitwise_invisible(dtype):
+    w = small_workloads(dtype)["turb16"]                        # 8 patches
+    outs = []
+    for ws in (None, 1):                                         # whole bunch at once / one patch per chunk
+        b = make_gpu(w, dtype, workspace_bytes=ws)
+        b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+        outs.append((b.download(), b.chunk))
+        b.close()
+    assert outs[0][1] == 8 and outs[1][1] == 1
+    assert np.array_equal(masked(outs[0][0], w.n), masked(outs[1][0], w.n))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_device_dt_path_equals_host_dt_path(dtype):
+    w = small_workloads(dtype)["ot64"]
+    a = make_gpu(w, dtype); a.fill_guards(); dt = a.cfl_dt(0.4, sync=True); a.step(dt)
+    b = make_gpu(w, dtype); b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+    assert np.array_equal(masked(a.download(), w.n), masked(b.download(), w.n))
+    c = make_gpu(w, dtype); c.fill_guards(); c.cfl_dt(0.4, sync=False); c.step_dev(dt_max=dt / 2)
+    d = make_gpu(w, dtype); d.fill_guards(); d.step(dt / 2)
+    assert np.array_equal(masked(c.download(), w.n), masked(d.download(), w.n))
+    for x in (a, b, c, d):
+        x.close()
+
+
+# -------------------------------------------------------------------- N steps -------
+def run_both(w, dtype, nsteps, limiter=1, emf_solver=0):
+    o = make_oracle(w, limiter, emf_solver)
+    U = w.U.astype(np.float64)
+    b = make_gpu(w, dtype, limiter, emf_solver)
+    for _ in range(nsteps):
+        o.fill_guards(U, w.nbr)
+        dt = o.cfl_dt(U, 0.4)
+        U = o.step(U, dt)
+        b.fill_guards()
+        b.step(dt)                                              # same dt sequence on both sides
+    got = b.download()
+    bad = b.status()
+    b.close()
+    return W.gather(got, w.n, w.P).astype(np.float64), W.gather(U, w.n, w.P), bad
+
+
+@pytest.mark.parametrize("name,nsteps", [("turb16", 20), ("ot64", 40), ("tube_z", 40)])
+def test_n_steps_fp64_totals_and_fields(name, nsteps):
+    w = small_workloads("f64")[name]
+    g, o, bad = run_both(w, "f64", nsteps)
+    assert bad == 0
+    tg, to = g[:5].sum(axis=(1, 2, 3)), o[:5].sum(axis=(1, 2, 3))
+    scale = np.array([to[0], np.abs(o[1:4]).sum(), np.abs(o[1:4]).sum(), np.abs(o[1:4]).sum(), to[4]])
+    assert np.all(np.abs(tg - to) <= TOL_TOTALS_F64 * scale), (tg - to) / scale
+    assert rel_err(g, o) <= 1e-10                                # per cell, after N steps
+
+
+@pytest.mark.parametrize("name,nsteps", [("turb16", 20), ("ot64", 40), ("tube_z", 40)])
+def test_n_steps_fp32_l1_norms(name, nsteps):
+    w = small_workloads("f32")[name]
+    g, o, bad = run_both(w, "f32", nsteps)
+    assert bad == 0
+    for a, b_ in ((0, 1), (1, 4), (4, 5), (5, 8)):
+        l1 = np.abs(g[a:b_] - o[a:b_]).sum() / max(np.abs(o[a:b_]).sum(), 1e-300)
+        assert l1 <= TOL_L1_F32, (name, a, l1)
+    tg, to = g[:5].sum(axis=(1, 2, 3)), o[:5].sum(axis=(1, 2, 3))
+    assert abs(tg[0] - to[0]) <= 1e-5 * to[0] and abs(tg[4] - to[4]) <= 1e-5 * to[4]
+
+
+# --------------------------------------------------------------- whole configs -------
+def gpu_run(w, dtype, t_end=None, max_steps=10 ** 9, limiter=1):
+    b = make_gpu(w, dtype, limiter)
+    t, steps = 0.0, 0
+    t_end = w.t_end if t_end is None else t_end
+    while t < t_end * (1 - 1e-14) and steps < max_steps:
+        b.fill_guards()
+        dt = min(b.cfl_dt(w.courant, sync=True), t_end - t)
+        b.step(dt)
+        t += dt
+        steps += 1
+    out = b.download()
+    bad = b.status()
+    b.close()
+    return out, t, steps, bad
+
+
+def test_config0_sod_on_gpu_against_exact_solution_and_oracle():
+    """BASELINE.json config 0: 256 cells, 8 patches of 32, fp64, CFL 0.4, t = 0.2."""
+    w = W.sod(256, 8)
+    U, t, steps, bad = gpu_run(w, "f64")
+    assert bad == 0 and 270 <= steps <= 290
+    g = W.gather(U, w.n, w.P)
+    x = (np.arange(256) + 0.5) / 256
+    ex = exact_riemann.sample((x - 0.5) / t, 1, 0, 1, 0.125, 0, 0.1, 1.4)
+    assert np.abs(g[0, 0, 0] - ex[0]).mean() <= 3.5e-3
+    assert not g[2:4].any() and not g[5:].any()
+    # the oracle over the same run (seconds)
+    o = make_oracle(w)
+    V = w.U.copy(); tt = 0.0
+    while tt < w.t_end * (1 - 1e-14):
+        o.fill_guards(V, w.nbr)
+        dt = min(o.cfl_dt(V, 0.4), w.t_end - tt)
+        V = o.step(V, dt); tt += dt
+    assert rel_err(g, W.gather(V, w.n, w.P)) <= 1e-10
+    # bunch of 8 == single patch, bitwise, on the GPU too
+    U1, _, s1, _ = gpu_run(W.sod(256, 1), "f64")
+    assert s1 == steps and np.array_equal(W.gather(U1, (256, 1, 1), (1, 1, 1)), g)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config1_orszag_tang_256_to_half(dtype):
+    """BASELINE.json config 1: 256^2 as 64 patches of 32^2, to t = 0.5: invariants at full
+    size and length; parity with the oracle over the first 30 steps."""
+    w = W.orszag_tang(256, 32, dtype=NPD[dtype])
+    U, t, steps, bad = gpu_run(w, dtype)
+    assert bad == 0 and 1200 <= steps <= 1700 and abs(t - 0.5) < 1e-12
+    g0 = W.gather(w.U, w.n, w.P).astype(np.float64)
+    g = W.gather(U, w.n, w.P).astype(np.float64)
+    eps = 1e-12 if dtype == "f64" else 2e-4
+    rot = lambda a: a[:, ::-1, ::-1]
+    assert np.abs(g[0] - rot(g[0])).max() <= eps * 100           # point symmetry
+    tot0, tot1 = g0[:5].sum(axis=(1, 2, 3)), g[:5].sum(axis=(1, 2, 3))
+    assert abs(tot1[0] - tot0[0]) <= eps * tot0[0] and abs(tot1[4] - tot0[4]) <= eps * tot0[4]
+    bx, by = g[5, 0], g[6, 0]
+    div = np.roll(bx, -1, 1) - bx + np.roll(by, -1, 0) - by
+    assert np.abs(div).max() / np.sqrt(np.mean(bx ** 2 + by ** 2)) <= (1e-12 if dtype == "f64" else 1e-4)
+    assert g[0].min() > 0.05 and g[0].max() < 0.6
+    gg, oo, _ = run_both(w, dtype, 30)
+    assert rel_err(gg, oo) <= (1e-10 if dtype == "f64" else 2e-4)
+
+
+def test_decomposition_invariance_on_gpu_bitwise():
+    a, b = W.turbulence(N=32, n=32, dtype=np.float32), W.turbulence(N=32, n=16, dtype=np.float32)
+    outs = []
+    for w in (a, b):
+        h = make_gpu(w, "f32")
+        dts = []
+        for _ in range(3):
+            h.fill_guards(); dts.append(h.cfl_dt(0.4, sync=True)); h.step(dts[-1])
+        outs.append((W.gather(h.download(), w.n, w.P), dts))
+        h.close()
+    assert outs[0][1] == outs[1][1]
+    assert np.array_equal(outs[0][0], outs[1][0])
+
+
+def test_run_to_run_determinism():
+    w = W.turbulence(N=32, n=16, dtype=np.float32)
+    outs = []
+    for _ in range(2):
+        h = make_gpu(w, "f32")
+        for _ in range(5):
+            h.fill_guards(); h.cfl_dt(0.4, sync=False); h.step_dev()
+        outs.append(h.download()); h.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------ edge cases -------
+def test_minimum_patch_size_and_single_patch():
+    w = W.turbulence(N=6, n=3, dtype=np.float64)               # n == ng: the thinnest legal patch
+    o = make_oracle(w)
+    U = o.fill_guards(w.U.copy(), w.nbr); dt = o.cfl_dt(U, 0.4); ref = o.step(U, dt)
+    b = make_gpu(w, "f64"); b.fill_guards(); b.step(dt)
+    assert rel_err(masked(b.download(), w.n), masked(ref, w.n)) <= 1e-12
+    b.close()
+
+
+def test_step_rejects_bad_dt_and_counts_bad_cells():
+    import ctypes as C
+    w = W.turbulence(N=16, n=8, dtype=np.float32)
+    b = make_gpu(w, "f32")
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        assert b.lib.mhd_bunch_step(b.h, bad) == -1
+    assert b.lib.mhd_bunch_cfl_dt(b.h, -0.4, None, None, None) == -1
+    assert b.status() == 0
+    U = w.U.copy(); U[4, 3, 5, 5, 5] = -1.0                     # negative energy => negative pressure
+    b.load(U); b.fill_guards(); b.step(1e-6)
+    assert b.status() >= 1
+    b.close()
+
+
+def test_launch_count_does_not_depend_on_bunch_size():
+    """bunching exists to amortise launches; here launches per step are
+    a constant of the dimensionality while the workspace holds the bunch."""
+    counts = []
+    for N in (16, 32):
+        w = W.turbulence(N=N, n=8, dtype=np.float32)             # 8 and 64 patches
+        b = make_gpu(w, "f32")
+        l0 = b.launches
+        b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+        counts.append(b.launches - l0)
+        b.close()
+    assert counts[0] == counts[1] <= 16
+
+
+# ------------------------------------------------------- full-size config 2 -------
+def test_config2_full_size_sampled_patches_and_invariants():
+    """BASELINE.json config 2 (512 patches of 32^3, fp32) in the launch configuration
+    bench.py times: sampled patches against the oracle, invariants over the whole bunch."""
+    w = W.turbulence(N=256, n=32, dtype=np.float32, config=2)
+    b = make_gpu(w, "f32")
+    b.fill_guards()
+    dt = b.cfl_dt(0.4, sync=True)
+    filled = b.download()
+    # guard fill at full size: sampled patches, bit-exact against the global periodic image
+    o_all = make_oracle(w)
+    ref_fill = o_all.fill_guards(w.U.astype(np.float64), w.nbr)
+    sample = [0, 73, 255, 300, 511]
+    for p in sample:
+        assert np.array_equal(filled[:, p].astype(np.float64), ref_fill[:, p])
+    dt_ref = o_all.cfl_dt(ref_fill, 0.4)
+    assert abs(dt - dt_ref) <= 2e-6 * dt_ref
+    b.step(dt_ref)
+    got = b.download()
+    assert b.status() == 0
+    import oracle
+    o = oracle.Oracle(w.n, len(sample), w.gamma, w.dx)
+    ref = o.step(np.ascontiguousarray(ref_fill[:, sample]), dt_ref)
+    err = rel_err(masked(got[:, sample], w.n), masked(ref, w.n))
+    assert err <= TOL_STEP["f32"], err
+    g0, g1 = W.gather(w.U, w.n, w.P).astype(np.float64), W.gather(got, w.n, w.P).astype(np.float64)
+    t0, t1 = g0[:5].sum(axis=(1, 2, 3)), g1[:5].sum(axis=(1, 2, 3))
+    assert abs(t1[0] - t0[0]) <= 2e-6 * t0[0] and abs(t1[4] - t0[4]) <= 2e-6 * t0[4]
+    div = np.roll(g1[5], -1, 2) - g1[5] + np.roll(g1[6], -1, 1) - g1[6] + np.roll(g1[7], -1, 0) - g1[7]
+    assert np.abs(div).max() / np.sqrt(np.mean(g1[5] ** 2 + g1[6] ** 2 + g1[7] ** 2)) <= 1e-4
+    b.close()
