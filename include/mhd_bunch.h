@@ -134,6 +134,12 @@ int mhd_bunch_status(mhd_bunch *b, int64_t *bad_cells);
 /* Number of kernel launches issued so far through this handle (for bench.py).           */
 int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 
+/* The step has two CUDA implementations: a fused path for bunches with three active
+ * dimensions (default there) and a general staged path (one kernel per stage of PAPER.md
+ * section 2.1.4) used for collapsed dimensions.  staged != 0 forces the staged path, for
+ * cross-checks and benchmarks; both run on the GPU.                                      */
+int mhd_bunch_set_path(mhd_bunch *b, int32_t staged);
+
 /* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
  * patches) the workspace allows.                                                        */
 int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);

@@ -18,7 +18,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
-    "mhd_bunch_chunk", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
 ]
 
 
@@ -63,6 +63,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_status.argtypes = [vp, C.POINTER(i64)]
     lib.mhd_bunch_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.mhd_bunch_chunk.argtypes = [vp, C.POINTER(i32)]
+    lib.mhd_bunch_set_path.argtypes = [vp, i32]
     lib.mhd_bunch_destroy.argtypes = [vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
@@ -196,6 +197,9 @@ class MhdBunch:
         v = C.c_int32(0)
         _check(self.lib.mhd_bunch_chunk(self.h, C.byref(v)), "mhd_bunch_chunk")
         return v.value
+
+    def set_path(self, staged):
+        _check(self.lib.mhd_bunch_set_path(self.h, 1 if staged else 0), "mhd_bunch_set_path")
 
     def set_timing(self, on):
         _check(self.lib.mhd_bunch_set_timing(self.h, 1 if on else 0), "mhd_bunch_set_timing")

@@ -1,0 +1,397 @@
+// stage_kernels.cuh -- guard fill, CFL reduction and the staged step kernels (one kernel per
+// stage of PAPER.md section 2.1.4 with HBM scratch).  The staged step is the general path
+// (any mix of active and collapsed dimensions); fused_kernels.cuh holds the fast 3D path.
+#pragma once
+#include <math.h>
+#include "bunch_types.cuh"
+#include "mhd_math.cuh"
+
+namespace mhd {
+
+// -------------------------------------------------------------------- guard fill ----
+// O1 (width 3 L212): every guard cell copies all 8 fields from
+// the neighbour's interior image, or from the nearest own interior cell (zero gradient).
+template <typename T>
+__global__ void __launch_bounds__(256) k_fill_guards(Geom G, T* __restrict__ U, const int* __restrict__ nbr) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long per = (long long)G.m[0] * G.m[1] * G.m[2];
+  if (t >= per * G.np) return;
+  const int p = (int)(t / per);
+  int r = (int)(t - (long long)p * per);
+  const int mxy = G.m[0] * G.m[1];
+  const int kk = r / mxy; r -= kk * mxy;
+  const int jj = r / G.m[0];
+  const int ii = r - jj * G.m[0];
+  const int c[3] = {ii - G.g[0], jj - G.g[1], kk - G.g[2]};
+  int o[3], src[3], cl[3];
+  bool guard = false;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    o[d] = c[d] < 0 ? -1 : (c[d] >= G.n[d] ? 1 : 0);
+    guard = guard || (o[d] != 0);
+    src[d] = c[d] - o[d] * G.n[d];
+    cl[d] = min(max(c[d], 0), G.n[d] - 1);
+  }
+  if (!guard) return;
+  const int q = nbr[p * 27 + (o[2] + 1) * 9 + (o[1] + 1) * 3 + (o[0] + 1)];
+  const long long dst = (long long)p * G.ps + G.lead + ii + (long long)jj * G.pitch + (long long)kk * G.pitch * G.m[1];
+  long long from;
+  if (q >= 0)
+    from = (long long)q * G.ps + G.lead + (src[0] + G.g[0]) + (long long)(src[1] + G.g[1]) * G.pitch +
+           (long long)(src[2] + G.g[2]) * G.pitch * G.m[1];
+  else
+    from = (long long)p * G.ps + G.lead + (cl[0] + G.g[0]) + (long long)(cl[1] + G.g[1]) * G.pitch +
+           (long long)(cl[2] + G.g[2]) * G.pitch * G.m[1];
+#pragma unroll
+  for (int f = 0; f < 8; ++f) {
+    if (q < 0 && f >= 5) {  // the closing face keeps its evolved value (O8)
+      const int a = f - 5, b = (a + 1) % 3, e = (a + 2) % 3;
+      if (G.act[a] && c[a] == G.n[a] && o[b] == 0 && o[e] == 0) continue;
+    }
+    U[f * G.fs + dst] = U[f * G.fs + from];
+  }
+}
+
+// -------------------------------------------------------------------------- CFL ----
+__device__ __forceinline__ unsigned long long enc_max(double x) { return (unsigned long long)__double_as_longlong(x); }
+
+// O9: rate = sum_d (|u_d| + c_f,d)/dx_d over active d; per-patch maximum.
+// Positive doubles order like their bit patterns, so the maximum is an integer atomicMax:
+// deterministic, no floating-point atomics.
+template <typename T>
+__global__ void __launch_bounds__(256) k_cfl(Params<T> P, unsigned long long* __restrict__ rate_bits) {
+  const Geom& G = P.G;
+  const int p = blockIdx.y;
+  const long long per = (long long)G.n[0] * G.n[1] * G.n[2];
+  double rmax = 0.0;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < per; t += (long long)gridDim.x * blockDim.x) {
+    int r = (int)t;
+    const int nxy = G.n[0] * G.n[1];
+    const int k = r / nxy; r -= k * nxy;
+    const int j = r / G.n[0];
+    const int i = r - j * G.n[0];
+    const long long c = (long long)p * G.ps + G.lead + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch +
+                        (long long)(k + G.g[2]) * G.pitch * G.m[1];
+    const T* U = P.U;
+    const T rho = U[c], irho = num<T>::rcp(rho);
+    const T u = U[G.fs + c] * irho, v = U[2 * G.fs + c] * irho, w = U[3 * G.fs + c] * irho;
+    const T bx = T(0.5) * (U[5 * G.fs + c] + U[5 * G.fs + c + G.s[0]]);
+    const T by = T(0.5) * (U[6 * G.fs + c] + U[6 * G.fs + c + G.s[1]]);
+    const T bz = T(0.5) * (U[7 * G.fs + c] + U[7 * G.fs + c + G.s[2]]);
+    const T b2 = bx * bx + by * by + bz * bz;
+    const T pr = (P.gamma - T(1)) * (U[4 * G.fs + c] - T(0.5) * rho * (u * u + v * v + w * w) - T(0.5) * b2);
+    const T gp = P.gamma * pr;
+    T rate = T(0);
+    if (G.act[0]) rate += (num<T>::abs(u) + fast_speed(gp, b2, bx * bx, irho)) * P.idx[0];
+    if (G.act[1]) rate += (num<T>::abs(v) + fast_speed(gp, b2, by * by, irho)) * P.idx[1];
+    if (G.act[2]) rate += (num<T>::abs(w) + fast_speed(gp, b2, bz * bz, irho)) * P.idx[2];
+    double rd = (double)rate;
+    if (!(rd == rd)) rd = INFINITY;  // a NaN cell forces dt = 0 rather than being ignored
+    rmax = fmax(rmax, rd);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
+  __shared__ double sm[8];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = rmax;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double v = threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) atomicMax(&rate_bits[p], enc_max(v));
+  }
+}
+
+// second stage: bunch-wide minimum step, optional per-patch steps
+__global__ void __launch_bounds__(256) k_cfl_final(const unsigned long long* __restrict__ rate_bits, int np, double courant,
+                                                   double* __restrict__ dt_out, double* __restrict__ dt_user,
+                                                   double* __restrict__ dt_patch) {
+  double rmax = 0.0;
+  for (int p = threadIdx.x; p < np; p += blockDim.x) {
+    const double r = __longlong_as_double((long long)rate_bits[p]);
+    if (dt_patch) dt_patch[p] = courant / r;
+    rmax = fmax(rmax, r);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
+  __shared__ double sm[8];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = rmax;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) rmax = fmax(rmax, sm[w]);
+    const double dt = courant / rmax;
+    *dt_out = dt;
+    if (dt_user) *dt_user = dt;
+  }
+}
+
+__global__ void k_zero_u64(unsigned long long* p, int n) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < n) p[t] = 0ull;
+}
+
+// dt for a step, on the device: either the host value or min(*dt_dev, dt_max)
+__global__ void k_set_dt(double* dst, const double* src, double host_dt, double dt_max) {
+  double dt = src ? *src : host_dt;
+  if (dt_max > 0.0 && dt > dt_max) dt = dt_max;
+  *dst = dt;
+}
+
+// ------------------------------------------------------------------- step stages ----
+// O2 (EOS L68): primitives on cells [-2, n+1]
+template <typename T>
+__global__ void __launch_bounds__(256) k_prim(Params<T> P, Box B, unsigned long long* __restrict__ bad) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const T* U = P.U;
+  const T rho = U[cu], irho = num<T>::rcp(rho);
+  const T u = U[G.fs + cu] * irho, v = U[2 * G.fs + cu] * irho, w = U[3 * G.fs + cu] * irho;
+  const T bx = T(0.5) * (U[5 * G.fs + cu] + U[5 * G.fs + cu + G.s[0]]);
+  const T by = T(0.5) * (U[6 * G.fs + cu] + U[6 * G.fs + cu + G.s[1]]);
+  const T bz = T(0.5) * (U[7 * G.fs + cu] + U[7 * G.fs + cu + G.s[2]]);
+  const T pr = (P.gamma - T(1)) *
+               (U[4 * G.fs + cu] - T(0.5) * rho * (u * u + v * v + w * w) - T(0.5) * (bx * bx + by * by + bz * bz));
+  T* q = P.W + W_Q * P.wfs + cw;
+  q[0] = rho; q[P.wfs] = u; q[2 * P.wfs] = v; q[3 * P.wfs] = w; q[4 * P.wfs] = pr;
+  q[5 * P.wfs] = bx; q[6 * P.wfs] = by; q[7 * P.wfs] = bz;
+  if (inside(G, i, j, k, 0, 0) && !(rho > T(0) && pr > T(0) && rho < T(INFINITY) && pr < T(INFINITY)))
+    atomicAdd(bad, 1ull);
+}
+
+// O4a: Eq. 7-11 and cyclic images, edges [-1, n+1]
+template <typename T>
+__global__ void __launch_bounds__(256) k_emf0(Params<T> P, Box B) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const long long sx = G.s[0], sy = G.s[1], sz = G.s[2];
+  const T* u = P.W + (W_Q + 1) * P.wfs + cw;
+  const T* v = P.W + (W_Q + 2) * P.wfs + cw;
+  const T* w = P.W + (W_Q + 3) * P.wfs + cw;
+  const T* bx = P.U + 5 * G.fs + cu;
+  const T* by = P.U + 6 * G.fs + cu;
+  const T* bz = P.U + 7 * G.fs + cu;
+  const T q4 = T(0.25), h = T(0.5);
+  T* e0 = P.W + W_E0 * P.wfs + cw;
+  {  // ez = <u><By> - <v><Bx> over cells (i-1..i, j-1..j)
+    const T ub = q4 * (u[0] + u[-sy] + u[-sx] + u[-sx - sy]);
+    const T vb = q4 * (v[0] + v[-sy] + v[-sx] + v[-sx - sy]);
+    e0[2 * P.wfs] = ub * (h * (by[0] + by[-sx])) - vb * (h * (bx[0] + bx[-sy]));
+  }
+  {  // ex = <v><Bz> - <w><By> over (j-1..j, k-1..k)
+    const T vb = q4 * (v[0] + v[-sz] + v[-sy] + v[-sy - sz]);
+    const T wb = q4 * (w[0] + w[-sz] + w[-sy] + w[-sy - sz]);
+    e0[0] = vb * (h * (bz[0] + bz[-sy])) - wb * (h * (by[0] + by[-sz]));
+  }
+  {  // ey = <w><Bx> - <u><Bz> over (k-1..k, i-1..i)
+    const T wb = q4 * (w[0] + w[-sx] + w[-sz] + w[-sz - sx]);
+    const T ub = q4 * (u[0] + u[-sx] + u[-sz] + u[-sz - sx]);
+    e0[P.wfs] = wb * (h * (bx[0] + bx[-sz])) - ub * (h * (bz[0] + bz[-sx]));
+  }
+}
+
+// O3 + O4b + O4c: limited slopes and the half-step predictor
+template <typename T>
+__global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const double* __restrict__ dtp) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const T dt = (T)(*dtp);
+  const T hdt = T(0.5) * dt;
+  const long long wfs = P.wfs;
+  const int cc[3] = {i, j, k};
+
+  // half-step face fields: Eq. 12 with dt/2
+  {
+    const T* e0 = P.W + W_E0 * wfs + cw;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const int b = (a + 1) % 3, e = (a + 2) % 3;
+      // faces [-1, n+1] along a, [-1, n] transversally
+      bool ok = true;
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+        if (G.act[d]) ok = ok && (d == a ? true : cc[d] <= G.n[d]);
+      if (!ok) continue;
+      const T* Ee = e0 + e * wfs;
+      const T* Eb = e0 + b * wfs;
+      T curl = T(0);  // differences along a collapsed dimension vanish identically
+      if (G.act[b]) curl += (Ee[G.s[b]] - Ee[0]) * P.idx[b];
+      if (G.act[e]) curl -= (Eb[G.s[e]] - Eb[0]) * P.idx[e];
+      P.W[(W_BH + a) * wfs + cw] = P.U[(5 + a) * G.fs + cu] + hdt * curl;
+    }
+  }
+  if (!inside(G, i, j, k, 1, 1)) return;
+
+  const T* q = P.W + W_Q * wfs + cw;
+  T qc[8];
+#pragma unroll
+  for (int f = 0; f < 8; ++f) qc[f] = q[f * wfs];
+  T dq[3][8];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+#pragma unroll
+    for (int f = 0; f < 8; ++f) {
+      T s = T(0);
+      if (G.act[d] && f != 5 + d) {
+        const T* qf = q + f * wfs;
+        s = limited_slope(G.limiter, qc[f] - qf[-G.s[d]], qf[G.s[d]] - qc[f]);
+      }
+      if (f != 5 + d) P.W[(W_DQ + d * 8 + f) * wfs + cw] = s;  // the normal-field slot is never read
+      dq[d][f] = s;
+    }
+  }
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      if (t == a) continue;
+      T s = T(0);
+      if (G.act[t]) {
+        const T* bf = P.U + (5 + a) * G.fs + cu;
+        s = limited_slope(G.limiter, bf[0] - bf[-G.s[t]], bf[G.s[t]] - bf[0]);
+      }
+      P.W[(W_DBF + dbf_index(a, t)) * wfs + cw] = s;
+    }
+  }
+  // primitive half step
+  T lam[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) lam[d] = G.act[d] ? hdt * P.idx[d] : T(0);
+  const T rho = qc[0], pr = qc[4], irho = num<T>::rcp(rho);
+  T rho_h = rho, p_h = pr, vh[3] = {qc[1], qc[2], qc[3]};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const T ud = qc[1 + d], dud = dq[d][1 + d];
+    rho_h -= lam[d] * (ud * dq[d][0] + rho * dud);
+    p_h -= lam[d] * (ud * dq[d][4] + P.gamma * pr * dud);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) vh[a] -= lam[d] * ud * dq[d][1 + a];
+  }
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const int b = (a + 1) % 3, e = (a + 2) % 3;
+    const T press = lam[a] * (dq[a][4] + qc[5 + b] * dq[a][5 + b] + qc[5 + e] * dq[a][5 + e]);
+    const T tens = lam[b] * qc[5 + b] * dq[b][5 + a] + lam[e] * qc[5 + e] * dq[e][5 + a];
+    vh[a] += (tens - press) * irho;
+  }
+  T* qh = P.W + W_QH * wfs + cw;
+  qh[0] = rho_h; qh[wfs] = vh[0]; qh[2 * wfs] = vh[1]; qh[3 * wfs] = vh[2]; qh[4 * wfs] = p_h;
+}
+
+// O5 + O6: face states and HLLD flux through the lower face along D
+template <typename T, int D>
+__global__ void __launch_bounds__(256) k_flux(Params<T> P, Box B) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cw = (long long)pl * G.ps + c, wfs = P.wfs;
+  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
+  const long long sd = G.s[D];
+  const T* qh = P.W + W_QH * wfs + cw;
+  const T* dq = P.W + (W_DQ + D * 8) * wfs + cw;
+  const T* bh = P.W + W_BH * wfs + cw;
+  const T h = T(0.5);
+  State1D<T> L, R;
+  // left state: upper face of cell c - e_D; right state: lower face of cell c
+  L.rho = qh[-sd] + h * dq[-sd];                               R.rho = qh[0] - h * dq[0];
+  L.u = qh[(1 + D) * wfs - sd] + h * dq[(1 + D) * wfs - sd];   R.u = qh[(1 + D) * wfs] - h * dq[(1 + D) * wfs];
+  L.v = qh[(1 + T1) * wfs - sd] + h * dq[(1 + T1) * wfs - sd]; R.v = qh[(1 + T1) * wfs] - h * dq[(1 + T1) * wfs];
+  L.w = qh[(1 + T2) * wfs - sd] + h * dq[(1 + T2) * wfs - sd]; R.w = qh[(1 + T2) * wfs] - h * dq[(1 + T2) * wfs];
+  L.p = qh[4 * wfs - sd] + h * dq[4 * wfs - sd];               R.p = qh[4 * wfs] - h * dq[4 * wfs];
+  // half-step centred transverse fields = mean of the two half-step faces
+  const T* b1 = bh + T1 * wfs;
+  const T* b2 = bh + T2 * wfs;
+  L.by = h * (b1[-sd] + b1[-sd + G.s[T1]]) + h * dq[(5 + T1) * wfs - sd];
+  R.by = h * (b1[0] + b1[G.s[T1]]) - h * dq[(5 + T1) * wfs];
+  L.bz = h * (b2[-sd] + b2[-sd + G.s[T2]]) + h * dq[(5 + T2) * wfs - sd];
+  R.bz = h * (b2[0] + b2[G.s[T2]]) - h * dq[(5 + T2) * wfs];
+  const Flux5<T> F = hlld_flux(P.gamma, L, R, bh[D * wfs]);
+  T* fl = P.W + (W_FLUX + D * 5) * wfs + cw;
+  fl[0] = F.d; fl[(1 + D) * wfs] = F.mu; fl[(1 + T1) * wfs] = F.mv; fl[(1 + T2) * wfs] = F.mw; fl[4 * wfs] = F.e;
+}
+
+// O5 + O7: corner states and the 2D Riemann problem at the edge along E
+template <typename T, int E>
+__global__ void __launch_bounds__(128) k_emf(Params<T> P, Box B) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cw = (long long)pl * G.ps + c, wfs = P.wfs;
+  constexpr int A = (E + 1) % 3, Bd = (E + 2) % 3;
+  const long long sa = G.s[A], sb = G.s[Bd], se = G.s[E];
+  const T* qh = P.W + W_QH * wfs + cw;
+  const T* da = P.W + (W_DQ + A * 8) * wfs + cw;
+  const T* db = P.W + (W_DQ + Bd * 8) * wfs + cw;
+  const T* bh = P.W + W_BH * wfs + cw;
+  const T h = T(0.5);
+  // corner of cell at offset o seen with signs (sga, sgb)
+  auto corner = [&](long long o, T sga, T sgb) {
+    Corner<T> q;
+    q.rho = qh[o] + sga * h * da[o] + sgb * h * db[o];
+    q.ua = qh[(1 + A) * wfs + o] + sga * h * da[(1 + A) * wfs + o] + sgb * h * db[(1 + A) * wfs + o];
+    q.ub = qh[(1 + Bd) * wfs + o] + sga * h * da[(1 + Bd) * wfs + o] + sgb * h * db[(1 + Bd) * wfs + o];
+    q.p = qh[4 * wfs + o] + sga * h * da[4 * wfs + o] + sgb * h * db[4 * wfs + o];
+    const T* be = bh + E * wfs + o;
+    q.be = h * (be[0] + be[se]) + sga * h * da[(5 + E) * wfs + o] + sgb * h * db[(5 + E) * wfs + o];
+    return q;
+  };
+  // SW = RT of cell (a-1,b-1), SE = LT of (a,b-1), NW = RB of (a-1,b), NE = LB of (a,b)
+  const Corner<T> sw = corner(-sa - sb, T(1), T(1)), se_ = corner(-sb, T(-1), T(1));
+  const Corner<T> nw = corner(-sa, T(1), T(-1)), ne = corner(0, T(-1), T(-1));
+  const T* dba = P.W + (W_DBF + dbf_index(A, Bd)) * wfs + cw;  // slope of b_A along B
+  const T* dbb = P.W + (W_DBF + dbf_index(Bd, A)) * wfs + cw;  // slope of b_B along A
+  const T* ba = bh + A * wfs;
+  const T* bb = bh + Bd * wfs;
+  const T AS = ba[-sb] + h * dba[-sb], AN = ba[0] - h * dba[0];
+  const T BW = bb[-sa] + h * dbb[-sa], BE = bb[0] - h * dbb[0];
+  P.W[(W_EMF + E) * wfs + cw] = emf_2d(P.gamma, G.emf_solver, sw, se_, nw, ne, AS, AN, BW, BE);
+}
+
+// O8: conservative update + constrained transport with the metric factor of each term
+// (Eq. 12; L154)
+template <typename T>
+__global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double* __restrict__ dtp) {
+  const Geom& G = P.G;
+  int pl, i, j, k; long long c;
+  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c, wfs = P.wfs;
+  const T dt = (T)(*dtp);
+  const int cc[3] = {i, j, k};
+  if (inside(G, i, j, k, 0, 0)) {
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      T v = P.U[f * G.fs + cu];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        if (!G.act[d]) continue;
+        const T* fl = P.W + (W_FLUX + d * 5 + f) * wfs + cw;
+        v -= dt * P.idx[d] * (fl[G.s[d]] - fl[0]);
+      }
+      P.Un[f * G.fs + cu] = v;
+    }
+  }
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const int b = (a + 1) % 3, e = (a + 2) % 3;
+    // faces 0..n along a (n = closing face), interior transversally
+    bool ok = true;
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+      if (G.act[d] && d != a) ok = ok && cc[d] < G.n[d];
+    if (!ok) continue;
+    const T* Ee = P.W + (W_EMF + e) * wfs + cw;
+    const T* Eb = P.W + (W_EMF + b) * wfs + cw;
+    T curl = T(0);
+    if (G.act[b]) curl += (Ee[G.s[b]] - Ee[0]) * P.idx[b];
+    if (G.act[e]) curl -= (Eb[G.s[e]] - Eb[0]) * P.idx[e];
+    P.Un[(5 + a) * G.fs + cu] = P.U[(5 + a) * G.fs + cu] + dt * curl;
+  }
+}
+
+
+}  // namespace mhd

@@ -96,6 +96,43 @@ def test_one_step_matches_oracle(name, dtype, limiter, emf_solver):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("limiter,emf_solver", [(1, 0), (2, 1)])
+@pytest.mark.parametrize("name", ["turb16", "turb_ragged", "turb_self"])
+def test_staged_path_on_3d_bunches_matches_oracle(name, dtype, limiter, emf_solver):
+    """3D bunches default to the fused kernels; the general staged kernels must agree with
+    the oracle there as well (they are the only path for collapsed dimensions)."""
+    w = small_workloads(dtype)[name]
+    o = make_oracle(w, limiter, emf_solver)
+    U = o.fill_guards(w.U.astype(np.float64), w.nbr)
+    dt = o.cfl_dt(U, 0.4)
+    ref = o.step(U, dt)
+    b = make_gpu(w, dtype, limiter, emf_solver, staged=True)
+    b.fill_guards()
+    b.step(dt)
+    err = rel_err(masked(b.download(), w.n), masked(ref, w.n))
+    assert err <= TOL_STEP[dtype], (name, dtype, err)
+    b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_fused_tiles_cover_large_and_odd_patches(dtype):
+    """Patch sizes that need several (x,y) tiles of the fused kernel with ragged edges:
+    40 x 20 x 12 cells (x tiles 32+8, y tiles 8+8+4) and 64 x 8 x 8."""
+    for N, n in (((80, 40, 24), (40, 20, 12)), ((64, 16, 16), (64, 8, 8))):
+        w = W.turbulence(N=N, n=n, dtype=NPD[dtype])
+        o = make_oracle(w)
+        U = o.fill_guards(w.U.astype(np.float64), w.nbr)
+        dt = o.cfl_dt(U, 0.4)
+        ref = o.step(U, dt)
+        b = make_gpu(w, dtype)
+        b.fill_guards()
+        b.step(dt)
+        err = rel_err(masked(b.download(), w.n), masked(ref, w.n))
+        assert err <= TOL_STEP[dtype], (n, dtype, err)
+        b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_sub_bunch_chunking_is_bitwise_invisible(dtype):
     w = small_workloads(dtype)["turb16"]                        # 8 patches
     outs = []
