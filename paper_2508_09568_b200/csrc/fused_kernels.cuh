@@ -50,11 +50,17 @@ template <typename T, int TXM, int TYM> struct FusedCfg {
   static constexpr int VE = 16 / (int)sizeof(T);                           // elements per 16 bytes
   static constexpr int DW = ((TXM + 2 + VE - 1) / VE) * VE, DH = TYM + 2, DC = DW * DH;
   static constexpr int FW = TXM + 1, FH = TYM + 1;
-  static constexpr int NTH = ((FW * FH + 31) / 32) * 32;
-  static constexpr int XV = 4;                                      // values per exchange pass
+  // Thread layout: threads [0, TXM*FH) own face columns 0..TXM-1 row by row (a warp never
+  // straddles tile rows unevenly, so shared-memory accesses are conflict-free); one more warp
+  // starting at CB owns the closing column fi = TXM, one lane per row.
+  static constexpr int CB = ((TXM * FH + 31) / 32) * 32;
+  static constexpr int NTH = CB + 32;
+  static_assert(FH <= 32 && 32 % TXM == 0, "tile shape");
+  static constexpr int XV = sizeof(T) == 8 ? 3 : 4;                 // values per y-exchange pass (7 in all)
+  static constexpr int XC = 7;                                      // values the closing column hands to column TXM-1
   static constexpr uint32_t slot_bytes = (uint32_t)(sizeof(T) * D_COUNT * DC);
   static constexpr uint32_t slot_stride = (slot_bytes + 127u) / 128u * 128u;   // TMA destinations: 128-byte aligned
-  static constexpr size_t smem = 2 * (size_t)slot_stride + sizeof(T) * (size_t)(XV * NTH) + 16;
+  static constexpr size_t smem = 2 * (size_t)slot_stride + sizeof(T) * (size_t)(XV * NTH + XC * 16) + 16;
 };
 
 // HLLD flux through the face between cell `cl` and cell `cr` along D; pointers address
@@ -154,24 +160,24 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   auto Bs = [&](int plane_, int a) { return QB + (((plane_ + 3) % 3) * 3 + a) * PA; };
   auto Es = [&](int plane_, int a) { return E + (((plane_ + 2) & 1) * 3 + a) * PA; };
 
-  T Ucur[8], Unxt[8], Uprev[8];
+  // Own-column registers.  The state of plane r is loaded at the top of iteration r but its
+  // hydro part is first used in iteration r+1 and its bx, by after the first barrier, so the
+  // loads overlap a whole iteration; only bz is needed at once and runs one plane ahead.
+  T Ucur[8], Uprev[8];
   T bxm[3] = {T(0), T(0), T(0)}, bym[3] = {T(0), T(0), T(0)};   // own raw bx, by at planes r-1, r-2, r-3
-  T bzm1 = T(0), bzm2 = T(0);                                   // own raw bz at planes r-1, r-2
+  T bznext = T(0);
 #pragma unroll
-  for (int f = 0; f < 8; ++f) { Ucur[f] = T(0); Unxt[f] = T(0); Uprev[f] = T(0); }
+  for (int f = 0; f < 8; ++f) { Ucur[f] = T(0); Uprev[f] = T(0); }
   const int rlo = -2, rhi = nz + 2;
-  if (rowok) {
-#pragma unroll
-    for (int f = 0; f < 8; ++f) Unxt[f] = P.U[f * fs + cbase + (long long)rlo * plane];
-  }
+  if (rowok) bznext = P.U[7 * fs + cbase + (long long)rlo * plane];
   unsigned int nbad = 0;
 
   for (int r = rlo; r <= rhi; ++r) {
+    Ucur[7] = bznext;
+    if (rowok) {
 #pragma unroll
-    for (int f = 0; f < 8; ++f) Ucur[f] = Unxt[f];
-    if (rowok && r + 1 <= rhi) {
-#pragma unroll
-      for (int f = 0; f < 8; ++f) Unxt[f] = P.U[f * fs + cbase + (long long)(r + 1) * plane];
+      for (int f = 0; f < 7; ++f) Ucur[f] = P.U[f * fs + cbase + (long long)r * plane];
+      if (r + 1 <= rhi) bznext = P.U[7 * fs + cbase + (long long)(r + 1) * plane];
     }
 
     // ---- primitives of plane r-1 (O2): needs bx(i+1), by(j+1) of plane r-1 and bz of plane r
@@ -218,14 +224,38 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
       const T* qc = Qs(kd, 0) + o;
       const T* qm = Qs(kd - 1, 0) + o;
       const T* qp = Qs(kd + 1, 0) + o;
-      T c[8], dq[3][8];
+      T* D = P.D + (long long)pl * P.DG.ps + (i + 1) + (long long)(j + 1) * P.DG.pitch +
+             (long long)(kd + 1) * P.DG.pitch * P.DG.ny;
+      const long long dfs = P.DG.fs;
+      T c[8];
 #pragma unroll
       for (int f = 0; f < 8; ++f) c[f] = qc[f * PA];
+      // slopes (O3) and the primitive half step (O4c), one direction at a time: every term of
+      // the predictor that involves direction d needs only the slopes along d
+      const T rho = c[0], p_ = c[4], ir = num<T>::rcp(rho);
+      const T lam[3] = {lx, ly, lz};
+      T rho_h = rho, p_h = p_, vh[3] = {c[1], c[2], c[3]};
 #pragma unroll
-      for (int f = 0; f < 8; ++f) {
-        dq[0][f] = (f == 5) ? T(0) : limited_slope(lim, c[f] - qc[f * PA - 1], qc[f * PA + 1] - c[f]);
-        dq[1][f] = (f == 6) ? T(0) : limited_slope(lim, c[f] - qc[f * PA - PW], qc[f * PA + PW] - c[f]);
-        dq[2][f] = (f == 7) ? T(0) : limited_slope(lim, c[f] - qm[f * PA], qp[f * PA] - c[f]);
+      for (int d = 0; d < 3; ++d) {
+        T dq[8];
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+          if (f == 5 + d) { dq[f] = T(0); continue; }
+          const T lo = d == 0 ? qc[f * PA - 1] : (d == 1 ? qc[f * PA - PW] : qm[f * PA]);
+          const T hi = d == 0 ? qc[f * PA + 1] : (d == 1 ? qc[f * PA + PW] : qp[f * PA]);
+          dq[f] = limited_slope(lim, c[f] - lo, hi - c[f]);
+          D[(long long)dq_slot(d, f) * dfs] = dq[f];
+        }
+        const int b = (d + 1) % 3, e = (d + 2) % 3;
+        const T ud = c[1 + d], dud = dq[1 + d];
+        rho_h -= lam[d] * (ud * dq[0] + rho * dud);
+        p_h -= lam[d] * (ud * dq[4] + P.gamma * p_ * dud);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) vh[a] -= lam[d] * ud * dq[1 + a];
+        // -(1/rho) d_d (p + B_b^2/2 + B_e^2/2) acts on u_d;  +(B_d/rho) d_d B_a acts on u_a, a != d
+        vh[d] -= lam[d] * (dq[4] + c[5 + b] * dq[5 + b] + c[5 + e] * dq[5 + e]) * ir;
+        vh[b] += lam[d] * c[5 + d] * dq[5 + b] * ir;
+        vh[e] += lam[d] * c[5 + d] * dq[5 + e] * ir;
       }
       const T *bx = Bs(kd, 0) + o, *by = Bs(kd, 1) + o, *bz = Bs(kd, 2) + o;
       const T bxc = bx[0], byc = by[0], bzc = bz[0];
@@ -248,48 +278,19 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
       const T bzu = Bs(kd + 1, 2)[o];
       const T bzh_up = bzu + (lx * (ey1[1] - ey1[0]) - ly * (ex1[PW] - ex1[0]));
       const T bchx = h * (bxh + bxh_at(1)), bchy = h * (byh + byh_at(PW)), bchz = h * (bzh + bzh_up);
-      // primitive half step (O4c)
-      const T rho = c[0], p_ = c[4], ir = num<T>::rcp(rho);
-      const T lam[3] = {lx, ly, lz};
-      T rho_h = rho, p_h = p_, vh[3] = {c[1], c[2], c[3]};
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        const T ud = c[1 + d], dud = dq[d][1 + d];
-        rho_h -= lam[d] * (ud * dq[d][0] + rho * dud);
-        p_h -= lam[d] * (ud * dq[d][4] + P.gamma * p_ * dud);
-#pragma unroll
-        for (int a = 0; a < 3; ++a) vh[a] -= lam[d] * ud * dq[d][1 + a];
-      }
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        const int b = (a + 1) % 3, e = (a + 2) % 3;
-        const T press = lam[a] * (dq[a][4] + c[5 + b] * dq[a][5 + b] + c[5 + e] * dq[a][5 + e]);
-        const T tens = lam[b] * c[5 + b] * dq[b][5 + a] + lam[e] * c[5 + e] * dq[e][5 + a];
-        vh[a] += (tens - press) * ir;
-      }
-      T* D = P.D + (long long)pl * P.DG.ps + (i + 1) + (long long)(j + 1) * P.DG.pitch +
-             (long long)(kd + 1) * P.DG.pitch * P.DG.ny;
-      const long long dfs = P.DG.fs;
       D[(D_QH + 0) * dfs] = rho_h; D[(D_QH + 1) * dfs] = vh[0]; D[(D_QH + 2) * dfs] = vh[1]; D[(D_QH + 3) * dfs] = vh[2];
       D[(D_QH + 4) * dfs] = p_h;
       D[(D_BCH + 0) * dfs] = bchx; D[(D_BCH + 1) * dfs] = bchy; D[(D_BCH + 2) * dfs] = bchz;
       D[(D_BH + 0) * dfs] = bxh; D[(D_BH + 1) * dfs] = byh; D[(D_BH + 2) * dfs] = bzh;
-#pragma unroll
-      for (int d = 0; d < 3; ++d)
-#pragma unroll
-        for (int f = 0; f < 8; ++f)
-          if (f != 5 + d) D[(long long)dq_slot(d, f) * dfs] = dq[d][f];
 #pragma unroll
       for (int a = 0; a < 6; ++a) D[(D_DBF + a) * dfs] = db[a];
     }
     // shift the own-column history
     bxm[2] = bxm[1]; bxm[1] = bxm[0]; bxm[0] = Ucur[5];
     bym[2] = bym[1]; bym[1] = bym[0]; bym[0] = Ucur[6];
-    bzm2 = bzm1; bzm1 = Ucur[7];
 #pragma unroll
     for (int f = 0; f < 8; ++f) Uprev[f] = Ucur[f];
   }
-  (void)bzm2;
   if (nbad) atomicAdd(bad, (unsigned long long)nbad);
 }
 
@@ -319,8 +320,9 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
   using C = FusedCfg<T, TXM, TYM>;
   constexpr int DC = C::DC, DW = C::DW, NTH = C::NTH;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* X = reinterpret_cast<T*>(smem_raw + 2 * C::slot_stride);                 // [XV][NTH]
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * C::slot_stride + sizeof(T) * C::XV * NTH);
+  T* X = reinterpret_cast<T*>(smem_raw + 2 * C::slot_stride);                 // [XV][NTH]  +y exchange
+  T* XCs = X + C::XV * NTH;                                                   // [XC][16]   closing column
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * C::slot_stride + sizeof(T) * (C::XV * NTH + C::XC * 16));
 
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
@@ -329,8 +331,11 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
   const int x0 = xt * TXM, y0 = yt * TYM;
   const int tw = min(TXM, nx - x0), th = min(TYM, ny - y0);
   const int t = threadIdx.x;
-  const int fj = t / C::FW, fi = t - fj * C::FW;
-  const bool active = (fi <= tw) && (fj <= th);
+  const bool colthr = t >= C::CB;                       // closing-column warp
+  const int fj = colthr ? t - C::CB : t / TXM;
+  const int fi = colthr ? TXM : t - fj * TXM;
+  const bool active = (fi <= tw) && (fj <= th) && (colthr ? fj < C::FH : t < TXM * C::FH);
+  const int ty = colthr ? t + 1 : t + TXM;              // thread that owns (fi, fj+1)
   const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1];
   const T dt = (T)(*dtp);
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
@@ -390,29 +395,69 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
       cey = edge_emf<T, DC, 1>(dp_ - 1, dc_ - 1, dp_, dc_, gamma, solver);
     }
 
-    // [B] exchange of the previous plane's in-plane values with the +x / +y neighbours.
-    // pass 1 also marks the point where every thread is done with slot prv (plane k-1).
+    // [B] exchange of the previous plane's in-plane values: the +x neighbour is the next lane
+    // (warp shuffle; the closing column hands its values over through XCs), the +y neighbour
+    // goes through X in two passes.  Barrier 1 also marks the point where every thread is
+    // done with slot prv (plane k-1), so the next plane can be prefetched into it.
     Flux5<T> xF = {}, yF = {};
     T xez = T(0), xey = T(0), yez = T(0), yex = T(0);
-    X[0 * NTH + t] = pFx.d; X[1 * NTH + t] = pFx.mu; X[2 * NTH + t] = pFx.mv; X[3 * NTH + t] = pFx.mw;
-    __syncthreads();
+    T un[8];
+#pragma unroll
+    for (int f = 0; f < 8; ++f) un[f] = T(0);
+    if (k >= 1) {
+      // U^n of the cell this thread updates: issued here so the loads fly during the exchange
+      const long long cu = ubase + (long long)(k - 1) * plane;
+      const long long fs = G.fs;
+      if (k - 1 < nz) {
+        if (cell) {
+#pragma unroll
+          for (int f = 0; f < 5; ++f) un[f] = P.U[f * fs + cu];
+        }
+        if (fj < th && (fi < tw || (fi == tw && lastx))) un[5] = P.U[5 * fs + cu];
+        if (fi < tw && (fj < th || (fj == th && lasty))) un[6] = P.U[6 * fs + cu];
+      }
+      if (cell) un[7] = P.U[7 * fs + cu];
+      if (colthr && fj < 16) {
+        XCs[0 * 16 + fj] = pFx.d; XCs[1 * 16 + fj] = pFx.mu; XCs[2 * 16 + fj] = pFx.mv; XCs[3 * 16 + fj] = pFx.mw;
+        XCs[4 * 16 + fj] = pFx.e; XCs[5 * 16 + fj] = pez;    XCs[6 * 16 + fj] = pey;
+      }
+    }
+    // +y exchange: 7 values in passes of XV through X; pass 0 is written before barrier 1
+    const T sendv[7] = {pFy.d, pFy.mu, pFy.mv, pFy.mw, pFy.e, pez, pex};
+    T recv[7] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    constexpr int NPASS = (7 + C::XV - 1) / C::XV;
+    if (k >= 1) {
+#pragma unroll
+      for (int v = 0; v < C::XV; ++v) X[v * NTH + t] = sendv[v];
+    }
+    __syncthreads();                                                   // barrier 1
     if (t == 0 && k + 1 <= nz) issue(k + 1, prv);   // prefetch plane k+1 while [B] and [C] run
     if (k >= 1) {
-      if (fi < tw) { xF.d = X[0 * NTH + t + 1]; xF.mu = X[1 * NTH + t + 1]; xF.mv = X[2 * NTH + t + 1]; xF.mw = X[3 * NTH + t + 1]; }
-      __syncthreads();
-      X[0 * NTH + t] = pFx.e; X[1 * NTH + t] = pez; X[2 * NTH + t] = pey; X[3 * NTH + t] = pex;
-      __syncthreads();
-      if (fi < tw) { xF.e = X[0 * NTH + t + 1]; xez = X[1 * NTH + t + 1]; xey = X[2 * NTH + t + 1]; }
-      if (fj < th) { yez = X[1 * NTH + t + C::FW]; yex = X[3 * NTH + t + C::FW]; }
-      __syncthreads();
-      X[0 * NTH + t] = pFy.d; X[1 * NTH + t] = pFy.mu; X[2 * NTH + t] = pFy.mv; X[3 * NTH + t] = pFy.mw;
-      __syncthreads();
-      if (fj < th) { yF.d = X[0 * NTH + t + C::FW]; yF.mu = X[1 * NTH + t + C::FW]; yF.mv = X[2 * NTH + t + C::FW]; yF.mw = X[3 * NTH + t + C::FW]; }
-      __syncthreads();
-      X[0 * NTH + t] = pFy.e;
-      __syncthreads();
-      if (fj < th) yF.e = X[0 * NTH + t + C::FW];
-      __syncthreads();
+      xF.d = __shfl_down_sync(0xffffffffu, pFx.d, 1);   xF.mu = __shfl_down_sync(0xffffffffu, pFx.mu, 1);
+      xF.mv = __shfl_down_sync(0xffffffffu, pFx.mv, 1); xF.mw = __shfl_down_sync(0xffffffffu, pFx.mw, 1);
+      xF.e = __shfl_down_sync(0xffffffffu, pFx.e, 1);
+      xez = __shfl_down_sync(0xffffffffu, pez, 1);      xey = __shfl_down_sync(0xffffffffu, pey, 1);
+      if (!colthr && fi == TXM - 1 && fj < 16) {       // the +x neighbour is the closing column
+        xF.d = XCs[0 * 16 + fj]; xF.mu = XCs[1 * 16 + fj]; xF.mv = XCs[2 * 16 + fj]; xF.mw = XCs[3 * 16 + fj];
+        xF.e = XCs[4 * 16 + fj]; xez = XCs[5 * 16 + fj];   xey = XCs[6 * 16 + fj];
+      }
+      const bool ynb = (fj < th) && active;
+#pragma unroll
+      for (int ps = 0; ps < NPASS; ++ps) {
+        if (ps > 0) {
+#pragma unroll
+          for (int v = 0; v < C::XV; ++v)
+            if (ps * C::XV + v < 7) X[v * NTH + t] = sendv[ps * C::XV + v];
+          __syncthreads();
+        }
+        if (ynb) {
+#pragma unroll
+          for (int v = 0; v < C::XV; ++v)
+            if (ps * C::XV + v < 7) recv[ps * C::XV + v] = X[v * NTH + ty];
+        }
+        __syncthreads();
+      }
+      yF.d = recv[0]; yF.mu = recv[1]; yF.mv = recv[2]; yF.mw = recv[3]; yF.e = recv[4]; yez = recv[5]; yex = recv[6];
 
       // update of plane k-1
       const long long cu = ubase + (long long)(k - 1) * plane;
@@ -420,22 +465,22 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
       if (k - 1 < nz) {
         if (cell) {
           // O8: U - dt * sum_d (F_d(c+e_d) - F_d(c)) / dx_d
-          P.Un[cu] = P.U[cu] - cx * (xF.d - pFx.d) - cy * (yF.d - pFy.d) - cz * (cFz.d - pFz.d);
+          P.Un[cu] = un[0] - cx * (xF.d - pFx.d) - cy * (yF.d - pFy.d) - cz * (cFz.d - pFz.d);
           // momentum components are stored by solver frame: x-face (mu,mv,mw)=(mx,my,mz);
           // y-face (mu,mv,mw)=(my,mz,mx); z-face (mu,mv,mw)=(mz,mx,my)
-          P.Un[fs + cu] = P.U[fs + cu] - cx * (xF.mu - pFx.mu) - cy * (yF.mw - pFy.mw) - cz * (cFz.mv - pFz.mv);
-          P.Un[2 * fs + cu] = P.U[2 * fs + cu] - cx * (xF.mv - pFx.mv) - cy * (yF.mu - pFy.mu) - cz * (cFz.mw - pFz.mw);
-          P.Un[3 * fs + cu] = P.U[3 * fs + cu] - cx * (xF.mw - pFx.mw) - cy * (yF.mv - pFy.mv) - cz * (cFz.mu - pFz.mu);
-          P.Un[4 * fs + cu] = P.U[4 * fs + cu] - cx * (xF.e - pFx.e) - cy * (yF.e - pFy.e) - cz * (cFz.e - pFz.e);
+          P.Un[fs + cu] = un[1] - cx * (xF.mu - pFx.mu) - cy * (yF.mw - pFy.mw) - cz * (cFz.mv - pFz.mv);
+          P.Un[2 * fs + cu] = un[2] - cx * (xF.mv - pFx.mv) - cy * (yF.mu - pFy.mu) - cz * (cFz.mw - pFz.mw);
+          P.Un[3 * fs + cu] = un[3] - cx * (xF.mw - pFx.mw) - cy * (yF.mv - pFy.mv) - cz * (cFz.mu - pFz.mu);
+          P.Un[4 * fs + cu] = un[4] - cx * (xF.e - pFx.e) - cy * (yF.e - pFy.e) - cz * (cFz.e - pFz.e);
         }
         // Eq. 12 with the metric factor of each term (L154)
         if (fj < th && (fi < tw || (fi == tw && lastx)))       // bx on faces x0..x0+tw (closing face at the patch end)
-          P.Un[5 * fs + cu] = P.U[5 * fs + cu] + (cy * (yez - pez) - cz * (cey - pey));
+          P.Un[5 * fs + cu] = un[5] + (cy * (yez - pez) - cz * (cey - pey));
         if (fi < tw && (fj < th || (fj == th && lasty)))
-          P.Un[6 * fs + cu] = P.U[6 * fs + cu] + (cz * (cex - pex) - cx * (xez - pez));
+          P.Un[6 * fs + cu] = un[6] + (cz * (cex - pex) - cx * (xez - pez));
       }
       if (cell)                                                 // bz on faces 0..nz (k-1 == nz: closing face)
-        P.Un[7 * fs + cu] = P.U[7 * fs + cu] + (cx * (xey - pey) - cy * (yex - pex));
+        P.Un[7 * fs + cu] = un[7] + (cx * (xey - pey) - cy * (yex - pex));
     }
 
     // [C] in-plane values of plane k become the "previous" set of the next iteration
