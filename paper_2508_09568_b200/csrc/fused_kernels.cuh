@@ -123,7 +123,7 @@ __device__ __forceinline__ T edge_emf(const T* __restrict__ csw, const T* __rest
 __host__ __device__ constexpr int predict_max_threads(int ty) { return ty == 8 ? 512 : 832; }
 
 template <typename T, int TY>
-__global__ void __launch_bounds__(predict_max_threads(TY), 1)
+__global__ void __launch_bounds__(predict_max_threads(TY), (TY == 8 && sizeof(T) == 4) ? 2 : 1)
 k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Geom& G = P.G;

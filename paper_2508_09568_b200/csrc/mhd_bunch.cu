@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <new>
 #include <vector>
@@ -190,9 +191,12 @@ inline unsigned blocks_for(long long threads, int bs) { return (unsigned)((threa
 template <typename T>
 int launch_fill(mhd_bunch* b) {
   const Geom& G = b->G;
-  const long long tot = (long long)G.m[0] * G.m[1] * G.m[2] * G.np;
-  { LaunchScope ls(b, KC_FILL);
-    k_fill_guards<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr); }
+  const FillMap M = make_fill_map(G);
+  const long long tot = (long long)M.start[6] * G.np;
+  if (tot > 0) {
+    LaunchScope ls(b, KC_FILL);
+    k_fill_guards<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, M, (T*)b->state[b->cur], b->d_nbr);
+  }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
 }
@@ -396,7 +400,9 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
     const bool f64 = desc->dtype == MHD_F64;
     b->DG = make_dgeom(b->G, b->esz, b->chunk);
     b->pred_ty = 0;
+    const char* env_ty = getenv("MHD_PREDICT_TY");   // tuning knob: force the predictor's y-tile
     for (int ty : {16, 8, 4}) {
+      if (env_ty && atoi(env_ty) != ty) continue;
       const size_t pa = (size_t)(b->G.n[0] + 5) * (ty + 5);
       if (pa <= (size_t)predict_max_threads(ty) && 39 * pa * b->esz <= (size_t)220 * 1024) { b->pred_ty = ty; break; }
     }

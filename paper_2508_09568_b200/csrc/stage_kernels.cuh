@@ -11,44 +11,81 @@ namespace mhd {
 // -------------------------------------------------------------------- guard fill ----
 // O1 (width 3 L212): every guard cell copies all 8 fields from
 // the neighbour's interior image, or from the nearest own interior cell (zero gradient).
+// Threads enumerate GUARD CELLS ONLY, slab by slab (z-low, z-high, y-low, y-high, x-low,
+// x-high) with x fastest, so the full-row slabs read and write contiguous runs; each thread
+// moves the 8 fields of one guard cell (8 independent loads in flight, then 8 stores).
+struct FillMap {
+  int start[7];      // first guard index of each slab; start[6] = guard cells per patch
+  int lo[6][3];      // first cell (i,j,k) of the slab, interior-relative
+  int ext[6][3];     // extents of the slab
+};
+
+inline FillMap make_fill_map(const Geom& G) {
+  FillMap M;
+  int n = 0, s = 0;
+  // the six slabs tile the guard shell: z slabs span the padded x,y range, y slabs the padded
+  // x range and interior z, x slabs interior y and z
+  for (int d = 2; d >= 0; --d) {
+    for (int side = 0; side < 2; ++side) {
+      M.start[s] = n;
+      for (int a = 0; a < 3; ++a) {
+        if (a == d) { M.lo[s][a] = side ? G.n[a] : -G.g[a]; M.ext[s][a] = G.g[a]; }
+        else if (a > d) { M.lo[s][a] = 0; M.ext[s][a] = G.n[a]; }
+        else { M.lo[s][a] = -G.g[a]; M.ext[s][a] = G.m[a]; }
+      }
+      n += M.ext[s][0] * M.ext[s][1] * M.ext[s][2];
+      ++s;
+    }
+  }
+  M.start[6] = n;
+  return M;
+}
+
 template <typename T>
-__global__ void __launch_bounds__(256) k_fill_guards(Geom G, T* __restrict__ U, const int* __restrict__ nbr) {
+__global__ void __launch_bounds__(256) k_fill_guards(Geom G, FillMap M, T* __restrict__ U, const int* __restrict__ nbr) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long per = (long long)G.m[0] * G.m[1] * G.m[2];
-  if (t >= per * G.np) return;
+  const int per = M.start[6];
+  if (t >= (long long)per * G.np) return;
   const int p = (int)(t / per);
   int r = (int)(t - (long long)p * per);
-  const int mxy = G.m[0] * G.m[1];
-  const int kk = r / mxy; r -= kk * mxy;
-  const int jj = r / G.m[0];
-  const int ii = r - jj * G.m[0];
-  const int c[3] = {ii - G.g[0], jj - G.g[1], kk - G.g[2]};
+  // slab parameters by an unrolled compare chain: indices into M stay compile-time, so the
+  // parameter struct is read from constant space and never copied to local memory
+  int st = 0, l0 = M.lo[0][0], l1 = M.lo[0][1], l2 = M.lo[0][2], e0 = M.ext[0][0], e1 = M.ext[0][1];
+#pragma unroll
+  for (int q = 1; q < 6; ++q) {
+    if (r >= M.start[q]) { st = M.start[q]; l0 = M.lo[q][0]; l1 = M.lo[q][1]; l2 = M.lo[q][2]; e0 = M.ext[q][0]; e1 = M.ext[q][1]; }
+  }
+  r -= st;
+  const int exy = e0 * e1;
+  const int kk = r / exy; r -= kk * exy;
+  const int jj = r / e0;
+  const int ii = r - jj * e0;
+  const int c[3] = {l0 + ii, l1 + jj, l2 + kk};
   int o[3], src[3], cl[3];
-  bool guard = false;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     o[d] = c[d] < 0 ? -1 : (c[d] >= G.n[d] ? 1 : 0);
-    guard = guard || (o[d] != 0);
     src[d] = c[d] - o[d] * G.n[d];
     cl[d] = min(max(c[d], 0), G.n[d] - 1);
   }
-  if (!guard) return;
   const int q = nbr[p * 27 + (o[2] + 1) * 9 + (o[1] + 1) * 3 + (o[0] + 1)];
-  const long long dst = (long long)p * G.ps + G.lead + ii + (long long)jj * G.pitch + (long long)kk * G.pitch * G.m[1];
+  const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1];
+  const long long dst = (long long)p * G.ps + G.lead + (c[0] + G.g[0]) + (c[1] + G.g[1]) * pitch + (c[2] + G.g[2]) * plane;
   long long from;
   if (q >= 0)
-    from = (long long)q * G.ps + G.lead + (src[0] + G.g[0]) + (long long)(src[1] + G.g[1]) * G.pitch +
-           (long long)(src[2] + G.g[2]) * G.pitch * G.m[1];
+    from = (long long)q * G.ps + G.lead + (src[0] + G.g[0]) + (src[1] + G.g[1]) * pitch + (src[2] + G.g[2]) * plane;
   else
-    from = (long long)p * G.ps + G.lead + (cl[0] + G.g[0]) + (long long)(cl[1] + G.g[1]) * G.pitch +
-           (long long)(cl[2] + G.g[2]) * G.pitch * G.m[1];
+    from = (long long)p * G.ps + G.lead + (cl[0] + G.g[0]) + (cl[1] + G.g[1]) * pitch + (cl[2] + G.g[2]) * plane;
+  T v[8];
+#pragma unroll
+  for (int f = 0; f < 8; ++f) v[f] = U[f * G.fs + from];
 #pragma unroll
   for (int f = 0; f < 8; ++f) {
     if (q < 0 && f >= 5) {  // the closing face keeps its evolved value (O8)
       const int a = f - 5, b = (a + 1) % 3, e = (a + 2) % 3;
       if (G.act[a] && c[a] == G.n[a] && o[b] == 0 && o[e] == 0) continue;
     }
-    U[f * G.fs + dst] = U[f * G.fs + from];
+    U[f * G.fs + dst] = v[f];
   }
 }
 
