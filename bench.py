@@ -49,23 +49,55 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-# algorithmic HBM bytes per interior cell-update of each kernel class, in units of
-# sizeof(real): compulsory reads + writes of that pass with perfect on-chip reuse
-# (DESIGN.md "Kernels").  m = padded/interior volume ratio of the pass's input halo.
-def algorithmic_values_per_cell(cls, n, ng=3):
+# Algorithmic work per interior cell-update of each kernel class.
+# bytes: compulsory HBM reads + writes of that pass with perfect on-chip reuse, in units of
+#        sizeof(real); r(a,b) = volume ratio of a pass that covers cells [-a, n-1+b].
+# flops: counted on the oracle's source by oracle/opcount.cpp at 32^3 (add+mul+div+sqrt,
+#        FMA = 2): whole step 3625.4, cfl 86; HLLD solve 392, HLLD-2D edge solve 453.
+STEP_FLOPS_32 = 3625.4
+CFL_FLOPS = 86.0
+
+
+def algorithmic_work(cls, n, ng=3):
     r = lambda a, b: ((n + a + b) / n) ** 3
+    f1 = (n + 1) / n
+    riemann_flops = 3 * f1 * (28 + 392) + 3 * f1 * f1 * (104 + 453) + 81     # face + edge states, solves, update
     table = {
-        "fill_guards": 2 * 8 * (r(ng, ng) - 1.0),                 # read + write the guard shell, 8 fields
-        "cfl": 8 + 3 / n,                                         # 8 fields (+ closing faces), one scalar out
-        "prim": 8 * r(2, 3) + 8 * r(2, 2),
-        "emf0": (3 + 3) * r(2, 2) + 3 * r(1, 2),
-        "predict": (8 + 3) * r(2, 2) + 3 * r(1, 2) + (21 + 6 + 5) * r(1, 1) + 3 * r(1, 2),
-        "hlld_flux": 3 * ((5 + 7) * r(1, 1) + 3 * r(1, 2) + 5 * r(0, 1)),      # three directions
-        "emf_2d": 3 * ((5 + 12 + 2) * r(1, 1) + 3 * r(1, 2) + 1 * r(0, 1)),    # three edge directions
-        "update": 8 + 15 * r(0, 1) + 3 * r(0, 1) + 8,
-        "fused_step": 8 * r(2, 3) + 8,
+        # class: (values per cell, flops per cell, bound)
+        "fill_guards": (2 * 8 * (r(ng, ng) - 1.0), 0.0, "hbm"),
+        "cfl": (8 + 3 / n, CFL_FLOPS, "hbm"),
+        "predict": (8 * r(2, 3) + 38 * r(1, 1), STEP_FLOPS_32 - riemann_flops, "hbm"),
+        "riemann_update": (38 * r(1, 1) + 8 + 8, riemann_flops, "alu"),
+        # staged path (general, collapsed dimensions)
+        "prim": (8 * r(2, 3) + 8 * r(2, 2), 40.0, "hbm"),
+        "emf0": ((3 + 3) * r(2, 2) + 3 * r(1, 2), 70.0, "hbm"),
+        "hlld_flux": (3 * ((5 + 7) * r(1, 1) + 3 * r(1, 2) + 5 * r(0, 1)), 3 * f1 * 420, "alu"),
+        "emf_2d": (3 * ((5 + 12 + 2) * r(1, 1) + 3 * r(1, 2) + 1 * r(0, 1)), 3 * f1 * f1 * 557, "alu"),
+        "update": (8 + 15 * r(0, 1) + 3 * r(0, 1) + 8, 81.0, "hbm"),
     }
     return table.get(cls)
+
+
+def ncu_traffic(workload, cls):
+    """DRAM bytes per launch of a kernel class from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "r1_ncu_traffic.txt")
+    try:
+        return json.load(open(path)).get(workload, {}).get(cls)
+    except Exception:
+        return None
+
+
+def aggregate_over_ranks(ms, cells_per_rank, steps, world, device=None):
+    """Whole-job throughput of N independent replicas: every rank processed cells_per_rank
+    cells per step; the job's time is the MAX over ranks (all_reduce), the value their sum
+    over that time.  Returns (value, ms_max).  world == 1 needs no process group."""
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([ms], dtype=torch.float64, device=device or "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return world * cells_per_rank * steps / (ms * 1e-3), ms
 
 
 class ClockSampler(threading.Thread):
@@ -201,11 +233,7 @@ def main():
     clocks = sampler.summary()
     launches = b.launches - l0
     bad = b.status()
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * w.cells * args.steps / (ms * 1e-3)
+    value, ms = aggregate_over_ranks(ms, w.cells, args.steps, world, device="cuda")
 
     # ---- per-kernel-class device times (separate pass, events around every launch) ----
     b.set_timing(True)
@@ -216,23 +244,41 @@ def main():
     b.set_timing(False)
     pk = peaks()
     esz = 4 if dtype == "f32" else 8
+    from paper_2508_09568_b200.binding import measure_alu_peak
+    alu_peak = measure_alu_peak(dtype, local)               # TFLOP/s, FMA-chain, measured now
+    alu_nominal = 148 * (128 if dtype == "f32" else 64) * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
     classes = {k: {"ms_per_step": v[0] / tsteps, "launches_per_step": v[1] / tsteps} for k, v in kt.items()}
     tot = sum(c["ms_per_step"] for c in classes.values())
     for k, c in classes.items():
         c["share"] = c["ms_per_step"] / tot
-        a = algorithmic_values_per_cell(k, n)
+        a = algorithmic_work(k, n)
         if a:
-            c["alg_bytes_per_cell"] = a * esz
-            c["alg_gbs"] = a * esz * w.cells / (c["ms_per_step"] * 1e-3) / 1e9
+            c["bound"] = a[2]
+            c["alg_bytes_per_cell"] = a[0] * esz
+            c["alg_flops_per_cell"] = a[1]
+            c["alg_gbs"] = a[0] * esz * w.cells / (c["ms_per_step"] * 1e-3) / 1e9
+            c["alg_tflops"] = a[1] * w.cells / (c["ms_per_step"] * 1e-3) / 1e12
+            c["hbm_frac"] = c["alg_gbs"] / pk["hbm_gbs"]
+            c["alu_frac"] = c["alg_tflops"] / alu_peak
     dom = max((k for k in classes if k != "misc"), key=lambda k: classes[k]["ms_per_step"])
     dc = classes[dom]
     per_launch_ms = dc["ms_per_step"] / dc["launches_per_step"]
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": dc.get("alg_gbs"), "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": (dc.get("alg_gbs") or 0.0) / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"],
-                "avg_launch_ms": per_launch_ms, "share_of_step": dc["share"],
-                "alg_bytes_per_launch": dc.get("alg_bytes_per_cell", 0) * w.cells / dc["launches_per_step"]}
-    # whole-step view: compulsory traffic of a fully fused step (16 values per cell)
-    step_view = {"compulsory_bytes_per_cell": 16 * esz,
+    if dc.get("bound") == "alu":
+        roofline = {"kernel": dom, "bound": "alu", "achieved": dc["alg_tflops"], "peak": alu_peak, "unit": "TFLOP/s",
+                    "frac": dc["alu_frac"], "peak_source": "measured FMA chain (mhd_bunch_measure_alu_peak), FMA = 2 flops",
+                    "peak_nominal": alu_nominal,
+                    "alg_flops_per_launch": dc["alg_flops_per_cell"] * w.cells / dc["launches_per_step"]}
+    else:
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": dc.get("alg_gbs"), "peak": pk["hbm_gbs"], "unit": "GB/s",
+                    "frac": dc.get("hbm_frac"), "peak_source": pk["source"],
+                    "alg_bytes_per_launch": dc.get("alg_bytes_per_cell", 0) * w.cells / dc["launches_per_step"]}
+    roofline.update({"traffic": ncu_traffic(args.workload, dom), "avg_launch_ms": per_launch_ms,
+                     "share_of_step": dc["share"], "hbm_frac": dc.get("hbm_frac"), "alu_frac": dc.get("alu_frac")})
+    # whole-pass view: counted flops of step + cfl, compulsory traffic of a fully fused step
+    pass_flops = STEP_FLOPS_32 + CFL_FLOPS
+    step_view = {"alg_flops_per_cell": pass_flops, "alg_tflops": pass_flops * value / world / 1e12,
+                 "alu_frac": pass_flops * value / world / 1e12 / alu_peak, "alu_peak_tflops": alu_peak,
+                 "compulsory_bytes_per_cell": 16 * esz,
                  "hbm_frac_at_compulsory_bytes": 16 * esz * value / world / 1e9 / pk["hbm_gbs"]}
 
     # ---- end to end through the host-buffer path of the C ABI -------------------------

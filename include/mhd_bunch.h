@@ -140,6 +140,11 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
  * cross-checks and benchmarks; both run on the GPU.                                      */
 int mhd_bunch_set_path(mhd_bunch *b, int32_t staged);
 
+/* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted
+ * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous; allocates
+ * and frees a small device buffer of its own (not part of any handle).                    */
+int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double *tflops);
+
 /* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
  * patches) the workspace allows.                                                        */
 int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);

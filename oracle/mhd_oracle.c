@@ -510,7 +510,7 @@ static void run_stages(const geom *G, const real *const Up[8], real dt, scratch 
         L[f] = S->qh[comp[f]][cl] + HALF * S->dq[d][comp[f]][cl];
         R[f] = S->qh[comp[f]][c] - HALF * S->dq[d][comp[f]][c];
       }
-      orc_hlld(G->gamma, L, R, S->bh[d][c], F);
+      orc_hlld((double)G->gamma, L, R, S->bh[d][c], F);
       S->flux[d][0][c] = F[0];
       S->flux[d][1 + d][c] = F[1];
       S->flux[d][1 + t1][c] = F[2];
@@ -542,7 +542,7 @@ static void run_stages(const geom *G, const real *const Up[8], real dt, scratch 
       real AN = S->bh[a][c] - HALF * dba[c];
       real BW = S->bh[b][c - s[a]] + HALF * dbb[c - s[a]];
       real BE = S->bh[b][c] - HALF * dbb[c];
-      S->emf[e][c] = orc_emf2d(G->gamma, G->emf_solver, (const real(*)[6])cs, AS, AN, BW, BE);
+      S->emf[e][c] = orc_emf2d((double)G->gamma, G->emf_solver, (const real(*)[6])cs, AS, AN, BW, BE);
     }
   }
 }

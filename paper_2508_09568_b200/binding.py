@@ -18,7 +18,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
-    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
 ]
 
 
@@ -64,6 +64,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.mhd_bunch_chunk.argtypes = [vp, C.POINTER(i32)]
     lib.mhd_bunch_set_path.argtypes = [vp, i32]
+    lib.mhd_bunch_measure_alu_peak.argtypes = [i32, i32, C.POINTER(dbl)]
     lib.mhd_bunch_destroy.argtypes = [vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
@@ -96,6 +97,14 @@ def query(desc):
     lay = Layout()
     _check(load_library().mhd_bunch_query(C.byref(desc), C.byref(lay)), "mhd_bunch_query")
     return lay
+
+
+def measure_alu_peak(dtype="f32", device=0):
+    """Measured FMA-chain peak in TFLOP/s (FMA = 2 flops) of the fp32 or fp64 pipe."""
+    v = C.c_double(0.0)
+    _check(load_library().mhd_bunch_measure_alu_peak(MHD_F32 if dtype == "f32" else MHD_F64, device, C.byref(v)),
+           "mhd_bunch_measure_alu_peak")
+    return v.value
 
 
 class MhdBunch:

@@ -41,7 +41,8 @@ struct mhd_bunch {
   int cur;
   char* ws;
   size_t ws_bytes;
-  int chunk;
+  int chunk;           // patches per sub-bunch of the fused path (D block)
+  int chunk_s;         // patches per sub-bunch of the staged path
   // carved from the workspace head
   int* d_nbr;
   unsigned long long* d_rate;  // [npatch]
@@ -160,11 +161,12 @@ int wave_aligned_chunk(const Geom& G, int chunk) {
   return chunk / 74 * 74;
 }
 size_t staged_bytes(const Geom& G, size_t esz, int chunk) { return align_up((size_t)W_COUNT * chunk * G.ps * esz, 256); }
-size_t scratch_bytes(const Geom& G, size_t esz, int chunk) {
-  size_t b = staged_bytes(G, esz, chunk);
-  if (all_active(G)) b += align_up((size_t)W_DCOUNT * make_dgeom(G, esz, chunk).fs * esz, 256);
-  return b;
+size_t dblock_bytes(const Geom& G, size_t esz, int chunk) {
+  return align_up((size_t)W_DCOUNT * make_dgeom(G, esz, chunk).fs * esz, 256);
 }
+// 3D bunches run the fused path: the D block scales with the chunk, the staged scratch (kept
+// for cross-checks) only needs a few patches.  Otherwise the staged scratch is all there is.
+int staged_patches_3d(const Geom& G) { return G.np < 16 ? G.np : 16; }
 
 template <typename T>
 Params<T> make_params(const mhd_bunch* b, int p0, int npl) {
@@ -173,7 +175,7 @@ Params<T> make_params(const mhd_bunch* b, int p0, int npl) {
   P.U = (const T*)b->state[b->cur] ;
   P.Un = (T*)b->state[1 - b->cur];
   P.W = (T*)b->d_scratch;
-  P.wfs = (long long)b->chunk * b->G.ps;
+  P.wfs = (long long)b->chunk_s * b->G.ps;
   P.DG = b->DG;
   P.D = (T*)b->d_dblock;
   P.p0 = p0;
@@ -234,8 +236,9 @@ int launch_step(mhd_bunch* b) {
       attr_done[sizeof(T) == 8] = true;
     }
   }
-  for (int p0 = 0; p0 < G.np; p0 += b->chunk) {
-    const int npl = (G.np - p0 < b->chunk) ? G.np - p0 : b->chunk;
+  const int ch = fused ? b->chunk : b->chunk_s;
+  for (int p0 = 0; p0 < G.np; p0 += ch) {
+    const int npl = (G.np - p0 < ch) ? G.np - p0 : ch;
     Params<T> P = make_params<T>(b, p0, npl);
     cudaStream_t st = b->stream;
     if (fused) {
@@ -334,13 +337,19 @@ int mhd_bunch_query(const mhd_bunch_desc* desc, mhd_bunch_layout* lay) {
   lay->origin = G.lead;
   lay->state_elems = 8 * G.fs;
   lay->state_bytes = (size_t)lay->state_elems * esz;
-  lay->workspace_min = head_bytes(G.np) + scratch_bytes(G, esz, 1);
   // the whole bunch in one chunk unless that needs more than 48 GiB of scratch
-  int chunk = G.np;
   const size_t cap = (size_t)48 << 30;
-  while (chunk > 1 && scratch_bytes(G, esz, chunk) > cap) chunk = (chunk + 1) / 2;
-  chunk = wave_aligned_chunk(G, chunk);
-  lay->workspace_best = head_bytes(G.np) + scratch_bytes(G, esz, chunk);
+  int chunk = G.np;
+  if (all_active(G)) {
+    lay->workspace_min = head_bytes(G.np) + staged_bytes(G, esz, 1) + dblock_bytes(G, esz, 1);
+    while (chunk > 1 && dblock_bytes(G, esz, chunk) > cap) chunk = (chunk + 1) / 2;
+    chunk = wave_aligned_chunk(G, chunk);
+    lay->workspace_best = head_bytes(G.np) + staged_bytes(G, esz, staged_patches_3d(G)) + dblock_bytes(G, esz, chunk);
+  } else {
+    lay->workspace_min = head_bytes(G.np) + staged_bytes(G, esz, 1);
+    while (chunk > 1 && staged_bytes(G, esz, chunk) > cap) chunk = (chunk + 1) / 2;
+    lay->workspace_best = head_bytes(G.np) + staged_bytes(G, esz, chunk);
+  }
   for (int a = 0; a < 3; ++a) lay->m[a] = G.m[a];
   return MHD_OK;
 }
@@ -390,11 +399,22 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->d_dt = (double*)p;               p += 256;
   b->d_scratch = p;
   const size_t avail = workspace_bytes - (size_t)(p - b->ws);
-  long long chunk = (long long)(avail / scratch_bytes(b->G, b->esz, 1));   // lower bound
-  if (chunk > desc->npatch) chunk = desc->npatch;
-  if (chunk < 1) { delete b; return MHD_ENOMEM; }
-  while (chunk < desc->npatch && scratch_bytes(b->G, b->esz, (int)chunk + 1) <= avail) ++chunk;
-  b->chunk = wave_aligned_chunk(b->G, (int)chunk);
+  {
+    const bool d3 = all_active(b->G);
+    // staged scratch first (a few patches in 3D, everything that fits otherwise), D block after it
+    int cs = d3 ? staged_patches_3d(b->G) : desc->npatch;
+    while (cs > 1 && staged_bytes(b->G, b->esz, cs) + (d3 ? dblock_bytes(b->G, b->esz, 1) : 0) > avail) --cs;
+    b->chunk_s = cs;
+    b->chunk = cs;
+    if (d3) {
+      const size_t left = avail - staged_bytes(b->G, b->esz, cs);
+      long long c = (long long)(left / dblock_bytes(b->G, b->esz, 1));
+      if (c > desc->npatch) c = desc->npatch;
+      if (c < 1) { delete b; return MHD_ENOMEM; }
+      while (c < desc->npatch && dblock_bytes(b->G, b->esz, (int)c + 1) <= left) ++c;
+      b->chunk = wave_aligned_chunk(b->G, (int)c);
+    }
+  }
   b->fused_ok = false;
   if (b->G.act[0] && b->G.act[1] && b->G.act[2]) {
     const bool f64 = desc->dtype == MHD_F64;
@@ -406,7 +426,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
       const size_t pa = (size_t)(b->G.n[0] + 5) * (ty + 5);
       if (pa <= (size_t)predict_max_threads(ty) && 39 * pa * b->esz <= (size_t)220 * 1024) { b->pred_ty = ty; break; }
     }
-    b->d_dblock = b->d_scratch + staged_bytes(b->G, b->esz, b->chunk);
+    b->d_dblock = b->d_scratch + staged_bytes(b->G, b->esz, b->chunk_s);
     const int bx = f64 ? FusedCfg<double, FusedTile<double>::TX, FusedTile<double>::TY>::DW
                        : FusedCfg<float, FusedTile<float>::TX, FusedTile<float>::TY>::DW;
     const int by = f64 ? FusedCfg<double, FusedTile<double>::TX, FusedTile<double>::TY>::DH
@@ -485,9 +505,41 @@ int mhd_bunch_set_path(mhd_bunch* b, int32_t staged) {
   return MHD_OK;
 }
 
+int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double* tflops) {
+  if (!tflops || (dtype != MHD_F32 && dtype != MHD_F64)) return MHD_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
+    return fail_cuda(cudaErrorNoDevice, "no CUDA device");
+  CUDA_TRY(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, device));
+  void* out = nullptr;
+  const int blocks = prop.multiProcessorCount * 8, iters = 4096;
+  CUDA_TRY(cudaMalloc(&out, (size_t)blocks * 256 * 8));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0, 0);
+    if (dtype == MHD_F64) k_fma_peak<double><<<blocks, 256>>>((double*)out, iters, 1.0000001, 1e-7);
+    else k_fma_peak<float><<<blocks, 256>>>((float*)out, iters, 1.0000001f, 1e-7f);
+    cudaEventRecord(e1, 0);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 16.0 * iters * (double)blocks * 256.0;
+    if (ms > 0.f && rep > 0) best = fmax(best, fl / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  CUDA_TRY(cudaGetLastError());
+  *tflops = best;
+  return MHD_OK;
+}
+
 int mhd_bunch_chunk(mhd_bunch* b, int32_t* chunk_patches) {
   if (!b || !chunk_patches) return MHD_ESTATE;
-  *chunk_patches = b->chunk;
+  *chunk_patches = (b->fused_ok && !b->force_staged) ? b->chunk : b->chunk_s;
   return MHD_OK;
 }
 

@@ -167,6 +167,23 @@ __global__ void k_zero_u64(unsigned long long* p, int n) {
   if (t < n) p[t] = 0ull;
 }
 
+// FMA-chain microbenchmark: 16 independent chains per thread, used to MEASURE the fp32/fp64
+// pipe peak that the ALU roofline of the step kernels is reported against
+template <typename T>
+__global__ void __launch_bounds__(256) k_fma_peak(T* out, int iters, T a, T b) {
+  T x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = T(threadIdx.x + i) * T(1e-3);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = x[i] * a + b;
+  }
+  T s = T(0);
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += x[i];
+  if (s == T(-1)) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true: keeps the chains alive
+}
+
 // dt for a step, on the device: either the host value or min(*dt_dev, dt_max)
 __global__ void k_set_dt(double* dst, const double* src, double host_dt, double dt_max) {
   double dt = src ? *src : host_dt;
