@@ -163,21 +163,34 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   // Own-column registers.  The state of plane r is loaded at the top of iteration r but its
   // hydro part is first used in iteration r+1 and its bx, by after the first barrier, so the
   // loads overlap a whole iteration; only bz is needed at once and runs one plane ahead.
+  // Every global load is issued at least one full iteration before its first use: the
+  // hydro part of plane r is used in iteration r+1 (as Uprev); bx, by of plane r are used in
+  // iteration r (shared-memory write), so they are loaded in iteration r-1; bz of plane r is
+  // used at the top of iteration r, so it runs two planes ahead.
   T Ucur[8], Uprev[8];
   T bxm[3] = {T(0), T(0), T(0)}, bym[3] = {T(0), T(0), T(0)};   // own raw bx, by at planes r-1, r-2, r-3
-  T bznext = T(0);
+  T bxn = T(0), byn = T(0), bzn1 = T(0), bzn2 = T(0);
 #pragma unroll
   for (int f = 0; f < 8; ++f) { Ucur[f] = T(0); Uprev[f] = T(0); }
   const int rlo = -2, rhi = nz + 2;
-  if (rowok) bznext = P.U[7 * fs + cbase + (long long)rlo * plane];
+  if (rowok) {
+    bxn = P.U[5 * fs + cbase + (long long)rlo * plane];
+    byn = P.U[6 * fs + cbase + (long long)rlo * plane];
+    bzn1 = P.U[7 * fs + cbase + (long long)rlo * plane];
+    bzn2 = P.U[7 * fs + cbase + (long long)(rlo + 1) * plane];
+  }
   unsigned int nbad = 0;
 
   for (int r = rlo; r <= rhi; ++r) {
-    Ucur[7] = bznext;
+    Ucur[5] = bxn; Ucur[6] = byn; Ucur[7] = bzn1; bzn1 = bzn2;
     if (rowok) {
 #pragma unroll
-      for (int f = 0; f < 7; ++f) Ucur[f] = P.U[f * fs + cbase + (long long)r * plane];
-      if (r + 1 <= rhi) bznext = P.U[7 * fs + cbase + (long long)(r + 1) * plane];
+      for (int f = 0; f < 5; ++f) Ucur[f] = P.U[f * fs + cbase + (long long)r * plane];
+      if (r + 1 <= rhi) {
+        bxn = P.U[5 * fs + cbase + (long long)(r + 1) * plane];
+        byn = P.U[6 * fs + cbase + (long long)(r + 1) * plane];
+      }
+      if (r + 2 <= rhi) bzn2 = P.U[7 * fs + cbase + (long long)(r + 2) * plane];
     }
 
     // ---- primitives of plane r-1 (O2): needs bx(i+1), by(j+1) of plane r-1 and bz of plane r
@@ -383,6 +396,13 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
     }
     const T* dc_ = slot(cur) + own;   // this cell, plane k
     const T* dp_ = slot(prv) + own;   // this cell, plane k-1
+    if (k >= 1 && active) {
+      // pull the U^n lines of plane k-1 towards L2 now: they are read after phase [A], and no
+      // registers can be spared to hold them across it
+      const T* up = P.U + ubase + (long long)(k - 1) * plane;
+#pragma unroll
+      for (int f = 0; f < 8; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(up + f * G.fs));
+    }
 
     // [A] values that couple planes k-1 and k: z-face flux and the x- and y-directed edges
     Flux5<T> cFz = {};

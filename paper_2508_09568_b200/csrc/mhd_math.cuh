@@ -21,16 +21,44 @@ template <> struct num<float> {
   static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
   static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
   static __device__ __forceinline__ float rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+  static __device__ __forceinline__ float rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
   static __device__ __forceinline__ float div(float a, float b) { return a * rcp(b); }
 };
 template <> struct num<double> {
   static __device__ __forceinline__ double eps() { return DBL_EPSILON; }
-  static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+  // fp64: MUFU seed (rcp/rsqrt.approx.ftz.f64, ~20 bits) + Newton steps in DFMA: ~1e-16
+  // relative error without the IEEE sequences' slow-path calls and branches (tolerance of
+  // the path is 1e-12 per cell and step).  Arguments here are normal, non-zero numbers;
+  // sqrt(0) is handled explicitly.
+  static __device__ __forceinline__ double rsqrt(double a) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double h = 0.5 * a;
+    y = y * fma(-h * y, y, 1.5);
+    y = y * fma(-h * y, y, 1.5);
+    return y;
+  }
+  static __device__ __forceinline__ double sqrt(double a) {
+    const double y = rsqrt(a);
+    double s = a * y;
+    s = fma(fma(-s, s, a), 0.5 * y, s);
+    return a > 0.0 ? s : 0.0;
+  }
   static __device__ __forceinline__ double abs(double x) { return fabs(x); }
   static __device__ __forceinline__ double min(double a, double b) { return fmin(a, b); }
   static __device__ __forceinline__ double max(double a, double b) { return fmax(a, b); }
-  static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
-  static __device__ __forceinline__ double div(double a, double b) { return a / b; }
+  static __device__ __forceinline__ double rcp(double a) {
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+    x = fma(x, fma(-a, x, 1.0), x);
+    x = fma(x, fma(-a, x, 1.0), x);
+    return x;
+  }
+  static __device__ __forceinline__ double div(double a, double b) {
+    const double r = rcp(b);
+    const double q = a * r;
+    return fma(fma(-b, q, a), r, q);   // one residual correction of the quotient
+  }
 };
 
 // ---- slope limiter: 0 at extrema; minmod (1) or monotonised central (2) -------------
@@ -47,11 +75,15 @@ __device__ __forceinline__ T limited_slope(int kind, T a, T b) {
 // ---- fast magnetosonic speed along a direction with normal field bn ---------------
 // gp = gamma*p, b2 = |B|^2, bn2 = bn^2, irho = 1/rho
 template <typename T>
-__device__ __forceinline__ T fast_speed(T gp, T b2, T bn2, T irho) {
+__device__ __forceinline__ T fast_speed2(T gp, T b2, T bn2, T irho) {   // c_f^2
   using N = num<T>;
   const T s = gp + b2;
   const T disc = N::max(s * s - T(4) * gp * bn2, T(0));
-  return N::sqrt(T(0.5) * (s + N::sqrt(disc)) * irho);
+  return T(0.5) * (s + N::sqrt(disc)) * irho;
+}
+template <typename T>
+__device__ __forceinline__ T fast_speed(T gp, T b2, T bn2, T irho) {
+  return num<T>::sqrt(fast_speed2(gp, b2, bn2, irho));
 }
 
 // primitive state seen by a 1D Riemann problem: normal velocity u, transverse (v,w),
@@ -71,9 +103,9 @@ __device__ __forceinline__ Flux5<T> hlld_flux(T gamma, const State1D<T>& L, cons
 
   const T b2L = bn2 + L.by * L.by + L.bz * L.bz, b2R = bn2 + R.by * R.by + R.bz * R.bz;
   const T pTL = L.p + half * b2L, pTR = R.p + half * b2R;
-  const T cfL = fast_speed(gamma * L.p, b2L, bn2, N::rcp(L.rho));
-  const T cfR = fast_speed(gamma * R.p, b2R, bn2, N::rcp(R.rho));
-  const T cmax = N::max(cfL, cfR);
+  // the square root is monotonic: one sqrt of the larger c_f^2
+  const T cmax = N::sqrt(N::max(fast_speed2(gamma * L.p, b2L, bn2, N::rcp(L.rho)),
+                                fast_speed2(gamma * R.p, b2R, bn2, N::rcp(R.rho))));
   const T SL = N::min(L.u, R.u) - cmax, SR = N::max(L.u, R.u) + cmax;
 
   const T sdL = SL - L.u, sdR = SR - R.u;
@@ -93,9 +125,10 @@ __device__ __forceinline__ Flux5<T> hlld_flux(T gamma, const State1D<T>& L, cons
   const T vsL = L.v - kvL * L.by, wsL = L.w - kvL * L.bz, bysL = L.by * kbL, bzsL = L.bz * kbL;
   const T vsR = R.v - kvR * R.by, wsR = R.w - kvR * R.bz, bysR = R.by * kbR, bzsR = R.bz * kbR;
 
-  const T rL = N::sqrt(rsL), rR = N::sqrt(rsR);
+  const T irL = N::rsqrt(rsL), irR = N::rsqrt(rsR);
+  const T rL = rsL * irL, rR = rsR * irR;             // sqrt(rho*) from the same MUFU result
   const T abn = N::abs(bn);
-  const T SsL = SM - N::div(abn, rL), SsR = SM + N::div(abn, rR);
+  const T SsL = SM - abn * irL, SsR = SM + abn * irR;
   const T sg = bn > T(0) ? T(1) : (bn < T(0) ? T(-1) : T(0));
 
   // which side holds the interface, and how deep into the fan it sits
@@ -185,10 +218,10 @@ __device__ __forceinline__ T emf_2d(T gamma, int solver, const Corner<T>& sw, co
   const T b2NW = AN2 + BW2 + nw.be * nw.be, b2NE = AN2 + BE2 + ne.be * ne.be;
   const T iSW = N::rcp(sw.rho), iSE = N::rcp(se.rho), iNW = N::rcp(nw.rho), iNE = N::rcp(ne.rho);
   const T gSW = gamma * sw.p, gSE = gamma * se.p, gNW = gamma * nw.p, gNE = gamma * ne.p;
-  const T ca = N::max(N::max(fast_speed(gSW, b2SW, AS2, iSW), fast_speed(gSE, b2SE, AS2, iSE)),
-                      N::max(fast_speed(gNW, b2NW, AN2, iNW), fast_speed(gNE, b2NE, AN2, iNE)));
-  const T cb = N::max(N::max(fast_speed(gSW, b2SW, BW2, iSW), fast_speed(gSE, b2SE, BE2, iSE)),
-                      N::max(fast_speed(gNW, b2NW, BW2, iNW), fast_speed(gNE, b2NE, BE2, iNE)));
+  const T ca = N::sqrt(N::max(N::max(fast_speed2(gSW, b2SW, AS2, iSW), fast_speed2(gSE, b2SE, AS2, iSE)),
+                              N::max(fast_speed2(gNW, b2NW, AN2, iNW), fast_speed2(gNE, b2NE, AN2, iNE))));
+  const T cb = N::sqrt(N::max(N::max(fast_speed2(gSW, b2SW, BW2, iSW), fast_speed2(gSE, b2SE, BE2, iSE)),
+                              N::max(fast_speed2(gNW, b2NW, BW2, iNW), fast_speed2(gNE, b2NE, BE2, iNE))));
   const T tW = N::min(N::min(sw.ua, se.ua), N::min(nw.ua, ne.ua)) - ca;
   const T tE = N::max(N::max(sw.ua, se.ua), N::max(nw.ua, ne.ua)) + ca;
   const T tS = N::min(N::min(sw.ub, se.ub), N::min(nw.ub, ne.ub)) - cb;
