@@ -134,11 +134,21 @@ int mhd_bunch_status(mhd_bunch *b, int64_t *bad_cells);
 /* Number of kernel launches issued so far through this handle (for bench.py).           */
 int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 
-/* The step has two CUDA implementations: a fused path for bunches with three active
- * dimensions (default there) and a general staged path (one kernel per stage of PAPER.md
- * section 2.1.4) used for collapsed dimensions.  staged != 0 forces the staged path, for
- * cross-checks and benchmarks; both run on the GPU.                                      */
-int mhd_bunch_set_path(mhd_bunch *b, int32_t staged);
+/* The step has three CUDA implementations, all on the GPU:
+ *   MHD_PATH_ONEPASS     the whole step in one kernel, nothing intermediate in HBM (three
+ *                        active dimensions, float32): the default where it applies;
+ *   MHD_PATH_TWO_KERNEL  predictor kernel + Riemann/update kernel with one scratch block in
+ *                        HBM (three active dimensions, any type);
+ *   MHD_PATH_STAGED      one kernel per stage of PAPER.md section 2.1.4 (general: collapsed
+ *                        dimensions, cross-checks).
+ * MHD_PATH_AUTO picks the first one that applies.  Asking for a path that does not apply to
+ * this bunch returns MHD_EINVAL.  mhd_bunch_get_path reports the one a step would run.    */
+#define MHD_PATH_AUTO        0
+#define MHD_PATH_STAGED      1
+#define MHD_PATH_TWO_KERNEL  2
+#define MHD_PATH_ONEPASS     3
+int mhd_bunch_set_path(mhd_bunch *b, int32_t path);
+int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
 
 /* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted
  * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous; allocates

@@ -12,13 +12,14 @@ import numpy as np
 from . import build as _build
 
 MHD_F32, MHD_F64 = 0, 1
+PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3}
 _ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
 
 ABI_SYMBOLS = [
     "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
-    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
 ]
 
 
@@ -64,6 +65,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.mhd_bunch_chunk.argtypes = [vp, C.POINTER(i32)]
     lib.mhd_bunch_set_path.argtypes = [vp, i32]
+    lib.mhd_bunch_get_path.argtypes = [vp, C.POINTER(i32)]
     lib.mhd_bunch_measure_alu_peak.argtypes = [i32, i32, C.POINTER(dbl)]
     lib.mhd_bunch_destroy.argtypes = [vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
@@ -207,8 +209,15 @@ class MhdBunch:
         _check(self.lib.mhd_bunch_chunk(self.h, C.byref(v)), "mhd_bunch_chunk")
         return v.value
 
-    def set_path(self, staged):
-        _check(self.lib.mhd_bunch_set_path(self.h, 1 if staged else 0), "mhd_bunch_set_path")
+    def set_path(self, path):
+        """'auto' | 'staged' | 'two_kernel' | 'onepass' (include/mhd_bunch.h, MHD_PATH_*)."""
+        _check(self.lib.mhd_bunch_set_path(self.h, PATHS[path]), "mhd_bunch_set_path")
+
+    @property
+    def path(self):
+        v = C.c_int32(0)
+        _check(self.lib.mhd_bunch_get_path(self.h, C.byref(v)), "mhd_bunch_get_path")
+        return {k: n for n, k in PATHS.items()}[v.value]
 
     def set_timing(self, on):
         _check(self.lib.mhd_bunch_set_timing(self.h, 1 if on else 0), "mhd_bunch_set_timing")

@@ -11,6 +11,7 @@
 #include "mhd_math.cuh"
 #include "stage_kernels.cuh"
 #include "fused_kernels.cuh"
+#include "onepass_kernel.cuh"
 
 #include <cuda_runtime.h>
 #include <math.h>
@@ -31,6 +32,8 @@ thread_local char g_cuda_err[256] = "";
 template <typename T> struct FusedTile;
 template <> struct FusedTile<float> { static constexpr int TX = 32, TY = 8; };
 template <> struct FusedTile<double> { static constexpr int TX = 16, TY = 8; };
+// one-pass kernel (onepass_kernel.cuh): tile and number of predictor warps
+struct OneTile { static constexpr int TX = 32, TY = 8, NPW = 6; };
 
 // ------------------------------------------------------------------------ handle ----
 struct mhd_bunch {
@@ -53,7 +56,9 @@ struct mhd_bunch {
   long long launches;
   size_t esz;
   // optional per-kernel-class timing (host-side objects only)
-  bool force_staged;   // run the general staged step even where the fused 3D path applies
+  int path;            // MHD_PATH_*: 0 = automatic choice
+  bool onepass_ok;     // three active dimensions, fp32, tensor maps of both state buffers built
+  CUtensorMap tm_h[2], tm_b[2];   // state buffers a/b: boxes of 5 hydro fields / 3 field components
   bool fused_ok;       // three active dimensions and the tensor maps could be built
   int pred_ty;         // y-tile of the fused predictor (16, 8 or 4)
   DGeom DG;            // geometry of the D block
@@ -66,9 +71,9 @@ struct mhd_bunch {
   long long cls_n[16];
 };
 
-enum KClass : int { KC_FILL = 0, KC_CFL, KC_PRIM, KC_EMF0, KC_PREDICT, KC_FLUX, KC_EMF, KC_UPDATE, KC_MISC, KC_RIEMANN, KC_COUNT };
+enum KClass : int { KC_FILL = 0, KC_CFL, KC_PRIM, KC_EMF0, KC_PREDICT, KC_FLUX, KC_EMF, KC_UPDATE, KC_MISC, KC_RIEMANN, KC_ONEPASS, KC_COUNT };
 static const char* const kclass_names[KC_COUNT] = {"fill_guards", "cfl", "prim", "emf0", "predict", "hlld_flux",
-                                                   "emf_2d", "update", "misc", "riemann_update"};
+                                                   "emf_2d", "update", "misc", "riemann_update", "step_onepass"};
 
 // brackets one launch with events when timing is on
 struct LaunchScope {
@@ -219,11 +224,47 @@ int launch_cfl(mhd_bunch* b, double courant, void* dt_dev, void* dt_patch) {
   return MHD_OK;
 }
 
+// which implementation of the step runs: MHD_PATH_ONEPASS, MHD_PATH_TWO_KERNEL or MHD_PATH_STAGED
+int effective_path(const mhd_bunch* b) {
+  if (b->path == MHD_PATH_STAGED) return MHD_PATH_STAGED;
+  if (b->path == MHD_PATH_TWO_KERNEL) return b->fused_ok ? MHD_PATH_TWO_KERNEL : MHD_PATH_STAGED;
+  if (b->onepass_ok) return MHD_PATH_ONEPASS;           // automatic, or asked for
+  return b->fused_ok ? MHD_PATH_TWO_KERNEL : MHD_PATH_STAGED;
+}
+
+template <typename T> struct OnePassLaunch {
+  static int run(mhd_bunch*, const double*) { return MHD_EINVAL; }
+};
+template <> struct OnePassLaunch<float> {
+  static int run(mhd_bunch* b, const double* dtp) {
+    using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
+    auto kern = k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
+    static bool attr_done = false;
+    if (!attr_done) {
+      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      attr_done = true;
+    }
+    const Geom& G = b->G;
+    Params<float> P = make_params<float>(b, 0, G.np);
+    const int xt = (G.n[0] + OneTile::TX - 1) / OneTile::TX, yt = (G.n[1] + OneTile::TY - 1) / OneTile::TY;
+    dim3 grid((unsigned)(xt * yt), (unsigned)G.np);
+    {
+      LaunchScope ls(b, KC_ONEPASS);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->tm_h[b->cur], b->tm_b[b->cur], dtp, b->d_bad, xt);
+    }
+    CUDA_TRY(cudaGetLastError());
+    b->cur = 1 - b->cur;
+    return MHD_OK;
+  }
+};
+
 template <typename T>
 int launch_step(mhd_bunch* b) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
-  const bool fused = b->fused_ok && !b->force_staged;
+  const int path = effective_path(b);
+  if (path == MHD_PATH_ONEPASS) return OnePassLaunch<T>::run(b, dtp);
+  const bool fused = path == MHD_PATH_TWO_KERNEL;
   if (fused) {
     static bool attr_done[2] = {false, false};
     if (!attr_done[sizeof(T) == 8]) {
@@ -434,6 +475,18 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
     b->fused_ok = b->pred_ty != 0 && make_bunch_tensor_map(&b->tmap_d, b->d_dblock, f64, b->DG.pitch, b->DG.ny, b->DG.nz, b->chunk, W_DCOUNT,
                                         b->DG.ps, b->DG.fs, bx, by, W_DCOUNT);
   }
+  b->onepass_ok = false;
+  if (all_active(b->G) && desc->dtype == MHD_F32) {
+    using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
+    bool ok = true;
+    for (int s = 0; s < 2 && ok; ++s) {
+      ok = make_bunch_tensor_map(&b->tm_h[s], b->state[s], false, b->G.pitch, b->G.m[1], b->G.m[2], desc->npatch, 8, b->G.ps,
+                                 b->G.fs, Cfg::BWX, Cfg::PH, 5) &&
+           make_bunch_tensor_map(&b->tm_b[s], b->state[s], false, b->G.pitch, b->G.m[1], b->G.m[2], desc->npatch, 8, b->G.ps,
+                                 b->G.fs, Cfg::BWX, Cfg::PH, 3);
+    }
+    b->onepass_ok = ok;
+  }
   cudaError_t e = cudaMemcpyAsync(b->d_nbr, nbr, sizeof(int) * 27 * (size_t)desc->npatch, cudaMemcpyHostToDevice, b->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(b->d_bad, 0, 512, b->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
@@ -499,9 +552,18 @@ int mhd_bunch_launch_count(mhd_bunch* b, int64_t* launches) {
   return MHD_OK;
 }
 
-int mhd_bunch_set_path(mhd_bunch* b, int32_t staged) {
+int mhd_bunch_set_path(mhd_bunch* b, int32_t path) {
   if (!b) return MHD_ESTATE;
-  b->force_staged = staged != 0;
+  if (path < MHD_PATH_AUTO || path > MHD_PATH_ONEPASS) return MHD_EINVAL;
+  if (path == MHD_PATH_ONEPASS && !b->onepass_ok) return MHD_EINVAL;
+  if (path == MHD_PATH_TWO_KERNEL && !b->fused_ok) return MHD_EINVAL;
+  b->path = path;
+  return MHD_OK;
+}
+
+int mhd_bunch_get_path(mhd_bunch* b, int32_t* path) {
+  if (!b || !path) return MHD_ESTATE;
+  *path = effective_path(b);
   return MHD_OK;
 }
 
@@ -539,7 +601,8 @@ int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double* tflops) {
 
 int mhd_bunch_chunk(mhd_bunch* b, int32_t* chunk_patches) {
   if (!b || !chunk_patches) return MHD_ESTATE;
-  *chunk_patches = (b->fused_ok && !b->force_staged) ? b->chunk : b->chunk_s;
+  const int path = effective_path(b);
+  *chunk_patches = path == MHD_PATH_ONEPASS ? b->G.np : (path == MHD_PATH_TWO_KERNEL ? b->chunk : b->chunk_s);
   return MHD_OK;
 }
 

@@ -41,11 +41,11 @@ def make_oracle(w, limiter=1, emf_solver=0):
     return oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, limiter=limiter, emf_solver=emf_solver)
 
 
-def make_gpu(w, dtype, limiter=1, emf_solver=0, workspace_bytes=None, staged=False):
+def make_gpu(w, dtype, limiter=1, emf_solver=0, workspace_bytes=None, path="auto"):
     from paper_2508_09568_b200.binding import MhdBunch
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, limiter=limiter, emf_solver=emf_solver,
                  workspace_bytes=workspace_bytes)
-    b.set_path(staged)
+    b.set_path(path)
     b.load(w.U)
     return b
 

@@ -106,7 +106,7 @@ def test_staged_path_on_3d_bunches_matches_oracle(name, dtype, limiter, emf_solv
     U = o.fill_guards(w.U.astype(np.float64), w.nbr)
     dt = o.cfl_dt(U, 0.4)
     ref = o.step(U, dt)
-    b = make_gpu(w, dtype, limiter, emf_solver, staged=True)
+    b = make_gpu(w, dtype, limiter, emf_solver, path="staged")
     b.fill_guards()
     b.step(dt)
     err = rel_err(masked(b.download(), w.n), masked(ref, w.n))
