@@ -68,6 +68,7 @@ def algorithmic_work(cls, n, ng=3):
         "cfl": (8 + 3 / n, CFL_FLOPS, "hbm"),
         "predict": (8 * r(2, 3) + 38 * r(1, 1), STEP_FLOPS_32 - riemann_flops, "hbm"),
         "riemann_update": (38 * r(1, 1) + 8 + 8, riemann_flops, "alu"),
+        "step_onepass": (8 * r(2, 3) + 8, STEP_FLOPS_32, "alu"),
         # staged path (general, collapsed dimensions)
         "prim": (8 * r(2, 3) + 8 * r(2, 2), 40.0, "hbm"),
         "emf0": ((3 + 3) * r(2, 2) + 3 * r(1, 2), 70.0, "hbm"),
@@ -165,6 +166,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=20, help="oracle steps for the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "two_kernel", "onepass"],
+                    help="which CUDA implementation of the step runs (include/mhd_bunch.h, MHD_PATH_*)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -202,6 +205,7 @@ def main():
     w = W.turbulence(N=N, n=n, dtype=np.float32 if dtype == "f32" else np.float64, config=2)
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, device=local)
     b.load(w.U)
+    b.set_path(args.path)
     stream = b.stream
     courant = 0.4
 
@@ -319,7 +323,7 @@ def main():
                 "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
                 "config": {"workload": wdesc, "patches": w.npatch, "patch": [n, n, n], "guard": 3, "courant": courant,
-                           "chunk_patches": b.chunk, "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "chunk_patches": b.chunk, "step_path": b.path, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (b.lay.state_bytes / 1e6)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "bad_cells": bad,
                 "roofline": roofline, "step_roofline": step_view, "kernel_classes": classes, "cpu_baseline": cpu}

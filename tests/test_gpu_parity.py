@@ -98,15 +98,18 @@ def test_one_step_matches_oracle(name, dtype, limiter, emf_solver):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("limiter,emf_solver", [(1, 0), (2, 1)])
 @pytest.mark.parametrize("name", ["turb16", "turb_ragged", "turb_self"])
-def test_staged_path_on_3d_bunches_matches_oracle(name, dtype, limiter, emf_solver):
-    """3D bunches default to the fused kernels; the general staged kernels must agree with
-    the oracle there as well (they are the only path for collapsed dimensions)."""
+@pytest.mark.parametrize("path", ["staged", "two_kernel"])
+def test_every_step_path_on_3d_bunches_matches_oracle(path, name, dtype, limiter, emf_solver):
+    """3D bunches default to the one-pass kernel (fp32) or the two fused kernels (fp64); the
+    other implementations of the step must agree with the oracle there as well (the staged
+    kernels are the only path for collapsed dimensions)."""
     w = small_workloads(dtype)[name]
     o = make_oracle(w, limiter, emf_solver)
     U = o.fill_guards(w.U.astype(np.float64), w.nbr)
     dt = o.cfl_dt(U, 0.4)
     ref = o.step(U, dt)
-    b = make_gpu(w, dtype, limiter, emf_solver, path="staged")
+    b = make_gpu(w, dtype, limiter, emf_solver, path=path)
+    assert b.path == path
     b.fill_guards()
     b.step(dt)
     err = rel_err(masked(b.download(), w.n), masked(ref, w.n))
@@ -137,7 +140,7 @@ def test_sub_bunch_chunking_is_bitwise_invisible(dtype):
     w = small_workloads(dtype)["turb16"]                        # 8 patches
     outs = []
     for ws in (None, 1):                                         # whole bunch at once / one patch per chunk
-        b = make_gpu(w, dtype, workspace_bytes=ws)
+        b = make_gpu(w, dtype, workspace_bytes=ws, path="two_kernel")   # the path that uses the workspace
         b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
         outs.append((b.download(), b.chunk))
         b.close()
