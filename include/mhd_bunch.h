@@ -89,8 +89,20 @@ int mhd_bunch_create(const mhd_bunch_desc *desc, const int32_t *nbr, void *state
 /* Guard fill of the current level: same-time, same-resolution copy of neighbour
  * interiors into the 3-deep guard shell, edges and corners included; -1 neighbours give
  * zero-gradient values and leave the closing face untouched (
- * DESIGN.md O1).  Must precede mhd_bunch_step.                                        */
+ * DESIGN.md O1).  Must precede mhd_bunch_step and mhd_bunch_cfl_dt.
+ *
+ * Deferred fill.  When the next step will run the one-pass kernel on a bunch all of whose
+ * neighbours exist, that kernel reads every halo straight from the neighbours' interiors,
+ * so this call only brings the closing faces up to date (if the caller may have written
+ * the buffer since the last fill) and marks the rest of the guard shell as owed.  The shell is written to HBM the moment anything reads it from there:
+ * mhd_bunch_current, mhd_bunch_download, mhd_bunch_sync_guards, mhd_bunch_set_path or a
+ * step by another path.  A caller that looks at guard cells of its own buffer must
+ * therefore go through one of those calls first (the Python binding always does).  What
+ * every entry point returns is identical to an immediate fill.                         */
 int mhd_bunch_fill_guards(mhd_bunch *b);
+
+/* Writes a deferred guard fill of the current level to HBM now (no-op if none is owed).  */
+int mhd_bunch_sync_guards(mhd_bunch *b);
 
 /* CFL time step of the current level: courant / max over interior cells of
  * sum_d (|u_d| + c_fast,d)/dx_d over active d (O9).
@@ -124,7 +136,11 @@ int mhd_bunch_download(mhd_bunch *b, void *host_state);
 int mhd_bunch_set_timing(mhd_bunch *b, int32_t enable);
 int mhd_bunch_kernel_times(mhd_bunch *b, int32_t cap, const char **names, double *ms, int64_t *count, int32_t *n);
 
-/* HOST out: which of state_a/state_b holds the current level.                           */
+/* HOST out: which of state_a/state_b holds the current level.  This is the call through
+ * which a caller gets at the state between library calls: a deferred guard fill is written
+ * out first, and the library assumes the caller may then modify the buffer (so the next
+ * mhd_bunch_fill_guards re-reads the closing faces).  Do not read or write the buffers
+ * behind the library's back without it (or mhd_bunch_upload / mhd_bunch_download).       */
 int mhd_bunch_current(mhd_bunch *b, void **state);
 
 /* Synchronises.  *bad_cells = number of interior cells met so far whose density or

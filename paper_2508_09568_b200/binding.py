@@ -19,7 +19,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
-    "mhd_bunch_chunk", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
 ]
 
 
@@ -43,9 +43,11 @@ def load_library(build_if_missing=True):
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.TARGET
-    if build_if_missing and _build.stale():
-        _build.build()
+    path = os.environ.get("MHD_BUNCH_LIB")       # an explicitly built library (e.g. a tuning variant)
+    if path is None:
+        path = _build.TARGET
+        if build_if_missing and _build.stale():
+            _build.build()
     if not os.path.exists(path):
         raise RuntimeError(f"{path} is missing: the CUDA extension must be built (no CPU fallback)")
     lib = C.CDLL(path)
@@ -53,6 +55,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_query.argtypes = [C.POINTER(Desc), C.POINTER(Layout)]
     lib.mhd_bunch_create.argtypes = [C.POINTER(Desc), vp, vp, vp, vp, C.c_size_t, C.POINTER(vp)]
     lib.mhd_bunch_fill_guards.argtypes = [vp]
+    lib.mhd_bunch_sync_guards.argtypes = [vp]
     lib.mhd_bunch_cfl_dt.argtypes = [vp, dbl, C.POINTER(dbl), vp, vp]
     lib.mhd_bunch_step.argtypes = [vp, dbl]
     lib.mhd_bunch_step_dev.argtypes = [vp, vp, dbl]
@@ -173,6 +176,10 @@ class MhdBunch:
     # ---- the path -------------------------------------------------------------------
     def fill_guards(self):
         _check(self.lib.mhd_bunch_fill_guards(self.h), "mhd_bunch_fill_guards")
+
+    def sync_guards(self):
+        """Write a deferred guard fill to HBM now (include/mhd_bunch.h)."""
+        _check(self.lib.mhd_bunch_sync_guards(self.h), "mhd_bunch_sync_guards")
 
     def cfl_dt(self, courant, sync=True, per_patch=False):
         dt = C.c_double(0.0)

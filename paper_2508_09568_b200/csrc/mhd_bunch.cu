@@ -57,8 +57,13 @@ struct mhd_bunch {
   size_t esz;
   // optional per-kernel-class timing (host-side objects only)
   int path;            // MHD_PATH_*: 0 = automatic choice
-  bool onepass_ok;     // three active dimensions, fp32, tensor maps of both state buffers built
-  CUtensorMap tm_h[2], tm_b[2];   // state buffers a/b: boxes of 5 hydro fields / 3 field components
+  bool onepass_ok;     // three active dimensions, fp32
+  bool gather_ok;      // the one-pass kernel can read halos from the neighbours' interiors: every
+                       // neighbour exists (no outflow side) and n_x is a whole number of 16-byte chunks
+  bool guards_stale;   // fill_guards was deferred: the guard shell of the current level is not in HBM
+  bool closing_ok;     // every closing face of the current level equals the neighbour's face 0: true after
+                       // any fill and kept by steps (both sides evaluate the same update on the same
+                       // data, bit for bit); false once the caller may have written the buffer
   bool fused_ok;       // three active dimensions and the tensor maps could be built
   int pred_ty;         // y-tile of the fused predictor (16, 8 or 4)
   DGeom DG;            // geometry of the D block
@@ -208,6 +213,28 @@ int launch_fill(mhd_bunch* b) {
   return MHD_OK;
 }
 
+// closing faces only (the part of the fill that cfl_dt and the one-pass kernel's update read)
+template <typename T>
+int launch_sync_closing(mhd_bunch* b) {
+  const Geom& G = b->G;
+  const long long per = (long long)G.n[1] * G.n[2] + (long long)G.n[0] * G.n[2] + (long long)G.n[0] * G.n[1];
+  const long long tot = per * G.np;
+  {
+    LaunchScope ls(b, KC_FILL);
+    k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
+
+// runs a deferred guard fill now (before anything reads the guard shell from HBM)
+int materialise_guards(mhd_bunch* b) {
+  if (!b->guards_stale) return MHD_OK;
+  b->guards_stale = false;
+  b->closing_ok = true;
+  return b->desc.dtype == MHD_F64 ? launch_fill<double>(b) : launch_fill<float>(b);
+}
+
 template <typename T>
 int launch_cfl(mhd_bunch* b, double courant, void* dt_dev, void* dt_patch) {
   const Geom& G = b->G;
@@ -250,10 +277,11 @@ template <> struct OnePassLaunch<float> {
     dim3 grid((unsigned)(xt * yt), (unsigned)G.np);
     {
       LaunchScope ls(b, KC_ONEPASS);
-      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->tm_h[b->cur], b->tm_b[b->cur], dtp, b->d_bad, xt);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt);
     }
     CUDA_TRY(cudaGetLastError());
     b->cur = 1 - b->cur;
+    b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
     return MHD_OK;
   }
 };
@@ -263,6 +291,11 @@ int launch_step(mhd_bunch* b) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
   const int path = effective_path(b);
+  if (path == MHD_PATH_ONEPASS && b->gather_ok) return OnePassLaunch<T>::run(b, dtp);
+  {  // every other route reads the guard shell from HBM
+    const int rc = materialise_guards(b);
+    if (rc != MHD_OK) return rc;
+  }
   if (path == MHD_PATH_ONEPASS) return OnePassLaunch<T>::run(b, dtp);
   const bool fused = path == MHD_PATH_TWO_KERNEL;
   if (fused) {
@@ -475,18 +508,12 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
     b->fused_ok = b->pred_ty != 0 && make_bunch_tensor_map(&b->tmap_d, b->d_dblock, f64, b->DG.pitch, b->DG.ny, b->DG.nz, b->chunk, W_DCOUNT,
                                         b->DG.ps, b->DG.fs, bx, by, W_DCOUNT);
   }
-  b->onepass_ok = false;
-  if (all_active(b->G) && desc->dtype == MHD_F32) {
-    using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
-    bool ok = true;
-    for (int s = 0; s < 2 && ok; ++s) {
-      ok = make_bunch_tensor_map(&b->tm_h[s], b->state[s], false, b->G.pitch, b->G.m[1], b->G.m[2], desc->npatch, 8, b->G.ps,
-                                 b->G.fs, Cfg::BWX, Cfg::PH, 5) &&
-           make_bunch_tensor_map(&b->tm_b[s], b->state[s], false, b->G.pitch, b->G.m[1], b->G.m[2], desc->npatch, 8, b->G.ps,
-                                 b->G.fs, Cfg::BWX, Cfg::PH, 3);
-    }
-    b->onepass_ok = ok;
-  }
+  b->onepass_ok = all_active(b->G) && desc->dtype == MHD_F32;
+  b->gather_ok = b->onepass_ok && b->G.n[0] % (int)(16 / b->esz) == 0;
+  for (long long c = 0; c < 27ll * desc->npatch && b->gather_ok; ++c)
+    if (nbr[c] < 0) b->gather_ok = false;
+  b->guards_stale = false;
+  b->closing_ok = false;
   cudaError_t e = cudaMemcpyAsync(b->d_nbr, nbr, sizeof(int) * 27 * (size_t)desc->npatch, cudaMemcpyHostToDevice, b->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(b->d_bad, 0, 512, b->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
@@ -497,7 +524,23 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
 
 int mhd_bunch_fill_guards(mhd_bunch* b) {
   if (!b) return MHD_ESTATE;
+  if (b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS) {
+    // deferred: the one-pass step reads halos from the neighbours' interiors, so only the
+    // closing faces are brought up to date now; the rest of the shell is written if and when
+    // something reads it from HBM (materialise_guards)
+    b->guards_stale = true;
+    if (b->closing_ok) return MHD_OK;
+    b->closing_ok = true;
+    return b->desc.dtype == MHD_F64 ? launch_sync_closing<double>(b) : launch_sync_closing<float>(b);
+  }
+  b->guards_stale = false;
+  b->closing_ok = true;
   return b->desc.dtype == MHD_F64 ? launch_fill<double>(b) : launch_fill<float>(b);
+}
+
+int mhd_bunch_sync_guards(mhd_bunch* b) {
+  if (!b) return MHD_ESTATE;
+  return materialise_guards(b);
 }
 
 int mhd_bunch_cfl_dt(mhd_bunch* b, double courant, double* dt_host, void* dt_dev, void* dt_per_patch_dev) {
@@ -533,6 +576,9 @@ int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
 
 int mhd_bunch_current(mhd_bunch* b, void** state) {
   if (!b || !state) return MHD_ESTATE;
+  const int rc = materialise_guards(b);   // the caller is about to look at the buffer
+  if (rc != MHD_OK) return rc;
+  b->closing_ok = false;                  // ... and may write it
   *state = b->state[b->cur];
   return MHD_OK;
 }
@@ -557,6 +603,8 @@ int mhd_bunch_set_path(mhd_bunch* b, int32_t path) {
   if (path < MHD_PATH_AUTO || path > MHD_PATH_ONEPASS) return MHD_EINVAL;
   if (path == MHD_PATH_ONEPASS && !b->onepass_ok) return MHD_EINVAL;
   if (path == MHD_PATH_TWO_KERNEL && !b->fused_ok) return MHD_EINVAL;
+  const int rc = materialise_guards(b);   // the other paths read the guard shell from HBM
+  if (rc != MHD_OK) return rc;
   b->path = path;
   return MHD_OK;
 }
@@ -623,12 +671,18 @@ static void drain_events(mhd_bunch* b, bool accumulate) {
 
 int mhd_bunch_upload(mhd_bunch* b, const void* host_state) {
   if (!b || !host_state) return MHD_ESTATE;
+  b->guards_stale = false;   // the whole buffer, guard shell included, is replaced
+  b->closing_ok = false;
   CUDA_TRY(cudaMemcpyAsync(b->state[b->cur], host_state, b->lay.state_bytes, cudaMemcpyHostToDevice, b->stream));
   return MHD_OK;
 }
 
 int mhd_bunch_download(mhd_bunch* b, void* host_state) {
   if (!b || !host_state) return MHD_ESTATE;
+  {
+    const int rc = materialise_guards(b);
+    if (rc != MHD_OK) return rc;
+  }
   CUDA_TRY(cudaMemcpyAsync(host_state, b->state[b->cur], b->lay.state_bytes, cudaMemcpyDeviceToHost, b->stream));
   CUDA_TRY(cudaStreamSynchronize(b->stream));
   return MHD_OK;

@@ -9,10 +9,14 @@
 // into three roles that run concurrently and hand data over through shared memory with
 // named barriers (bar.sync / bar.arrive), so that the issue slots of the SM stay busy:
 //
-//   P  predictor   U^n planes arrive by TMA (cp.async.bulk.tensor.5d on an mbarrier) into a
-//                  ring of raw planes; P forms primitives, edge EMFs, slopes and the half
-//                  step and writes the "D data" of one plane (38 arrays, see
-//                  fused_kernels.cuh) into one of two shared-memory slots.
+//   P  predictor   U^n planes arrive by 16-byte asynchronous copies (cp.async) into a ring of
+//                  raw planes.  In GATHER mode the halo of a plane is read straight from
+//                  the interiors of the neighbouring patches through the neighbour table
+//                  (guard fill O1 folded into the load: PAPER.md L124, L188, L241), so the
+//                  guard shell in HBM is neither written nor read; otherwise the patch's
+//                  own (already filled) guard cells are read.  P forms primitives, edge
+//                  EMFs, slopes and the half step and writes the "D data" of one plane
+//                  (38 arrays, see fused_kernels.cuh) into one of two shared-memory slots.
 //   A  z-coupled   reads D planes k-1 and k: HLLD at the z-face, 2D Riemann problems at the
 //                  x- and y-directed edges; finishes the update of plane k-1 and of b_z.
 //   C  in-plane    reads D plane k: HLLD at the x- and y-faces, 2D Riemann problem at the
@@ -30,6 +34,11 @@ namespace mhd {
 
 __device__ __forceinline__ void nb_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+// 16-byte asynchronous copy global -> shared (L2 only), and the wait for all of a thread's copies
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <typename T, int TX, int TY, int NPW> struct OneCfg {
   static constexpr int PW = TX + 5, PH = TY + 5, PA = PW * PH;     // predictor positions: cells x0-2.., y0-2..
@@ -55,9 +64,10 @@ template <typename T, int TX, int TY, int NPW> struct OneCfg {
   static constexpr size_t o_xe = o_pu + al(sizeof(T) * 7 * FA);        // [2][NR]   A: ex, ey of the neighbours
   static constexpr size_t o_xy = o_xe + al(sizeof(T) * 2 * NR);        // [6][NR]   C: +y exchange
   static constexpr size_t o_xc = o_xy + al(sizeof(T) * 6 * NR);        // [6][32]   C: closing column -> column TX-1
-  static constexpr size_t o_bar = o_xc + al(sizeof(T) * 6 * 32);       // 2 mbarriers
-  static constexpr size_t smem = o_bar + 64;
-  static constexpr uint32_t bytes_h = (uint32_t)(sizeof(T) * 5 * RA), bytes_b = (uint32_t)(sizeof(T) * 3 * RA);
+  static constexpr size_t o_nb = o_xc + al(sizeof(T) * 6 * 32);        // [27] source patch per neighbour class
+  static constexpr size_t smem = o_nb + 128;
+  static constexpr int VEC = 16 / sizeof(T), CPR = BWX / VEC;          // elements per 16-byte copy, copies per row
+  static_assert(BWX % VEC == 0, "raw rows are whole 16-byte chunks");
 };
 
 // named barrier ids (0 is __syncthreads)
@@ -103,8 +113,8 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
 
 template <typename T, int TX, int TY, int NPW>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
-k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_b,
-               const double* __restrict__ dtp, unsigned long long* __restrict__ bad, int xtiles) {
+k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
+               unsigned long long* __restrict__ bad, int xtiles) {
   using C = OneCfg<T, TX, TY, NPW>;
   constexpr int PW = C::PW, PH = C::PH, PA = C::PA, BWX = C::BWX, RA = C::RA, DW = C::DW, DC = C::DC;
   constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL;
@@ -116,7 +126,7 @@ k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __gr
   T* const XE = reinterpret_cast<T*>(smem_raw + C::o_xe);
   T* const XY = reinterpret_cast<T*>(smem_raw + C::o_xy);
   T* const XC = reinterpret_cast<T*>(smem_raw + C::o_xc);
-  uint64_t* const bar = reinterpret_cast<uint64_t*>(smem_raw + C::o_bar);
+  int* const NBS = reinterpret_cast<int*>(smem_raw + C::o_nb);
 
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
@@ -130,11 +140,9 @@ k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __gr
   const T dt = (T)(*dtp);
   const T gamma = P.gamma;
 
-  if (t == 0) {
-    mbar_init(&bar[0], 1);
-    mbar_init(&bar[1], 1);
-    fence_mbar_init();
-  }
+  // source patch of each of the 27 neighbour classes: the neighbour table in gather mode,
+  // the patch itself (whose guard cells are then read) otherwise
+  if (t < 27) NBS[t] = gather ? nbr[(long long)(P.p0 + pl) * 27 + t] : P.p0 + pl;
   __syncthreads();
 
   auto dslot = [&](int plane) { return Dm + (size_t)((plane + 2) & 1) * (D_COUNT * DC); };
@@ -150,20 +158,43 @@ k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __gr
     auto RH = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawh + (size_t)((plane + 2) & 1) * C::rawh_slot); };
     auto RB = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawb + (size_t)((plane + 4) & 3) * C::rawb_slot); };
     const int rlo = -2, rhi = nz + 2;
-    auto issue = [&](int plane) {   // one thread: U^n plane -> raw ring (two boxes: 5 hydro fields, 3 field components)
-      uint64_t* b = &bar[(plane + 2) & 1];
-      mbar_arrive_expect_tx(b, C::bytes_h + C::bytes_b);
-      tma_load_5d(const_cast<T*>(RH(plane)), &tm_h, b, x0, y0 + 1, plane + 3, P.p0 + pl, 0);
-      tma_load_5d(const_cast<T*>(RB(plane)), &tm_b, b, x0, y0 + 1, plane + 3, P.p0 + pl, 5);
+    // U^n plane -> raw ring, one 16-byte chunk of a row per copy, all 8 fields.  A chunk lies
+    // in one patch (x0 and, in gather mode, n_x are multiples of the chunk); its source is
+    // the image cell in the neighbour of class (ox,oy,oz) -- O1 -- or, without gather, the
+    // same cell of the own patch.  Chunks past the data a tile needs are skipped.
+    auto issue = [&](int plane) {
+      const long long zplane = (long long)G.pitch * G.m[1];
+      const int oz = gather ? (plane < 0 ? -1 : (plane >= nz ? 1 : 0)) : 0;
+      const long long zoff = (long long)(plane - oz * nz + G.g[2]) * zplane;
+      T* const dh = const_cast<T*>(RH(plane));
+      T* const db = const_cast<T*>(RB(plane));
+      for (int it = tp; it < PH * C::CPR; it += NP) {
+        const int row = it / C::CPR, ch = it - row * C::CPR;
+        const int x = x0 - 4 + ch * C::VEC, y = y0 - 2 + row;   // first cell of the chunk (raw column 0 is cell x0-4)
+        int ox = 0, oy = 0;
+        if (gather) { ox = x < 0 ? -1 : (x >= nx ? 1 : 0); oy = y < 0 ? -1 : (y >= ny ? 1 : 0); }
+        const int xs = x - ox * nx, ys = y - oy * ny;
+        const bool ok = gather ? (xs + C::VEC <= nx && ys < ny && xs >= 0 && ys >= 0)
+                               : (G.lead + G.g[0] + xs + C::VEC <= G.pitch && ys + G.g[1] < G.m[1]);
+        if (!ok) continue;
+        const int q = NBS[(oz + 1) * 9 + (oy + 1) * 3 + (ox + 1)];
+        const T* src = P.U + (long long)q * G.ps + zoff + (long long)(ys + G.g[1]) * G.pitch + (G.lead + G.g[0] + xs);
+        const int o = row * BWX + ch * C::VEC;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) cp_async16(dh + f * RA + o, src + f * G.fs);
+#pragma unroll
+        for (int f = 0; f < 3; ++f) cp_async16(db + f * RA + o, src + (5 + f) * G.fs);
+      }
     };
-    if (tp == 0) issue(rlo);
+    issue(rlo);
+    cp_async_wait_all();
+    nb_sync(NB_P, NP);
     T cbx[C::PASS3], cby[C::PASS3];   // backward z-differences of the raw bx, by of the own D cells
 #pragma unroll
     for (int s = 0; s < C::PASS3; ++s) { cbx[s] = T(0); cby[s] = T(0); }
     unsigned int nbad = 0;
 
     for (int r = rlo; r <= rhi; ++r) {
-      mbar_wait(&bar[(r + 2) & 1], (uint32_t)(((r + 2) >> 1) & 1));
       // ---- primitives of plane r-1 (O2): needs bx(i+1), by(j+1) of plane r-1 and bz of plane r
       if (r - 1 >= rlo) {
         const T* hy = RH(r - 1);
@@ -193,7 +224,7 @@ k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __gr
       }
       nb_sync(NB_P, NP);
       // every P thread is past iteration r-1: the slots of hydro plane r-1 and field plane r-3 are free
-      if (tp == 0 && r + 1 <= rhi) issue(r + 1);
+      if (r + 1 <= rhi) issue(r + 1);
 
       // ---- edge EMFs of plane r-1 (O4a: Eq. 7-11 and cyclic images)
       if (r - 2 >= rlo) {
@@ -308,7 +339,8 @@ k_step_onepass(Params<T> P, const __grid_constant__ CUtensorMap tm_h, const __gr
           nb_arrive(NB_FULL + ((kd + 2) & 1), NALL);
         }
       }
-      nb_sync(NB_P, NP);   // the rings are rewritten by the next iteration
+      cp_async_wait_all();   // own chunks of plane r+1 have landed ...
+      nb_sync(NB_P, NP);     // ... and everybody's; the rings are rewritten by the next iteration
     }
     if (nbad) atomicAdd(bad, (unsigned long long)nbad);
     return;

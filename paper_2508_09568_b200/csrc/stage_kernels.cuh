@@ -89,6 +89,33 @@ __global__ void __launch_bounds__(256) k_fill_guards(Geom G, FillMap M, T* __res
   }
 }
 
+// The closing faces alone (O8: face n_a of the normal field b_a sits in the first high guard
+// slot): the neighbour's face 0 overwrites it, an outflow side keeps the evolved value.
+// This is the only part of the guard shell that cfl_dt and the one-pass kernel's update read
+// from HBM, so it is all a deferred fill has to do up front.
+template <typename T>
+__global__ void __launch_bounds__(256) k_sync_closing_faces(Geom G, T* __restrict__ U, const int* __restrict__ nbr) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int fx = G.n[1] * G.n[2], fy = G.n[0] * G.n[2], fz = G.n[0] * G.n[1];
+  const int per = fx + fy + fz;
+  if (t >= (long long)per * G.np) return;
+  const int p = (int)(t / per);
+  int r = (int)(t - (long long)p * per);
+  int a, c[3];
+  if (r < fx) { a = 0; c[0] = G.n[0]; c[1] = r % G.n[1]; c[2] = r / G.n[1]; }
+  else if (r < fx + fy) { r -= fx; a = 1; c[0] = r % G.n[0]; c[1] = G.n[1]; c[2] = r / G.n[0]; }
+  else { r -= fx + fy; a = 2; c[0] = r % G.n[0]; c[1] = r / G.n[0]; c[2] = G.n[2]; }
+  if (!G.act[a]) return;
+  const int cls = 13 + (a == 0 ? 1 : (a == 1 ? 3 : 9));      // neighbour class with offset +1 along a
+  const int q = nbr[p * 27 + cls];
+  if (q < 0) return;
+  const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1];
+  const long long dst = (long long)p * G.ps + G.lead + (c[0] + G.g[0]) + (c[1] + G.g[1]) * pitch + (c[2] + G.g[2]) * plane;
+  c[a] = 0;
+  const long long from = (long long)q * G.ps + G.lead + (c[0] + G.g[0]) + (c[1] + G.g[1]) * pitch + (c[2] + G.g[2]) * plane;
+  U[(5 + a) * G.fs + dst] = U[(5 + a) * G.fs + from];
+}
+
 // -------------------------------------------------------------------------- CFL ----
 __device__ __forceinline__ unsigned long long enc_max(double x) { return (unsigned long long)__double_as_longlong(x); }
 

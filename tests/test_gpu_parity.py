@@ -58,6 +58,48 @@ def test_fill_guards_mixed_outflow_periodic_3d():
     b.close()
 
 
+@pytest.mark.parametrize("name", ["turb16", "turb_ragged", "turb_self"])
+def test_deferred_fill_is_indistinguishable_from_an_immediate_one(name):
+    """fp32 periodic 3D bunches defer the fill (the one-pass kernel reads halos from the
+    neighbours' interiors; include/mhd_bunch.h).  Whatever the caller can see must equal an
+    immediate fill: (a) the guard shell after download, bit for bit against the oracle's
+    fill, also after steps; (b) a step that read neighbours' interiors equals, bit for bit,
+    the same steps with the guard shell written first; the launch count shows which route
+    ran."""
+    w = small_workloads("f32")[name]
+    o = make_oracle(w)
+    # (a) random data, guards included
+    rng = np.random.default_rng(11)
+    w.U = rng.normal(size=w.U.shape).astype(np.float32)
+    b = make_gpu(w, "f32")
+    assert b.path == "onepass"
+    b.fill_guards()
+    l0 = b.launches
+    got = b.download()
+    deferred = (b.launches - l0) == 1          # the owed fill ran when the buffer was looked at
+    assert deferred == (bool((w.nbr >= 0).all()) and w.n[0] % 4 == 0)
+    assert np.array_equal(got.astype(np.float64), o.fill_guards(w.U.astype(np.float64).copy(), w.nbr))
+    b.close()
+    # (b) physical data: deferred fill + step, against fill written first (sync_guards) + step
+    w = small_workloads("f32")[name]
+    outs = []
+    for force in (False, True):
+        b = make_gpu(w, "f32")
+        for _ in range(3):
+            b.fill_guards()
+            if force:
+                b.sync_guards()
+            b.cfl_dt(0.4, sync=False)
+            b.step_dev()
+        b.fill_guards()
+        outs.append(b.download())
+        b.close()
+    assert np.array_equal(outs[0], outs[1])
+    ref = o.fill_guards(outs[0].astype(np.float64).copy(), w.nbr)
+    assert np.array_equal(outs[0].astype(np.float64), ref)
+    assert deferred, "periodic fp32 3D bunches with n_x % 4 == 0 are expected to take the deferred route"
+
+
 # ------------------------------------------------------------------------ CFL -------
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-13), ("f32", 2e-6)])
 @pytest.mark.parametrize("name", ["sod_x", "tube_z", "ot_ragged", "turb_ragged"])
