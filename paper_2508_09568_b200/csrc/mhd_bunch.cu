@@ -33,7 +33,10 @@ template <typename T> struct FusedTile;
 template <> struct FusedTile<float> { static constexpr int TX = 32, TY = 8; };
 template <> struct FusedTile<double> { static constexpr int TX = 16, TY = 8; };
 // one-pass kernel (onepass_kernel.cuh): tile and number of predictor warps
-struct OneTile { static constexpr int TX = 32, TY = 8, NPW = 6; };
+#ifndef ONEPASS_NPW
+#define ONEPASS_NPW 6
+#endif
+struct OneTile { static constexpr int TX = 32, TY = 8, NPW = ONEPASS_NPW; };
 
 // ------------------------------------------------------------------------ handle ----
 struct mhd_bunch {
