@@ -268,13 +268,14 @@ template <typename T> struct OnePassLaunch {
 template <> struct OnePassLaunch<float> {
   static int run(mhd_bunch* b, const double* dtp) {
     using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
-    auto kern = k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
-    static bool attr_done = false;
-    if (!attr_done) {
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
-      attr_done = true;
-    }
     const Geom& G = b->G;
+    auto kern = G.limiter == 1 ? k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW, 1>
+                               : k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW, 2>;
+    static bool attr_done[3] = {false, false, false};
+    if (!attr_done[G.limiter]) {
+      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      attr_done[G.limiter] = true;
+    }
     Params<float> P = make_params<float>(b, 0, G.np);
     const int xt = (G.n[0] + OneTile::TX - 1) / OneTile::TX, yt = (G.n[1] + OneTile::TY - 1) / OneTile::TY;
     dim3 grid((unsigned)(xt * yt), (unsigned)G.np);

@@ -50,7 +50,10 @@ template <typename T, int TX, int TY, int NPW> struct OneCfg {
   static constexpr int NP = NPW * 32;                              // threads of role P
   static constexpr int NTH = 2 * NR + NP;
   static constexpr int NALL = NTH;
-  static constexpr int PASS1 = (PA + NP - 1) / NP, PASS3 = (DC + NP - 1) / NP;
+  // compact index spaces of the predictor passes: primitives on columns 0..PW-2 and rows
+  // 0..PH-2, edge EMFs on columns 1..PW-2 and rows 1..PH-2, D cells
+  static constexpr int W1 = PW - 1, N1 = W1 * (PH - 1), W2 = PW - 2, N2 = W2 * (PH - 2);
+  static constexpr int PASS1 = (N1 + NP - 1) / NP, PASS2 = (N2 + NP - 1) / NP, PASS3 = (DC + NP - 1) / NP;
   static_assert(FH <= 32 && 32 % TX == 0, "tile shape");
   static constexpr size_t al(size_t x) { return (x + 127) / 128 * 128; }
   // shared-memory map (bytes)
@@ -111,7 +114,7 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
   return c[(D_BH + X) * DC] + s * c[dbf_slot(X, ALONG) * DC];
 }
 
-template <typename T, int TX, int TY, int NPW>
+template <typename T, int TX, int TY, int NPW, int LIM>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
                unsigned long long* __restrict__ bad, int xtiles) {
@@ -152,7 +155,6 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
     const int tp = t - 2 * NR;
     const T q4 = T(0.25), hdt = h * dt;
     const T lx = hdt * P.idx[0], ly = hdt * P.idx[1], lz = hdt * P.idx[2];
-    const int lim = G.limiter;
     auto Qs = [&](int plane, int f) { return Q + (((plane + 3) % 3) * 8 + f) * PA; };
     auto Es = [&](int plane, int a) { return Em + (((plane + 2) & 1) * 3 + a) * PA; };
     auto RH = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawh + (size_t)((plane + 2) & 1) * C::rawh_slot); };
@@ -203,9 +205,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 #pragma unroll
         for (int s = 0; s < C::PASS1; ++s) {
           const int pos = tp + s * NP;
-          const int pr = pos / PW, pc = pos - pr * PW;
-          if (pos < PA && pc <= PW - 2 && pr <= PH - 2) {
-            const int o = pos, ob = pr * BWX + pc + 2;
+          const int pr = pos / C::W1, pc = pos - pr * C::W1;
+          if (pos < C::N1) {
+            const int o = pr * PW + pc, ob = pr * BWX + pc + 2;
             const T rho = hy[ob], ir = num<T>::rcp(rho);
             const T u = hy[RA + ob] * ir, v = hy[2 * RA + ob] * ir, w = hy[3 * RA + ob] * ir;
             const T bz0 = bb[2 * RA + ob];
@@ -231,11 +233,11 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         const T* b1 = RB(r - 1);
         const T* b2 = RB(r - 2);
 #pragma unroll
-        for (int s = 0; s < C::PASS1; ++s) {
+        for (int s = 0; s < C::PASS2; ++s) {
           const int pos = tp + s * NP;
-          const int pr = pos / PW, pc = pos - pr * PW;
-          if (pos < PA && pc >= 1 && pr >= 1 && pc <= PW - 2 && pr <= PH - 2) {
-            const int o = pos, ob = pr * BWX + pc + 2;
+          const int pr = pos / C::W2 + 1, pc = pos - (pr - 1) * C::W2 + 1;
+          if (pos < C::N2) {
+            const int o = pr * PW + pc, ob = pr * BWX + pc + 2;
             const T *u1 = Qs(r - 1, 1) + o, *v1 = Qs(r - 1, 2) + o, *w1 = Qs(r - 1, 3) + o;
             const T *u2 = Qs(r - 2, 1) + o, *v2 = Qs(r - 2, 2) + o, *w2 = Qs(r - 2, 3) + o;
             const T *bx1 = b1 + ob, *by1 = b1 + RA + ob, *bz1 = b1 + 2 * RA + ob;
@@ -296,7 +298,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
                   if (f == 5 + d) { dq[f] = T(0); continue; }
                   const T lo = d == 0 ? qc[f * PA - 1] : (d == 1 ? qc[f * PA - PW] : qm[f * PA]);
                   const T hi = d == 0 ? qc[f * PA + 1] : (d == 1 ? qc[f * PA + PW] : qp[f * PA]);
-                  dq[f] = limited_slope(lim, c[f] - lo, hi - c[f]);
+                  dq[f] = limited_slope_k<LIM>(c[f] - lo, hi - c[f]);
                   D[dq_slot(d, f) * DC] = dq[f];
                 }
                 const int b = (d + 1) % 3, e = (d + 2) % 3;
@@ -311,12 +313,12 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
                 vh[e] += lam[d] * c[5 + d] * dq[5 + e] * ir;
               }
               // face-field transverse slopes: dy bx, dz bx, dx by, dz by, dx bz, dy bz
-              D[(D_DBF + 0) * DC] = limited_slope(lim, bxc - bx[-BWX], bx[BWX] - bxc);
-              D[(D_DBF + 1) * DC] = limited_slope(lim, cbx[s], fwx);
-              D[(D_DBF + 2) * DC] = limited_slope(lim, byc - by[-1], by[1] - byc);
-              D[(D_DBF + 3) * DC] = limited_slope(lim, cby[s], fwy);
-              D[(D_DBF + 4) * DC] = limited_slope(lim, bzc - bz[-1], bz[1] - bzc);
-              D[(D_DBF + 5) * DC] = limited_slope(lim, bzc - bz[-BWX], bz[BWX] - bzc);
+              D[(D_DBF + 0) * DC] = limited_slope_k<LIM>(bxc - bx[-BWX], bx[BWX] - bxc);
+              D[(D_DBF + 1) * DC] = limited_slope_k<LIM>(cbx[s], fwx);
+              D[(D_DBF + 2) * DC] = limited_slope_k<LIM>(byc - by[-1], by[1] - byc);
+              D[(D_DBF + 3) * DC] = limited_slope_k<LIM>(cby[s], fwy);
+              D[(D_DBF + 4) * DC] = limited_slope_k<LIM>(bzc - bz[-1], bz[1] - bzc);
+              D[(D_DBF + 5) * DC] = limited_slope_k<LIM>(bzc - bz[-BWX], bz[BWX] - bzc);
               // half-step faces (Eq. 12 with dt/2) of this cell and of its +x, +y, +z neighbours
               const T *ex0 = Es(kd, 0) + o, *ey0 = Es(kd, 1) + o, *ez0 = Es(kd, 2) + o;
               const T *ex1 = Es(kd + 1, 0) + o, *ey1 = Es(kd + 1, 1) + o;
