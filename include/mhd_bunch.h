@@ -127,6 +127,49 @@ int mhd_bunch_step_dev(mhd_bunch *b, const void *dt_dev, double dt_max);
 int mhd_bunch_upload(mhd_bunch *b, const void *host_state);
 int mhd_bunch_download(mhd_bunch *b, void *host_state);
 
+/* Host-streaming path (bunches handed to the GPU
+ * round-robin with several in flight; L243-247: asynchronous host<->device staging).  The
+ * bunch lives in HOST memory in the COMPACT layout  host[field][patch][k][j][i]  (interior
+ * cells only, n_z*n_y*n_x per patch and field, fields in Eq. 6's order; B components on the
+ * lower faces; host_bytes long; pinned memory lets the copies run asynchronously).  One
+ * call advances it by one step: chunks of patches cross PCIe on two library-owned copy
+ * streams, are scattered into the padded HBM layout, stepped chunk by chunk as soon as the
+ * chunks holding their neighbours have arrived (the neighbour table decides), gathered and
+ * copied back -- so uploads, kernels and downloads overlap.  Guard zones never cross PCIe.
+ *
+ *   mhd_bunch_host_query   HOST out *layout for a chunk size (<= 0: library default):
+ *                          host_bytes, the staging size, the number of chunks, and whether
+ *                          the fully overlapped schedule applies (one-pass path with every
+ *                          neighbour present); otherwise uploads, a whole-bunch step and
+ *                          downloads run back to back, still through the same chunks.
+ *   mhd_bunch_host_attach  staging_dev: DEVICE, caller-owned, >= staging_bytes, 16-byte
+ *                          aligned, borrowed until detach/destroy.  MHD_EINVAL for bunches
+ *                          with outflow (-1) neighbours: their evolved closing faces have
+ *                          no slot in the compact layout.  Creates the streams and events.
+ *   mhd_bunch_step_host    host_in: HOST const, time level n; host_out: HOST, receives level
+ *                          n+1 (may equal host_in only if dt == 0 or the schedule is not
+ *                          overlapped -- keep them distinct).  dt > 0: step with this dt
+ *                          (uploads and steps overlap); dt == 0: the step is the CFL step
+ *                          courant/max rate of level n, which needs every chunk on the
+ *                          device first.  HOST out, nullable: *dt_used, and *dt_next =
+ *                          the CFL step of level n+1 (so the next call can pass dt > 0).
+ *                          Synchronises: on return host_out is complete.  The device keeps
+ *                          level n+1 as the current level.
+ */
+typedef struct {
+  size_t  host_bytes;      /* bytes of a compact host state                                */
+  size_t  staging_bytes;   /* bytes of device staging mhd_bunch_host_attach needs          */
+  int32_t chunk_patches;   /* patches per chunk                                            */
+  int32_t nchunk;          /* chunks per bunch                                             */
+  int32_t pipelined;       /* 1: uploads, steps and downloads overlap chunk by chunk       */
+  int32_t reserved;
+} mhd_bunch_host_layout;
+int mhd_bunch_host_query(mhd_bunch *b, int32_t chunk_patches, mhd_bunch_host_layout *layout);
+int mhd_bunch_host_attach(mhd_bunch *b, void *staging_dev, size_t staging_bytes, int32_t chunk_patches);
+int mhd_bunch_step_host(mhd_bunch *b, const void *host_in, void *host_out, double dt, double courant,
+                        double *dt_used, double *dt_next);
+int mhd_bunch_host_detach(mhd_bunch *b);
+
 /* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
  * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
  * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to

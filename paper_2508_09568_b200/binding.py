@@ -20,6 +20,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
     "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_host_query", "mhd_bunch_host_attach", "mhd_bunch_step_host", "mhd_bunch_host_detach",
 ]
 
 
@@ -33,6 +34,11 @@ class Layout(C.Structure):
     _fields_ = [("stride", C.c_int64 * 5), ("origin", C.c_int64), ("state_elems", C.c_int64),
                 ("state_bytes", C.c_size_t), ("workspace_min", C.c_size_t), ("workspace_best", C.c_size_t),
                 ("m", C.c_int32 * 3), ("reserved", C.c_int32)]
+
+
+class HostLayout(C.Structure):
+    _fields_ = [("host_bytes", C.c_size_t), ("staging_bytes", C.c_size_t), ("chunk_patches", C.c_int32),
+                ("nchunk", C.c_int32), ("pipelined", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -71,6 +77,10 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_get_path.argtypes = [vp, C.POINTER(i32)]
     lib.mhd_bunch_measure_alu_peak.argtypes = [i32, i32, C.POINTER(dbl)]
     lib.mhd_bunch_destroy.argtypes = [vp]
+    lib.mhd_bunch_host_query.argtypes = [vp, i32, C.POINTER(HostLayout)]
+    lib.mhd_bunch_host_attach.argtypes = [vp, vp, C.c_size_t, i32]
+    lib.mhd_bunch_step_host.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.mhd_bunch_host_detach.argtypes = [vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
     lib.mhd_bunch_last_cuda_error.restype = C.c_char_p
@@ -198,6 +208,25 @@ class MhdBunch:
 
     def download_host(self, host_tensor):
         _check(self.lib.mhd_bunch_download(self.h, host_tensor.data_ptr()), "mhd_bunch_download")
+
+    # ---- host-streaming path (include/mhd_bunch.h: mhd_bunch_host_*) -------------------
+    def host_attach(self, chunk_patches=0):
+        """Allocate the device staging (a torch tensor) and attach it; returns the layout."""
+        lay = HostLayout()
+        _check(self.lib.mhd_bunch_host_query(self.h, chunk_patches, C.byref(lay)), "mhd_bunch_host_query")
+        self.host_staging = self.torch.empty(lay.staging_bytes, dtype=self.torch.uint8, device=self.device)
+        _check(self.lib.mhd_bunch_host_attach(self.h, self.host_staging.data_ptr(), lay.staging_bytes,
+                                              lay.chunk_patches), "mhd_bunch_host_attach")
+        self.host_lay = lay
+        return lay
+
+    def step_host(self, host_in, host_out, dt=0.0, courant=0.4):
+        """host_in/host_out: pinned torch CPU tensors in the compact layout [8, npatch, nz, ny, nx].
+        Returns (dt_used, dt_next)."""
+        used, nxt = C.c_double(0.0), C.c_double(0.0)
+        _check(self.lib.mhd_bunch_step_host(self.h, host_in.data_ptr(), host_out.data_ptr(), dt, courant,
+                                            C.byref(used), C.byref(nxt)), "mhd_bunch_step_host")
+        return used.value, nxt.value
 
     def status(self):
         v = C.c_int64(0)

@@ -12,6 +12,7 @@
 #include "stage_kernels.cuh"
 #include "fused_kernels.cuh"
 #include "onepass_kernel.cuh"
+#include "host_stream_kernels.cuh"
 
 #include <cuda_runtime.h>
 #include <math.h>
@@ -20,6 +21,8 @@
 #include <string.h>
 #include <new>
 #include <vector>
+#include <algorithm>
+#include <type_traits>
 
 using namespace mhd;
 
@@ -72,6 +75,18 @@ struct mhd_bunch {
   DGeom DG;            // geometry of the D block
   char* d_dblock;
   CUtensorMap tmap_d;  // D block of the scratch: [38][chunk][mz][my][pitch]
+  // host-streaming path (mhd_bunch_host_attach / mhd_bunch_step_host)
+  struct HostStream {
+    char* stage_up; char* stage_dn;      // DEVICE staging, one chunk each (caller-owned)
+    int chunk, nchunk;                   // patches per chunk, number of chunks
+    cudaStream_t s_up, s_dn;             // copy-in and copy-out streams (library-owned)
+    cudaEvent_t ev_begin, ev_all_steps;
+    std::vector<cudaEvent_t> ev_up, ev_step;   // per upload position / per chunk
+    std::vector<int> up_order, step_order, ready;   // ready[c]: upload position after which chunk c may step
+  };
+  HostStream* hs;
+  std::vector<int>* h_nbr;   // HOST copy of the neighbour table (schedules of the host-streaming path)
+  bool all_nbr;        // no -1 entry in the neighbour table
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
   std::vector<Ev>* events;
@@ -218,13 +233,14 @@ int launch_fill(mhd_bunch* b) {
 
 // closing faces only (the part of the fill that cfl_dt and the one-pass kernel's update read)
 template <typename T>
-int launch_sync_closing(mhd_bunch* b) {
+int launch_sync_closing(mhd_bunch* b, int p0 = 0, int npl = -1) {
   const Geom& G = b->G;
+  if (npl < 0) npl = G.np;
   const long long per = (long long)G.n[1] * G.n[2] + (long long)G.n[0] * G.n[2] + (long long)G.n[0] * G.n[1];
-  const long long tot = per * G.np;
+  const long long tot = per * npl;
   {
     LaunchScope ls(b, KC_FILL);
-    k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr);
+    k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr, p0, npl);
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
@@ -263,10 +279,11 @@ int effective_path(const mhd_bunch* b) {
 }
 
 template <typename T> struct OnePassLaunch {
-  static int run(mhd_bunch*, const double*) { return MHD_EINVAL; }
+  static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true) { return MHD_EINVAL; }
 };
 template <> struct OnePassLaunch<float> {
-  static int run(mhd_bunch* b, const double* dtp) {
+  // patches [p0, p0+npl) of the bunch (npl < 0: all); `last` flips the buffers
+  static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true) {
     using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
     const Geom& G = b->G;
     auto kern = G.limiter == 1 ? k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW, 1>
@@ -276,16 +293,19 @@ template <> struct OnePassLaunch<float> {
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       attr_done[G.limiter] = true;
     }
-    Params<float> P = make_params<float>(b, 0, G.np);
+    if (npl < 0) npl = G.np;
+    Params<float> P = make_params<float>(b, p0, npl);
     const int xt = (G.n[0] + OneTile::TX - 1) / OneTile::TX, yt = (G.n[1] + OneTile::TY - 1) / OneTile::TY;
-    dim3 grid((unsigned)(xt * yt), (unsigned)G.np);
+    dim3 grid((unsigned)(xt * yt), (unsigned)npl);
     {
       LaunchScope ls(b, KC_ONEPASS);
       kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt);
     }
     CUDA_TRY(cudaGetLastError());
-    b->cur = 1 - b->cur;
-    b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
+    if (last) {
+      b->cur = 1 - b->cur;
+      b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
+    }
     return MHD_OK;
   }
 };
@@ -514,8 +534,13 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   }
   b->onepass_ok = all_active(b->G) && desc->dtype == MHD_F32;
   b->gather_ok = b->onepass_ok && b->G.n[0] % (int)(16 / b->esz) == 0;
-  for (long long c = 0; c < 27ll * desc->npatch && b->gather_ok; ++c)
-    if (nbr[c] < 0) b->gather_ok = false;
+  b->all_nbr = true;
+  for (long long c = 0; c < 27ll * desc->npatch && b->all_nbr; ++c)
+    if (nbr[c] < 0) b->all_nbr = false;
+  b->gather_ok = b->gather_ok && b->all_nbr;
+  b->hs = nullptr;
+  b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
+  if (!b->h_nbr) { delete b->events; delete b; return MHD_ENOMEM; }
   b->guards_stale = false;
   b->closing_ok = false;
   cudaError_t e = cudaMemcpyAsync(b->d_nbr, nbr, sizeof(int) * 27 * (size_t)desc->npatch, cudaMemcpyHostToDevice, b->stream);
@@ -717,10 +742,278 @@ int mhd_bunch_kernel_times(mhd_bunch* b, int32_t cap, const char** names, double
   return MHD_OK;
 }
 
+}  // extern "C"
+
+// ------------------------------------------------------- host-streaming path ----
+namespace {
+
+size_t hs_chunk_bytes(const mhd_bunch* b, int chunk) {
+  return align_up((size_t)8 * chunk * b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz, 256);
+}
+
+void hs_release(mhd_bunch* b) {
+  mhd_bunch::HostStream* h = b->hs;
+  if (!h) return;
+  cudaStreamSynchronize(h->s_up);
+  cudaStreamSynchronize(h->s_dn);
+  for (cudaEvent_t e : h->ev_up) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->ev_step) cudaEventDestroy(e);
+  cudaEventDestroy(h->ev_begin);
+  cudaEventDestroy(h->ev_all_steps);
+  cudaStreamDestroy(h->s_up);
+  cudaStreamDestroy(h->s_dn);
+  delete h;
+  b->hs = nullptr;
+}
+
+template <typename T, bool PACK>
+int launch_pack(mhd_bunch* b, cudaStream_t st, void* state, char* stage, int p0, int npl) {
+  const Geom& G = b->G;
+  const int vec = (int)(16 / sizeof(T));
+  const long long n = (long long)8 * npl * G.n[0] * G.n[1] * G.n[2];
+  b->launches += 1;
+  if (G.n[0] % vec == 0) {
+    const unsigned blocks = blocks_for(n / vec, 256);
+    k_pack_unpack<T, (int)(16 / sizeof(T)), PACK><<<blocks, 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl);
+  } else {
+    k_pack_unpack<T, 1, PACK><<<blocks_for(n, 256), 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
+
+// one strided copy per chunk: rows = the eight fields, host[f][p0 .. p0+npl) <-> stage[f][0 .. npl)
+int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device) {
+  const size_t per = (size_t)b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
+  char* h = host + (size_t)p0 * per;
+  const size_t hp = (size_t)b->G.np * per, dp = (size_t)npl * per;
+  if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, hp, dp, 8, cudaMemcpyHostToDevice, st));
+  else CUDA_TRY(cudaMemcpy2DAsync(h, hp, stage, dp, dp, 8, cudaMemcpyDeviceToHost, st));
+  return MHD_OK;
+}
+
+// Schedule of one host-streamed step for a chunk size.  Uploads run in rotated order (last
+// chunk first: a periodic stack of slabs can then start stepping after three uploads); a
+// chunk may step once the last upload carrying one of its neighbours has landed (ready[c] =
+// that upload's position); chunks step in order of readiness.
+struct HsPlan { std::vector<int> up_order, ready, step_order; };
+HsPlan hs_plan(const mhd_bunch* b, int chunk) {
+  HsPlan pl;
+  const int np = b->G.np, C = (np + chunk - 1) / chunk;
+  pl.up_order.resize(C);
+  std::vector<int> upos(C);
+  for (int u = 0; u < C; ++u) { pl.up_order[u] = (u + C - 1) % C; upos[pl.up_order[u]] = u; }
+  pl.ready.assign(C, 0);
+  const std::vector<int>& nb = *b->h_nbr;
+  for (int p = 0; p < np; ++p) {
+    const int c = p / chunk;
+    int r = upos[c];
+    for (int k = 0; k < 27; ++k) {
+      const int q = nb[(size_t)p * 27 + k];
+      if (q >= 0) r = std::max(r, upos[q / chunk]);
+    }
+    pl.ready[c] = std::max(pl.ready[c], r);
+  }
+  pl.step_order.resize(C);
+  for (int c = 0; c < C; ++c) pl.step_order[c] = c;
+  std::stable_sort(pl.step_order.begin(), pl.step_order.end(), [&](int a, int c2) {
+    return pl.ready[a] != pl.ready[c2] ? pl.ready[a] < pl.ready[c2] : upos[a] < upos[c2];
+  });
+  return pl;
+}
+// Makespan of that schedule in units of "one patch across PCIe": uploads back to back, a
+// step costs `alpha` per patch, a download 1 per patch, `eps` of fixed cost per transfer.
+double hs_makespan(const mhd_bunch* b, int chunk, const HsPlan& pl, double alpha, double eps) {
+  const int np = b->G.np, C = (int)pl.up_order.size();
+  auto size = [&](int c) { return (double)std::min(chunk, np - c * chunk); };
+  std::vector<double> t_up(C);
+  double t = 0.0;
+  for (int u = 0; u < C; ++u) { t += size(pl.up_order[u]) + eps; t_up[u] = t; }
+  double t_step = 0.0, t_dn = 0.0;
+  for (int s2 = 0; s2 < C; ++s2) {
+    const int c = pl.step_order[s2];
+    t_step = std::max(t_step, t_up[pl.ready[c]]) + alpha * size(c) + eps;
+    t_dn = std::max(t_dn, t_step) + size(c) + eps;
+  }
+  return t_dn;
+}
+// default chunk: the candidate with the shortest simulated step (transfers dominate: a step
+// of a patch costs about a third of its transfer; ~30 us of fixed cost per chunk and stream)
+int hs_default_chunk(const mhd_bunch* b) {
+  const int np = b->G.np;
+  int best = np;
+  double best_t = 1e300;
+  for (int k : {1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64}) {
+    const int chunk = (np + k - 1) / k;
+    if (chunk < 1) break;
+    const double tt = hs_makespan(b, chunk, hs_plan(b, chunk), 0.3, 1.5);
+    if (tt < best_t - 1e-9) { best_t = tt; best = chunk; }
+    if (chunk == 1) break;
+  }
+  return best;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mhd_bunch_host_query(mhd_bunch* b, int32_t chunk_patches, mhd_bunch_host_layout* out) {
+  if (!b || !out) return MHD_ESTATE;
+  int chunk = chunk_patches;
+  if (chunk <= 0) chunk = hs_default_chunk(b);
+  if (chunk > b->G.np) chunk = b->G.np;
+  out->chunk_patches = chunk;
+  out->nchunk = (b->G.np + chunk - 1) / chunk;
+  out->host_bytes = (size_t)8 * b->G.np * b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
+  out->staging_bytes = 2 * hs_chunk_bytes(b, chunk);
+  out->pipelined = (b->all_nbr && b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS) ? 1 : 0;
+  return MHD_OK;
+}
+
+int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes, int32_t chunk_patches) {
+  if (!b) return MHD_ESTATE;
+  if (!staging_dev || ((uintptr_t)staging_dev & 15)) return MHD_EINVAL;
+  if (!b->all_nbr) return MHD_EINVAL;   // the compact host layout has no room for evolved closing faces
+  mhd_bunch_host_layout lay;
+  int rc = mhd_bunch_host_query(b, chunk_patches, &lay);
+  if (rc != MHD_OK) return rc;
+  if (staging_bytes < lay.staging_bytes) return MHD_ENOMEM;
+  hs_release(b);
+  mhd_bunch::HostStream* h = new (std::nothrow) mhd_bunch::HostStream;
+  if (!h) return MHD_ENOMEM;
+  h->chunk = lay.chunk_patches;
+  h->nchunk = lay.nchunk;
+  h->stage_up = (char*)staging_dev;
+  h->stage_dn = (char*)staging_dev + hs_chunk_bytes(b, h->chunk);
+  CUDA_TRY(cudaSetDevice(b->desc.device));
+  CUDA_TRY(cudaStreamCreateWithFlags(&h->s_up, cudaStreamNonBlocking));
+  CUDA_TRY(cudaStreamCreateWithFlags(&h->s_dn, cudaStreamNonBlocking));
+  CUDA_TRY(cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming));
+  CUDA_TRY(cudaEventCreateWithFlags(&h->ev_all_steps, cudaEventDisableTiming));
+  h->ev_up.resize(h->nchunk);
+  h->ev_step.resize(h->nchunk);
+  for (int c = 0; c < h->nchunk; ++c) {
+    CUDA_TRY(cudaEventCreateWithFlags(&h->ev_up[c], cudaEventDisableTiming));
+    CUDA_TRY(cudaEventCreateWithFlags(&h->ev_step[c], cudaEventDisableTiming));
+  }
+  HsPlan pl = hs_plan(b, h->chunk);
+  h->up_order = pl.up_order;
+  h->ready = pl.ready;
+  h->step_order = pl.step_order;
+  b->hs = h;
+  return MHD_OK;
+}
+
+int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant,
+                        double* dt_used, double* dt_next) {
+  if (!b) return MHD_ESTATE;
+  mhd_bunch::HostStream* h = b->hs;
+  if (!h) return MHD_ESTATE;
+  if (!host_in || !host_out) return MHD_EINVAL;
+  if (!(courant > 0.0) || !isfinite(courant) || !isfinite(dt) || dt < 0.0) return MHD_EINVAL;
+  const bool f64 = b->desc.dtype == MHD_F64;
+  const bool have_dt = dt > 0.0;
+  const bool pipelined = b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS;
+  const Geom& G = b->G;
+  const int C = h->nchunk;
+  auto range = [&](int c, int& p0, int& npl) { p0 = c * h->chunk; npl = std::min(h->chunk, G.np - p0); };
+  int rc;
+
+  // the copy streams start after whatever the caller's stream has enqueued so far
+  CUDA_TRY(cudaEventRecord(h->ev_begin, b->stream));
+  CUDA_TRY(cudaStreamWaitEvent(h->s_up, h->ev_begin, 0));
+  CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_begin, 0));
+
+  // ---- uploads: host -> staging -> interiors of the current level --------------------
+  for (int u = 0; u < C; ++u) {
+    int p0, npl;
+    range(h->up_order[u], p0, npl);
+    if ((rc = hs_copy(b, h->s_up, h->stage_up, (char*)const_cast<void*>(host_in), p0, npl, true)) != MHD_OK) return rc;
+    rc = f64 ? launch_pack<double, false>(b, h->s_up, b->state[b->cur], h->stage_up, p0, npl)
+             : launch_pack<float, false>(b, h->s_up, b->state[b->cur], h->stage_up, p0, npl);
+    if (rc != MHD_OK) return rc;
+    CUDA_TRY(cudaEventRecord(h->ev_up[u], h->s_up));
+  }
+  b->closing_ok = false;
+  b->guards_stale = false;
+
+  const bool overlap_up = pipelined && have_dt;   // steps start while later chunks still upload
+  if (!overlap_up) {
+    CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[C - 1], 0));
+    if ((rc = mhd_bunch_fill_guards(b)) != MHD_OK) return rc;    // deferred on the one-pass path: closing faces only
+    if (!have_dt) {
+      rc = f64 ? launch_cfl<double>(b, courant, nullptr, nullptr) : launch_cfl<float>(b, courant, nullptr, nullptr);
+      if (rc != MHD_OK) return rc;
+    }
+  }
+  { LaunchScope ls(b, KC_MISC);
+    k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, have_dt ? nullptr : b->d_dt, dt, 0.0); }
+
+  // ---- steps, and the way back: interiors of the new level -> staging -> host --------
+  void* const next = b->state[1 - b->cur];
+  auto download = [&](int c) -> int {
+    int p0, npl;
+    range(c, p0, npl);
+    int r2 = f64 ? launch_pack<double, true>(b, h->s_dn, next, h->stage_dn, p0, npl)
+                 : launch_pack<float, true>(b, h->s_dn, next, h->stage_dn, p0, npl);
+    if (r2 != MHD_OK) return r2;
+    return hs_copy(b, h->s_dn, h->stage_dn, (char*)host_out, p0, npl, false);
+  };
+  if (pipelined) {
+    for (int s2 = 0; s2 < C; ++s2) {
+      const int c = h->step_order[s2];
+      int p0, npl;
+      range(c, p0, npl);
+      if (overlap_up) {
+        CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[h->ready[c]], 0));
+        if ((rc = launch_sync_closing<float>(b, p0, npl)) != MHD_OK) return rc;
+      }
+      if ((rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, s2 == C - 1)) != MHD_OK) return rc;
+      CUDA_TRY(cudaEventRecord(h->ev_step[c], b->stream));
+      CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_step[c], 0));
+      if ((rc = download(c)) != MHD_OK) return rc;
+    }
+    b->guards_stale = true;   // the new level's shell is owed (deferred fill), its closing faces are current
+    b->closing_ok = true;
+  } else {
+    if ((rc = step_common(b)) != MHD_OK) return rc;
+    CUDA_TRY(cudaEventRecord(h->ev_all_steps, b->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_all_steps, 0));
+    for (int c = 0; c < C; ++c)
+      if ((rc = download(c)) != MHD_OK) return rc;
+    if ((rc = mhd_bunch_fill_guards(b)) != MHD_OK) return rc;   // cfl of the new level reads its closing faces
+  }
+
+  // ---- CFL step of the new level (overlaps the last downloads) -----------------------
+  double dts[2] = {0.0, 0.0};
+  CUDA_TRY(cudaMemcpyAsync(&dts[1], b->d_dt + 1, sizeof(double), cudaMemcpyDeviceToHost, b->stream));
+  rc = f64 ? launch_cfl<double>(b, courant, nullptr, nullptr) : launch_cfl<float>(b, courant, nullptr, nullptr);
+  if (rc != MHD_OK) return rc;
+  CUDA_TRY(cudaMemcpyAsync(&dts[0], b->d_dt, sizeof(double), cudaMemcpyDeviceToHost, b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->s_dn));
+  CUDA_TRY(cudaStreamSynchronize(h->s_up));
+  if (dt_used) *dt_used = dts[1];
+  if (dt_next) *dt_next = dts[0];
+  return MHD_OK;
+}
+
+int mhd_bunch_host_detach(mhd_bunch* b) {
+  if (!b) return MHD_ESTATE;
+  hs_release(b);
+  return MHD_OK;
+}
+
+}  // extern "C"
+
+extern "C" {
+
 int mhd_bunch_destroy(mhd_bunch* b) {
   if (!b) return MHD_ESTATE;
   cudaStreamSynchronize(b->stream);
   drain_events(b, false);
+  hs_release(b);
+  delete b->h_nbr;
   delete b->events;
   delete b;
   return MHD_OK;

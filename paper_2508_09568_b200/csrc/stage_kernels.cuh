@@ -94,13 +94,14 @@ __global__ void __launch_bounds__(256) k_fill_guards(Geom G, FillMap M, T* __res
 // This is the only part of the guard shell that cfl_dt and the one-pass kernel's update read
 // from HBM, so it is all a deferred fill has to do up front.
 template <typename T>
-__global__ void __launch_bounds__(256) k_sync_closing_faces(Geom G, T* __restrict__ U, const int* __restrict__ nbr) {
+__global__ void __launch_bounds__(256) k_sync_closing_faces(Geom G, T* __restrict__ U, const int* __restrict__ nbr,
+                                                            int p0, int npl) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int fx = G.n[1] * G.n[2], fy = G.n[0] * G.n[2], fz = G.n[0] * G.n[1];
   const int per = fx + fy + fz;
-  if (t >= (long long)per * G.np) return;
-  const int p = (int)(t / per);
-  int r = (int)(t - (long long)p * per);
+  if (t >= (long long)per * npl) return;
+  const int p = p0 + (int)(t / per);
+  int r = (int)(t % per);
   int a, c[3];
   if (r < fx) { a = 0; c[0] = G.n[0]; c[1] = r % G.n[1]; c[2] = r / G.n[1]; }
   else if (r < fx + fy) { r -= fx; a = 1; c[0] = r % G.n[0]; c[1] = G.n[1]; c[2] = r / G.n[0]; }

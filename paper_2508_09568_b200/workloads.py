@@ -96,6 +96,22 @@ def gather(U, n, P, ng=NG):
     return out
 
 
+def to_compact(U, n, ng=NG):
+    """Dense bunch array [8, npatch, mz, my, mx] -> compact host layout [8, npatch, nz, ny, nx]
+    (interior cells only; include/mhd_bunch.h, host-streaming path)."""
+    g = [ng if k > 1 else 0 for k in n]
+    return np.ascontiguousarray(U[:, :, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]])
+
+
+def from_compact(Uc, n, ng=NG):
+    """Compact host layout -> dense bunch array with every guard cell zero."""
+    mx, my, mz = padded(n, ng)
+    g = [ng if k > 1 else 0 for k in n]
+    U = np.zeros(Uc.shape[:2] + (mz, my, mx), dtype=Uc.dtype)
+    U[:, :, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]] = Uc
+    return U
+
+
 def conserved_from_primitive(rho, vel, p, bfaces, gamma):
     """Definition of the initial state (EOS): returns cons5 [5,Nz,Ny,Nx].
     Cell-centred B is the mean of the two faces (reading O2/Q5)."""
