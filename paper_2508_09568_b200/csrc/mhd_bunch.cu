@@ -282,26 +282,34 @@ template <typename T> struct OnePassLaunch {
   static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true) { return MHD_EINVAL; }
 };
 template <> struct OnePassLaunch<float> {
-  // patches [p0, p0+npl) of the bunch (npl < 0: all); `last` flips the buffers
-  static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true) {
-    using Cfg = OneCfg<float, OneTile::TX, OneTile::TY, OneTile::NPW>;
+  // one tile shape: patches [p0, p0+npl) of the bunch
+  template <int TX, int TY>
+  static int launch(mhd_bunch* b, const double* dtp, int p0, int npl) {
+    using Cfg = OneCfg<float, TX, TY, OneTile::NPW>;
     const Geom& G = b->G;
-    auto kern = G.limiter == 1 ? k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW, 1>
-                               : k_step_onepass<float, OneTile::TX, OneTile::TY, OneTile::NPW, 2>;
+    auto kern = G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1>
+                               : k_step_onepass<float, TX, TY, OneTile::NPW, 2>;
     static bool attr_done[3] = {false, false, false};
     if (!attr_done[G.limiter]) {
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       attr_done[G.limiter] = true;
     }
-    if (npl < 0) npl = G.np;
     Params<float> P = make_params<float>(b, p0, npl);
-    const int xt = (G.n[0] + OneTile::TX - 1) / OneTile::TX, yt = (G.n[1] + OneTile::TY - 1) / OneTile::TY;
+    const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
     dim3 grid((unsigned)(xt * yt), (unsigned)npl);
     {
       LaunchScope ls(b, KC_ONEPASS);
       kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt);
     }
     CUDA_TRY(cudaGetLastError());
+    return MHD_OK;
+  }
+  // patches [p0, p0+npl) of the bunch (npl < 0: all); `last` flips the buffers.  Rows of up to
+  // 16 cells take the 16 x 16 tile (a 32-wide tile would leave half of every warp idle).
+  static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true) {
+    if (npl < 0) npl = b->G.np;
+    const int rc = b->G.n[0] <= 16 ? launch<16, 16>(b, dtp, p0, npl) : launch<OneTile::TX, OneTile::TY>(b, dtp, p0, npl);
+    if (rc != MHD_OK) return rc;
     if (last) {
       b->cur = 1 - b->cur;
       b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
