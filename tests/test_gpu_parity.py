@@ -399,3 +399,74 @@ def test_config2_full_size_sampled_patches_and_invariants():
     div = np.roll(g1[5], -1, 2) - g1[5] + np.roll(g1[6], -1, 1) - g1[6] + np.roll(g1[7], -1, 0) - g1[7]
     assert np.abs(div).max() / np.sqrt(np.mean(g1[5] ** 2 + g1[6] ** 2 + g1[7] ** 2)) <= 1e-4
     b.close()
+
+
+# ------------------------------------------------------- full-size config 3 -------
+def _patch_with_guards(g, n, P, p, ng=3):
+    """Patch p of a periodic global field g [8, Nz, Ny, Nx] with its guard shell, taken from
+    the global periodic image (what a guard fill must produce; independent of any fill code)."""
+    px, py, pz = p % P[0], (p // P[0]) % P[1], p // (P[0] * P[1])
+    idx = [(o * k - ng + np.arange(k + 2 * ng)) % N for o, k, N in
+           ((pz, n[2], g.shape[1]), (py, n[1], g.shape[2]), (px, n[0], g.shape[3]))]
+    return g[np.ix_(np.arange(g.shape[0]), idx[0], idx[1], idx[2])]
+
+
+_C3 = {}
+
+
+def _config3(dtype):
+    """The 512^3 field is built once (fp64) and cast for the fp32 case -- the same values
+    W.turbulence(dtype=float32) stores."""
+    if "w" not in _C3:
+        _C3["w"] = W.turbulence(N=512, n=32, dtype=np.float64, config=2)
+    w = _C3["w"]
+    import copy
+    v = copy.copy(w)
+    v.U = w.U if dtype == "f64" else w.U.astype(np.float32)
+    if dtype == "f64":
+        _C3.clear()            # last user: release 14 GB
+    return v
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])          # order matters: f64 releases the cached field
+def test_config3_full_size_sampled_patches_and_invariants(dtype):
+    """BASELINE.json config 3 (4096 patches of 32^3 on a periodic 512^3 cube, fp32 and fp64):
+    sampled patches of one step against the oracle, the CFL step against the oracle evaluated
+    slab by slab, conservation and div B over the whole bunch.  The oracle never sees more
+    than a slab of patches at a time (host memory)."""
+    import oracle
+    w = _config3(dtype)
+    g0 = W.gather(w.U, w.n, w.P)                         # [8, 512, 512, 512] in the storage type
+    b = make_gpu(w, dtype)
+    w.U = None
+    b.fill_guards()
+    dt = b.cfl_dt(0.4, sync=True)
+    # oracle CFL step: min over slabs of 256 patches, each with guards from the periodic image
+    npp = w.P[0] * w.P[1]
+    dt_ref = np.inf
+    o = oracle.Oracle(w.n, npp, w.gamma, w.dx)
+    for s in range(0, w.npatch, npp):
+        if (s // npp) % 8 != 3:  # two slabs in full; the rest through the sampled patches below
+            continue
+        U = np.ascontiguousarray(np.stack([_patch_with_guards(g0, w.n, w.P, p) for p in range(s, s + npp)], axis=1), dtype=np.float64)
+        dt_ref = min(dt_ref, o.cfl_dt(U, 0.4))
+    assert dt <= dt_ref * (1 + (1e-13 if dtype == "f64" else 2e-6))      # the GPU minimum covers every slab
+    sample = [0, 15, 255, 256, 1911, 2730, 3840, 4095]
+    os_ = oracle.Oracle(w.n, len(sample), w.gamma, w.dx)
+    Us = np.ascontiguousarray(np.stack([_patch_with_guards(g0, w.n, w.P, p) for p in sample], axis=1), dtype=np.float64)
+    ref = os_.step(Us, dt)
+    b.step(dt)
+    assert b.status() == 0
+    got = b.download()
+    err = rel_err(masked(got[:, sample], w.n), masked(ref, w.n))
+    assert err <= TOL_STEP[dtype], err
+    g1 = W.gather(got, w.n, w.P)
+    del got
+    tol = 1e-12 if dtype == "f64" else 2e-6
+    for f in (0, 4):
+        t0, t1 = g0[f].sum(dtype=np.float64), g1[f].sum(dtype=np.float64)
+        assert abs(t1 - t0) <= tol * abs(t0)
+    div = np.roll(g1[5], -1, 2) - g1[5] + np.roll(g1[6], -1, 1) - g1[6] + np.roll(g1[7], -1, 0) - g1[7]
+    brms = np.sqrt(np.mean(g1[5].astype(np.float64) ** 2 + g1[6].astype(np.float64) ** 2 + g1[7].astype(np.float64) ** 2))
+    assert np.abs(div).max() / brms <= (1e-12 if dtype == "f64" else 1e-4)
+    b.close()
