@@ -403,6 +403,23 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       Flux5<T> cFz = {};
       T cex = T(0), cey = T(0);
       if (doFz) cFz = hlld_flux(gamma, Lz, face_state<T, DC, 2>(dc_, -h), dc_[(D_BH + 2) * DC]);
+      // The hydro part of plane k-1 only waits for this flux: finish it now (C is ahead, its
+      // partial update is normally there already), so that the previous plane's flux is dead
+      // while the two edge problems are solved.
+      const long long cu = ubase + (long long)(k - 1) * plane;
+      const T* pu = PU + fidx;
+      if (k >= 1) {
+        nb_sync(NB_PUF, 2 * NR);
+        if (cell) {
+          // O8: (U - dt*dFx/dx - dt*dFy/dy) - dt*dFz/dz; z-face frame (mu,mv,mw) = (mz,mx,my)
+          P.Un[cu] = pu[0] - cz * (cFz.d - pFz.d);
+          P.Un[fs + cu] = pu[FA] - cz * (cFz.mv - pFz.mv);
+          P.Un[2 * fs + cu] = pu[2 * FA] - cz * (cFz.mw - pFz.mw);
+          P.Un[3 * fs + cu] = pu[3 * FA] - cz * (cFz.mu - pFz.mu);
+          P.Un[4 * fs + cu] = pu[4 * FA] - cz * (cFz.e - pFz.e);
+        }
+      }
+      pFz = cFz;
       if (doEx)
         cex = emf_2d(gamma, solver, xsw, xse, corner_state<T, DC, 0>(dc_ - DW, h, -h), corner_state<T, DC, 0>(dc_, -h, -h),
                      xAS, edge_field<T, DC, 1, 2>(dc_, -h), edge_field<T, DC, 2, 1>(dc_ - DW, h), edge_field<T, DC, 2, 1>(dc_, -h));
@@ -417,22 +434,11 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       // b_z on the lower z-face of plane k (k = nz: closing face) -- Eq. 12
       if (cell) P.Un[7 * fs + ubase + (long long)k * plane] = u7 + (cx * (xey - cey) - cy * (yex - cex));
       if (k >= 1) {
-        nb_sync(NB_PUF, 2 * NR);
-        const long long cu = ubase + (long long)(k - 1) * plane;
-        const T* pu = PU + fidx;
-        if (cell) {
-          // O8: (U - dt*dFx/dx - dt*dFy/dy) - dt*dFz/dz; z-face frame (mu,mv,mw) = (mz,mx,my)
-          P.Un[cu] = pu[0] - cz * (cFz.d - pFz.d);
-          P.Un[fs + cu] = pu[FA] - cz * (cFz.mv - pFz.mv);
-          P.Un[2 * fs + cu] = pu[2 * FA] - cz * (cFz.mw - pFz.mw);
-          P.Un[3 * fs + cu] = pu[3 * FA] - cz * (cFz.mu - pFz.mu);
-          P.Un[4 * fs + cu] = pu[4 * FA] - cz * (cFz.e - pFz.e);
-        }
         if (xface) P.Un[5 * fs + cu] = pu[5 * FA] - cz * (cey - pey);
         if (yface) P.Un[6 * fs + cu] = pu[6 * FA] + cz * (cex - pex);
         if (k <= nz - 1) nb_arrive(NB_PUE, 2 * NR);
       }
-      pFz = cFz; pex = cex; pey = cey;
+      pex = cex; pey = cey;
     }
     return;
   }
