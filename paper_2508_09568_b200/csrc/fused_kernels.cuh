@@ -124,7 +124,8 @@ __host__ __device__ constexpr int predict_max_threads(int ty) { return ty == 8 ?
 
 template <typename T, int TY>
 __global__ void __launch_bounds__(predict_max_threads(TY), (TY == 8 && sizeof(T) == 4) ? 2 : 1)
-k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad) {
+k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad,
+                const int* __restrict__ nbr, int gather) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
@@ -146,6 +147,20 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1], fs = G.fs;
   const long long cbase = (long long)(P.p0 + pl) * G.ps + G.lead + (i + G.g[0]) + (long long)(j + G.g[1]) * pitch +
                           (long long)G.g[2] * plane;
+  // GATHER mode (guard fill O1 folded into the loads, as in the one-pass kernel): a position
+  // outside the patch reads the image cell of the neighbour of class (ox,oy,oz) through the
+  // neighbour table, so the guard shell in HBM is neither written nor read.  The column of a
+  // thread crosses at most three patches along z: one base each.
+  long long cb0 = cbase, cbm = cbase, cbp = cbase;
+  if (gather && rowok) {
+    const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0), oy = j < 0 ? -1 : (j >= ny ? 1 : 0);
+    const long long inner = G.lead + (i - ox * nx + G.g[0]) + (long long)(j - oy * ny + G.g[1]) * pitch + (long long)G.g[2] * plane;
+    const int* tb = nbr + (long long)(P.p0 + pl) * 27 + (oy + 1) * 3 + (ox + 1);
+    cbm = (long long)tb[0] * G.ps + inner + (long long)nz * plane;
+    cb0 = (long long)tb[9] * G.ps + inner;
+    cbp = (long long)tb[18] * G.ps + inner - (long long)nz * plane;
+  }
+  auto at = [&](int rr) { return (rr < 0 ? cbm : (rr >= nz ? cbp : cb0)) + (long long)rr * plane; };
   const T h = T(0.5), q4 = T(0.25);
   const T dt = (T)(*dtp), hdt = h * dt;
   const T lx = hdt * P.idx[0], ly = hdt * P.idx[1], lz = hdt * P.idx[2];
@@ -174,23 +189,25 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   for (int f = 0; f < 8; ++f) { Ucur[f] = T(0); Uprev[f] = T(0); }
   const int rlo = -2, rhi = nz + 2;
   if (rowok) {
-    bxn = P.U[5 * fs + cbase + (long long)rlo * plane];
-    byn = P.U[6 * fs + cbase + (long long)rlo * plane];
-    bzn1 = P.U[7 * fs + cbase + (long long)rlo * plane];
-    bzn2 = P.U[7 * fs + cbase + (long long)(rlo + 1) * plane];
+    bxn = P.U[5 * fs + at(rlo)];
+    byn = P.U[6 * fs + at(rlo)];
+    bzn1 = P.U[7 * fs + at(rlo)];
+    bzn2 = P.U[7 * fs + at(rlo + 1)];
   }
   unsigned int nbad = 0;
 
   for (int r = rlo; r <= rhi; ++r) {
     Ucur[5] = bxn; Ucur[6] = byn; Ucur[7] = bzn1; bzn1 = bzn2;
     if (rowok) {
+      const long long cr = at(r);
 #pragma unroll
-      for (int f = 0; f < 5; ++f) Ucur[f] = P.U[f * fs + cbase + (long long)r * plane];
+      for (int f = 0; f < 5; ++f) Ucur[f] = P.U[f * fs + cr];
       if (r + 1 <= rhi) {
-        bxn = P.U[5 * fs + cbase + (long long)(r + 1) * plane];
-        byn = P.U[6 * fs + cbase + (long long)(r + 1) * plane];
+        const long long c1 = at(r + 1);
+        bxn = P.U[5 * fs + c1];
+        byn = P.U[6 * fs + c1];
       }
-      if (r + 2 <= rhi) bzn2 = P.U[7 * fs + cbase + (long long)(r + 2) * plane];
+      if (r + 2 <= rhi) bzn2 = P.U[7 * fs + at(r + 2)];
     }
 
     // ---- primitives of plane r-1 (O2): needs bx(i+1), by(j+1) of plane r-1 and bz of plane r

@@ -66,6 +66,7 @@ struct mhd_bunch {
   bool onepass_ok;     // three active dimensions, fp32
   bool gather_ok;      // the one-pass kernel can read halos from the neighbours' interiors: every
                        // neighbour exists (no outflow side) and n_x is a whole number of 16-byte chunks
+  bool gather2_ok;     // the two-kernel path can do the same (predictor loads through the neighbour table)
   bool guards_stale;   // fill_guards was deferred: the guard shell of the current level is not in HBM
   bool closing_ok;     // every closing face of the current level equals the neighbour's face 0: true after
                        // any fill and kept by steps (both sides evaluate the same update on the same
@@ -278,6 +279,13 @@ int effective_path(const mhd_bunch* b) {
   return b->fused_ok ? MHD_PATH_TWO_KERNEL : MHD_PATH_STAGED;
 }
 
+// true if the step that would run gathers its halos from the neighbours' interiors, so that the
+// guard shell need not exist in HBM (deferred fill)
+bool step_gathers(const mhd_bunch* b) {
+  const int path = effective_path(b);
+  return (path == MHD_PATH_ONEPASS && b->gather_ok) || (path == MHD_PATH_TWO_KERNEL && b->gather2_ok);
+}
+
 template <typename T> struct OnePassLaunch {
   static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true) { return MHD_EINVAL; }
 };
@@ -318,54 +326,77 @@ template <> struct OnePassLaunch<float> {
   }
 };
 
+// two-kernel path on patches [q0, q0+nq): sub-bunches of at most b->chunk patches (D block)
+template <typename T>
+int launch_fused_range(mhd_bunch* b, int q0, int nq) {
+  const Geom& G = b->G;
+  const double* dtp = b->d_dt + 1;
+  static bool attr_done[2] = {false, false};
+  if (!attr_done[sizeof(T) == 8]) {
+    CUDA_TRY(cudaFuncSetAttribute(k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>::smem));
+    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr_done[sizeof(T) == 8] = true;
+  }
+  const int gather = (b->gather2_ok && b->guards_stale) ? 1 : 0;   // shell not in HBM: read through the table
+  cudaStream_t st = b->stream;
+  for (int p0 = q0; p0 < q0 + nq; p0 += b->chunk) {
+    const int npl = (q0 + nq - p0 < b->chunk) ? q0 + nq - p0 : b->chunk;
+    Params<T> P = make_params<T>(b, p0, npl);
+    const int ty = b->pred_ty;
+    const int pa = (G.n[0] + 5) * (ty + 5);
+    const size_t sm = (size_t)39 * pa * sizeof(T);
+    dim3 grid((unsigned)((G.n[1] + ty - 1) / ty), (unsigned)npl);
+    const unsigned nth = (unsigned)((pa + 31) / 32 * 32);
+    {
+      LaunchScope ls(b, KC_PREDICT);
+      if (ty == 16) k_predict_fused<T, 16><<<grid, nth, sm, st>>>(P, dtp, b->d_bad, b->d_nbr, gather);
+      else if (ty == 8) k_predict_fused<T, 8><<<grid, nth, sm, st>>>(P, dtp, b->d_bad, b->d_nbr, gather);
+      else k_predict_fused<T, 4><<<grid, nth, sm, st>>>(P, dtp, b->d_bad, b->d_nbr, gather);
+    }
+    using Cfg = FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>;
+    const int xt = (G.n[0] + FusedTile<T>::TX - 1) / FusedTile<T>::TX, yt = (G.n[1] + FusedTile<T>::TY - 1) / FusedTile<T>::TY;
+    dim3 grid2((unsigned)(xt * yt), (unsigned)npl);
+    LaunchScope ls(b, KC_RIEMANN);
+    k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY><<<grid2, Cfg::NTH, Cfg::smem, st>>>(P, b->tmap_d, dtp, xt);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
+
 template <typename T>
 int launch_step(mhd_bunch* b) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
   const int path = effective_path(b);
   if (path == MHD_PATH_ONEPASS && b->gather_ok) return OnePassLaunch<T>::run(b, dtp);
+  if (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) {
+    // halos come through the neighbour table if the fill was deferred, from the shell otherwise
+    const int rc = launch_fused_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
+    b->cur = 1 - b->cur;
+    b->guards_stale = false;
+    return MHD_OK;
+  }
   {  // every other route reads the guard shell from HBM
     const int rc = materialise_guards(b);
     if (rc != MHD_OK) return rc;
   }
   if (path == MHD_PATH_ONEPASS) return OnePassLaunch<T>::run(b, dtp);
-  const bool fused = path == MHD_PATH_TWO_KERNEL;
-  if (fused) {
-    static bool attr_done[2] = {false, false};
-    if (!attr_done[sizeof(T) == 8]) {
-      CUDA_TRY(cudaFuncSetAttribute(k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY>,
-                                    cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>::smem));
-      CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-      CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-      CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-      attr_done[sizeof(T) == 8] = true;
-    }
+  if (path == MHD_PATH_TWO_KERNEL) {
+    const int rc = launch_fused_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
+    b->cur = 1 - b->cur;
+    return MHD_OK;
   }
-  const int ch = fused ? b->chunk : b->chunk_s;
+  const int ch = b->chunk_s;
   for (int p0 = 0; p0 < G.np; p0 += ch) {
     const int npl = (G.np - p0 < ch) ? G.np - p0 : ch;
     Params<T> P = make_params<T>(b, p0, npl);
     cudaStream_t st = b->stream;
-    if (fused) {
-      const int ty = b->pred_ty;
-      const int pa = (G.n[0] + 5) * (ty + 5);
-      const size_t sm = (size_t)39 * pa * sizeof(T);
-      dim3 grid((unsigned)((G.n[1] + ty - 1) / ty), (unsigned)npl);
-      const unsigned nth = (unsigned)((pa + 31) / 32 * 32);
-      {
-        LaunchScope ls(b, KC_PREDICT);
-        if (ty == 16) k_predict_fused<T, 16><<<grid, nth, sm, st>>>(P, dtp, b->d_bad);
-        else if (ty == 8) k_predict_fused<T, 8><<<grid, nth, sm, st>>>(P, dtp, b->d_bad);
-        else k_predict_fused<T, 4><<<grid, nth, sm, st>>>(P, dtp, b->d_bad);
-      }
-      using Cfg = FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>;
-      const int xt = (G.n[0] + FusedTile<T>::TX - 1) / FusedTile<T>::TX, yt = (G.n[1] + FusedTile<T>::TY - 1) / FusedTile<T>::TY;
-      dim3 grid2((unsigned)(xt * yt), (unsigned)npl);
-      LaunchScope ls(b, KC_RIEMANN);
-      k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY><<<grid2, Cfg::NTH, Cfg::smem, st>>>(P, b->tmap_d, dtp, xt);
-      continue;
-    }
     {
       Box B = make_box(G, 2, 2);
       LaunchScope ls(b, KC_PRIM);
@@ -546,6 +577,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   for (long long c = 0; c < 27ll * desc->npatch && b->all_nbr; ++c)
     if (nbr[c] < 0) b->all_nbr = false;
   b->gather_ok = b->gather_ok && b->all_nbr;
+  b->gather2_ok = b->fused_ok && b->all_nbr;
   b->hs = nullptr;
   b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
   if (!b->h_nbr) { delete b->events; delete b; return MHD_ENOMEM; }
@@ -561,7 +593,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
 
 int mhd_bunch_fill_guards(mhd_bunch* b) {
   if (!b) return MHD_ESTATE;
-  if (b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS) {
+  if (step_gathers(b)) {
     // deferred: the one-pass step reads halos from the neighbours' interiors, so only the
     // closing faces are brought up to date now; the rest of the shell is written if and when
     // something reads it from HBM (materialise_guards)
@@ -874,7 +906,7 @@ int mhd_bunch_host_query(mhd_bunch* b, int32_t chunk_patches, mhd_bunch_host_lay
   out->nchunk = (b->G.np + chunk - 1) / chunk;
   out->host_bytes = (size_t)8 * b->G.np * b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
   out->staging_bytes = 2 * hs_chunk_bytes(b, chunk);
-  out->pipelined = (b->all_nbr && b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS) ? 1 : 0;
+  out->pipelined = (b->all_nbr && step_gathers(b)) ? 1 : 0;
   return MHD_OK;
 }
 
@@ -921,7 +953,8 @@ int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, doubl
   if (!(courant > 0.0) || !isfinite(courant) || !isfinite(dt) || dt < 0.0) return MHD_EINVAL;
   const bool f64 = b->desc.dtype == MHD_F64;
   const bool have_dt = dt > 0.0;
-  const bool pipelined = b->gather_ok && effective_path(b) == MHD_PATH_ONEPASS;
+  const bool pipelined = step_gathers(b);
+  const bool onepass = effective_path(b) == MHD_PATH_ONEPASS;
   const Geom& G = b->G;
   const int C = h->nchunk;
   auto range = [&](int c, int& p0, int& npl) { p0 = c * h->chunk; npl = std::min(h->chunk, G.np - p0); };
@@ -974,13 +1007,18 @@ int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, doubl
       range(c, p0, npl);
       if (overlap_up) {
         CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[h->ready[c]], 0));
-        if ((rc = launch_sync_closing<float>(b, p0, npl)) != MHD_OK) return rc;
+        rc = f64 ? launch_sync_closing<double>(b, p0, npl) : launch_sync_closing<float>(b, p0, npl);
+        if (rc != MHD_OK) return rc;
+        b->guards_stale = true;    // halos of this chunk come through the neighbour table
       }
-      if ((rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, s2 == C - 1)) != MHD_OK) return rc;
+      if (onepass) rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, false);
+      else rc = f64 ? launch_fused_range<double>(b, p0, npl) : launch_fused_range<float>(b, p0, npl);
+      if (rc != MHD_OK) return rc;
       CUDA_TRY(cudaEventRecord(h->ev_step[c], b->stream));
       CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_step[c], 0));
       if ((rc = download(c)) != MHD_OK) return rc;
     }
+    b->cur = 1 - b->cur;
     b->guards_stale = true;   // the new level's shell is owed (deferred fill), its closing faces are current
     b->closing_ok = true;
   } else {

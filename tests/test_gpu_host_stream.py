@@ -39,6 +39,24 @@ def oracle_step(w, dt=None, courant=0.4):
     return dt_ref, new, o.cfl_dt(new_f, courant)
 
 
+@pytest.mark.parametrize("path", ["two_kernel", "staged"])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_step_host_on_the_other_step_paths(dtype, path):
+    """fp32 3D bunches default to the one-pass kernel; the same call through the two-kernel path
+    (overlapped schedule, predictor gathers halos) and the staged path (whole-bunch step)."""
+    import torch
+    w = workloads(dtype)["turb_slabs"]
+    dt_ref, ref, dt_next_ref = oracle_step(w)
+    b = make_gpu(w, dtype, path=path)
+    b.host_attach(2)
+    hin = pinned(W.to_compact(w.U, w.n))
+    hout = torch.zeros_like(hin).pin_memory()
+    used, nxt = b.step_host(hin, hout, dt=dt_ref, courant=0.4)
+    assert rel_err(hout.numpy().astype(np.float64), W.to_compact(ref, w.n)) <= TOL_STEP[dtype]
+    assert abs(nxt - dt_next_ref) <= 10 * TOL_STEP[dtype] * dt_next_ref
+    b.close()
+
+
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("chunk", [1, 3, 0])
 @pytest.mark.parametrize("given_dt", [True, False])
@@ -104,8 +122,11 @@ def test_host_stream_schedule_and_rejections():
     b = make_gpu(w, "f32")
     lay = b.host_attach(1)
     assert (lay.chunk_patches, lay.nchunk, lay.pipelined) == (1, 8, 1)
-    b.set_path("two_kernel")
     lay2 = HostLayout()
+    b.set_path("two_kernel")            # its predictor gathers halos too: same overlapped schedule
+    _check(b.lib.mhd_bunch_host_query(b.h, 3, C.byref(lay2)), "q")
+    assert (lay2.chunk_patches, lay2.nchunk, lay2.pipelined) == (3, 3, 1)
+    b.set_path("staged")                # reads the guard shell from HBM: whole-bunch step between the copies
     _check(b.lib.mhd_bunch_host_query(b.h, 3, C.byref(lay2)), "q")
     assert (lay2.chunk_patches, lay2.nchunk, lay2.pipelined) == (3, 3, 0)
     b.close()

@@ -100,6 +100,34 @@ def test_deferred_fill_is_indistinguishable_from_an_immediate_one(name):
     assert deferred, "periodic fp32 3D bunches with n_x % 4 == 0 are expected to take the deferred route"
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["turb16", "turb_ragged", "turb_self"])
+def test_two_kernel_path_defers_the_fill_too(name, dtype):
+    """The two-kernel path (the fp64 default) reads halos through the neighbour table in its
+    predictor when every neighbour exists: three steps with the fill deferred equal, bit for bit,
+    three steps with the guard shell written first, and the shell a caller then sees equals the
+    oracle's fill of the result."""
+    w = small_workloads(dtype)[name]
+    outs, launches = [], []
+    for force in (False, True):
+        b = make_gpu(w, dtype, path="two_kernel")
+        l0 = b.launches
+        for _ in range(3):
+            b.fill_guards()
+            if force:
+                b.sync_guards()
+            b.cfl_dt(0.4, sync=False)
+            b.step_dev()
+        launches.append(b.launches - l0)
+        b.fill_guards()
+        outs.append(b.download())
+        b.close()
+    assert np.array_equal(outs[0], outs[1])
+    assert launches[0] < launches[1]                      # no fill kernel inside the deferred loop
+    ref = make_oracle(w).fill_guards(outs[0].astype(np.float64).copy(), w.nbr)
+    assert np.array_equal(outs[0].astype(np.float64), ref)
+
+
 # ------------------------------------------------------------------------ CFL -------
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-13), ("f32", 2e-6)])
 @pytest.mark.parametrize("name", ["sod_x", "tube_z", "ot_ragged", "turb_ragged"])
