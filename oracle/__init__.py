@@ -24,7 +24,7 @@ STAGE_SLICES = {
 
 class _Desc(C.Structure):
     _fields_ = [("n", C.c_int32 * 3), ("ng", C.c_int32), ("npatch", C.c_int32),
-                ("limiter", C.c_int32), ("emf_solver", C.c_int32), ("pad_", C.c_int32),
+                ("limiter", C.c_int32), ("emf_solver", C.c_int32), ("flux_solver", C.c_int32),
                 ("gamma", C.c_double), ("dx", C.c_double * 3)]
 
 
@@ -54,6 +54,8 @@ def _lib(key):
         lib.orc_limiter.argtypes = [C.c_int32, real, real]
         lib.orc_hlld.restype = None
         lib.orc_hlld.argtypes = [C.c_double, rp, rp, real, rp]
+        lib.orc_hll.restype = None
+        lib.orc_hll.argtypes = [C.c_double, rp, rp, real, rp]
         lib.orc_emf2d.restype = real
         lib.orc_emf2d.argtypes = [C.c_double, C.c_int32, rp, real, real, real, real]
         lib.orc_fast_speed.restype = real
@@ -67,13 +69,13 @@ def _ptr(a):
 
 
 class Oracle:
-    def __init__(self, n, npatch, gamma, dx, ng=3, limiter=1, emf_solver=0, dtype="f64"):
+    def __init__(self, n, npatch, gamma, dx, ng=3, limiter=1, emf_solver=0, dtype="f64", flux_solver=0):
         self.key = dtype
         self.np_dtype = np.float64 if dtype == "f64" else np.float32
         self.lib = _lib(dtype)
         d = _Desc()
         d.n[:] = list(n)
-        d.ng, d.npatch, d.limiter, d.emf_solver = ng, npatch, limiter, emf_solver
+        d.ng, d.npatch, d.limiter, d.emf_solver, d.flux_solver = ng, npatch, limiter, emf_solver, flux_solver
         d.gamma = gamma
         d.dx[:] = list(dx)
         self.desc = d
@@ -130,6 +132,15 @@ def hlld(gamma, L, R, bn, dtype="f64"):
     L = np.ascontiguousarray(L, dtype=t); R = np.ascontiguousarray(R, dtype=t)
     F = np.zeros(7, dtype=t)
     _lib(dtype).orc_hlld(gamma, _ptr(L), _ptr(R), float(bn), _ptr(F))
+    return F
+
+
+def hll(gamma, L, R, bn, dtype="f64"):
+    """HLL flux (PAPER.md 2.1.1); same arguments and layout as hlld."""
+    t = np.float64 if dtype == "f64" else np.float32
+    L = np.ascontiguousarray(L, dtype=t); R = np.ascontiguousarray(R, dtype=t)
+    F = np.zeros(7, dtype=t)
+    _lib(dtype).orc_hll(gamma, _ptr(L), _ptr(R), float(bn), _ptr(F))
     return F
 
 

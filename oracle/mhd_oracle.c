@@ -34,7 +34,7 @@ typedef struct {
   long M;    /* cells per patch, guards included */
   int np;
   real gamma, dx[3];
-  int limiter, emf_solver;
+  int limiter, emf_solver, flux_solver;
 } geom;
 
 static void mkgeom(const orc_desc *d, geom *G) {
@@ -53,6 +53,7 @@ static void mkgeom(const orc_desc *d, geom *G) {
   G->gamma = (real)d->gamma;
   G->limiter = d->limiter;
   G->emf_solver = d->emf_solver;
+  G->flux_solver = d->flux_solver;
 }
 
 /* index of the cell with interior-relative coordinates (i,j,k) */
@@ -247,6 +248,31 @@ void orc_hlld(double gamma_, const real L[7], const real R[7], real bn, real F[7
     else if (SsR >= ZERO) F[f] = FsR + SsR * (UssR[f] - UsR[f]);
     else if (SR >= ZERO)  F[f] = FsR;
     else                  F[f] = FR[f];
+  }
+}
+
+/* HLL (section 2.1.1; Harten, Lax & van Leer 1983): three regions, the
+ * star state is the integral average of the solution between the two outer waves,
+ *     U* = (SR UR - SL UL - (FR - FL)) / (SR - SL),
+ * and the flux through x = 0 follows from the jump condition across either outer wave,
+ *     F* = FL + SL (U* - UL)   [ = FR + SR (U* - UR) ].
+ * Outer speeds as in O6.  Same argument and flux layout as orc_hlld.                    */
+void orc_hll(double gamma_, const real L[7], const real R[7], real bn, real F[7]) {
+  real gamma = (real)gamma_;
+  real UL[7], UR[7], FL[7], FR[7], pTL, pTR;
+  phys_flux(gamma, L, bn, UL, FL, &pTL);
+  phys_flux(gamma, R, bn, UR, FR, &pTR);
+  real cfL = orc_fast_speed(gamma_, L[0], L[4], bn, L[5], L[6]);
+  real cfR = orc_fast_speed(gamma_, R[0], R[4], bn, R[5], R[6]);
+  real cmax = rmax(cfL, cfR);
+  real SL = rmin(L[1], R[1]) - cmax;
+  real SR = rmax(L[1], R[1]) + cmax;
+  for (int f = 0; f < 7; ++f) {
+    if (SL > ZERO) F[f] = FL[f];
+    else if (SR >= ZERO) {
+      real Us = (SR * UR[f] - SL * UL[f] - (FR[f] - FL[f])) / (SR - SL);
+      F[f] = FL[f] + SL * (Us - UL[f]);
+    } else F[f] = FR[f];
   }
 }
 
@@ -510,7 +536,8 @@ static void run_stages(const geom *G, const real *const Up[8], real dt, scratch 
         L[f] = S->qh[comp[f]][cl] + HALF * S->dq[d][comp[f]][cl];
         R[f] = S->qh[comp[f]][c] - HALF * S->dq[d][comp[f]][c];
       }
-      orc_hlld((double)G->gamma, L, R, S->bh[d][c], F);
+      if (G->flux_solver == 1) orc_hll((double)G->gamma, L, R, S->bh[d][c], F);
+      else orc_hlld((double)G->gamma, L, R, S->bh[d][c], F);
       S->flux[d][0][c] = F[0];
       S->flux[d][1 + d][c] = F[1];
       S->flux[d][1 + t1][c] = F[2];

@@ -34,7 +34,7 @@ typedef struct {
   int32_t npatch;     /* bunch size                                      */
   int32_t limiter;    /* 1 = minmod, 2 = monotonised central                             */
   int32_t emf_solver; /* 0 = HLLD-2D, 1 = HLL-2D                                         */
-  int32_t pad_;
+  int32_t flux_solver;/* 0 = HLLD (PAPER.md 2.1.2), 1 = HLL (PAPER.md 2.1.1)            */
   double gamma;       /* adiabatic index                                  */
   double dx[3];       /* cell sizes                                                      */
 } orc_desc;
@@ -66,6 +66,7 @@ void orc_stages(const orc_desc *d, const real *U, int32_t patch, double dt, real
 /* pointwise pieces, exported for the pins */
 real orc_limiter(int32_t kind, real a, real b);                               /* O3 */
 void orc_hlld(double gamma, const real L[7], const real R[7], real bn, real F[7]); /* O6 */
+void orc_hll(double gamma, const real L[7], const real R[7], real bn, real F[7]);  /* PAPER.md 2.1.1 */
 /* O7: corner c = 0:SW 1:SE 2:NW 3:NE, each (rho, ua, ub, ue, p, Be);
  *     A = in-plane field along a (south, north), B = in-plane field along b (west, east) */
 real orc_emf2d(double gamma, int32_t solver, const real c[4][6],

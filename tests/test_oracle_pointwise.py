@@ -415,3 +415,93 @@ def test_emf2d_hlld_and_hll_agree_for_weak_field_smooth_data():
         e0 = oracle.emf2d(G, 0, c, A + d[0], A + d[1], B + d[2], B + d[3])
         e1 = oracle.emf2d(G, 1, c, A + d[0], A + d[1], B + d[2], B + d[3])
         assert abs(e0 - e1) <= 5e-3 * (1 + abs(e0)) * 1e-1
+
+
+# ----------------------------------------------------------------------- HLL ------
+# PAPER.md section 2.1.1 (L70-72): three regions; the star state is the integral average of
+# the solution between the two outer waves.  Pinned through what that sentence fixes.
+def _outer_speeds(L, R, bn):
+    c = max(oracle.fast_speed(G, L[0], L[4], bn, L[5], L[6]), oracle.fast_speed(G, R[0], R[4], bn, R[5], R[6]))
+    return min(L[1], R[1]) - c, max(L[1], R[1]) + c
+
+
+def test_hll_consistency_and_supersonic_upwinding():
+    rng = np.random.default_rng(21)
+    for _ in range(300):
+        q, L, R = rand_state(rng), rand_state(rng), rand_state(rng)
+        bn = rng.normal()
+        ref = phys_flux(q, bn, G)
+        assert np.allclose(oracle.hll(G, q, q, bn), ref, rtol=0, atol=2e-13 * (1 + np.abs(ref).max()))
+        for shift, side in ((+30.0, L), (-30.0, R)):
+            Ls, Rs, s = L.copy(), R.copy(), side.copy()
+            Ls[1] += shift; Rs[1] += shift; s[1] += shift
+            assert np.allclose(oracle.hll(G, Ls, Rs, bn), phys_flux(s, bn, G), rtol=1e-14, atol=0)
+
+
+def test_hll_star_state_is_the_integral_average_and_both_jumps_hold():
+    """Integrating the conservation law over [SL*t, SR*t] x [0, t] gives the average state
+    U* = (SR UR - SL UL - (FR - FL)) / (SR - SL); the flux at x = 0 inside the fan must then
+    satisfy the jump condition across BOTH outer waves with that one state."""
+    rng = np.random.default_rng(22)
+    n_sub = 0
+    for _ in range(400):
+        L, R = rand_state(rng, mach=0.7), rand_state(rng, mach=0.7)
+        bn = rng.normal()
+        SL, SR = _outer_speeds(L, R, bn)
+        if not (SL < 0 < SR):
+            continue
+        n_sub += 1
+        UL, UR, FL, FR = cons(L, bn, G), cons(R, bn, G), phys_flux(L, bn, G), phys_flux(R, bn, G)
+        Us = (SR * UR - SL * UL - (FR - FL)) / (SR - SL)
+        F = oracle.hll(G, L, R, bn)
+        scale = 1 + max(np.abs(FL).max(), np.abs(FR).max())
+        assert np.allclose(F - FL, SL * (Us - UL), rtol=0, atol=1e-12 * scale)
+        assert np.allclose(F - FR, SR * (Us - UR), rtol=0, atol=1e-12 * scale)
+        assert Us[0] > 0                                   # the average density is positive
+    assert n_sub > 200
+
+
+def test_hll_galilean_fan_is_one_linear_piece():
+    """G(V) = F(V) - V U(V) of the boosted problem is linear in V inside the fan with slope
+    -U* (one star state), and equals F_K - V U_K outside: three regions, no more."""
+    rng = np.random.default_rng(23)
+    for _ in range(40):
+        L, R = rand_state(rng), rand_state(rng)
+        bn = rng.normal()
+        SL, SR = _outer_speeds(L, R, bn)
+
+        def Gv(V):
+            Lb, Rb = L.copy(), R.copy()
+            Lb[1] -= V; Rb[1] -= V
+            Fp = oracle.hll(G, Lb, Rb, bn)
+            g = Fp.copy()
+            g[1] = Fp[1] + V * Fp[0]
+            g[4] = Fp[4] + V * Fp[1] + 0.5 * V * V * Fp[0]
+            return g
+        UL, UR = cons(L, bn, G), cons(R, bn, G)
+        Us = (SR * UR - SL * UL - (phys_flux(R, bn, G) - phys_flux(L, bn, G))) / (SR - SL)
+        Vs = np.linspace(SL + 1e-3 * (SR - SL), SR - 1e-3 * (SR - SL), 9)
+        g = np.array([Gv(V) for V in Vs])
+        slope = (g[-1] - g[0]) / (Vs[-1] - Vs[0])
+        scale = 1 + np.abs(g).max()
+        assert np.allclose(slope, -Us, rtol=0, atol=1e-10 * scale)
+        assert np.allclose(g, g[0] + np.outer(Vs - Vs[0], slope), rtol=0, atol=1e-10 * scale)
+        for V, q in ((SL - 0.5, L), (SR + 0.5, R)):
+            assert np.allclose(Gv(V), phys_flux(q, bn, G) - V * cons(q, bn, G), rtol=1e-12, atol=1e-12 * scale)
+
+
+def test_hll_mirror_symmetry_and_diffusive_contact():
+    rng = np.random.default_rng(24)
+    flip = np.array([-1, 1, -1, -1, -1, -1, -1.0])     # same parity as test_hlld_mirror_symmetry
+    for _ in range(300):
+        L, R = rand_state(rng), rand_state(rng)
+        bn = rng.normal()
+        Lm, Rm = R.copy(), L.copy()
+        Lm[1] *= -1; Rm[1] *= -1
+        F = oracle.hll(G, L, R, bn)
+        Fm = oracle.hll(G, Lm, Rm, -bn)
+        assert np.allclose(Fm, flip * F, rtol=0, atol=1e-12 * (1 + np.abs(F).max()))
+    # a stationary contact: HLLD keeps it exactly (zero mass flux), HLL smears it (the paper: "quite diffusive")
+    L = np.array([1.0, 0, 0, 0, 1.0, 0.3, -0.2]); R = np.array([0.25, 0, 0, 0, 1.0, 0.3, -0.2])
+    assert oracle.hlld(G, L, R, 0.5)[0] == 0.0
+    assert oracle.hll(G, L, R, 0.5)[0] > 1e-2

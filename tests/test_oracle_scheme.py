@@ -12,8 +12,8 @@ from paper_2508_09568_b200 import workloads as W
 NG = 3
 
 
-def run(w, limiter=1, emf_solver=0, t_end=None, max_steps=10 ** 9, courant=None):
-    o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, limiter=limiter, emf_solver=emf_solver)
+def run(w, limiter=1, emf_solver=0, t_end=None, max_steps=10 ** 9, courant=None, flux_solver=0):
+    o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, limiter=limiter, emf_solver=emf_solver, flux_solver=flux_solver)
     U = w.U.copy()
     t, steps = 0.0, 0
     t_end = w.t_end if t_end is None else t_end
@@ -272,3 +272,48 @@ def test_mirror_reflection_of_2d_data():
         dt = o.cfl_dt(Ua, 0.4)
         Ua, Ub = o.step(Ua, dt), o.step(Ub, dt)
     assert np.abs(reflect(W.gather(Ua, w.n, w.P)) - W.gather(Ub, w.n, w.P)).max() <= 1e-13
+
+
+# ------------------------------------------------- HLL flux variant (PAPER.md 2.1.1) ----
+def test_hll_variant_sod_converges_to_the_exact_solution_and_is_more_diffusive():
+    """The scheme with the HLL flux still converges to the exact Sod solution; its error is
+    larger than HLLD's at the same resolution ("quite diffusive")."""
+    errs = {}
+    for fs in (0, 1):
+        for N in (128, 256):
+            w = W.sod(N, 8)
+            U, t, _ = run(w, flux_solver=fs)
+            g = W.gather(U, w.n, w.P)
+            x = (np.arange(N) + 0.5) / N
+            ex = exact_riemann.sample((x - 0.5) / t, 1, 0, 1, 0.125, 0, 0.1, 1.4)
+            errs[fs, N] = np.abs(g[0, 0, 0] - ex[0]).mean()
+            assert abs(g[0].sum() / N - 0.5625) < 1e-14
+    assert errs[1, 256] <= 4.5e-3 and np.log2(errs[1, 128] / errs[1, 256]) > 0.7, errs
+    assert errs[1, 256] > errs[0, 256] and errs[1, 128] > errs[0, 128], errs
+
+
+def test_hll_variant_conserves_and_keeps_div_b_on_periodic_3d_data():
+    w = W.turbulence(N=16, n=8, dtype=np.float64)
+    U, _, steps = run(w, flux_solver=1, t_end=1.0, max_steps=5)
+    assert steps == 5
+    g0, g1 = W.gather(w.U, w.n, w.P), W.gather(U, w.n, w.P)
+    for f in range(5):
+        t0, t1 = g0[f].sum(), g1[f].sum()
+        assert abs(t1 - t0) <= 1e-12 * max(abs(t0), np.abs(g0[f]).sum() * 1e-3 + 1e-300), f
+    div = np.roll(g1[5], -1, 2) - g1[5] + np.roll(g1[6], -1, 1) - g1[6] + np.roll(g1[7], -1, 0) - g1[7]
+    assert np.abs(div).max() <= 1e-13 * np.abs(g1[5:]).max() * 16
+    assert np.abs(g1 - g0).max() > 1e-4            # the state did move
+
+
+def test_hll_variant_is_direction_blind():
+    """One MHD tube along x, y and z with the HLL flux: identical up to relabelling."""
+    left, right = (1.0, 0.2, 0.3, -0.1, 1.0, 1.0, 0.4), (0.125, -0.1, -0.2, 0.25, 0.1, -1.0, 0.2)
+    prof = []
+    for axis in range(3):
+        w = W.mhd_tube(left, right, 0.75, 2.0, ncell=64, npatch=2, axis=axis, t_end=0.05)
+        U, _, _ = run(w, flux_solver=1)
+        g = W.gather(U, w.n, w.P)
+        line = g[(slice(None),) + tuple(slice(None) if 2 - a == axis else 0 for a in range(3))]   # [8, ncell]
+        perm = [0] + [1 + (axis + k) % 3 for k in range(3)] + [4] + [5 + (axis + k) % 3 for k in range(3)]
+        prof.append(line[perm])
+    assert np.abs(prof[1] - prof[0]).max() <= 1e-11 and np.abs(prof[2] - prof[0]).max() <= 1e-11
