@@ -54,7 +54,7 @@ typedef struct {
   int32_t limiter;     /* 1 = minmod (default), 2 = monotonised central */
   int32_t emf_solver;  /* 0 = HLLD-2D (default), 1 = HLL-2D          */
   int32_t device;      /* CUDA ordinal                                                  */
-  int32_t reserved;
+  int32_t flux_solver; /* 0 = HLLD (default, PAPER.md 2.1.2), 1 = HLL (PAPER.md 2.1.1)  */
   double  gamma;       /* adiabatic index                                               */
   double  dx[3];       /* cell sizes, uniform over the bunch                            */
   void   *stream;      /* cudaStream_t supplied by the caller (0 = default stream)      */

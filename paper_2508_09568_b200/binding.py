@@ -26,7 +26,7 @@ ABI_SYMBOLS = [
 
 class Desc(C.Structure):
     _fields_ = [("n", C.c_int32 * 3), ("ng", C.c_int32), ("npatch", C.c_int32), ("dtype", C.c_int32),
-                ("limiter", C.c_int32), ("emf_solver", C.c_int32), ("device", C.c_int32), ("reserved", C.c_int32),
+                ("limiter", C.c_int32), ("emf_solver", C.c_int32), ("device", C.c_int32), ("flux_solver", C.c_int32),
                 ("gamma", C.c_double), ("dx", C.c_double * 3), ("stream", C.c_void_p)]
 
 
@@ -98,10 +98,11 @@ def _check(rc, what):
         raise RuntimeError(f"{what}: {_ERR.get(rc, rc)} ({msg}) {cu}")
 
 
-def make_desc(n, npatch, gamma, dx, dtype=MHD_F32, limiter=1, emf_solver=0, device=0, stream=0, ng=3):
+def make_desc(n, npatch, gamma, dx, dtype=MHD_F32, limiter=1, emf_solver=0, device=0, stream=0, ng=3, flux_solver=0):
     d = Desc()
     d.n[:] = list(n)
     d.ng, d.npatch, d.dtype, d.limiter, d.emf_solver, d.device = ng, npatch, dtype, limiter, emf_solver, device
+    d.flux_solver = flux_solver
     d.gamma = gamma
     d.dx[:] = list(dx)
     d.stream = stream
@@ -130,7 +131,7 @@ class MhdBunch:
     """
 
     def __init__(self, n, npatch, nbr, gamma, dx, dtype="f32", limiter=1, emf_solver=0, device=0,
-                 workspace_bytes=None, stream=None):
+                 workspace_bytes=None, stream=None, flux_solver=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("MhdBunch needs a CUDA device: there is no CPU fallback")
@@ -143,7 +144,7 @@ class MhdBunch:
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream()
         self.desc = make_desc(n, npatch, gamma, dx, MHD_F32 if dtype == "f32" else MHD_F64, limiter, emf_solver,
-                              device, self.stream.cuda_stream)
+                              device, self.stream.cuda_stream, flux_solver=flux_solver)
         self.lay = query(self.desc)
         self.m = tuple(self.lay.m)
         ws = self.lay.workspace_best if workspace_bytes is None else max(int(workspace_bytes), self.lay.workspace_min)

@@ -12,7 +12,7 @@ struct Geom {
   long long ps;        // elements per patch
   long long fs;        // elements per field of a state buffer (= npatch*ps)
   int np;
-  int limiter, emf_solver;
+  int limiter, emf_solver, flux_solver;
 };
 
 struct Box { int lo[3], ext[3]; long long cells; };

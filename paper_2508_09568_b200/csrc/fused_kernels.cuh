@@ -66,7 +66,7 @@ template <typename T, int TXM, int TYM> struct FusedCfg {
 // HLLD flux through the face between cell `cl` and cell `cr` along D; pointers address
 // array 0 of the respective cells, arrays are DC elements apart
 template <typename T, int DC, int D>
-__device__ __forceinline__ Flux5<T> face_flux(const T* __restrict__ cl, const T* __restrict__ cr, T gamma) {
+__device__ __forceinline__ Flux5<T> face_flux(const T* __restrict__ cl, const T* __restrict__ cr, T gamma, int flux_solver) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
   const T h = T(0.5);
   State1D<T> L, R;
@@ -84,7 +84,7 @@ __device__ __forceinline__ Flux5<T> face_flux(const T* __restrict__ cl, const T*
   R.p = cr[(D_QH + 4) * DC] - h * cr[dq_slot(D, 4) * DC];
   R.by = cr[(D_BCH + T1) * DC] - h * cr[dq_slot(D, 5 + T1) * DC];
   R.bz = cr[(D_BCH + T2) * DC] - h * cr[dq_slot(D, 5 + T2) * DC];
-  return hlld_flux(gamma, L, R, cr[(D_BH + D) * DC]);
+  return riemann_flux(flux_solver, gamma, L, R, cr[(D_BH + D) * DC]);
 }
 
 // EMF at the edge along E shared by cells sw=(a-1,b-1), se=(a,b-1), nw=(a-1,b), ne=(a,b)
@@ -370,7 +370,7 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
   const T dt = (T)(*dtp);
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
   const T gamma = P.gamma;
-  const int solver = G.emf_solver;
+  const int solver = G.emf_solver, fsolver = G.flux_solver;
 
   // D-block coordinates of the tile's first cell (i = x0-1, j = y0-1): cell -1 sits at 0, so
   // the start column x0 is a multiple of TXM and the box start is 16-byte aligned (TMA)
@@ -425,7 +425,7 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
     Flux5<T> cFz = {};
     T cex = T(0), cey = T(0);
     if (k <= nz && active) {
-      cFz = face_flux<T, DC, 2>(dp_, dc_, gamma);
+      cFz = face_flux<T, DC, 2>(dp_, dc_, gamma, fsolver);
       // ex: in-plane (y,z): sw=(j-1,k-1) se=(j,k-1) nw=(j-1,k) ne=(j,k)
       cex = edge_emf<T, DC, 0>(dp_ - DW, dp_, dc_ - DW, dc_, gamma, solver);
       // ey: in-plane (z,x): sw=(k-1,i-1) se=(k,i-1) nw=(k-1,i) ne=(k,i)
@@ -522,8 +522,8 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
 
     // [C] in-plane values of plane k become the "previous" set of the next iteration
     if (k <= nz && active) {
-      pFx = face_flux<T, DC, 0>(dc_ - 1, dc_, gamma);
-      pFy = face_flux<T, DC, 1>(dc_ - DW, dc_, gamma);
+      pFx = face_flux<T, DC, 0>(dc_ - 1, dc_, gamma, fsolver);
+      pFy = face_flux<T, DC, 1>(dc_ - DW, dc_, gamma, fsolver);
       // ez: in-plane (x,y): sw=(i-1,j-1) se=(i,j-1) nw=(i-1,j) ne=(i,j)
       pez = edge_emf<T, DC, 2>(dc_ - DW - 1, dc_ - DW, dc_ - 1, dc_, gamma, solver);
     }

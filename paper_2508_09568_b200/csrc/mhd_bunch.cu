@@ -137,6 +137,7 @@ int build_geom(const mhd_bunch_desc* d, Geom* G) {
   if (d->dtype != MHD_F32 && d->dtype != MHD_F64) return MHD_EINVAL;
   if (d->limiter != 1 && d->limiter != 2) return MHD_EINVAL;
   if (d->emf_solver != 0 && d->emf_solver != 1) return MHD_EINVAL;
+  if (d->flux_solver != 0 && d->flux_solver != 1) return MHD_EINVAL;
   if (!(d->gamma > 1.0) || !isfinite(d->gamma)) return MHD_EINVAL;
   int nact = 0;
   for (int a = 0; a < 3; ++a) {
@@ -166,6 +167,7 @@ int build_geom(const mhd_bunch_desc* d, Geom* G) {
   G->fs = (long long)d->npatch * G->ps;
   G->limiter = d->limiter;
   G->emf_solver = d->emf_solver;
+  G->flux_solver = d->flux_solver;
   return MHD_OK;
 }
 
@@ -295,12 +297,14 @@ template <> struct OnePassLaunch<float> {
   static int launch(mhd_bunch* b, const double* dtp, int p0, int npl) {
     using Cfg = OneCfg<float, TX, TY, OneTile::NPW>;
     const Geom& G = b->G;
-    auto kern = G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1>
-                               : k_step_onepass<float, TX, TY, OneTile::NPW, 2>;
-    static bool attr_done[3] = {false, false, false};
-    if (!attr_done[G.limiter]) {
+    // limiter and flux solver are compile-time parameters of the kernel
+    auto kern = G.flux_solver == 1
+                    ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 1> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 1>)
+                    : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 0> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 0>);
+    static bool attr_done[6] = {false, false, false, false, false, false};
+    if (!attr_done[G.limiter + 3 * G.flux_solver]) {
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
-      attr_done[G.limiter] = true;
+      attr_done[G.limiter + 3 * G.flux_solver] = true;
     }
     Params<float> P = make_params<float>(b, p0, npl);
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;

@@ -185,6 +185,45 @@ __device__ __forceinline__ Flux5<T> hlld_flux(T gamma, const State1D<T>& L, cons
   return F;
 }
 
+// ---- HLL flux (section 2.1.1) --------------------------------------
+// Three regions; the star state is the integral average between the outer waves, so the
+// flux through the interface is (SR FL - SL FR + SL SR (UR - UL)) / (SR - SL) inside the fan.
+// With SL clipped to <= 0 and SR to >= 0 the same expression returns FL / FR outside it.
+template <typename T>
+__device__ __forceinline__ Flux5<T> hll_flux(T gamma, const State1D<T>& L, const State1D<T>& R, T bn) {
+  using N = num<T>;
+  const T half = T(0.5), bn2 = bn * bn;
+  const T igm1 = N::rcp(gamma - T(1));
+  const T b2L = bn2 + L.by * L.by + L.bz * L.bz, b2R = bn2 + R.by * R.by + R.bz * R.bz;
+  const T pTL = L.p + half * b2L, pTR = R.p + half * b2R;
+  const T cmax = N::sqrt(N::max(fast_speed2(gamma * L.p, b2L, bn2, N::rcp(L.rho)),
+                                fast_speed2(gamma * R.p, b2R, bn2, N::rcp(R.rho))));
+  const T SL = N::min(N::min(L.u, R.u) - cmax, T(0)), SR = N::max(N::max(L.u, R.u) + cmax, T(0));
+  const T EL = L.p * igm1 + half * L.rho * (L.u * L.u + L.v * L.v + L.w * L.w) + half * b2L;
+  const T ER = R.p * igm1 + half * R.rho * (R.u * R.u + R.v * R.v + R.w * R.w) + half * b2R;
+  const T ubL = L.u * bn + L.v * L.by + L.w * L.bz, ubR = R.u * bn + R.v * R.by + R.w * R.bz;
+  const T mL = L.rho * L.u, mR = R.rho * R.u;
+  const T inv = N::rcp(SR - SL), ss = SL * SR;
+  Flux5<T> F;
+  F.d = (SR * mL - SL * mR + ss * (R.rho - L.rho)) * inv;
+  F.mu = (SR * (mL * L.u + pTL - bn2) - SL * (mR * R.u + pTR - bn2) + ss * (mR - mL)) * inv;
+  F.mv = (SR * (mL * L.v - L.by * bn) - SL * (mR * R.v - R.by * bn) + ss * (R.rho * R.v - L.rho * L.v)) * inv;
+  F.mw = (SR * (mL * L.w - L.bz * bn) - SL * (mR * R.w - R.bz * bn) + ss * (R.rho * R.w - L.rho * L.w)) * inv;
+  F.e = (SR * (L.u * (EL + pTL) - bn * ubL) - SL * (R.u * (ER + pTR) - bn * ubR) + ss * (ER - EL)) * inv;
+  return F;
+}
+
+// flux solver of the faces: 0 = HLLD, 1 = HLL (mhd_bunch_desc.flux_solver)
+template <typename T>
+__device__ __forceinline__ Flux5<T> riemann_flux(int flux_solver, T gamma, const State1D<T>& L, const State1D<T>& R, T bn) {
+  return flux_solver == 1 ? hll_flux(gamma, L, R, bn) : hlld_flux(gamma, L, R, bn);
+}
+template <int FS, typename T>
+__device__ __forceinline__ Flux5<T> riemann_flux_k(T gamma, const State1D<T>& L, const State1D<T>& R, T bn) {
+  if (FS == 1) return hll_flux(gamma, L, R, bn);
+  return hlld_flux(gamma, L, R, bn);
+}
+
 // ---- two-dimensional Riemann problem at an edge -------------------------------------
 // Corner states (rho, ua, ub, p, be) with be the out-of-plane field; in-plane fields are
 // single-valued per side: A (component a) south/north, B (component b) west/east.

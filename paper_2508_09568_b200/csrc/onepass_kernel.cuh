@@ -114,7 +114,7 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
   return c[(D_BH + X) * DC] + s * c[dbf_slot(X, ALONG) * DC];
 }
 
-template <typename T, int TX, int TY, int NPW, int LIM>
+template <typename T, int TX, int TY, int NPW, int LIM, int FS>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
                unsigned long long* __restrict__ bad, int xtiles) {
@@ -402,7 +402,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 
       Flux5<T> cFz = {};
       T cex = T(0), cey = T(0);
-      if (doFz) cFz = hlld_flux(gamma, Lz, face_state<T, DC, 2>(dc_, -h), dc_[(D_BH + 2) * DC]);
+      if (doFz) cFz = riemann_flux_k<FS>(gamma, Lz, face_state<T, DC, 2>(dc_, -h), dc_[(D_BH + 2) * DC]);
       // The hydro part of plane k-1 only waits for this flux: finish it now (C is ahead, its
       // partial update is normally there already), so that the previous plane's flux is dead
       // while the two edge problems are solved.
@@ -464,8 +464,8 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         if (xface) un[5] = P.U[5 * fs + cu];
         if (yface) un[6] = P.U[6 * fs + cu];
         const T* dc_ = dslot(kd) + own;
-        if (doFx) Fx = hlld_flux(gamma, face_state<T, DC, 0>(dc_ - 1, h), face_state<T, DC, 0>(dc_, -h), dc_[(D_BH + 0) * DC]);
-        if (doFy) Fy = hlld_flux(gamma, face_state<T, DC, 1>(dc_ - DW, h), face_state<T, DC, 1>(dc_, -h), dc_[(D_BH + 1) * DC]);
+        if (doFx) Fx = riemann_flux_k<FS>(gamma, face_state<T, DC, 0>(dc_ - 1, h), face_state<T, DC, 0>(dc_, -h), dc_[(D_BH + 0) * DC]);
+        if (doFy) Fy = riemann_flux_k<FS>(gamma, face_state<T, DC, 1>(dc_ - DW, h), face_state<T, DC, 1>(dc_, -h), dc_[(D_BH + 1) * DC]);
         if (active)   // ez, in-plane (x,y): sw=(i-1,j-1) se=(i,j-1) nw=(i-1,j) ne=(i,j)
           ez = emf_2d(gamma, solver, corner_state<T, DC, 2>(dc_ - DW - 1, h, h), corner_state<T, DC, 2>(dc_ - DW, -h, h),
                       corner_state<T, DC, 2>(dc_ - 1, h, -h), corner_state<T, DC, 2>(dc_, -h, -h),

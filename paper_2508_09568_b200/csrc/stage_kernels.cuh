@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(256) k_flux(Params<T> P, Box B) {
   R.by = h * (b1[0] + b1[G.s[T1]]) - h * dq[(5 + T1) * wfs];
   L.bz = h * (b2[-sd] + b2[-sd + G.s[T2]]) + h * dq[(5 + T2) * wfs - sd];
   R.bz = h * (b2[0] + b2[G.s[T2]]) - h * dq[(5 + T2) * wfs];
-  const Flux5<T> F = hlld_flux(P.gamma, L, R, bh[D * wfs]);
+  const Flux5<T> F = riemann_flux(G.flux_solver, P.gamma, L, R, bh[D * wfs]);
   T* fl = P.W + (W_FLUX + D * 5) * wfs + cw;
   fl[0] = F.d; fl[(1 + D) * wfs] = F.mu; fl[(1 + T1) * wfs] = F.mv; fl[(1 + T2) * wfs] = F.mw; fl[4 * wfs] = F.e;
 }

@@ -37,14 +37,14 @@ def updated_mask(n, ng=3):
     return m
 
 
-def make_oracle(w, limiter=1, emf_solver=0):
-    return oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, limiter=limiter, emf_solver=emf_solver)
+def make_oracle(w, limiter=1, emf_solver=0, flux_solver=0):
+    return oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, limiter=limiter, emf_solver=emf_solver, flux_solver=flux_solver)
 
 
-def make_gpu(w, dtype, limiter=1, emf_solver=0, workspace_bytes=None, path="auto"):
+def make_gpu(w, dtype, limiter=1, emf_solver=0, workspace_bytes=None, path="auto", flux_solver=0):
     from paper_2508_09568_b200.binding import MhdBunch
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, limiter=limiter, emf_solver=emf_solver,
-                 workspace_bytes=workspace_bytes)
+                 workspace_bytes=workspace_bytes, flux_solver=flux_solver)
     b.set_path(path)
     b.load(w.U)
     return b

@@ -70,6 +70,7 @@ def test_query_rejects_bad_descriptions():
     assert rc(dtype=5) == -1
     assert rc(limiter=3) == -1
     assert rc(emf_solver=2) == -1
+    assert rc(flux_solver=2) == -1 and rc(flux_solver=1) == 0
     assert lib.mhd_bunch_query(None, C.byref(lay)) == -1
     assert lib.mhd_bunch_strerror(-1) and lib.mhd_bunch_strerror(-3)
 

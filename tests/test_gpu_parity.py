@@ -188,6 +188,36 @@ def test_every_step_path_on_3d_bunches_matches_oracle(path, name, dtype, limiter
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("path", ["auto", "staged", "two_kernel"])
+@pytest.mark.parametrize("name", ["sod_x", "tube_z", "ot_ragged", "turb16", "turb_ragged", "turb_self"])
+def test_hll_flux_variant_matches_oracle(name, path, dtype):
+    """flux_solver = 1: the HLL flux of PAPER.md 2.1.1 at the faces, on every
+    implementation of the step; three chained steps so that the variant's own states feed back."""
+    w = small_workloads(dtype)[name]
+    if path == "two_kernel" and not all(k > 1 for k in w.n):
+        pytest.skip("the two-kernel path needs three active dimensions")
+    o = make_oracle(w, 2, 1, flux_solver=1)
+    b = make_gpu(w, dtype, 2, 1, path=path, flux_solver=1)
+    U = w.U.astype(np.float64)
+    for _ in range(3):
+        U = o.fill_guards(U, w.nbr)
+        dt = o.cfl_dt(U, 0.4)
+        U = o.step(U, dt)
+        b.fill_guards()
+        b.step(dt)
+    err = rel_err(masked(b.download(), w.n), masked(U, w.n))
+    assert err <= 3 * TOL_STEP[dtype], (name, dtype, err)
+    # and it is a different scheme: the HLLD result differs
+    o2 = make_oracle(w, 2, 1)
+    V = o2.fill_guards(w.U.astype(np.float64), w.nbr)
+    V = o2.step(V, o2.cfl_dt(V, 0.4))
+    W1 = o.step(o.fill_guards(w.U.astype(np.float64), w.nbr), o2.cfl_dt(o2.fill_guards(w.U.astype(np.float64), w.nbr), 0.4))
+    assert rel_err(masked(W1, w.n), masked(V, w.n)) > 100 * TOL_STEP["f64"]
+    assert b.status() == 0
+    b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_fused_tiles_cover_large_and_odd_patches(dtype):
     """Patch sizes that need several (x,y) tiles of the fused kernel with ragged edges:
     40 x 20 x 12 cells (x tiles 32+8, y tiles 8+8+4) and 64 x 8 x 8."""
