@@ -58,9 +58,10 @@ template <typename T, int TXM, int TYM> struct FusedCfg {
   static_assert(FH <= 32 && 32 % TXM == 0, "tile shape");
   static constexpr int XV = sizeof(T) == 8 ? 3 : 4;                 // values per y-exchange pass (7 in all)
   static constexpr int XC = 7;                                      // values the closing column hands to column TXM-1
+  static constexpr int XR = FH <= 16 ? 16 : 32;                     // rows of that hand-over buffer
   static constexpr uint32_t slot_bytes = (uint32_t)(sizeof(T) * D_COUNT * DC);
   static constexpr uint32_t slot_stride = (slot_bytes + 127u) / 128u * 128u;   // TMA destinations: 128-byte aligned
-  static constexpr size_t smem = 2 * (size_t)slot_stride + sizeof(T) * (size_t)(XV * NTH + XC * 16) + 16;
+  static constexpr size_t smem = 2 * (size_t)slot_stride + sizeof(T) * (size_t)(XV * NTH + XC * XR) + 16;
 };
 
 // HLLD flux through the face between cell `cl` and cell `cr` along D; pointers address
@@ -344,15 +345,16 @@ __global__ void __launch_bounds__(256) k_pack_d(Params<T> P, Box B) {
   }
 }
 
+// two CTAs per SM where two tiles' planes fit in shared memory (fp32 32x8), one otherwise (fp64 16x16)
 template <typename T, int TXM, int TYM>
-__global__ void __launch_bounds__(FusedCfg<T, TXM, TYM>::NTH, 2)
+__global__ void __launch_bounds__(FusedCfg<T, TXM, TYM>::NTH, (FusedCfg<T, TXM, TYM>::smem > 116 * 1024) ? 1 : 2)
 k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const double* __restrict__ dtp, int xtiles) {
   using C = FusedCfg<T, TXM, TYM>;
   constexpr int DC = C::DC, DW = C::DW, NTH = C::NTH;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* X = reinterpret_cast<T*>(smem_raw + 2 * C::slot_stride);                 // [XV][NTH]  +y exchange
-  T* XCs = X + C::XV * NTH;                                                   // [XC][16]   closing column
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * C::slot_stride + sizeof(T) * (C::XV * NTH + C::XC * 16));
+  T* XCs = X + C::XV * NTH;                                                   // [XC][XR]   closing column
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * C::slot_stride + sizeof(T) * (C::XV * NTH + C::XC * C::XR));
 
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
@@ -454,9 +456,9 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
         if (fi < tw && (fj < th || (fj == th && lasty))) un[6] = P.U[6 * fs + cu];
       }
       if (cell) un[7] = P.U[7 * fs + cu];
-      if (colthr && fj < 16) {
-        XCs[0 * 16 + fj] = pFx.d; XCs[1 * 16 + fj] = pFx.mu; XCs[2 * 16 + fj] = pFx.mv; XCs[3 * 16 + fj] = pFx.mw;
-        XCs[4 * 16 + fj] = pFx.e; XCs[5 * 16 + fj] = pez;    XCs[6 * 16 + fj] = pey;
+      if (colthr && fj < C::XR) {
+        XCs[0 * C::XR + fj] = pFx.d; XCs[1 * C::XR + fj] = pFx.mu; XCs[2 * C::XR + fj] = pFx.mv; XCs[3 * C::XR + fj] = pFx.mw;
+        XCs[4 * C::XR + fj] = pFx.e; XCs[5 * C::XR + fj] = pez;    XCs[6 * C::XR + fj] = pey;
       }
     }
     // +y exchange: 7 values in passes of XV through X; pass 0 is written before barrier 1
@@ -474,9 +476,9 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
       xF.mv = __shfl_down_sync(0xffffffffu, pFx.mv, 1); xF.mw = __shfl_down_sync(0xffffffffu, pFx.mw, 1);
       xF.e = __shfl_down_sync(0xffffffffu, pFx.e, 1);
       xez = __shfl_down_sync(0xffffffffu, pez, 1);      xey = __shfl_down_sync(0xffffffffu, pey, 1);
-      if (!colthr && fi == TXM - 1 && fj < 16) {       // the +x neighbour is the closing column
-        xF.d = XCs[0 * 16 + fj]; xF.mu = XCs[1 * 16 + fj]; xF.mv = XCs[2 * 16 + fj]; xF.mw = XCs[3 * 16 + fj];
-        xF.e = XCs[4 * 16 + fj]; xez = XCs[5 * 16 + fj];   xey = XCs[6 * 16 + fj];
+      if (!colthr && fi == TXM - 1 && fj < C::XR) {       // the +x neighbour is the closing column
+        xF.d = XCs[0 * C::XR + fj]; xF.mu = XCs[1 * C::XR + fj]; xF.mv = XCs[2 * C::XR + fj]; xF.mw = XCs[3 * C::XR + fj];
+        xF.e = XCs[4 * C::XR + fj]; xez = XCs[5 * C::XR + fj];   xey = XCs[6 * C::XR + fj];
       }
       const bool ynb = (fj < th) && active;
 #pragma unroll

@@ -30,11 +30,17 @@ namespace {
 thread_local char g_cuda_err[256] = "";
 }
 
-// (x,y) tile of the fused kernel per arithmetic type: 2 CTAs/SM fit 2 x 38 arrays of
-// (TX+2..) x (TY+2) cells in shared memory
+// (x,y) tile of the fused kernel per arithmetic type.  fp32: 32 x 8, two CTAs per SM (2 x 38
+// arrays of 36 x 10 cells each).  fp64: 16 x 16 with ONE CTA of 10 warps per SM -- a double
+// takes two registers, so occupancy is register-bound either way, and the square tile does
+// 5 % less halo work than 16 x 8 with two CTAs (riemann_update 7.81 -> 7.24 ms on the
+// config-2 shape).
 template <typename T> struct FusedTile;
 template <> struct FusedTile<float> { static constexpr int TX = 32, TY = 8; };
-template <> struct FusedTile<double> { static constexpr int TX = 16, TY = 8; };
+#ifndef FUSED_F64_TY
+#define FUSED_F64_TY 16
+#endif
+template <> struct FusedTile<double> { static constexpr int TX = 16, TY = FUSED_F64_TY; };
 // one-pass kernel (onepass_kernel.cuh): tile and number of predictor warps
 #ifndef ONEPASS_NPW
 #define ONEPASS_NPW 6
