@@ -26,22 +26,19 @@ template <> struct num<float> {
 };
 template <> struct num<double> {
   static __device__ __forceinline__ double eps() { return DBL_EPSILON; }
-  // fp64: MUFU seed (rcp/rsqrt.approx.ftz.f64, ~20 bits) + Newton steps in DFMA: ~1e-16
-  // relative error without the IEEE sequences' slow-path calls and branches (tolerance of
-  // the path is 1e-12 per cell and step).  Arguments here are normal, non-zero numbers;
-  // sqrt(0) is handled explicitly.
+  // fp64: MUFU seed (rcp/rsqrt.approx.ftz.f64, relative error below 2^-20) refined by ONE
+  // third-order step in DFMA -- the residual e of the seed leaves e^3 < 2^-60, i.e. the result
+  // is good to a few units of 1e-16 without the IEEE sequences' slow-path calls and branches
+  // and with fewer DFMA than two Newton steps (tolerance of the path: 1e-12 per cell and
+  // step).  Arguments here are normal, non-zero numbers; sqrt(0) is handled explicitly.
   static __device__ __forceinline__ double rsqrt(double a) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-    const double h = 0.5 * a;
-    y = y * fma(-h * y, y, 1.5);
-    y = y * fma(-h * y, y, 1.5);
-    return y;
+    const double e = fma(-(a * y), y, 1.0);            // 1 - a y^2
+    return fma(y, fma(0.375, e, 0.5) * e, y);          // y (1 + e/2 + 3 e^2/8)
   }
   static __device__ __forceinline__ double sqrt(double a) {
-    const double y = rsqrt(a);
-    double s = a * y;
-    s = fma(fma(-s, s, a), 0.5 * y, s);
+    const double s = a * rsqrt(a);
     return a > 0.0 ? s : 0.0;
   }
   static __device__ __forceinline__ double abs(double x) { return fabs(x); }
@@ -50,15 +47,10 @@ template <> struct num<double> {
   static __device__ __forceinline__ double rcp(double a) {
     double x;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
-    x = fma(x, fma(-a, x, 1.0), x);
-    x = fma(x, fma(-a, x, 1.0), x);
-    return x;
+    const double e = fma(-a, x, 1.0);                  // 1 - a x
+    return fma(x, fma(e, e, e), x);                    // x (1 + e + e^2)
   }
-  static __device__ __forceinline__ double div(double a, double b) {
-    const double r = rcp(b);
-    const double q = a * r;
-    return fma(fma(-b, q, a), r, q);   // one residual correction of the quotient
-  }
+  static __device__ __forceinline__ double div(double a, double b) { return a * rcp(b); }
 };
 
 // ---- slope limiter: 0 at extrema; minmod (1) or monotonised central (2) -------------
