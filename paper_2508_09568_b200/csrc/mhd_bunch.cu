@@ -269,7 +269,10 @@ int launch_cfl(mhd_bunch* b, double courant, void* dt_dev, void* dt_patch) {
   Params<T> P = make_params<T>(b, 0, G.np);
   { LaunchScope ls(b, KC_MISC); k_zero_u64<<<blocks_for(G.np, 256), 256, 0, b->stream>>>(b->d_rate, G.np); }
   const long long per = (long long)G.n[0] * G.n[1] * G.n[2];
-  int bx = (int)((per + 256 * 8 - 1) / (256 * 8));
+#ifndef CFL_CPT
+#define CFL_CPT 8
+#endif
+  int bx = (int)((per + 256 * CFL_CPT - 1) / (256 * CFL_CPT));
   if (bx < 1) bx = 1;
   dim3 grid((unsigned)bx, (unsigned)G.np);
   { LaunchScope ls(b, KC_CFL); k_cfl<T><<<grid, 256, 0, b->stream>>>(P, b->d_rate); }
@@ -804,14 +807,15 @@ size_t hs_chunk_bytes(const mhd_bunch* b, int chunk) {
 void hs_release(mhd_bunch* b) {
   mhd_bunch::HostStream* h = b->hs;
   if (!h) return;
-  cudaStreamSynchronize(h->s_up);
-  cudaStreamSynchronize(h->s_dn);
-  for (cudaEvent_t e : h->ev_up) cudaEventDestroy(e);
-  for (cudaEvent_t e : h->ev_step) cudaEventDestroy(e);
-  cudaEventDestroy(h->ev_begin);
-  cudaEventDestroy(h->ev_all_steps);
-  cudaStreamDestroy(h->s_up);
-  cudaStreamDestroy(h->s_dn);
+  // members are null until created (a failed attach releases what it got so far)
+  if (h->s_up) cudaStreamSynchronize(h->s_up);
+  if (h->s_dn) cudaStreamSynchronize(h->s_dn);
+  for (cudaEvent_t e : h->ev_up) if (e) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->ev_step) if (e) cudaEventDestroy(e);
+  if (h->ev_begin) cudaEventDestroy(h->ev_begin);
+  if (h->ev_all_steps) cudaEventDestroy(h->ev_all_steps);
+  if (h->s_up) cudaStreamDestroy(h->s_up);
+  if (h->s_dn) cudaStreamDestroy(h->s_dn);
   delete h;
   b->hs = nullptr;
 }
@@ -929,8 +933,15 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   if (rc != MHD_OK) return rc;
   if (staging_bytes < lay.staging_bytes) return MHD_ENOMEM;
   hs_release(b);
-  mhd_bunch::HostStream* h = new (std::nothrow) mhd_bunch::HostStream;
+  mhd_bunch::HostStream* h = new (std::nothrow) mhd_bunch::HostStream();
   if (!h) return MHD_ENOMEM;
+  h->s_up = h->s_dn = nullptr;
+  h->ev_begin = h->ev_all_steps = nullptr;
+  b->hs = h;                               // owned by the handle from here on: released by detach / destroy,
+  struct Guard {                           // or right here if the attach fails half way
+    mhd_bunch* b; bool ok;
+    ~Guard() { if (!ok) hs_release(b); }
+  } guard{b, false};
   h->chunk = lay.chunk_patches;
   h->nchunk = lay.nchunk;
   h->stage_up = (char*)staging_dev;
@@ -940,8 +951,8 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   CUDA_TRY(cudaStreamCreateWithFlags(&h->s_dn, cudaStreamNonBlocking));
   CUDA_TRY(cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming));
   CUDA_TRY(cudaEventCreateWithFlags(&h->ev_all_steps, cudaEventDisableTiming));
-  h->ev_up.resize(h->nchunk);
-  h->ev_step.resize(h->nchunk);
+  h->ev_up.assign(h->nchunk, nullptr);
+  h->ev_step.assign(h->nchunk, nullptr);
   for (int c = 0; c < h->nchunk; ++c) {
     CUDA_TRY(cudaEventCreateWithFlags(&h->ev_up[c], cudaEventDisableTiming));
     CUDA_TRY(cudaEventCreateWithFlags(&h->ev_step[c], cudaEventDisableTiming));
@@ -950,7 +961,7 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   h->up_order = pl.up_order;
   h->ready = pl.ready;
   h->step_order = pl.step_order;
-  b->hs = h;
+  guard.ok = true;
   return MHD_OK;
 }
 
