@@ -220,8 +220,18 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    def totals():
+        """mass and total energy over the interior cells (fp64 sums on the device, outside the timed region)"""
+        v = b.view()
+        g = [3 if k > 1 else 0 for k in w.n]
+        I = v[:, :, g[2]:g[2] + w.n[2], g[1]:g[1] + w.n[1], g[0]:g[0] + w.n[0]]
+        return float(I[0].sum(dtype=torch.float64)), float(I[4].sum(dtype=torch.float64))
+
     for _ in range(max(3, args.warmup)):
         one_step()
+    barrier()
+    tot0 = totals()
+    b.fill_guards()            # looking at the buffer made the library re-validate the closing faces: do it here, untimed
     barrier()
     l0 = b.launches
     sampler = ClockSampler(local)
@@ -238,6 +248,9 @@ def main():
     clocks = sampler.summary()
     launches = b.launches - l0
     bad = b.status()
+    tot1 = totals()
+    conservation = {"mass_rel_drift": abs(tot1[0] - tot0[0]) / abs(tot0[0]), "energy_rel_drift": abs(tot1[1] - tot0[1]) / abs(tot0[1]),
+                    "note": "interior totals before/after the timed steps (periodic bunch: conserved up to round-off)"}
     value, ms = aggregate_over_ranks(ms, w.cells, args.steps, world, device="cuda")
 
     # ---- per-kernel-class device times (separate pass, events around every launch) ----
@@ -331,7 +344,7 @@ def main():
                 "config": {"workload": wdesc, "patches": w.npatch, "patch": [n, n, n], "guard": 3, "courant": courant,
                            "chunk_patches": b.chunk, "step_path": b.path, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (b.lay.state_bytes / 1e6)},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "bad_cells": bad,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "bad_cells": bad, "conservation": conservation,
                 "roofline": roofline, "step_roofline": step_view, "kernel_classes": classes, "cpu_baseline": cpu}
         print(json.dumps(line))
     b.close()

@@ -289,6 +289,25 @@ def test_n_steps_fp64_totals_and_fields(name, nsteps):
     assert rel_err(g, o) <= 1e-10                                # per cell, after N steps
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_n_steps_on_a_128_cube_cut_of_config2(dtype):
+    """N-step parity on a 128^3 cut (64 patches of 32^3, the bench's patch size, several
+    tiles per SM) with the config-2 field construction: 8 steps against the oracle."""
+    w = W.turbulence(N=128, n=32, dtype=NPD[dtype], config=2)
+    g, o, bad = run_both(w, dtype, 8)
+    assert bad == 0
+    tg, to = g[:5].sum(axis=(1, 2, 3)), o[:5].sum(axis=(1, 2, 3))
+    scale = np.array([to[0], np.abs(o[1:4]).sum(), np.abs(o[1:4]).sum(), np.abs(o[1:4]).sum(), to[4]])
+    if dtype == "f64":
+        assert np.all(np.abs(tg - to) <= TOL_TOTALS_F64 * scale), (tg - to) / scale
+        assert rel_err(g, o) <= 1e-10
+    else:
+        for a, b_ in ((0, 1), (1, 4), (4, 5), (5, 8)):
+            l1 = np.abs(g[a:b_] - o[a:b_]).sum() / max(np.abs(o[a:b_]).sum(), 1e-300)
+            assert l1 <= TOL_L1_F32, (a, l1)
+        assert np.all(np.abs(tg - to) <= 2e-6 * scale)
+
+
 @pytest.mark.parametrize("name,nsteps", [("turb16", 20), ("ot64", 40), ("tube_z", 40)])
 def test_n_steps_fp32_l1_norms(name, nsteps):
     w = small_workloads("f32")[name]
