@@ -127,7 +127,7 @@ template <typename T, int TY>
 __global__ void __launch_bounds__(predict_max_threads(TY), (TY == 8 && sizeof(T) == 4) ? 2 : 1)
 k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad,
                 const int* __restrict__ nbr, int gather) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
   const int PW = nx + 5, PH = TY + 5, PA = PW * PH;
