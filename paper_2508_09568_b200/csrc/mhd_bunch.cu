@@ -69,6 +69,7 @@ struct mhd_bunch {
   size_t esz;
   // optional per-kernel-class timing (host-side objects only)
   int path;            // MHD_PATH_*: 0 = automatic choice
+  int nsm;             // multiprocessors of the device
   bool onepass_ok;     // three active dimensions, fp32
   bool gather_ok;      // the one-pass kernel can read halos from the neighbours' interiors: every
                        // neighbour exists (no outflow side) and n_x is a whole number of 16-byte chunks
@@ -317,10 +318,21 @@ template <> struct OnePassLaunch<float> {
     }
     Params<float> P = make_params<float>(b, p0, npl);
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
-    dim3 grid((unsigned)(xt * yt), (unsigned)npl);
+    // fewer tiles than SMs: cut the columns into z segments of at least 8 planes so that the
+    // launch covers the GPU about twice (each segment pays a five-plane run-in, so only then)
+    int zseg = 1;
+    const long long tiles = (long long)xt * yt * npl;
+    if (tiles < b->nsm) {
+      zseg = (int)((2ll * b->nsm + tiles - 1) / tiles);
+      const int zmax = G.n[2] / 8 > 1 ? G.n[2] / 8 : 1;
+      if (zseg > zmax) zseg = zmax;
+    }
+    const char* env_z = getenv("MHD_ONEPASS_ZSEG");   // tuning knob
+    if (env_z && atoi(env_z) >= 1) zseg = atoi(env_z) < G.n[2] ? atoi(env_z) : G.n[2];
+    dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
-      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt, zseg);
     }
     CUDA_TRY(cudaGetLastError());
     return MHD_OK;
@@ -585,6 +597,8 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
                                         b->DG.ps, b->DG.fs, bx, by, W_DCOUNT);
   }
   b->onepass_ok = all_active(b->G) && desc->dtype == MHD_F32;
+  b->nsm = 148;
+  cudaDeviceGetAttribute(&b->nsm, cudaDevAttrMultiProcessorCount, desc->device);
   b->gather_ok = b->onepass_ok && b->G.n[0] % (int)(16 / b->esz) == 0;
   b->all_nbr = true;
   for (long long c = 0; c < 27ll * desc->npatch && b->all_nbr; ++c)

@@ -117,7 +117,7 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
 template <typename T, int TX, int TY, int NPW, int LIM, int FS>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
-               unsigned long long* __restrict__ bad, int xtiles) {
+               unsigned long long* __restrict__ bad, int xtiles, int zseg) {
   using C = OneCfg<T, TX, TY, NPW>;
   constexpr int PW = C::PW, PH = C::PH, PA = C::PA, BWX = C::BWX, RA = C::RA, DW = C::DW, DC = C::DC;
   constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL;
@@ -133,6 +133,11 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
+  // Small bunches have fewer tiles than the GPU has SMs; their columns are then cut into zseg
+  // segments along z (blockIdx.z), each a CTA of its own that marches planes [za, zb) after a
+  // five-plane run-in through its lower neighbour's planes.  zseg == 1: za = 0, zb = nz.
+  const int zlen = (nz + zseg - 1) / zseg;
+  const int za = (int)blockIdx.z * zlen, zb = min(nz, za + zlen);
   const int pl = blockIdx.y;
   const int xt = blockIdx.x % xtiles, yt = blockIdx.x / xtiles;
   const int x0 = xt * TX, y0 = yt * TY;
@@ -159,7 +164,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
     auto Es = [&](int plane, int a) { return Em + (((plane + 2) & 1) * 3 + a) * PA; };
     auto RH = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawh + (size_t)((plane + 2) & 1) * C::rawh_slot); };
     auto RB = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawb + (size_t)((plane + 4) & 3) * C::rawb_slot); };
-    const int rlo = -2, rhi = nz + 2;
+    const int rlo = za - 2, rhi = zb + 2;
     // U^n plane -> raw ring, one 16-byte chunk of a row per copy, all 8 fields.  A chunk lies
     // in one patch (x0 and, in gather mode, n_x are multiples of the chunk); its source is
     // the image cell in the neighbour of class (ox,oy,oz) -- O1 -- or, without gather, the
@@ -218,7 +223,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
             T* q = Qs(r - 1, 0) + o;
             q[0] = rho; q[PA] = u; q[2 * PA] = v; q[3 * PA] = w; q[4 * PA] = pr_; q[5 * PA] = bcx; q[6 * PA] = bcy; q[7 * PA] = bcz;
             const int ci = pc - 2, cj = pr - 2;   // tile-relative cell
-            if (ci >= 0 && ci < tw && cj >= 0 && cj < th && r - 1 >= 0 && r - 1 < nz &&
+            if (ci >= 0 && ci < tw && cj >= 0 && cj < th && r - 1 >= za && r - 1 < zb &&
                 !(rho > T(0) && pr_ > T(0) && rho < T(INFINITY) && pr_ < T(INFINITY)))
               ++nbad;
           }
@@ -263,9 +268,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 
       // ---- D data of plane kd = r-2 -> shared slot
       const int kd = r - 2;
-      if (kd >= -2) {
+      if (kd >= rlo) {
         T* const Dw = dslot(kd);
-        if (kd >= 1) nb_sync(NB_EMPTY + ((kd + 2) & 1), NALL);   // A and C are done with plane kd-2
+        if (kd >= za + 1) nb_sync(NB_EMPTY + ((kd + 2) & 1), NALL);   // A and C are done with plane kd-2
         const T* b0 = RB(kd);
         const T* b1 = RB(kd + 1);
 #pragma unroll
@@ -278,7 +283,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
             const T bxc = bx[0], byc = by[0], bzc = bz[0];
             const T bxu = b1[ob], byu = b1[RA + ob], bzu = b1[2 * RA + ob];   // raw fields one plane up
             const T fwx = bxu - bxc, fwy = byu - byc;
-            if (kd >= -1) {
+            if (kd >= za - 1) {
               const T* qc = Qs(kd, 0) + o;
               const T* qm = Qs(kd - 1, 0) + o;
               const T* qp = Qs(kd + 1, 0) + o;
@@ -336,7 +341,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
             cbx[s] = fwx; cby[s] = fwy;
           }
         }
-        if (kd >= -1) {
+        if (kd >= za - 1) {
           __threadfence_block();
           nb_arrive(NB_FULL + ((kd + 2) & 1), NALL);
         }
@@ -376,8 +381,8 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
     const bool doEy = active && (fj < th);      // ey(i..i+1, j): bx faces and b_z
     Flux5<T> pFz = {};
     T pex = T(0), pey = T(0);
-    nb_sync(NB_FULL + 1, NALL);                 // plane -1
-    for (int k = 0; k <= nz; ++k) {
+    nb_sync(NB_FULL + ((za + 1) & 1), NALL);    // plane za-1
+    for (int k = za; k <= zb; ++k) {
       nb_sync(NB_FULL + ((k + 2) & 1), NALL);   // plane k
       const T* dp_ = dslot(k - 1) + own;
       const T* dc_ = dslot(k) + own;
@@ -398,7 +403,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         ynw = corner_state<T, DC, 1>(dp_, h, -h);
         yBW = edge_field<T, DC, 0, 2>(dp_, h);
       }
-      if (k + 1 <= nz) nb_arrive(NB_EMPTY + ((k + 1) & 1), NALL);   // slot of plane k-1
+      if (k + 1 <= zb) nb_arrive(NB_EMPTY + ((k + 1) & 1), NALL);   // slot of plane k-1
 
       Flux5<T> cFz = {};
       T cex = T(0), cey = T(0);
@@ -408,7 +413,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       // while the two edge problems are solved.
       const long long cu = ubase + (long long)(k - 1) * plane;
       const T* pu = PU + fidx;
-      if (k >= 1) {
+      if (k >= za + 1) {
         nb_sync(NB_PUF, 2 * NR);
         if (cell) {
           // O8: (U - dt*dFx/dx - dt*dFy/dy) - dt*dFz/dz; z-face frame (mu,mv,mw) = (mz,mx,my)
@@ -432,11 +437,12 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       nb_sync(NB_A, NR);
       const T yex = XE[tyn], xey = XE[NR + txn];
       // b_z on the lower z-face of plane k (k = nz: closing face) -- Eq. 12
-      if (cell) P.Un[7 * fs + ubase + (long long)k * plane] = u7 + (cx * (xey - cey) - cy * (yex - cex));
-      if (k >= 1) {
+      // (face zb belongs to the next segment unless it is the patch's closing face)
+      if (cell && (k < zb || zb == nz)) P.Un[7 * fs + ubase + (long long)k * plane] = u7 + (cx * (xey - cey) - cy * (yex - cex));
+      if (k >= za + 1) {
         if (xface) P.Un[5 * fs + cu] = pu[5 * FA] - cz * (cey - pey);
         if (yface) P.Un[6 * fs + cu] = pu[6 * FA] + cz * (cex - pex);
-        if (k <= nz - 1) nb_arrive(NB_PUE, 2 * NR);
+        if (k <= zb - 1) nb_arrive(NB_PUE, 2 * NR);
       }
       pex = cex; pey = cey;
     }
@@ -447,9 +453,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   {
     const bool doFx = active && (fj < th);
     const bool doFy = active && (fi < tw);
-    for (int kd = -1; kd <= nz; ++kd) {
+    for (int kd = za - 1; kd <= zb; ++kd) {
       nb_sync(NB_FULL + ((kd + 2) & 1), NALL);
-      const bool work = (kd >= 0) && (kd <= nz - 1);
+      const bool work = (kd >= za) && (kd <= zb - 1);
       Flux5<T> Fx = {}, Fy = {};
       T ez = T(0);
       T un[7];
@@ -472,7 +478,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
                       edge_field<T, DC, 0, 1>(dc_ - DW, h), edge_field<T, DC, 0, 1>(dc_, -h),
                       edge_field<T, DC, 1, 0>(dc_ - 1, h), edge_field<T, DC, 1, 0>(dc_, -h));
       }
-      if (kd + 2 <= nz) nb_arrive(NB_EMPTY + ((kd + 2) & 1), NALL);   // done with plane kd
+      if (kd + 2 <= zb) nb_arrive(NB_EMPTY + ((kd + 2) & 1), NALL);   // done with plane kd
       if (!work) continue;
 
       // neighbours: +x by warp shuffle (the closing column hands its values over through XC),
@@ -498,7 +504,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       yF.d = XY[ty_]; yF.mu = XY[NR + ty_]; yF.mv = XY[2 * NR + ty_]; yF.mw = XY[3 * NR + ty_]; yF.e = XY[4 * NR + ty_];
       const T yez = XY[5 * NR + ty_];
 
-      if (kd >= 1) nb_sync(NB_PUE, 2 * NR);   // A has consumed the previous plane
+      if (kd >= za + 1) nb_sync(NB_PUE, 2 * NR);   // A has consumed the previous plane
       T* pu = PU + fidx;
       if (cell) {
         // momentum components by solver frame: x-face (mu,mv,mw)=(mx,my,mz); y-face (mu,mv,mw)=(my,mz,mx)
