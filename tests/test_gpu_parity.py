@@ -445,6 +445,34 @@ def test_launch_count_does_not_depend_on_bunch_size():
     assert counts[0] == counts[1] <= 16
 
 
+def test_z_segments_are_bitwise_invisible(monkeypatch):
+    """Small bunches are cut along z into several CTAs per column (MHD_ONEPASS_ZSEG overrides the
+    automatic choice): whatever the cut, ragged or not, the result is the same bit for bit, and
+    equals the oracle within the one-step tolerance."""
+    w = W.turbulence(N=(32, 32, 40), n=(32, 32, 40), dtype=np.float32)      # one patch, its own neighbour
+    outs = {}
+    for z in ("1", "auto", "3", "5", "40"):
+        if z == "auto":
+            monkeypatch.delenv("MHD_ONEPASS_ZSEG", raising=False)
+        else:
+            monkeypatch.setenv("MHD_ONEPASS_ZSEG", z)
+        b = make_gpu(w, "f32")
+        assert b.path == "onepass"
+        for _ in range(2):
+            b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+        outs[z] = b.download()
+        assert b.status() == 0
+        b.close()
+    for z in outs:
+        assert np.array_equal(outs[z], outs["1"]), z
+    o = make_oracle(w)
+    U = w.U.astype(np.float64)
+    for _ in range(2):
+        U = o.fill_guards(U, w.nbr)
+        U = o.step(U, o.cfl_dt(U, 0.4))
+    assert rel_err(masked(outs["auto"], w.n), masked(U, w.n)) <= 2 * TOL_STEP["f32"]
+
+
 # ------------------------------------------------------- full-size config 2 -------
 def test_config2_full_size_sampled_patches_and_invariants():
     """BASELINE.json config 2 (512 patches of 32^3, fp32) in the launch configuration
