@@ -170,6 +170,17 @@ int mhd_bunch_step_host(mhd_bunch *b, const void *host_in, void *host_out, doubl
                         double *dt_used, double *dt_next);
 int mhd_bunch_host_detach(mhd_bunch *b);
 
+/* HOST only, no device needed: the schedule mhd_bunch_step_host would follow for a neighbour
+ * table (HOST int32 [npatch][27]) and a chunk size (<= 0: the library's choice, the candidate
+ * with the shortest simulated makespan).  Outputs (HOST; the three arrays nullable, capacity
+ * `cap` >= *nchunk else MHD_ENOMEM): up_order[u] = chunk uploaded u-th; ready[c] = position
+ * of the last upload that carries a neighbour of chunk c (its step may start after it);
+ * step_order[s] = chunk stepped s-th; *makespan = simulated length of the step in units of
+ * "one patch across PCIe" (a step costs 0.3 per patch, each transfer 1.5 fixed).           */
+int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t chunk_patches, int32_t *chunk_out,
+                            int32_t *nchunk_out, int32_t *up_order, int32_t *ready, int32_t *step_order, int32_t cap,
+                            double *makespan);
+
 /* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
  * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
  * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to

@@ -21,6 +21,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
     "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
     "mhd_bunch_host_query", "mhd_bunch_host_attach", "mhd_bunch_step_host", "mhd_bunch_host_detach",
+    "mhd_bunch_host_schedule",
 ]
 
 
@@ -81,6 +82,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_host_attach.argtypes = [vp, vp, C.c_size_t, i32]
     lib.mhd_bunch_step_host.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.mhd_bunch_host_detach.argtypes = [vp]
+    lib.mhd_bunch_host_schedule.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, i32, C.POINTER(dbl)]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
     lib.mhd_bunch_last_cuda_error.restype = C.c_char_p
@@ -121,6 +123,22 @@ def measure_alu_peak(dtype="f32", device=0):
     _check(load_library().mhd_bunch_measure_alu_peak(MHD_F32 if dtype == "f32" else MHD_F64, device, C.byref(v)),
            "mhd_bunch_measure_alu_peak")
     return v.value
+
+
+def host_schedule(nbr, chunk_patches=0):
+    """Schedule of the host-streaming step for a neighbour table (host only, no device):
+    dict with chunk, up_order, ready, step_order (numpy int32) and the simulated makespan."""
+    nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+    npatch = nbr.shape[0]
+    chunk, nchunk, span = C.c_int32(0), C.c_int32(0), C.c_double(0.0)
+    up, ready, order = (np.zeros(npatch, dtype=np.int32) for _ in range(3))
+    _check(load_library().mhd_bunch_host_schedule(nbr.ctypes.data_as(C.c_void_p), npatch, chunk_patches, C.byref(chunk),
+                                                  C.byref(nchunk), up.ctypes.data_as(C.c_void_p),
+                                                  ready.ctypes.data_as(C.c_void_p), order.ctypes.data_as(C.c_void_p),
+                                                  npatch, C.byref(span)), "mhd_bunch_host_schedule")
+    n = nchunk.value
+    return {"chunk": chunk.value, "nchunk": n, "up_order": up[:n].copy(), "ready": ready[:n].copy(),
+            "step_order": order[:n].copy(), "makespan": span.value}
 
 
 class MhdBunch:

@@ -865,14 +865,13 @@ int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int 
 // chunk may step once the last upload carrying one of its neighbours has landed (ready[c] =
 // that upload's position); chunks step in order of readiness.
 struct HsPlan { std::vector<int> up_order, ready, step_order; };
-HsPlan hs_plan(const mhd_bunch* b, int chunk) {
+HsPlan hs_plan(const int* nb, int np, int chunk) {
   HsPlan pl;
-  const int np = b->G.np, C = (np + chunk - 1) / chunk;
+  const int C = (np + chunk - 1) / chunk;
   pl.up_order.resize(C);
   std::vector<int> upos(C);
   for (int u = 0; u < C; ++u) { pl.up_order[u] = (u + C - 1) % C; upos[pl.up_order[u]] = u; }
   pl.ready.assign(C, 0);
-  const std::vector<int>& nb = *b->h_nbr;
   for (int p = 0; p < np; ++p) {
     const int c = p / chunk;
     int r = upos[c];
@@ -891,8 +890,8 @@ HsPlan hs_plan(const mhd_bunch* b, int chunk) {
 }
 // Makespan of that schedule in units of "one patch across PCIe": uploads back to back, a
 // step costs `alpha` per patch, a download 1 per patch, `eps` of fixed cost per transfer.
-double hs_makespan(const mhd_bunch* b, int chunk, const HsPlan& pl, double alpha, double eps) {
-  const int np = b->G.np, C = (int)pl.up_order.size();
+double hs_makespan(int np, int chunk, const HsPlan& pl, double alpha, double eps) {
+  const int C = (int)pl.up_order.size();
   auto size = [&](int c) { return (double)std::min(chunk, np - c * chunk); };
   std::vector<double> t_up(C);
   double t = 0.0;
@@ -907,14 +906,13 @@ double hs_makespan(const mhd_bunch* b, int chunk, const HsPlan& pl, double alpha
 }
 // default chunk: the candidate with the shortest simulated step (transfers dominate: a step
 // of a patch costs about a third of its transfer; ~30 us of fixed cost per chunk and stream)
-int hs_default_chunk(const mhd_bunch* b) {
-  const int np = b->G.np;
+int hs_default_chunk(const int* nb, int np) {
   int best = np;
   double best_t = 1e300;
   for (int k : {1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64}) {
     const int chunk = (np + k - 1) / k;
     if (chunk < 1) break;
-    const double tt = hs_makespan(b, chunk, hs_plan(b, chunk), 0.3, 1.5);
+    const double tt = hs_makespan(np, chunk, hs_plan(nb, np, chunk), 0.3, 1.5);
     if (tt < best_t - 1e-9) { best_t = tt; best = chunk; }
     if (chunk == 1) break;
   }
@@ -928,13 +926,37 @@ extern "C" {
 int mhd_bunch_host_query(mhd_bunch* b, int32_t chunk_patches, mhd_bunch_host_layout* out) {
   if (!b || !out) return MHD_ESTATE;
   int chunk = chunk_patches;
-  if (chunk <= 0) chunk = hs_default_chunk(b);
+  if (chunk <= 0) chunk = hs_default_chunk(b->h_nbr->data(), b->G.np);
   if (chunk > b->G.np) chunk = b->G.np;
   out->chunk_patches = chunk;
   out->nchunk = (b->G.np + chunk - 1) / chunk;
   out->host_bytes = (size_t)8 * b->G.np * b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
   out->staging_bytes = 2 * hs_chunk_bytes(b, chunk);
   out->pipelined = (b->all_nbr && step_gathers(b)) ? 1 : 0;
+  return MHD_OK;
+}
+
+int mhd_bunch_host_schedule(const int32_t* nbr, int32_t npatch, int32_t chunk_patches, int32_t* chunk_out,
+                            int32_t* nchunk_out, int32_t* up_order, int32_t* ready, int32_t* step_order, int32_t cap,
+                            double* makespan) {
+  if (!nbr || npatch < 1 || !chunk_out || !nchunk_out) return MHD_EINVAL;
+  for (long long c = 0; c < 27ll * npatch; ++c)
+    if (nbr[c] < -1 || nbr[c] >= npatch) return MHD_EINVAL;
+  int chunk = chunk_patches > 0 ? chunk_patches : hs_default_chunk(nbr, npatch);
+  if (chunk > npatch) chunk = npatch;
+  const HsPlan pl = hs_plan(nbr, npatch, chunk);
+  const int C = (int)pl.up_order.size();
+  *chunk_out = chunk;
+  *nchunk_out = C;
+  if (makespan) *makespan = hs_makespan(npatch, chunk, pl, 0.3, 1.5);
+  if (up_order || ready || step_order) {
+    if (cap < C) return MHD_ENOMEM;
+    for (int c = 0; c < C; ++c) {
+      if (up_order) up_order[c] = pl.up_order[c];
+      if (ready) ready[c] = pl.ready[c];
+      if (step_order) step_order[c] = pl.step_order[c];
+    }
+  }
   return MHD_OK;
 }
 
@@ -971,7 +993,7 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
     CUDA_TRY(cudaEventCreateWithFlags(&h->ev_up[c], cudaEventDisableTiming));
     CUDA_TRY(cudaEventCreateWithFlags(&h->ev_step[c], cudaEventDisableTiming));
   }
-  HsPlan pl = hs_plan(b, h->chunk);
+  HsPlan pl = hs_plan(b->h_nbr->data(), b->G.np, h->chunk);
   h->up_order = pl.up_order;
   h->ready = pl.ready;
   h->step_order = pl.step_order;
