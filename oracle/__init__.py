@@ -10,6 +10,7 @@ Arrays are numpy, dense, shape [8, npatch, mz, my, mx] (guards included), dtype
 float64 (or float32 with dtype="f32", a diagnostic build of the same source).
 """
 import ctypes as C
+import os
 
 import numpy as np
 
@@ -33,10 +34,21 @@ _LIBS = {}
 
 def _lib(key):
     if key not in _LIBS:
-        paths = _build.build()
-        lib = C.CDLL(paths[key])
+        # MHD_ORACLE_LIBDIR: load liboracle_<key>.so from there instead of building the committed
+        # source -- how tests/test_oracle_mutations.py points the pins at a deliberately broken
+        # copy of the oracle.  "f64_omp" is the OpenMP build of the same source (bench.py).
+        alt = os.environ.get("MHD_ORACLE_LIBDIR")
+        if key == "f64_omp":
+            path = _build.build_omp()
+        elif alt:
+            path = os.path.join(alt, "liboracle_%s.so" % key)
+        else:
+            path = _build.build()[key]
+        lib = C.CDLL(path)
         rp = C.c_void_p
         lib.orc_sizeof_real.restype = C.c_int
+        lib.orc_threads.restype = C.c_int
+        lib.orc_threads.argtypes = [C.c_int]
         lib.orc_patch_cells.restype = C.c_int64
         lib.orc_patch_cells.argtypes = [C.POINTER(_Desc)]
         lib.orc_state_elems.restype = C.c_int64
@@ -49,7 +61,7 @@ def _lib(key):
         lib.orc_step.argtypes = [C.POINTER(_Desc), rp, rp, C.c_double]
         lib.orc_stages.restype = None
         lib.orc_stages.argtypes = [C.POINTER(_Desc), rp, C.c_int32, C.c_double, rp]
-        real = C.c_double if key == "f64" else C.c_float
+        real = C.c_float if key == "f32" else C.c_double
         lib.orc_limiter.restype = real
         lib.orc_limiter.argtypes = [C.c_int32, real, real]
         lib.orc_hlld.restype = None
@@ -71,7 +83,7 @@ def _ptr(a):
 class Oracle:
     def __init__(self, n, npatch, gamma, dx, ng=3, limiter=1, emf_solver=0, dtype="f64", flux_solver=0):
         self.key = dtype
-        self.np_dtype = np.float64 if dtype == "f64" else np.float32
+        self.np_dtype = np.float32 if dtype == "f32" else np.float64
         self.lib = _lib(dtype)
         d = _Desc()
         d.n[:] = list(n)
@@ -120,6 +132,11 @@ class Oracle:
     def interior(self, U):
         sl = [slice(self.ng, self.ng + k) if k > 1 else slice(0, 1) for k in self.n]
         return U[:, :, sl[2], sl[1], sl[0]]
+
+
+def threads(want=0, dtype="f64_omp"):
+    """Threads the per-patch loops of the OpenMP build use (set if want > 0); 1 for the plain builds."""
+    return _lib(dtype).orc_threads(want)
 
 
 def limiter(kind, a, b, dtype="f64"):

@@ -78,6 +78,14 @@ static box mkbox(const geom *G, int ax, int bx, int ay, int by, int az, int bz) 
       for (int i = (B).lo[0]; i <= (B).hi[0]; ++i)
 
 int orc_sizeof_real(void) { return (int)sizeof(real); }
+
+/* threads of the OpenMP build (bench.py's all-cores timing leg); 1 in the plain build */
+#ifdef _OPENMP
+#include <omp.h>
+int orc_threads(int want) { if (want > 0) omp_set_num_threads(want); return omp_get_max_threads(); }
+#else
+int orc_threads(int want) { (void)want; return 1; }
+#endif
 int64_t orc_patch_cells(const orc_desc *d) { geom G; mkgeom(d, &G); return G.M; }
 int64_t orc_state_elems(const orc_desc *d) { geom G; mkgeom(d, &G); return 8 * (int64_t)G.np * G.M; }
 
@@ -87,6 +95,9 @@ int64_t orc_state_elems(const orc_desc *d) { geom G; mkgeom(d, &G); return 8 * (
 void orc_fill_guards(const orc_desc *d, const int32_t *nbr, real *U) {
   geom G; mkgeom(d, &G);
   box all = mkbox(&G, G.g[0], G.g[0], G.g[1], G.g[1], G.g[2], G.g[2]);
+  /* patches only read each other's INTERIOR cells here, so they are independent: the pragma is
+   * inert unless the file is built with -fopenmp (bench.py's all-cores timing leg only)        */
+#pragma omp parallel for schedule(dynamic)
   for (int p = 0; p < G.np; ++p) {
     BOXLOOP(all) {
       int c[3] = {i, j, k}, o[3], src[3], clamp[3];
@@ -607,10 +618,12 @@ static void update_patch(const geom *G, const real *const Up[8], real *const Un[
 
 void orc_step(const orc_desc *d, const real *U, real *Unew, double dt) {
   geom G; mkgeom(d, &G);
-  real *buf = (real *)malloc(sizeof(real) * ORC_NSTAGE * G.M);
-  scratch S; scratch_bind(&S, buf, G.M);
   memcpy(Unew, U, sizeof(real) * 8 * (size_t)G.np * G.M);
+  /* patches are independent between guard fills; each gets its own scratch */
+#pragma omp parallel for schedule(dynamic)
   for (int p = 0; p < G.np; ++p) {
+    real *buf = (real *)malloc(sizeof(real) * ORC_NSTAGE * G.M);
+    scratch S; scratch_bind(&S, buf, G.M);
     const real *Up[8]; real *Un[8];
     for (int f = 0; f < 8; ++f) {
       Up[f] = U + ((long)f * G.np + p) * G.M;
@@ -618,8 +631,8 @@ void orc_step(const orc_desc *d, const real *U, real *Unew, double dt) {
     }
     run_stages(&G, Up, (real)dt, &S);
     update_patch(&G, Up, Un, (real)dt, &S);
+    free(buf);
   }
-  free(buf);
 }
 
 void orc_stages(const orc_desc *d, const real *U, int32_t patch, double dt, real *out) {
@@ -635,6 +648,8 @@ double orc_cfl_dt(const orc_desc *d, const real *U, double courant, double *per_
   geom G; mkgeom(d, &G);
   box I = mkbox(&G, 0, 0, 0, 0, 0, 0);
   double dtmin = INFINITY;
+  double *dts = (double *)malloc(sizeof(double) * (size_t)G.np);
+#pragma omp parallel for schedule(dynamic)
   for (int p = 0; p < G.np; ++p) {
     const real *Up[8];
     for (int f = 0; f < 8; ++f) Up[f] = U + ((long)f * G.np + p) * G.M;
@@ -655,9 +670,12 @@ double orc_cfl_dt(const orc_desc *d, const real *U, double courant, double *per_
       }
       if (!(rate <= rate_max)) rate_max = rate; /* NaN propagates into the maximum */
     }
-    double dtp = courant / (double)rate_max;
-    if (per_patch) per_patch[p] = dtp;
-    if (!(dtp >= dtmin)) dtmin = dtp;
+    dts[p] = courant / (double)rate_max;
   }
+  for (int p = 0; p < G.np; ++p) {
+    if (per_patch) per_patch[p] = dts[p];
+    if (!(dts[p] >= dtmin)) dtmin = dts[p];
+  }
+  free(dts);
   return dtmin;
 }

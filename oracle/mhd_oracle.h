@@ -17,7 +17,16 @@
  * match of orc_emf2d (HLLD-2D) to the RAMSES routine the paper copied, whose
  * formulas the paper does not print: "parity unpinned" for that match.  What IS
  * pinned for orc_emf2d: planar reduction to orc_hlld's induction flux, uniform
- * state, x<->y antisymmetry, supersonic upwinding.
+ * state, x<->y antisymmetry, supersonic upwinding, the upwind weighting of the
+ * edge-side star fields (step 5: one-way supersonic flow reduces the edge to the
+ * upwind row's / column's 1D problem) and a second typing of the whole reading
+ * (see DESIGN.md).  tests/test_oracle_mutations.py compiles deliberately broken
+ * copies of this file and requires every one of them to fail a pin.
+ *
+ * The `#pragma omp parallel for` lines over patches are inert in the builds the
+ * tests use; oracle/build.py's build_omp() (-fopenmp) activates them for bench.py's
+ * all-cores timing leg.  Patches are independent between guard fills (PAPER.md
+ * L124), so the arithmetic is the same (checked bit for bit in the tests).
  */
 #ifndef MHD_ORACLE_H
 #define MHD_ORACLE_H
@@ -44,6 +53,9 @@ typedef struct {
 #define ORC_NSTAGE 70
 
 int     orc_sizeof_real(void);
+/* OpenMP build only (-fopenmp, bench.py's all-cores leg): set (want > 0) and return the number
+ * of threads the per-patch loops use; the plain build returns 1.                              */
+int     orc_threads(int want);
 int64_t orc_patch_cells(const orc_desc *d);              /* m_x*m_y*m_z                 */
 int64_t orc_state_elems(const orc_desc *d);              /* 8*npatch*patch_cells        */
 

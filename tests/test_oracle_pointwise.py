@@ -386,6 +386,162 @@ def test_emf2d_supersonic_in_one_direction_ignores_downwind_column():
         assert oracle.emf2d(G, 0, c2, AS, AN, BW, BE) == e0
 
 
+def _one_way_case(rng, sign):
+    """Corner set with flow supersonic towards sign*b and (mostly) subsonic along a, built so that
+    the DOWNWIND row can change nothing but the quantities under test:
+      * every corner of a column has the column's u_a, so min/max u_a come from the upwind row;
+      * the downwind row is denser (rho x kappa >= 1), colder, carries no A field and a weaker
+        out-of-plane field, so its fast speeds lie below the upwind row's (c_f grows with p, with
+        every field component and with 1/rho), i.e. the outer speeds are the upwind row's;
+      * total pressure is equal along each row, so both rows' contact speeds are the same |m|-weighted
+        mean of u_W and u_E; with A = 0 the downwind row's Alfven bounds collapse onto that contact
+        speed, strictly inside the upwind row's bounds: the inner speeds are the upwind row's too.
+    Returns (corners, AS, AN, BW, BE, L, R, bn): L, R, bn = the 1D problem of the upwind row."""
+    c = rand_corners(rng)
+    up, dn = ((0, 1), (2, 3)) if sign > 0 else ((2, 3), (0, 1))
+    A_up = rng.choice([-1.0, 1.0]) * rng.uniform(0.4, 1.5)
+    BW, BE = rng.normal(size=2)
+    c[:, 2] += 40.0 * sign
+    # equal total pressure along the upwind row: adjust the pressure of its east corner
+    w, e = up
+    pT = c[w, 4] + 0.5 * (A_up ** 2 + BW ** 2 + c[w, 5] ** 2)
+    c[e, 4] = pT - 0.5 * (A_up ** 2 + BE ** 2 + c[e, 5] ** 2)
+    if c[e, 4] <= 0.05:
+        return None
+    kappa = rng.uniform(1.0, 3.0)
+    for k in (0, 1):
+        c[dn[k], 0] = kappa * c[up[k], 0]
+        c[dn[k], 1] = c[up[k], 1]
+        c[dn[k], 3] = rng.normal()
+        c[dn[k], 5] = rng.uniform(-1, 1) * abs(c[up[k], 5])
+    pTd = rng.uniform(0.3, 0.9) * min(c[up[0], 4], c[up[1], 4]) + 0.5 * max(BW ** 2 + c[dn[0], 5] ** 2, BE ** 2 + c[dn[1], 5] ** 2)
+    c[dn[0], 4] = pTd - 0.5 * (BW ** 2 + c[dn[0], 5] ** 2)
+    c[dn[1], 4] = pTd - 0.5 * (BE ** 2 + c[dn[1], 5] ** 2)
+    if min(c[dn[0], 4], c[dn[1], 4]) <= 0 or max(c[dn[0], 4], c[dn[1], 4]) > min(c[up[0], 4], c[up[1], 4]):
+        return None
+    AS, AN = (A_up, 0.0) if sign > 0 else (0.0, A_up)
+    # precondition, checked with the (separately pinned) fast speed: the maxima are upwind
+    A = [AS, AS, AN, AN]; B = [BW, BE, BW, BE]
+    cfa = [oracle.fast_speed(G, c[q, 0], c[q, 4], A[q], B[q], c[q, 5]) for q in range(4)]
+    cfb = [oracle.fast_speed(G, c[q, 0], c[q, 4], B[q], A[q], c[q, 5]) for q in range(4)]
+    assert max(cfa[dn[0]], cfa[dn[1]]) < max(cfa[up[0]], cfa[up[1]])
+    assert max(cfb[dn[0]], cfb[dn[1]]) < max(cfb[up[0]], cfb[up[1]])
+    L = [c[w, 0], c[w, 1], c[w, 2], c[w, 3], c[w, 4], BW, c[w, 5]]
+    R = [c[e, 0], c[e, 1], c[e, 2], c[e, 3], c[e, 4], BE, c[e, 5]]
+    return c, AS, AN, BW, BE, L, R, A_up
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_emf2d_supersonic_along_b_takes_the_upwind_rows_star_fields(sign):
+    """O7 step 5.  Flow supersonic towards +b: S_S = 0, so the weights of the composition are 1 on
+    the south row and 0 on the north row -- for the corner EMFs AND for the edge-side star fields
+    B*_W, B*_E that feed the x-dissipation term.  The 2D problem then IS the 1D problem of the south
+    row along a: the edge EMF must equal O6's induction flux of that row (a separately pinned
+    function) while the flow is subsonic along a, so that the dissipation weight is not zero.  A
+    solver that weighted the star fields the other way round would pick the north row's values."""
+    rng = np.random.default_rng(31 + sign)
+    done = subsonic = 0
+    while done < 300:
+        case = _one_way_case(rng, sign)
+        if case is None:
+            continue
+        c, AS, AN, BW, BE, L, R, bn = case
+        F = oracle.hlld(G, L, R, bn)
+        e = oracle.emf2d(G, 0, c, AS, AN, BW, BE)
+        assert abs(e - F[5]) <= 5e-13 * (1 + abs(F[5])), (e, F[5])
+        # ... bit for bit whatever the downwind row holds (inside the precondition)
+        dn = (2, 3) if sign > 0 else (0, 1)
+        c2 = c.copy()
+        c2[dn[0], 3] += 0.7; c2[dn[1], 3] -= 0.3                       # out-of-plane velocity
+        c2[dn[0], 0] *= 1.25; c2[dn[1], 0] *= 1.25                     # density (same factor: same contact speed)
+        assert oracle.emf2d(G, 0, c2, AS, AN, BW, BE) == e
+        done += 1
+        cf = max(oracle.fast_speed(G, L[0], L[4], bn, L[5], L[6]), oracle.fast_speed(G, R[0], R[4], bn, R[5], R[6]))
+        subsonic += (min(L[1], R[1]) - cf < 0 < max(L[1], R[1]) + cf)
+    assert subsonic > 200          # the x-dissipation term was exercised
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_emf2d_supersonic_along_a_takes_the_upwind_columns_star_fields(sign):
+    """The same statement with the roles of a and b exchanged (weights a_E, a_W of A*_S, A*_N):
+    the case above mapped by a <-> b (u_a <-> u_b, A <-> B, SE <-> NW), under which the EMF changes
+    sign; expected value = minus O6's flux of the upwind COLUMN's 1D problem along b."""
+    rng = np.random.default_rng(41 + sign)
+    done = 0
+    while done < 300:
+        case = _one_way_case(rng, sign)
+        if case is None:
+            continue
+        c, AS, AN, BW, BE, L, R, bn = case
+        F = oracle.hlld(G, L, R, bn)
+        cs = c[[0, 2, 1, 3]].copy()
+        cs[:, [1, 2]] = cs[:, [2, 1]]
+        e = oracle.emf2d(G, 0, cs, BW, BE, AS, AN)
+        assert abs(e + F[5]) <= 5e-13 * (1 + abs(F[5])), (e, F[5])
+        done += 1
+
+
+def _hlld2d_typed(c, AS, AN, BW, BE):
+    """DESIGN.md reading O7 typed from its text; the Miyoshi-Kusano star
+    relations of a 1D sub-problem with prescribed outer speeds are typed from O6."""
+    SW_, SE_, NW_, NE_ = 0, 1, 2, 3
+    A = [AS, AS, AN, AN]; B = [BW, BE, BW, BE]
+    rho, ua, ub, p, be = c[:, 0], c[:, 1], c[:, 2], c[:, 4], c[:, 5]
+    emf = [ua[q] * B[q] - ub[q] * A[q] for q in range(4)]
+    pT = [p[q] + 0.5 * (A[q] ** 2 + B[q] ** 2 + be[q] ** 2) for q in range(4)]
+    ca = max(oracle.fast_speed(G, rho[q], p[q], A[q], B[q], be[q]) for q in range(4))
+    cb = max(oracle.fast_speed(G, rho[q], p[q], B[q], A[q], be[q]) for q in range(4))
+    tW, tE, tS, tN = ua.min() - ca, ua.max() + ca, ub.min() - cb, ub.max() + cb       # step 1
+
+    def sub(l, r, un, bt_l, bt_r, bn, SL, SR):                                          # step 2
+        mL, mR = rho[l] * (SL - un[l]), rho[r] * (SR - un[r])
+        SM = (mR * un[r] - mL * un[l] - pT[r] + pT[l]) / (mR - mL)
+        rsL, rsR = mL / (SL - SM), mR / (SR - SM)
+        star = []
+        for m, S, u, bt in ((mL, SL, un[l], bt_l), (mR, SR, un[r], bt_r)):
+            D = m * (S - SM) - bn ** 2
+            star.append(bt if abs(D) <= 16 * np.finfo(float).eps * m * (S - u) else bt * (m * (S - u) - bn ** 2) / D)
+        return star[0], star[1], SM - abs(bn) / np.sqrt(rsL), SM + abs(bn) / np.sqrt(rsR)
+
+    xS = sub(SW_, SE_, ua, BW, BE, AS, tW, tE)
+    xN = sub(NW_, NE_, ua, BW, BE, AN, tW, tE)
+    yW = sub(SW_, NW_, ub, AS, AN, BW, tS, tN)
+    yE = sub(SE_, NE_, ub, AS, AN, BE, tS, tN)
+    S_W = 0.0 if tW >= 0 else min(0.0, xS[2], xN[2])                                   # step 3
+    S_E = 0.0 if tE <= 0 else max(0.0, xS[3], xN[3])
+    S_S = 0.0 if tS >= 0 else min(0.0, yW[2], yE[2])
+    S_N = 0.0 if tN <= 0 else max(0.0, yW[3], yE[3])
+    Bs = {SW_: xS[0], SE_: xS[1], NW_: xN[0], NE_: xN[1]}
+    As = {SW_: yW[0], NW_: yW[1], SE_: yE[0], NE_: yE[1]}
+    Sx = {SW_: min(tW, 0.0), NW_: min(tW, 0.0), SE_: max(tE, 0.0), NE_: max(tE, 0.0)}   # step 4
+    Sy = {SW_: min(tS, 0.0), SE_: min(tS, 0.0), NW_: max(tN, 0.0), NE_: max(tN, 0.0)}
+    es = {q: emf[q] + Sx[q] * (Bs[q] - B[q]) - Sy[q] * (As[q] - A[q]) for q in range(4)}
+    BsW = (S_N * Bs[SW_] - S_S * Bs[NW_]) / (S_N - S_S)                                 # step 5
+    BsE = (S_N * Bs[SE_] - S_S * Bs[NE_]) / (S_N - S_S)
+    AsS = (S_E * As[SW_] - S_W * As[SE_]) / (S_E - S_W)
+    AsN = (S_E * As[NW_] - S_W * As[NE_]) / (S_E - S_W)
+    return (S_E * S_N * es[SW_] - S_W * S_N * es[SE_] - S_E * S_S * es[NW_] + S_W * S_S * es[NE_]) \
+        / ((S_E - S_W) * (S_N - S_S)) + S_W * S_E / (S_E - S_W) * (BsE - BsW) - S_S * S_N / (S_N - S_S) * (AsN - AsS)   # step 6
+
+
+def test_emf2d_hlld_matches_typed_reading():
+    """HLLD-2D against DESIGN.md's reading O7 typed a second time (numpy, in the printed form of
+    the formulas, weights of step 5 included), on non-planar subsonic corner sets where both
+    dissipation terms are active and the star fields of the two rows / columns differ."""
+    rng = np.random.default_rng(28)
+    n = 0
+    while n < 400:
+        c = rand_corners(rng)
+        c[:, 1:3] *= 0.5                                    # subsonic in both directions
+        AS, AN, BW, BE = rng.normal(size=4)
+        ref = _hlld2d_typed(c, AS, AN, BW, BE)
+        if not np.isfinite(ref):
+            continue
+        e = oracle.emf2d(G, 0, c, AS, AN, BW, BE)
+        assert abs(e - ref) <= 1e-11 * (1 + abs(ref)), (e, ref)
+        n += 1
+
+
 def test_emf2d_hll_matches_typed_formula():
     """HLL-2D is the composition (dagger) of DESIGN.md O7 with the corner values and the
     fast speeds clipped at zero -- typed here from that formula in its printed form."""

@@ -453,3 +453,18 @@ def test_cfl_skips_collapsed_dimensions():
     o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx)
     dt = o.cfl_dt(w.U, 0.4)
     assert np.isclose(dt, 0.4 * (1 / 64) / np.sqrt(1.4), rtol=1e-14)   # c = sqrt(gamma p/rho) = sqrt(1.4) on the left
+
+
+def test_openmp_build_of_the_oracle_is_bitwise_the_plain_build():
+    """bench.py's all-cores leg uses the same source built with -fopenmp: same bits."""
+    w = W.turbulence(N=16, n=8, dtype=np.float64)
+    res = {}
+    for key in ("f64", "f64_omp"):
+        o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, dtype=key)
+        U = o.fill_guards(w.U.copy(), w.nbr)
+        dt, pp = o.cfl_dt(U, 0.4, per_patch=True)
+        res[key] = (dt, pp, o.step(U, dt))
+    assert res["f64"][0] == res["f64_omp"][0]
+    assert np.array_equal(res["f64"][1], res["f64_omp"][1])
+    assert np.array_equal(res["f64"][2], res["f64_omp"][2])
+    assert oracle.threads(0, "f64") == 1 and oracle.threads(0) >= 1
