@@ -82,7 +82,13 @@ int mhd_bunch_query(const mhd_bunch_desc *desc, mhd_bunch_layout *layout);
  *   state_a/b  DEVICE, state_bytes each, 16-byte aligned.  state_a holds time level n.
  *   workspace  DEVICE, workspace_bytes >= layout.workspace_min, 16-byte aligned.  Nothing
  *              is allocated or freed after create (static work arrays).
- * Synchronises desc.stream once (table upload).                                          */
+ * Synchronises desc.stream once (table upload).
+ * The fast routes that read halos through the table (deferred fill, below) are taken only if
+ * the table has no -1 entry and composes like translations: nbr[p][centre] = p and
+ * nbr[nbr[p][c1]][c2] = nbr[p][c1+c2] wherever c1+c2 is again one of the 27 classes (true for
+ * any periodic arrangement of patches).  Any other table is still handled correctly, by an
+ * explicit guard fill before every step.  Every later call runs on desc.device, whatever the
+ * caller's current device is.                                                            */
 int mhd_bunch_create(const mhd_bunch_desc *desc, const int32_t *nbr, void *state_a, void *state_b,
                      void *workspace, size_t workspace_bytes, mhd_bunch **out);
 
@@ -220,10 +226,21 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 int mhd_bunch_set_path(mhd_bunch *b, int32_t path);
 int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
 
+/* Launch-shape knobs (tests and tuning runs; the library reads no environment variables).
+ *   MHD_TUNE_ONEPASS_ZSEG  z segments per tile column of the one-pass kernel (0 = automatic:
+ *                          1 unless the bunch has fewer tiles than the device has SMs);
+ *                          results do not depend on it, bit for bit.
+ *   MHD_TUNE_PREDICT_TY    y-tile of the two-kernel path's predictor: 16, 8 or 4.
+ * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
+#define MHD_TUNE_ONEPASS_ZSEG 1
+#define MHD_TUNE_PREDICT_TY   2
+int mhd_bunch_set_tuning(mhd_bunch *b, int32_t key, int32_t value);
+
 /* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted
- * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous; allocates
- * and frees a small device buffer of its own (not part of any handle).                    */
-int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double *tflops);
+ * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous.
+ *   scratch_dev  DEVICE, caller-owned, >= 8 * 256 * 8 * (number of SMs) bytes (4 MiB is
+ *                always enough; MHD_ENOMEM otherwise): the library allocates nothing.     */
+int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, void *scratch_dev, size_t scratch_bytes, double *tflops);
 
 /* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
  * patches) the workspace allows.                                                        */

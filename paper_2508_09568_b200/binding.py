@@ -13,13 +13,14 @@ from . import build as _build
 
 MHD_F32, MHD_F64 = 0, 1
 PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3}
+TUNE = {"onepass_zseg": 1, "predict_ty": 2}
 _ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
 
 ABI_SYMBOLS = [
     "mhd_bunch_query", "mhd_bunch_create", "mhd_bunch_fill_guards", "mhd_bunch_cfl_dt", "mhd_bunch_step",
     "mhd_bunch_step_dev", "mhd_bunch_upload", "mhd_bunch_download", "mhd_bunch_set_timing",
     "mhd_bunch_kernel_times", "mhd_bunch_current", "mhd_bunch_status", "mhd_bunch_launch_count",
-    "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
+    "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_set_tuning", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
     "mhd_bunch_host_query", "mhd_bunch_host_attach", "mhd_bunch_step_host", "mhd_bunch_host_detach",
     "mhd_bunch_host_schedule",
 ]
@@ -50,11 +51,9 @@ def load_library(build_if_missing=True):
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("MHD_BUNCH_LIB")       # an explicitly built library (e.g. a tuning variant)
-    if path is None:
-        path = _build.TARGET
-        if build_if_missing and _build.stale():
-            _build.build()
+    path = _build.TARGET
+    if build_if_missing and _build.stale():
+        _build.build()
     if not os.path.exists(path):
         raise RuntimeError(f"{path} is missing: the CUDA extension must be built (no CPU fallback)")
     lib = C.CDLL(path)
@@ -76,7 +75,8 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_chunk.argtypes = [vp, C.POINTER(i32)]
     lib.mhd_bunch_set_path.argtypes = [vp, i32]
     lib.mhd_bunch_get_path.argtypes = [vp, C.POINTER(i32)]
-    lib.mhd_bunch_measure_alu_peak.argtypes = [i32, i32, C.POINTER(dbl)]
+    lib.mhd_bunch_measure_alu_peak.argtypes = [i32, i32, vp, C.c_size_t, C.POINTER(dbl)]
+    lib.mhd_bunch_set_tuning.argtypes = [vp, i32, i32]
     lib.mhd_bunch_destroy.argtypes = [vp]
     lib.mhd_bunch_host_query.argtypes = [vp, i32, C.POINTER(HostLayout)]
     lib.mhd_bunch_host_attach.argtypes = [vp, vp, C.c_size_t, i32]
@@ -119,9 +119,11 @@ def query(desc):
 
 def measure_alu_peak(dtype="f32", device=0):
     """Measured FMA-chain peak in TFLOP/s (FMA = 2 flops) of the fp32 or fp64 pipe."""
+    import torch
     v = C.c_double(0.0)
-    _check(load_library().mhd_bunch_measure_alu_peak(MHD_F32 if dtype == "f32" else MHD_F64, device, C.byref(v)),
-           "mhd_bunch_measure_alu_peak")
+    scratch = torch.empty(4 << 20, dtype=torch.uint8, device=torch.device("cuda", device))
+    _check(load_library().mhd_bunch_measure_alu_peak(MHD_F32 if dtype == "f32" else MHD_F64, device, scratch.data_ptr(),
+                                                     scratch.numel(), C.byref(v)), "mhd_bunch_measure_alu_peak")
     return v.value
 
 
@@ -273,6 +275,10 @@ class MhdBunch:
         v = C.c_int32(0)
         _check(self.lib.mhd_bunch_get_path(self.h, C.byref(v)), "mhd_bunch_get_path")
         return {k: n for n, k in PATHS.items()}[v.value]
+
+    def set_tuning(self, key, value):
+        """key: 'onepass_zseg' | 'predict_ty' (include/mhd_bunch.h, MHD_TUNE_*)."""
+        _check(self.lib.mhd_bunch_set_tuning(self.h, TUNE[key], int(value)), "mhd_bunch_set_tuning")
 
     def set_timing(self, on):
         _check(self.lib.mhd_bunch_set_timing(self.h, 1 if on else 0), "mhd_bunch_set_timing")

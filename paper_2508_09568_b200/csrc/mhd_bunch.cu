@@ -95,6 +95,8 @@ struct mhd_bunch {
   HostStream* hs;
   std::vector<int>* h_nbr;   // HOST copy of the neighbour table (schedules of the host-streaming path)
   bool all_nbr;        // no -1 entry in the neighbour table
+  bool nbr_consistent; // the table composes like translations (see table_is_consistent)
+  int tune_zseg;       // MHD_TUNE_ONEPASS_ZSEG: 0 = automatic
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
   std::vector<Ev>* events;
@@ -102,9 +104,11 @@ struct mhd_bunch {
   long long cls_n[16];
 };
 
-enum KClass : int { KC_FILL = 0, KC_CFL, KC_PRIM, KC_EMF0, KC_PREDICT, KC_FLUX, KC_EMF, KC_UPDATE, KC_MISC, KC_RIEMANN, KC_ONEPASS, KC_COUNT };
+enum KClass : int { KC_FILL = 0, KC_CFL, KC_PRIM, KC_EMF0, KC_PREDICT, KC_FLUX, KC_EMF, KC_UPDATE, KC_MISC, KC_RIEMANN, KC_ONEPASS,
+                    KC_CLOSING, KC_COUNT };
 static const char* const kclass_names[KC_COUNT] = {"fill_guards", "cfl", "prim", "emf0", "predict", "hlld_flux",
-                                                   "emf_2d", "update", "misc", "riemann_update", "step_onepass"};
+                                                   "emf_2d", "update", "misc", "riemann_update", "step_onepass",
+                                                   "sync_closing_faces"};
 
 // brackets one launch with events when timing is on
 struct LaunchScope {
@@ -249,7 +253,7 @@ int launch_sync_closing(mhd_bunch* b, int p0 = 0, int npl = -1) {
   const long long per = (long long)G.n[1] * G.n[2] + (long long)G.n[0] * G.n[2] + (long long)G.n[0] * G.n[1];
   const long long tot = per * npl;
   {
-    LaunchScope ls(b, KC_FILL);
+    LaunchScope ls(b, KC_CLOSING);
     k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr, p0, npl);
   }
   CUDA_TRY(cudaGetLastError());
@@ -299,22 +303,22 @@ bool step_gathers(const mhd_bunch* b) {
 }
 
 template <typename T> struct OnePassLaunch {
+  static int prepare(mhd_bunch*) { return MHD_OK; }
   static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true) { return MHD_EINVAL; }
 };
 template <> struct OnePassLaunch<float> {
   // one tile shape: patches [p0, p0+npl) of the bunch
   template <int TX, int TY>
-  static int launch(mhd_bunch* b, const double* dtp, int p0, int npl) {
+  static int launch(mhd_bunch* b, const double* dtp, int p0, int npl, bool attr_only = false) {
     using Cfg = OneCfg<float, TX, TY, OneTile::NPW>;
     const Geom& G = b->G;
     // limiter and flux solver are compile-time parameters of the kernel
     auto kern = G.flux_solver == 1
                     ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 1> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 1>)
                     : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 0> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 0>);
-    static bool attr_done[6] = {false, false, false, false, false, false};
-    if (!attr_done[G.limiter + 3 * G.flux_solver]) {
+    if (attr_only) {   // called once from create, on the handle's device (the attribute is per device)
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
-      attr_done[G.limiter + 3 * G.flux_solver] = true;
+      return MHD_OK;
     }
     Params<float> P = make_params<float>(b, p0, npl);
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
@@ -327,8 +331,7 @@ template <> struct OnePassLaunch<float> {
       const int zmax = G.n[2] / 8 > 1 ? G.n[2] / 8 : 1;
       if (zseg > zmax) zseg = zmax;
     }
-    const char* env_z = getenv("MHD_ONEPASS_ZSEG");   // tuning knob
-    if (env_z && atoi(env_z) >= 1) zseg = atoi(env_z) < G.n[2] ? atoi(env_z) : G.n[2];
+    if (b->tune_zseg >= 1) zseg = b->tune_zseg < G.n[2] ? b->tune_zseg : G.n[2];   // mhd_bunch_set_tuning
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
@@ -339,6 +342,9 @@ template <> struct OnePassLaunch<float> {
   }
   // patches [p0, p0+npl) of the bunch (npl < 0: all); `last` flips the buffers.  Rows of up to
   // 16 cells take the 16 x 16 tile (a 32-wide tile would leave half of every warp idle).
+  static int prepare(mhd_bunch* b) {
+    return b->G.n[0] <= 16 ? launch<16, 16>(b, nullptr, 0, 0, true) : launch<OneTile::TX, OneTile::TY>(b, nullptr, 0, 0, true);
+  }
   static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true) {
     if (npl < 0) npl = b->G.np;
     const int rc = b->G.n[0] <= 16 ? launch<16, 16>(b, dtp, p0, npl) : launch<OneTile::TX, OneTile::TY>(b, dtp, p0, npl);
@@ -351,21 +357,54 @@ template <> struct OnePassLaunch<float> {
   }
 };
 
+// dynamic shared memory opt-in of the fused kernels: per device, so done once per handle in create
+template <typename T>
+int prepare_fused() {
+  CUDA_TRY(cudaFuncSetAttribute(k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+  CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+  CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+  return MHD_OK;
+}
+
+// The deferred fill trusts that a patch's evolved closing face equals its neighbour's face 0 bit
+// for bit, and the gathered halos that what a patch sees across a side is what its neighbour
+// sees of itself.  Both hold when the table composes like translations: nbr[p][0] = p and
+// nbr[nbr[p][c1]][c2] = nbr[p][c1+c2] whenever c1+c2 is again one of the 27 classes.  Tables
+// with -1 entries never take those routes.
+bool table_is_consistent(const int32_t* nb, int np) {
+  for (int p = 0; p < np; ++p) {
+    const int32_t* tp = nb + (size_t)p * 27;
+    if (tp[13] != p) return false;
+    for (int c1 = 0; c1 < 27; ++c1) {
+      const int q = tp[c1];
+      if (q < 0) return false;
+      const int a[3] = {c1 % 3 - 1, (c1 / 3) % 3 - 1, c1 / 9 - 1};
+      for (int c2 = 0; c2 < 27; ++c2) {
+        const int e[3] = {a[0] + c2 % 3 - 1, a[1] + (c2 / 3) % 3 - 1, a[2] + c2 / 9 - 1};
+        if (e[0] < -1 || e[0] > 1 || e[1] < -1 || e[1] > 1 || e[2] < -1 || e[2] > 1) continue;
+        if (nb[(size_t)q * 27 + c2] != tp[(e[2] + 1) * 9 + (e[1] + 1) * 3 + (e[0] + 1)]) return false;
+      }
+    }
+  }
+  return true;
+}
+
+// every launching entry point runs on the handle's device, whatever the caller's current one is
+#define ENTER(b)                                                   \
+  do {                                                             \
+    if (!(b)) return MHD_ESTATE;                                   \
+    cudaError_t e_ = cudaSetDevice((b)->desc.device);              \
+    if (e_ != cudaSuccess) return fail_cuda(e_, "cudaSetDevice");  \
+  } while (0)
+
 // two-kernel path on patches [q0, q0+nq): sub-bunches of at most b->chunk patches (D block)
 template <typename T>
 int launch_fused_range(mhd_bunch* b, int q0, int nq) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
-  static bool attr_done[2] = {false, false};
-  if (!attr_done[sizeof(T) == 8]) {
-    CUDA_TRY(cudaFuncSetAttribute(k_riemann_update<T, FusedTile<T>::TX, FusedTile<T>::TY>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)FusedCfg<T, FusedTile<T>::TX, FusedTile<T>::TY>::smem));
-    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    CUDA_TRY(cudaFuncSetAttribute(k_predict_fused<T, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done[sizeof(T) == 8] = true;
-  }
   const int gather = (b->gather2_ok && b->guards_stale) ? 1 : 0;   // shell not in HBM: read through the table
   cudaStream_t st = b->stream;
   for (int p0 = q0; p0 < q0 + nq; p0 += b->chunk) {
@@ -572,7 +611,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
       const size_t left = avail - staged_bytes(b->G, b->esz, cs);
       long long c = (long long)(left / dblock_bytes(b->G, b->esz, 1));
       if (c > desc->npatch) c = desc->npatch;
-      if (c < 1) { delete b; return MHD_ENOMEM; }
+      if (c < 1) { delete b->events; delete b; return MHD_ENOMEM; }
       while (c < desc->npatch && dblock_bytes(b->G, b->esz, (int)c + 1) <= left) ++c;
       b->chunk = wave_aligned_chunk(b->G, (int)c);
     }
@@ -582,9 +621,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
     const bool f64 = desc->dtype == MHD_F64;
     b->DG = make_dgeom(b->G, b->esz, b->chunk);
     b->pred_ty = 0;
-    const char* env_ty = getenv("MHD_PREDICT_TY");   // tuning knob: force the predictor's y-tile
     for (int ty : {16, 8, 4}) {
-      if (env_ty && atoi(env_ty) != ty) continue;
       const size_t pa = (size_t)(b->G.n[0] + 5) * (ty + 5);
       if (pa <= (size_t)predict_max_threads(ty) && 39 * pa * b->esz <= (size_t)220 * 1024) { b->pred_ty = ty; break; }
     }
@@ -603,8 +640,10 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->all_nbr = true;
   for (long long c = 0; c < 27ll * desc->npatch && b->all_nbr; ++c)
     if (nbr[c] < 0) b->all_nbr = false;
-  b->gather_ok = b->gather_ok && b->all_nbr;
-  b->gather2_ok = b->fused_ok && b->all_nbr;
+  b->nbr_consistent = b->all_nbr && table_is_consistent(nbr, desc->npatch);
+  b->gather_ok = b->gather_ok && b->nbr_consistent;
+  b->gather2_ok = b->fused_ok && b->nbr_consistent;
+  b->tune_zseg = 0;
   b->hs = nullptr;
   b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
   if (!b->h_nbr) { delete b->events; delete b; return MHD_ENOMEM; }
@@ -613,13 +652,19 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   cudaError_t e = cudaMemcpyAsync(b->d_nbr, nbr, sizeof(int) * 27 * (size_t)desc->npatch, cudaMemcpyHostToDevice, b->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(b->d_bad, 0, 512, b->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
-  if (e != cudaSuccess) { delete b; return fail_cuda(e, "create: table upload"); }
+  if (e != cudaSuccess) { delete b->h_nbr; delete b->events; delete b; return fail_cuda(e, "create: table upload"); }
+  {  // dynamic shared memory opt-ins of the kernels this handle can launch, on ITS device
+    int ra = MHD_OK;
+    if (b->fused_ok) ra = desc->dtype == MHD_F64 ? prepare_fused<double>() : prepare_fused<float>();
+    if (ra == MHD_OK && b->onepass_ok) ra = OnePassLaunch<float>::prepare(b);
+    if (ra != MHD_OK) { delete b->h_nbr; delete b->events; delete b; return ra; }
+  }
   *out = b;
   return MHD_OK;
 }
 
 int mhd_bunch_fill_guards(mhd_bunch* b) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (step_gathers(b)) {
     // deferred: the one-pass step reads halos from the neighbours' interiors, so only the
     // closing faces are brought up to date now; the rest of the shell is written if and when
@@ -635,12 +680,12 @@ int mhd_bunch_fill_guards(mhd_bunch* b) {
 }
 
 int mhd_bunch_sync_guards(mhd_bunch* b) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   return materialise_guards(b);
 }
 
 int mhd_bunch_cfl_dt(mhd_bunch* b, double courant, double* dt_host, void* dt_dev, void* dt_per_patch_dev) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (!(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
   const int rc = b->desc.dtype == MHD_F64 ? launch_cfl<double>(b, courant, dt_dev, dt_per_patch_dev)
                                            : launch_cfl<float>(b, courant, dt_dev, dt_per_patch_dev);
@@ -657,14 +702,14 @@ static int step_common(mhd_bunch* b) {
 }
 
 int mhd_bunch_step(mhd_bunch* b, double dt) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (!(dt > 0.0) || !isfinite(dt)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0); }
   return step_common(b);
 }
 
 int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (!dt_dev || !(dt_max >= 0.0)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, (const double*)dt_dev, 0.0, dt_max); }
   return step_common(b);
@@ -672,6 +717,7 @@ int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
 
 int mhd_bunch_current(mhd_bunch* b, void** state) {
   if (!b || !state) return MHD_ESTATE;
+  ENTER(b);
   const int rc = materialise_guards(b);   // the caller is about to look at the buffer
   if (rc != MHD_OK) return rc;
   b->closing_ok = false;                  // ... and may write it
@@ -681,6 +727,7 @@ int mhd_bunch_current(mhd_bunch* b, void** state) {
 
 int mhd_bunch_status(mhd_bunch* b, int64_t* bad_cells) {
   if (!b || !bad_cells) return MHD_ESTATE;
+  ENTER(b);
   unsigned long long v = 0;
   CUDA_TRY(cudaMemcpyAsync(&v, b->d_bad, sizeof(v), cudaMemcpyDeviceToHost, b->stream));
   CUDA_TRY(cudaStreamSynchronize(b->stream));
@@ -695,7 +742,7 @@ int mhd_bunch_launch_count(mhd_bunch* b, int64_t* launches) {
 }
 
 int mhd_bunch_set_path(mhd_bunch* b, int32_t path) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (path < MHD_PATH_AUTO || path > MHD_PATH_ONEPASS) return MHD_EINVAL;
   if (path == MHD_PATH_ONEPASS && !b->onepass_ok) return MHD_EINVAL;
   if (path == MHD_PATH_TWO_KERNEL && !b->fused_ok) return MHD_EINVAL;
@@ -705,23 +752,41 @@ int mhd_bunch_set_path(mhd_bunch* b, int32_t path) {
   return MHD_OK;
 }
 
+int mhd_bunch_set_tuning(mhd_bunch* b, int32_t key, int32_t value) {
+  ENTER(b);
+  if (value < 0) return MHD_EINVAL;
+  if (key == MHD_TUNE_ONEPASS_ZSEG) {
+    b->tune_zseg = value;
+    return MHD_OK;
+  }
+  if (key == MHD_TUNE_PREDICT_TY) {
+    if (!b->fused_ok) return MHD_EINVAL;
+    if (value != 16 && value != 8 && value != 4) return MHD_EINVAL;
+    const size_t pa = (size_t)(b->G.n[0] + 5) * (value + 5);
+    if (!(pa <= (size_t)predict_max_threads(value) && 39 * pa * b->esz <= (size_t)220 * 1024)) return MHD_EINVAL;
+    b->pred_ty = value;
+    return MHD_OK;
+  }
+  return MHD_EINVAL;
+}
+
 int mhd_bunch_get_path(mhd_bunch* b, int32_t* path) {
   if (!b || !path) return MHD_ESTATE;
   *path = effective_path(b);
   return MHD_OK;
 }
 
-int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double* tflops) {
-  if (!tflops || (dtype != MHD_F32 && dtype != MHD_F64)) return MHD_EINVAL;
+int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, void* scratch_dev, size_t scratch_bytes, double* tflops) {
+  if (!tflops || !scratch_dev || (dtype != MHD_F32 && dtype != MHD_F64)) return MHD_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
     return fail_cuda(cudaErrorNoDevice, "no CUDA device");
   CUDA_TRY(cudaSetDevice(device));
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, device));
-  void* out = nullptr;
+  void* out = scratch_dev;
   const int blocks = prop.multiProcessorCount * 8, iters = 4096;
-  CUDA_TRY(cudaMalloc(&out, (size_t)blocks * 256 * 8));
+  if (scratch_bytes < (size_t)blocks * 256 * 8) return MHD_ENOMEM;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
   double best = 0.0;
@@ -737,7 +802,6 @@ int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, double* tflops) {
     if (ms > 0.f && rep > 0) best = fmax(best, fl / (ms * 1e-3) / 1e12);
   }
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(out);
   CUDA_TRY(cudaGetLastError());
   *tflops = best;
   return MHD_OK;
@@ -767,6 +831,7 @@ static void drain_events(mhd_bunch* b, bool accumulate) {
 
 int mhd_bunch_upload(mhd_bunch* b, const void* host_state) {
   if (!b || !host_state) return MHD_ESTATE;
+  ENTER(b);
   b->guards_stale = false;   // the whole buffer, guard shell included, is replaced
   b->closing_ok = false;
   CUDA_TRY(cudaMemcpyAsync(b->state[b->cur], host_state, b->lay.state_bytes, cudaMemcpyHostToDevice, b->stream));
@@ -775,6 +840,7 @@ int mhd_bunch_upload(mhd_bunch* b, const void* host_state) {
 
 int mhd_bunch_download(mhd_bunch* b, void* host_state) {
   if (!b || !host_state) return MHD_ESTATE;
+  ENTER(b);
   {
     const int rc = materialise_guards(b);
     if (rc != MHD_OK) return rc;
@@ -785,7 +851,7 @@ int mhd_bunch_download(mhd_bunch* b, void* host_state) {
 }
 
 int mhd_bunch_set_timing(mhd_bunch* b, int32_t enable) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   CUDA_TRY(cudaStreamSynchronize(b->stream));
   drain_events(b, false);
   for (int c = 0; c < 16; ++c) { b->cls_ms[c] = 0.0; b->cls_n[c] = 0; }
@@ -795,6 +861,7 @@ int mhd_bunch_set_timing(mhd_bunch* b, int32_t enable) {
 
 int mhd_bunch_kernel_times(mhd_bunch* b, int32_t cap, const char** names, double* ms, int64_t* count, int32_t* n) {
   if (!b || !n) return MHD_ESTATE;
+  ENTER(b);
   CUDA_TRY(cudaStreamSynchronize(b->stream));
   drain_events(b, true);
   int k = 0;
@@ -961,7 +1028,7 @@ int mhd_bunch_host_schedule(const int32_t* nbr, int32_t npatch, int32_t chunk_pa
 }
 
 int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes, int32_t chunk_patches) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   if (!staging_dev || ((uintptr_t)staging_dev & 15)) return MHD_EINVAL;
   if (!b->all_nbr) return MHD_EINVAL;   // the compact host layout has no room for evolved closing faces
   mhd_bunch_host_layout lay;
@@ -1001,9 +1068,25 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   return MHD_OK;
 }
 
+static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant,
+                          double* dt_used, double* dt_next);
+
 int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant,
                         double* dt_used, double* dt_next) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
+  const int rc = step_host_impl(b, host_in, host_out, dt, courant, dt_used, dt_next);
+  if (rc != MHD_OK && b->hs) {
+    // copies into / out of the caller's host buffers may still be in flight: drain them before
+    // the caller sees the error and reuses the buffers
+    cudaStreamSynchronize(b->stream);
+    if (b->hs->s_up) cudaStreamSynchronize(b->hs->s_up);
+    if (b->hs->s_dn) cudaStreamSynchronize(b->hs->s_dn);
+  }
+  return rc;
+}
+
+static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant,
+                          double* dt_used, double* dt_next) {
   mhd_bunch::HostStream* h = b->hs;
   if (!h) return MHD_ESTATE;
   if (!host_in || !host_out) return MHD_EINVAL;
@@ -1102,7 +1185,7 @@ int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, doubl
 }
 
 int mhd_bunch_host_detach(mhd_bunch* b) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   hs_release(b);
   return MHD_OK;
 }
@@ -1112,7 +1195,7 @@ int mhd_bunch_host_detach(mhd_bunch* b) {
 extern "C" {
 
 int mhd_bunch_destroy(mhd_bunch* b) {
-  if (!b) return MHD_ESTATE;
+  ENTER(b);
   cudaStreamSynchronize(b->stream);
   drain_events(b, false);
   hs_release(b);

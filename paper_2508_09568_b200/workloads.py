@@ -250,7 +250,12 @@ def _band_limited(rng, N, power, kmin=1, kmax=8, base=32):
     for sz, dz_ in ((slice(0, h), slice(0, h)), (slice(base - h + 1, base), slice(Nz - h + 1, Nz))):
         for sy, dy_ in ((slice(0, h), slice(0, h)), (slice(base - h + 1, base), slice(Ny - h + 1, Ny))):
             big[dz_, dy_, :h] = spec[sz, sy, :h]
-    f = np.fft.irfftn(big, s=(Nz, Ny, Nx), axes=(0, 1, 2)) * (Nz * Ny * Nx / base ** 3)
+    try:                       # the same pocketfft transform on all cores (bitwise the numpy result)
+        from scipy import fft as _sfft
+        f = _sfft.irfftn(big, s=(Nz, Ny, Nx), axes=(0, 1, 2), workers=-1)
+    except ImportError:
+        f = np.fft.irfftn(big, s=(Nz, Ny, Nx), axes=(0, 1, 2))
+    f *= (Nz * Ny * Nx / base ** 3)
     f -= f.mean()
     f /= f.std()
     return f

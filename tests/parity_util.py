@@ -10,18 +10,72 @@ GROUPS = [(0, 1), (1, 4), (4, 5), (5, 8)]      # rho; momentum; E; B
 TOL_STEP = {"f64": 1e-12, "f32": 2e-5}         # BASELINE.json north_star: per-cell relative error after one step
 TOL_TOTALS_F64 = 1e-12                         # conserved totals after N steps
 TOL_L1_F32 = 1e-4                              # L1 field norms after N steps
+# Regression bounds, a decade above what the kernels are observed to do (Q21):
+# the north_star tolerances leave two to four orders of headroom, these do not.
+TIGHT_STEP = {"f64": 2e-14, "f32": 2e-6}
+# Secondary metric of Q21: PURE relative error |g-o|/|o|, per component, over cells with
+# |o| > PURE_FLOOR * s_f, held to the same north_star tolerance.  (In fp32 the update U - dt*dF/dx
+# of a small component cancels fluxes of the group's magnitude, so this is the tighter of the two
+# statements there: observed 1.2e-5 at worst against 1.4e-7 for the scale-relative metric.)
+PURE_FLOOR = 1e-3
+TOL_PURE = {"f64": 1e-12, "f32": 2e-5}
 
 
 def rel_err(g, o):
-    """max over cells of |g-o| / max(|o|, s_f), s_f = max|o| of the field group (1 if 0)."""
+    """Q21, primary: max over cells of |g-o| / max(|o|, s_f), s_f = max|o| of the field group
+    (rho; momentum; E; B) over the bunch, 1 if the group is identically zero.  Since |o| <= s_f this
+    is the maximum-norm error of the group in units of its scale; the per-cell statement proper is
+    rel_err_pure."""
     worst = 0.0
     for a, b in GROUPS:
         s = np.abs(o[a:b]).max()
         s = s if s > 0 else 1.0
-        # compare at the scale of the group: a cell near zero is measured against s_f
         e = np.abs(g[a:b].astype(np.float64) - o[a:b]) / np.maximum(np.abs(o[a:b]), s)
         worst = max(worst, float(e.max()))
     return worst
+
+
+def rel_err_pure(g, o, floor=PURE_FLOOR):
+    """Q21, secondary: max over components f and cells with |o_f| > floor * s_f of |g_f-o_f|/|o_f|
+    (s_f = max|o| of the component's field group).  A cell at a thousandth of the scale that is
+    wrong by a percent fails this, which the primary metric alone would not notice."""
+    worst = 0.0
+    for a, b in GROUPS:
+        s = np.abs(o[a:b]).max()
+        if not s > 0:
+            continue
+        for f in range(a, b):
+            of = o[f]
+            m = np.abs(of) > floor * s
+            if m.any():
+                e = np.abs(g[f].astype(np.float64)[m] - of[m]) / np.abs(of[m])
+                worst = max(worst, float(e.max()))
+    return worst
+
+
+def assert_step_parity(g, o, dtype, what=(), tight=True):
+    """Both Q21 metrics of a stepped state against the oracle's, at the north_star tolerance and
+    (tight) at the regression bound; returns (primary, secondary)."""
+    e1, e2 = rel_err(g, o), rel_err_pure(g, o)
+    assert e1 <= (TIGHT_STEP if tight else TOL_STEP)[dtype], (what, dtype, "scale-relative", e1)
+    assert e2 <= TOL_PURE[dtype], (what, dtype, "pure relative", e2)
+    return e1, e2
+
+
+def assert_nstep_parity(g, o, dtype, what=()):
+    """north_star's N-step criteria on interior data [8, ...]: conserved totals of rho, m, E to 1e-12
+    relative in fp64, relative L1 norm of each field group to 1e-4 in fp32 (and in fp64, where it is
+    far smaller)."""
+    g = g.astype(np.float64)
+    ax = tuple(range(1, g.ndim))
+    tg, to = g[:5].sum(axis=ax), o[:5].sum(axis=ax)
+    msum = np.abs(o[1:4]).sum()
+    scale = np.array([abs(to[0]), msum, msum, msum, abs(to[4])])
+    if dtype == "f64":
+        assert np.all(np.abs(tg - to) <= TOL_TOTALS_F64 * scale), (what, (tg - to) / scale)
+    for a, b in GROUPS:
+        l1 = np.abs(g[a:b] - o[a:b]).sum() / max(np.abs(o[a:b]).sum(), 1e-300)
+        assert l1 <= TOL_L1_F32, (what, dtype, a, l1)
 
 
 def updated_mask(n, ng=3):
