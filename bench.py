@@ -1,14 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the bunch MHD update on B200 (cell-updates/s).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c3f64|small]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c3f64|c2f64|small|c4]
+                    [--sub c2f64,c3,c3f64 | --sub none]
     python bench.py --impl reference ...      # the CPU oracle on a bounded sample
 
 A step = one pass of the whole hot path over the bunch: fill_guards -> cfl_dt (dt stays
-on the device) -> step.  The default workload is BASELINE.json config 2 (512 patches of
-32^3, fp32, seeded turbulence-like field).  Prints ONE JSON line (see DESIGN.md,
-"Measurement").  Multi-GPU: the path does not shard (north_star: one GPU) -- under
-torchrun every rank runs an independent replica ("replicas only").
+on the device) -> step.  The headline workload is BASELINE.json config 2 (512 patches of
+32^3, fp32, seeded turbulence-like field); the metric is quoted "(fp32/fp64)", so the same
+JSON line carries sub-records for the config-2 shape in fp64 and for config 3 (4096 patches)
+in fp32 and fp64, each with its own value, roofline fraction and end-to-end number.
+`--workload c4` runs BASELINE.json's bunching sweep instead.  Prints ONE JSON line (see
+DESIGN.md, "Measurement").  Multi-GPU: the path does not shard (north_star: one GPU) --
+under torchrun every rank runs an independent replica ("replicas only").
 """
 import argparse
 import json
@@ -36,8 +40,10 @@ WORKLOADS = {
     "c2f64": (256, 32, "f64", "config2 shape in fp64: 512 patches x 32^3"),
     "small": (64, 32, "f32", "8 patches x 32^3, fp32 (smoke size)"),
 }
-# the CPU oracle's bounded sample: the same seeded field construction on 64^3 cells
-SAMPLE_N = 64
+# the CPU oracle's bounded samples: the same seeded field construction on a cut of the cube
+SAMPLE_1 = (64, 64, 64)          # 8 patches of 32^3, single thread
+SAMPLE_ALL = (128, 128, 64)      # 32 patches of 32^3, OpenMP over patches on all host cores
+TRAFFIC_FILE = os.path.join("profiles", "r2_ncu_traffic.txt")
 
 
 def peaks():
@@ -65,10 +71,12 @@ def algorithmic_work(cls, n, ng=3):
     table = {
         # class: (values per cell, flops per cell, bound)
         "fill_guards": (2 * 8 * (r(ng, ng) - 1.0), 0.0, "hbm"),
+        "sync_closing_faces": (2 * 3 / n, 0.0, "hbm"),
         "cfl": (8 + 3 / n, CFL_FLOPS, "hbm"),
         "predict": (8 * r(2, 3) + 38 * r(1, 1), STEP_FLOPS_32 - riemann_flops, "hbm"),
         "riemann_update": (38 * r(1, 1) + 8 + 8, riemann_flops, "alu"),
         "step_onepass": (8 * r(2, 3) + 8, STEP_FLOPS_32, "alu"),
+        "step_onepass_cfl": (8 * r(2, 3) + 8, STEP_FLOPS_32 + CFL_FLOPS, "alu"),
         # staged path (general, collapsed dimensions)
         "prim": (8 * r(2, 3) + 8 * r(2, 2), 40.0, "hbm"),
         "emf0": ((3 + 3) * r(2, 2) + 3 * r(1, 2), 70.0, "hbm"),
@@ -80,10 +88,10 @@ def algorithmic_work(cls, n, ng=3):
 
 
 def ncu_traffic(workload, cls):
-    """DRAM bytes per launch of a kernel class from the committed ncu capture, or None."""
-    path = os.path.join(ROOT, "profiles", "r1_ncu_traffic.txt")
+    """DRAM bytes per launch of a kernel class from the committed ncu capture of this round
+    (a cross-reference, not something this run measured), or None."""
     try:
-        return json.load(open(path)).get(workload, {}).get(cls)
+        return json.load(open(os.path.join(ROOT, TRAFFIC_FILE))).get(workload, {}).get(cls)
     except Exception:
         return None
 
@@ -134,12 +142,18 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def run_oracle_sample(steps, warmup):
-    """The oracle as it stands on the bounded sample; returns (cell-updates/s, seconds, description)."""
+def run_oracle_sample(steps, warmup, all_cores=False):
+    """The oracle as it stands on a bounded sample; returns dict(value, seconds, cores, sample).
+    all_cores: the same source built with -fopenmp (`parallel for` over patches, patches being
+    independent between guard fills) on every host core."""
     import oracle
-    w = W.turbulence(N=SAMPLE_N, n=32, dtype=np.float32, config=2)
-    o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx)
+    N = SAMPLE_ALL if all_cores else SAMPLE_1
+    w = W.turbulence(N=N, n=32, dtype=np.float32, config=2)
+    key = "f64_omp" if all_cores else "f64"
+    cores = oracle.threads(os.cpu_count() or 1) if all_cores else 1
+    o = oracle.Oracle(w.n, w.npatch, w.gamma, w.dx, dtype=key)
     U = w.U.astype(np.float64)
+
     def one(U):
         o.fill_guards(U, w.nbr)
         dt = o.cfl_dt(U, 0.4)
@@ -151,64 +165,31 @@ def run_oracle_sample(steps, warmup):
         U = one(U)
     el = time.perf_counter() - t0
     assert np.isfinite(U).all()
-    desc = (f"config-2 field construction on {SAMPLE_N}^3 cells = {w.npatch} patches x 32^3, fp64 oracle, "
-            f"fill+cfl+step, {steps} steps, single thread")
-    return w.cells * steps / el, el, desc
+    desc = (f"config-2 field construction on {N[0]}x{N[1]}x{N[2]} cells = {w.npatch} patches x 32^3, fp64 oracle, "
+            f"fill+cfl+step, {steps} steps after {warmup} warm-up, " +
+            (f"OpenMP over patches on {cores} threads (nproc = {os.cpu_count()})" if all_cores else "single thread"))
+    return {"value": w.cells * steps / el, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": el}
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
-    ap.add_argument("--cpu-steps", type=int, default=20, help="oracle steps for the cpu_baseline leg")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--host-chunk", type=int, default=0, help="patches per chunk of the host-streaming path (0: library default)")
-    ap.add_argument("--path", default="auto", choices=["auto", "staged", "two_kernel", "onepass"],
-                    help="which CUDA implementation of the step runs (include/mhd_bunch.h, MHD_PATH_*)")
-    args = ap.parse_args()
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    N, n, dtype, wdesc = WORKLOADS[args.workload]
-
-    # ---------------------------------------------------------------- reference arm ----
-    if args.impl == "reference":
-        if rank != 0:
-            return 0
-        steps = max(1, args.steps)
-        val, el, desc = run_oracle_sample(steps, max(0, min(args.warmup, 2)))
-        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-                "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": wdesc, "sample": desc},
-                "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
-                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-                "gpu_launches": 0}
-        print(json.dumps(line))
-        return 0
-
-    # --------------------------------------------------------------------- our arm ----
+# ------------------------------------------------------------------- one workload ----
+def measure(name, args, local, world, rank, field_cache, headline):
+    """Resident loop, per-class times with rooflines, and the end-to-end host-buffer loop of one
+    workload.  Returns the record (dict)."""
     import torch
     import torch.distributed as dist
-    from paper_2508_09568_b200.binding import MhdBunch
-
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    w = W.turbulence(N=N, n=n, dtype=np.float32 if dtype == "f32" else np.float64, config=2)
+    from paper_2508_09568_b200.binding import MhdBunch, measure_alu_peak
+    N, n, dtype, wdesc = WORKLOADS[name]
+    npd = np.float32 if dtype == "f32" else np.float64
+    if N not in field_cache:                       # the fp64 field serves both types (same values as a direct build)
+        field_cache.clear()
+        field_cache[N] = W.turbulence(N=N, n=n, dtype=np.float64, config=2)
+    w = field_cache[N]
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, device=local)
-    b.load(w.U)
+    b.load(w.U if dtype == "f64" else w.U.astype(np.float32))
     b.set_path(args.path)
     stream = b.stream
     courant = 0.4
+    steps = args.steps if headline else max(3, min(args.steps, args.sub_steps))
 
     def one_step():
         b.fill_guards()
@@ -227,7 +208,8 @@ def main():
         I = v[:, :, g[2]:g[2] + w.n[2], g[1]:g[1] + w.n[1], g[0]:g[0] + w.n[0]]
         return float(I[0].sum(dtype=torch.float64)), float(I[4].sum(dtype=torch.float64))
 
-    for _ in range(max(3, args.warmup)):
+    warm = max(3, args.warmup)
+    for _ in range(warm):
         one_step()
     barrier()
     tot0 = totals()
@@ -240,7 +222,7 @@ def main():
     barrier()
     with torch.cuda.stream(stream):
         ev0.record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             one_step()
         ev1.record(stream)
     barrier()
@@ -251,18 +233,18 @@ def main():
     tot1 = totals()
     conservation = {"mass_rel_drift": abs(tot1[0] - tot0[0]) / abs(tot0[0]), "energy_rel_drift": abs(tot1[1] - tot0[1]) / abs(tot0[1]),
                     "note": "interior totals before/after the timed steps (periodic bunch: conserved up to round-off)"}
-    value, ms = aggregate_over_ranks(ms, w.cells, args.steps, world, device="cuda")
+    value, ms = aggregate_over_ranks(ms, w.cells, steps, world, device="cuda")
 
     # ---- per-kernel-class device times (separate pass, events around every launch) ----
+    b.fill_guards()
     b.set_timing(True)
-    tsteps = min(args.steps, 10)
+    tsteps = min(steps, 10)
     for _ in range(tsteps):
         one_step()
     kt = b.kernel_times()
     b.set_timing(False)
     pk = peaks()
     esz = 4 if dtype == "f32" else 8
-    from paper_2508_09568_b200.binding import measure_alu_peak
     alu_peak = measure_alu_peak(dtype, local)               # TFLOP/s, FMA-chain, measured now
     alu_nominal = 148 * (128 if dtype == "f32" else 64) * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
     classes = {k: {"ms_per_step": v[0] / tsteps, "launches_per_step": v[1] / tsteps} for k, v in kt.items()}
@@ -270,7 +252,9 @@ def main():
     for k, c in classes.items():
         c["share"] = c["ms_per_step"] / tot
         a = algorithmic_work(k, n)
-        if a:
+        # a class that does not run every step (e.g. the closing-face sync after the caller looked at the
+        # buffer) has no per-step rate: no fraction is printed for it
+        if a and c["launches_per_step"] >= 1.0:
             c["bound"] = a[2]
             c["alg_bytes_per_cell"] = a[0] * esz
             c["alg_flops_per_cell"] = a[1]
@@ -290,7 +274,7 @@ def main():
         roofline = {"kernel": dom, "bound": "hbm", "achieved": dc.get("alg_gbs"), "peak": pk["hbm_gbs"], "unit": "GB/s",
                     "frac": dc.get("hbm_frac"), "peak_source": pk["source"],
                     "alg_bytes_per_launch": dc.get("alg_bytes_per_cell", 0) * w.cells / dc["launches_per_step"]}
-    roofline.update({"traffic": ncu_traffic(args.workload, dom), "avg_launch_ms": per_launch_ms,
+    roofline.update({"traffic": ncu_traffic(name, dom), "traffic_source": TRAFFIC_FILE, "avg_launch_ms": per_launch_ms,
                      "share_of_step": dc["share"], "hbm_frac": dc.get("hbm_frac"), "alu_frac": dc.get("alu_frac")})
     # whole-pass view: counted flops of step + cfl, compulsory traffic of a fully fused step
     pass_flops = STEP_FLOPS_32 + CFL_FLOPS
@@ -311,7 +295,7 @@ def main():
         hin = torch.from_numpy(W.to_compact(cur, w.n)).pin_memory()
         hout = torch.empty_like(hin).pin_memory()
         del cur
-        esteps = max(2, min(args.steps, 10))
+        esteps = max(2, min(steps, 10))
         _, dt_next = b.step_host(hin, hout, dt=0.0, courant=courant)      # warm-up, and the first dt
         hin, hout = hout, hin
         barrier()
@@ -330,24 +314,200 @@ def main():
                "chunk_patches": int(hl.chunk_patches), "chunks": int(hl.nchunk), "overlapped": bool(hl.pipelined),
                "note": "mhd_bunch_step_host: compact host state (interiors only) uploaded from pinned memory, "
                        "stepped and downloaded every step in chunks on two copy streams; wall clock"}
+        del hin, hout
+    rec = {"workload": name, "value": value, "unit": UNIT, "steps": steps, "warmup": warm, "ms_per_step": ms / steps,
+           "dtype": dtype,
+           "config": {"workload": wdesc, "patches": w.npatch, "patch": [n, n, n], "guard": 3, "courant": courant,
+                      "chunk_patches": b.chunk, "step_path": b.path,
+                      "parallelism": "replicas only" if world > 1 else "single GPU",
+                      "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (b.lay.state_bytes / 1e6)},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "bad_cells": bad, "conservation": conservation,
+           "roofline": roofline, "step_roofline": step_view, "kernel_classes": classes}
+    b.close()
+    del b
+    torch.cuda.empty_cache()
+    return rec
 
-    # ---- the oracle beside it (rank 0, N=1 only) ---------------------------------------
-    cpu = None
+
+# ---------------------------------------------------------------- config 4: the sweep ----
+ARRANGE = {1: (1, 1, 1), 8: (2, 2, 2), 64: (4, 4, 4), 300: (5, 6, 10), 512: (8, 8, 8), 4096: (16, 16, 16)}
+
+
+def replicated_bunch(n, P, dtype, device, max_side=256):
+    """A periodic bunch of P patches whose global field would be too large to build on the host:
+    the seeded field is built on a block of at most max_side cells per side and repeated
+    periodically ON THE DEVICE (patch (px,py,pz) holds block patch (px mod Bx, ...)), which is again
+    a periodic field.  Returns (MhdBunch, Workload of the block, block arrangement)."""
+    import torch
+    from paper_2508_09568_b200.binding import MhdBunch
+    B = tuple(min(p, max(1, max_side // n)) for p in P)
+    wb = W.turbulence(N=tuple(n * k for k in B), n=n, dtype=np.float32 if dtype == "f32" else np.float64, config=2, patches=B)
+    nbr = W.neighbour_table(P, (True, True, True))
+    npatch = P[0] * P[1] * P[2]
+    dx = tuple(1.0 / (n * max(P)) for _ in range(3))
+    b = MhdBunch(wb.n, npatch, nbr, wb.gamma, dx, dtype=dtype, device=device, workspace_bytes=1 << 30)
+    src = torch.from_numpy(wb.U).to(b.device)                 # [8, block patches, mz, my, mx]
+    v = b.view()
+    ids = np.arange(npatch)
+    px, py, pz = ids % P[0], (ids // P[0]) % P[1], ids // (P[0] * P[1])
+    img = (px % B[0]) + B[0] * ((py % B[1]) + B[1] * (pz % B[2]))
+    for q in range(B[0] * B[1] * B[2]):
+        sel = torch.from_numpy(ids[img == q]).to(b.device)
+        for f in range(8):                                    # field by field: no large temporaries
+            v[f].index_copy_(0, sel, src[f, q].unsqueeze(0).expand(len(sel), -1, -1, -1))
+    b.stream.synchronize()
+    return b, wb, B
+
+
+def sweep(args, local):
+    """BASELINE.json config 4: patch sizes x bunch sizes, fp32, config-2 field construction; per
+    point the resident loop's rate, device-busy time (events around every launch) and the
+    launch-overhead share 1 - busy/wall."""
+    import torch
+    from paper_2508_09568_b200.binding import MhdBunch
+    sizes = [int(x) for x in args.sizes.split(",")]
+    bunches = [int(x) for x in args.bunches.split(",")]
+    pts = [(n, k) for n in sizes for k in bunches] + ([(24, 300)] if 24 in sizes else [])
+    out = []
+    for n, k in pts:
+        P = ARRANGE[k]
+        N = tuple(n * p for p in P)
+        rec = {"patch": n, "bunch": k, "cells": k * n ** 3}
+        try:
+            if max(N) > 512:
+                b, wb, B = replicated_bunch(n, P, "f32", local)
+                rec["field"] = "block of %dx%dx%d patches repeated periodically on the device" % B
+            else:
+                w = W.turbulence(N=N, n=n, dtype=np.float32, config=2, patches=P)
+                b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype="f32", device=local)
+                b.load(w.U)
+        except Exception as e:
+            rec["skipped"] = str(e).splitlines()[0][:100]
+            out.append(rec)
+            continue
+
+        def one():
+            b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+        steps = max(3, min(args.steps, 20))
+        for _ in range(3):
+            one()
+        torch.cuda.synchronize()
+        l0 = b.launches
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            one()
+        torch.cuda.synchronize()
+        wall = (time.perf_counter() - t0) / steps
+        launches = (b.launches - l0) / steps
+        b.set_timing(True)
+        for _ in range(steps):
+            one()
+        kt = b.kernel_times()
+        b.set_timing(False)
+        busy = sum(v[0] for v in kt.values()) * 1e-3 / steps
+        rec.update({"step_path": b.path, "launches_per_step": launches, "wall_us": wall * 1e6, "busy_us": busy * 1e6,
+                    "value": rec["cells"] / wall, "launch_overhead_share": max(0.0, 1.0 - busy / wall), "bad_cells": b.status()})
+        b.close()
+        del b
+        torch.cuda.empty_cache()
+        out.append(rec)
+        print(json.dumps(rec), file=sys.stderr, flush=True)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS) + ["c4"])
+    ap.add_argument("--sub", default="c2f64,c3,c3f64",
+                    help="sub-records added to the default (c2) line: comma list of workloads, or 'none'")
+    ap.add_argument("--sub-steps", type=int, default=20, help="timed steps of each sub-record")
+    ap.add_argument("--cpu-steps", type=int, default=20, help="oracle steps for the cpu_baseline legs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--host-chunk", type=int, default=0, help="patches per chunk of the host-streaming path (0: library default)")
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "two_kernel", "onepass"],
+                    help="which CUDA implementation of the step runs (include/mhd_bunch.h, MHD_PATH_*)")
+    ap.add_argument("--sizes", default="16,24,32,64", help="c4: patch sizes")
+    ap.add_argument("--bunches", default="1,8,64,512,4096", help="c4: bunch sizes")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    # ---------------------------------------------------------------- reference arm ----
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        steps = max(1, args.steps)
+        warm = max(0, min(args.warmup, 2))          # the oracle has no caches to warm: two steps at most
+        r = run_oracle_sample(steps, warm)
+        wdesc = WORKLOADS[args.workload if args.workload in WORKLOADS else "c2"][3]
+        line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+                "warmup": warm, "ms_per_step": 1e3 * r["seconds"] / steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": wdesc, "sample": r["sample"]},
+                "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+                "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    # --------------------------------------------------------------------- our arm ----
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    if args.workload == "c4":
+        pts = sweep(args, local) if rank == 0 else []
+        if rank == 0:
+            best = max((p for p in pts if "value" in p), key=lambda p: p["value"])
+            print(json.dumps({"metric": METRIC, "value": best["value"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                              "warmup": 3, "ms_per_step": best["wall_us"] / 1e3, "higher_is_better": True, "scaling": "weak",
+                              "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                              "config": {"workload": "config4: bunching sweep, value = best point", "best": [best["patch"], best["bunch"]]},
+                              "sweep": pts}))
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    field_cache = {}
+    head = measure(args.workload, args, local, world, rank, field_cache, headline=True)
+    subs = []
+    if args.workload == "c2" and args.sub != "none":
+        for name in [s for s in args.sub.split(",") if s]:
+            try:
+                r = measure(name, args, local, world, rank, field_cache, headline=False)
+                subs.append({k: r[k] for k in ("workload", "dtype", "value", "unit", "steps", "ms_per_step", "config", "e2e",
+                                               "gpu_launches", "bad_cells", "roofline", "step_roofline", "kernel_classes")})
+            except Exception as e:                       # a sub-record must never cost the headline
+                subs.append({"workload": name, "error": str(e).splitlines()[0][:200]})
+    field_cache.clear()
+
+    # ---- the oracle beside it (rank 0, N=1 only): one thread, and all host cores --------
+    cpu = cpu_all = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        val, el, desc = run_oracle_sample(args.cpu_steps, 1)
-        cpu = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": el}
+        cpu = run_oracle_sample(args.cpu_steps, 1)
+        cpu_all = run_oracle_sample(args.cpu_steps, 1, all_cores=True)
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
-                "config": {"workload": wdesc, "patches": w.npatch, "patch": [n, n, n], "guard": 3, "courant": courant,
-                           "chunk_patches": b.chunk, "step_path": b.path, "parallelism": "replicas only" if world > 1 else "single GPU",
-                           "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (b.lay.state_bytes / 1e6)},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "bad_cells": bad, "conservation": conservation,
-                "roofline": roofline, "step_roofline": step_view, "kernel_classes": classes, "cpu_baseline": cpu}
+        line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": head["steps"],
+                "warmup": head["warmup"], "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic",
+                "config": head["config"], "clocks": head["clocks"], "e2e": head["e2e"], "gpu_launches": head["gpu_launches"],
+                "bad_cells": head["bad_cells"], "conservation": head["conservation"], "roofline": head["roofline"],
+                "step_roofline": head["step_roofline"], "kernel_classes": head["kernel_classes"],
+                "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "sub_records": subs}
         print(json.dumps(line))
-    b.close()
     if world > 1:
         dist.destroy_process_group()
     return 0

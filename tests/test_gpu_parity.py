@@ -619,3 +619,53 @@ def test_config3_full_size_sampled_patches_and_invariants(dtype):
     brms = np.sqrt(np.mean(g1[5].astype(np.float64) ** 2 + g1[6].astype(np.float64) ** 2 + g1[7].astype(np.float64) ** 2))
     assert np.abs(div).max() / brms <= (1e-12 if dtype == "f64" else 1e-4)
     b.close()
+
+
+# ------------------------------------- config 4's largest point: 64-bit offsets -------
+def test_config4_corner_4096_patches_of_64_cubed():
+    """BASELINE.json config 4's largest point, 4096 patches of 64^3 in fp32: 11.6 G elements per
+    state buffer, the only case whose element offsets exceed 2^31 (and 2^32).  The global field
+    (1024^3 cells) is not built on the host: the seeded field of a 256^3 block (4 x 4 x 4 patches)
+    is repeated periodically on the device, which is again a periodic field.  Checks: sampled
+    patches from the low, middle and high end of the buffer against the oracle (one step), and
+    every patch bit for bit equal to its periodic image among the 64 patches of the block -- an
+    offset that wrapped anywhere would break one of them."""
+    import importlib.util
+    import os
+    import oracle
+    import torch
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    free, _ = torch.cuda.mem_get_info()
+    if free < 110 * 2 ** 30:
+        pytest.skip("needs 2 x 46 GB of device memory")
+    n, P = 64, (16, 16, 16)
+    b, wb, B = bench.replicated_bunch(n, P, "f32", 0)
+    assert b.lay.state_elems > 2 ** 33 and b.path == "onepass"
+    b.fill_guards()
+    dt = b.cfl_dt(0.4, sync=True)
+    # the oracle on the block with the bunch's cell size: same field, same step
+    ob = oracle.Oracle(wb.n, wb.npatch, wb.gamma, b.desc.dx[:])
+    Ub = ob.fill_guards(wb.U.astype(np.float64), wb.nbr)
+    dt_ref = ob.cfl_dt(Ub, 0.4)
+    assert abs(dt - dt_ref) <= 2e-6 * dt_ref
+    b.step(dt_ref)
+    assert b.status() == 0
+    v = b.view()                                                  # the new level, on the device
+    ids = np.arange(4096)
+    px, py, pz = ids % 16, (ids // 16) % 16, ids // 256
+    img = (px % B[0]) + B[0] * ((py % B[1]) + B[1] * (pz % B[2]))
+    sample = [0, 1911, 4095]
+    simg = [int(img[p]) for p in sample]
+    osub = oracle.Oracle(wb.n, len(sample), wb.gamma, b.desc.dx[:])
+    ref = osub.step(np.ascontiguousarray(Ub[:, simg]), dt_ref)
+    got = v[:, sample].cpu().numpy()
+    assert_step_parity(masked(got, wb.n), masked(ref, wb.n), "f32", "64^3 x 4096")
+    I = (slice(3, 3 + n),) * 3
+    for q in range(64):
+        same = torch.from_numpy(ids[img == q]).to(v.device)
+        first = v[:, int(same[0])][(slice(None),) + I]
+        for p in same[1:].tolist():
+            assert torch.equal(v[:, p][(slice(None),) + I], first), (q, p)
+    b.close()
