@@ -23,7 +23,8 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return TARGET
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, *SOURCES, "-o", TARGET + ".tmp"]
+    extra = os.environ.get("MHD_BUNCH_NVCC_FLAGS", "").split()      # build-time knobs (e.g. -DONEPASS_NPW=4)
+    cmd = [nvcc, *NVCC_FLAGS, *extra, *SOURCES, "-o", TARGET + ".tmp"]
     r = subprocess.run(cmd, capture_output=True, text=True, cwd=HERE)
     log = r.stdout + r.stderr
     with open(os.path.join(HERE, "build.log"), "w") as fh:

@@ -43,7 +43,7 @@ template <> struct FusedTile<float> { static constexpr int TX = 32, TY = 8; };
 template <> struct FusedTile<double> { static constexpr int TX = 16, TY = FUSED_F64_TY; };
 // one-pass kernel (onepass_kernel.cuh): tile and number of predictor warps
 #ifndef ONEPASS_NPW
-#define ONEPASS_NPW 6
+#define ONEPASS_NPW 7
 #endif
 struct OneTile { static constexpr int TX = 32, TY = 8, NPW = ONEPASS_NPW; };
 

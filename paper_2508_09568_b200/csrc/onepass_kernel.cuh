@@ -32,43 +32,82 @@
 
 namespace mhd {
 
-__device__ __forceinline__ void nb_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+// Named barriers.  bar.sync / bar.arrive are the .aligned forms: they ASSERT that the whole warp
+// executes them together, and ptxas uses that assertion -- it may place the reconvergence point of
+// a preceding divergent `if` after the barrier and drop a __syncwarp() in front of it as redundant,
+// so that a warp whose lanes took different sides arrives twice (seen in SASS; the barrier count
+// then drifts and the CTA hangs).  Hence: the non-aligned forms, which assert nothing, behind a
+// __syncwarp() that makes the warp whole; and the predictor passes keep their lanes together
+// (tasks are clamped, not skipped, inside a partly filled warp).  Every call site is reached by
+// all non-exited lanes of its warp.
+__device__ __forceinline__ void nb_sync(int id, int n) {
+  __syncwarp();
+  asm volatile("barrier.sync %0, %1;" ::"r"(id), "r"(n) : "memory");
+}
+__device__ __forceinline__ void nb_arrive(int id, int n) {
+  __syncwarp();
+  asm volatile("barrier.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
+}
 // 16-byte asynchronous copy global -> shared (L2 only), and the wait for all of a thread's copies
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// two consecutive elements moved by one 8-byte (float) or 16-byte (double) shared-memory access
+template <typename T> struct Pair;
+template <> struct Pair<float> { using V = float2; };
+template <> struct Pair<double> { using V = double2; };
+template <typename T> struct V2 { T a, b; };
+template <typename T> __device__ __forceinline__ V2<T> ld2(const T* p) {
+  const typename Pair<T>::V v = *reinterpret_cast<const typename Pair<T>::V*>(p);
+  return V2<T>{v.x, v.y};
+}
+template <typename T> __device__ __forceinline__ void st2(T* p, T a, T b) {
+  typename Pair<T>::V v;
+  v.x = a; v.y = b;
+  *reinterpret_cast<typename Pair<T>::V*>(p) = v;
+}
+
+// Geometry of a tile.  Every plane array of the predictor (raw U^n, primitives, time-n EMFs) has
+// PH rows of BWX columns; column rc holds cell x0-4+rc (so that 16-byte chunks of a state row land
+// on 16-byte boundaries), row pr holds y0-2+pr.  Predictor threads work on STRIPS of two
+// consecutive columns (rc = 2s, 2s+1; 8/16-byte shared accesses, x-differences shared between the
+// two cells).  The D arrays handed to the solver roles hold cells rc = 3..TX+4 (x0-1..x0+TX),
+// rows dr = pr-1 = 0..TY+1, at index dr*DP + rc with DP = TX+4: columns 0..2 of a row are unused,
+// and the strip stores that overhang the row on either side (rc = 2, rc = TX+5) fall into those
+// unused slots of this row and the next one.
 template <typename T, int TX, int TY, int NPW> struct OneCfg {
-  static constexpr int PW = TX + 5, PH = TY + 5, PA = PW * PH;     // predictor positions: cells x0-2.., y0-2..
-  static constexpr int BWX = TX + 8, RA = BWX * PH;                // raw box: columns x0-4.. (16-byte aligned start)
-  static constexpr int DW = TX + 2, DH = TY + 2, DC = DW * DH;     // D cells: x0-1.., y0-1..
+  static constexpr int PH = TY + 5;
+  static constexpr int BWX = TX + 8, RA = BWX * PH;
+  static constexpr int DP = TX + 4, DH = TY + 2, DCS = DH * DP + 4;   // D arrays: row pitch, rows, elements per array
   static constexpr int FW = TX + 1, FH = TY + 1, FA = FW * FH;     // faces / edges
   static constexpr int CB = ((TX * FH + 31) / 32) * 32;            // first thread of the closing-column warp
   static constexpr int NR = CB + 32;                               // threads of role A and of role C
   static constexpr int NP = NPW * 32;                              // threads of role P
   static constexpr int NTH = 2 * NR + NP;
   static constexpr int NALL = NTH;
-  // compact index spaces of the predictor passes: primitives on columns 0..PW-2 and rows
-  // 0..PH-2, edge EMFs on columns 1..PW-2 and rows 1..PH-2, D cells
-  static constexpr int W1 = PW - 1, N1 = W1 * (PH - 1), W2 = PW - 2, N2 = W2 * (PH - 2);
-  static constexpr int PASS1 = (N1 + NP - 1) / NP, PASS2 = (N2 + NP - 1) / NP, PASS3 = (DC + NP - 1) / NP;
-  static_assert(FH <= 32 && 32 % TX == 0, "tile shape");
+  // strips s = 1..NS cover rc = 2..TX+5; tasks of the three predictor passes: primitives on rows
+  // 0..PH-2, edge EMFs on rows 1..PH-2, D cells on rows 1..PH-3
+  static constexpr int NS = (TX + 4) / 2;
+  static constexpr int NT1 = NS * (PH - 1), NT2 = NS * (PH - 2), NT3 = NS * (PH - 3);
+  static constexpr int PASS1 = (NT1 + NP - 1) / NP, PASS2 = (NT2 + NP - 1) / NP, PASS3 = (NT3 + NP - 1) / NP;
+  static_assert(FH <= 32 && 32 % TX == 0 && TX % 4 == 0, "tile shape");
   static constexpr size_t al(size_t x) { return (x + 127) / 128 * 128; }
   // shared-memory map (bytes)
   static constexpr size_t rawh_slot = al(sizeof(T) * 5 * RA), rawb_slot = al(sizeof(T) * 3 * RA);
-  static constexpr size_t o_rawh = 0;                                  // [2] hydro planes (TMA destinations)
-  static constexpr size_t o_rawb = o_rawh + 2 * rawh_slot;             // [4] field planes (TMA destinations)
-  static constexpr size_t o_d = o_rawb + 4 * rawb_slot;                // [2][38][DC]
-  static constexpr size_t o_q = o_d + al(sizeof(T) * 2 * D_COUNT * DC);   // [3][8][PA]
-  static constexpr size_t o_e = o_q + al(sizeof(T) * 3 * 8 * PA);      // [2][3][PA]
-  static constexpr size_t o_pu = o_e + al(sizeof(T) * 2 * 3 * PA);     // [7][FA]   C -> A partial update
+  static constexpr size_t o_rawh = 0;                                  // [1] hydro plane (cp.async destination)
+  static constexpr size_t o_rawb = o_rawh + rawh_slot;                 // [4] field planes (cp.async destinations)
+  static constexpr size_t o_d = o_rawb + 4 * rawb_slot;                // [2][38][DCS]
+  static constexpr size_t o_q = o_d + al(sizeof(T) * 2 * D_COUNT * DCS);  // [3][8][RA]
+  static constexpr size_t o_e = o_q + al(sizeof(T) * 3 * 8 * RA);      // [2][3][RA]
+  static constexpr size_t o_pu = o_e + al(sizeof(T) * 2 * 3 * RA);     // [7][FA]   C -> A partial update
   static constexpr size_t o_xe = o_pu + al(sizeof(T) * 7 * FA);        // [2][NR]   A: ex, ey of the neighbours
   static constexpr size_t o_xy = o_xe + al(sizeof(T) * 2 * NR);        // [6][NR]   C: +y exchange
   static constexpr size_t o_xc = o_xy + al(sizeof(T) * 6 * NR);        // [6][32]   C: closing column -> column TX-1
   static constexpr size_t o_nb = o_xc + al(sizeof(T) * 6 * 32);        // [27] source patch per neighbour class
   static constexpr size_t smem = o_nb + 128;
+  static_assert(smem <= 227 * 1024, "shared memory of one CTA");
   static constexpr int VEC = 16 / sizeof(T), CPR = BWX / VEC;          // elements per 16-byte copy, copies per row
   static_assert(BWX % VEC == 0, "raw rows are whole 16-byte chunks");
 };
@@ -78,29 +117,29 @@ enum : int { NB_FULL = 1, NB_EMPTY = 3, NB_PUF = 5, NB_PUE = 6, NB_P = 7, NB_A =
 
 // face state of cell c along D: q^h + s*dq  (s = +1/2: upper face, left state of the next
 // face; s = -1/2: lower face, right state) -- O5
-template <typename T, int DC, int D>
+template <typename T, int DCS, int D>
 __device__ __forceinline__ State1D<T> face_state(const T* __restrict__ c, T s) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
   State1D<T> q;
-  q.rho = c[(D_QH + 0) * DC] + s * c[dq_slot(D, 0) * DC];
-  q.u = c[(D_QH + 1 + D) * DC] + s * c[dq_slot(D, 1 + D) * DC];
-  q.v = c[(D_QH + 1 + T1) * DC] + s * c[dq_slot(D, 1 + T1) * DC];
-  q.w = c[(D_QH + 1 + T2) * DC] + s * c[dq_slot(D, 1 + T2) * DC];
-  q.p = c[(D_QH + 4) * DC] + s * c[dq_slot(D, 4) * DC];
-  q.by = c[(D_BCH + T1) * DC] + s * c[dq_slot(D, 5 + T1) * DC];
-  q.bz = c[(D_BCH + T2) * DC] + s * c[dq_slot(D, 5 + T2) * DC];
+  q.rho = c[(D_QH + 0) * DCS] + s * c[dq_slot(D, 0) * DCS];
+  q.u = c[(D_QH + 1 + D) * DCS] + s * c[dq_slot(D, 1 + D) * DCS];
+  q.v = c[(D_QH + 1 + T1) * DCS] + s * c[dq_slot(D, 1 + T1) * DCS];
+  q.w = c[(D_QH + 1 + T2) * DCS] + s * c[dq_slot(D, 1 + T2) * DCS];
+  q.p = c[(D_QH + 4) * DCS] + s * c[dq_slot(D, 4) * DCS];
+  q.by = c[(D_BCH + T1) * DCS] + s * c[dq_slot(D, 5 + T1) * DCS];
+  q.bz = c[(D_BCH + T2) * DCS] + s * c[dq_slot(D, 5 + T2) * DCS];
   return q;
 }
 // corner state of cell c seen from the edge along E: q^h + sa*d_A q + sb*d_B q
-template <typename T, int DC, int E>
+template <typename T, int DCS, int E>
 __device__ __forceinline__ Corner<T> corner_state(const T* __restrict__ c, T sa, T sb) {
   constexpr int A = (E + 1) % 3, B = (E + 2) % 3;
   Corner<T> q;
-  q.rho = c[(D_QH + 0) * DC] + sa * c[dq_slot(A, 0) * DC] + sb * c[dq_slot(B, 0) * DC];
-  q.ua = c[(D_QH + 1 + A) * DC] + sa * c[dq_slot(A, 1 + A) * DC] + sb * c[dq_slot(B, 1 + A) * DC];
-  q.ub = c[(D_QH + 1 + B) * DC] + sa * c[dq_slot(A, 1 + B) * DC] + sb * c[dq_slot(B, 1 + B) * DC];
-  q.p = c[(D_QH + 4) * DC] + sa * c[dq_slot(A, 4) * DC] + sb * c[dq_slot(B, 4) * DC];
-  q.be = c[(D_BCH + E) * DC] + sa * c[dq_slot(A, 5 + E) * DC] + sb * c[dq_slot(B, 5 + E) * DC];
+  q.rho = c[(D_QH + 0) * DCS] + sa * c[dq_slot(A, 0) * DCS] + sb * c[dq_slot(B, 0) * DCS];
+  q.ua = c[(D_QH + 1 + A) * DCS] + sa * c[dq_slot(A, 1 + A) * DCS] + sb * c[dq_slot(B, 1 + A) * DCS];
+  q.ub = c[(D_QH + 1 + B) * DCS] + sa * c[dq_slot(A, 1 + B) * DCS] + sb * c[dq_slot(B, 1 + B) * DCS];
+  q.p = c[(D_QH + 4) * DCS] + sa * c[dq_slot(A, 4) * DCS] + sb * c[dq_slot(B, 4) * DCS];
+  q.be = c[(D_BCH + E) * DCS] + sa * c[dq_slot(A, 5 + E) * DCS] + sb * c[dq_slot(B, 5 + E) * DCS];
   return q;
 }
 // D slot of the slope of face field b_a along t (a != t)
@@ -109,9 +148,9 @@ __host__ __device__ constexpr int dbf_slot(int a, int t) {
 }
 // in-plane field of the edge along E on the side of cell c: component X (A or B of the edge),
 // extrapolated along the other in-plane direction with sign s
-template <typename T, int DC, int X, int ALONG>
+template <typename T, int DCS, int X, int ALONG>
 __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
-  return c[(D_BH + X) * DC] + s * c[dbf_slot(X, ALONG) * DC];
+  return c[(D_BH + X) * DCS] + s * c[dbf_slot(X, ALONG) * DCS];
 }
 
 template <typename T, int TX, int TY, int NPW, int LIM, int FS>
@@ -119,8 +158,8 @@ __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
                unsigned long long* __restrict__ bad, int xtiles, int zseg) {
   using C = OneCfg<T, TX, TY, NPW>;
-  constexpr int PW = C::PW, PH = C::PH, PA = C::PA, BWX = C::BWX, RA = C::RA, DW = C::DW, DC = C::DC;
-  constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL;
+  constexpr int PH = C::PH, BWX = C::BWX, RA = C::RA, DP = C::DP, DCS = C::DCS;
+  constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL, NS = C::NS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* const Dm = reinterpret_cast<T*>(smem_raw + C::o_d);
   T* const Q = reinterpret_cast<T*>(smem_raw + C::o_q);
@@ -153,28 +192,31 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   if (t < 27) NBS[t] = gather ? nbr[(long long)(P.p0 + pl) * 27 + t] : P.p0 + pl;
   __syncthreads();
 
-  auto dslot = [&](int plane) { return Dm + (size_t)((plane + 2) & 1) * (D_COUNT * DC); };
+  auto dslot = [&](int plane) { return Dm + (size_t)((plane + 2) & 1) * (D_COUNT * DCS); };
 
   if (t >= 2 * NR) {
     // =============================================================== role P ==========
     const int tp = t - 2 * NR;
     const T q4 = T(0.25), hdt = h * dt;
     const T lx = hdt * P.idx[0], ly = hdt * P.idx[1], lz = hdt * P.idx[2];
-    auto Qs = [&](int plane, int f) { return Q + (((plane + 3) % 3) * 8 + f) * PA; };
-    auto Es = [&](int plane, int a) { return Em + (((plane + 2) & 1) * 3 + a) * PA; };
-    auto RH = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawh + (size_t)((plane + 2) & 1) * C::rawh_slot); };
-    auto RB = [&](int plane) { return reinterpret_cast<const T*>(smem_raw + C::o_rawb + (size_t)((plane + 4) & 3) * C::rawb_slot); };
+    const T gm1 = gamma - T(1);
+    auto Qs = [&](int plane) { return Q + ((plane + 3) % 3) * (8 * RA); };              // [8][RA]
+    auto Es = [&](int plane) { return Em + ((plane + 2) & 1) * (3 * RA); };             // [3][RA]
+    T* const RHs = reinterpret_cast<T*>(smem_raw + C::o_rawh);                           // [5][RA], one plane
+    auto RB = [&](int plane) { return reinterpret_cast<T*>(smem_raw + C::o_rawb + (size_t)((plane + 4) & 3) * C::rawb_slot); };
     const int rlo = za - 2, rhi = zb + 2;
-    // U^n plane -> raw ring, one 16-byte chunk of a row per copy, all 8 fields.  A chunk lies
-    // in one patch (x0 and, in gather mode, n_x are multiples of the chunk); its source is
-    // the image cell in the neighbour of class (ox,oy,oz) -- O1 -- or, without gather, the
-    // same cell of the own patch.  Chunks past the data a tile needs are skipped.
-    auto issue = [&](int plane) {
+    // U^n -> raw planes, one 16-byte chunk of a row per copy: the hydro fields of plane ph into the
+    // single hydro slot, the face fields of plane pb into the field ring.  A chunk lies in one patch
+    // (x0 and, in gather mode, n_x are multiples of the chunk); its source is the image cell in the
+    // neighbour of class (ox,oy,oz) -- O1 -- or, without gather, the same cell of the own patch.
+    // Chunks past the data a tile needs are skipped.
+    auto issue = [&](int ph, int pb, bool with_h) {
       const long long zplane = (long long)G.pitch * G.m[1];
-      const int oz = gather ? (plane < 0 ? -1 : (plane >= nz ? 1 : 0)) : 0;
-      const long long zoff = (long long)(plane - oz * nz + G.g[2]) * zplane;
-      T* const dh = const_cast<T*>(RH(plane));
-      T* const db = const_cast<T*>(RB(plane));
+      const int ozh = gather ? (ph < 0 ? -1 : (ph >= nz ? 1 : 0)) : 0;
+      const int ozb = gather ? (pb < 0 ? -1 : (pb >= nz ? 1 : 0)) : 0;
+      const long long zoffh = (long long)(ph - ozh * nz + G.g[2]) * zplane;
+      const long long zoffb = (long long)(pb - ozb * nz + G.g[2]) * zplane;
+      T* const db = RB(pb);
       for (int it = tp; it < PH * C::CPR; it += NP) {
         const int row = it / C::CPR, ch = it - row * C::CPR;
         const int x = x0 - 4 + ch * C::VEC, y = y0 - 2 + row;   // first cell of the chunk (raw column 0 is cell x0-4)
@@ -184,83 +226,131 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         const bool ok = gather ? (xs + C::VEC <= nx && ys < ny && xs >= 0 && ys >= 0)
                                : (G.lead + G.g[0] + xs + C::VEC <= G.pitch && ys + G.g[1] < G.m[1]);
         if (!ok) continue;
-        const int q = NBS[(oz + 1) * 9 + (oy + 1) * 3 + (ox + 1)];
-        const T* src = P.U + (long long)q * G.ps + zoff + (long long)(ys + G.g[1]) * G.pitch + (G.lead + G.g[0] + xs);
+        const int cls = (oy + 1) * 3 + (ox + 1);
+        const long long inp = (long long)(ys + G.g[1]) * G.pitch + (G.lead + G.g[0] + xs);
         const int o = row * BWX + ch * C::VEC;
+        const T* sb = P.U + (long long)NBS[(ozb + 1) * 9 + cls] * G.ps + zoffb + inp;
 #pragma unroll
-        for (int f = 0; f < 5; ++f) cp_async16(dh + f * RA + o, src + f * G.fs);
+        for (int f = 0; f < 3; ++f) cp_async16(db + f * RA + o, sb + (5 + f) * G.fs);
+        if (with_h) {
+          const T* sh = P.U + (long long)NBS[(ozh + 1) * 9 + cls] * G.ps + zoffh + inp;
 #pragma unroll
-        for (int f = 0; f < 3; ++f) cp_async16(db + f * RA + o, src + (5 + f) * G.fs);
+          for (int f = 0; f < 5; ++f) cp_async16(RHs + f * RA + o, sh + f * G.fs);
+        }
       }
     };
-    issue(rlo);
+    issue(rlo, rlo, false);
     cp_async_wait_all();
     nb_sync(NB_P, NP);
-    T cbx[C::PASS3], cby[C::PASS3];   // backward z-differences of the raw bx, by of the own D cells
+    // backward z-differences of the raw bx, by of the own D cells (carried from plane to plane)
+    T cbx[C::PASS3][2], cby[C::PASS3][2];
 #pragma unroll
-    for (int s = 0; s < C::PASS3; ++s) { cbx[s] = T(0); cby[s] = T(0); }
+    for (int s_ = 0; s_ < C::PASS3; ++s_) { cbx[s_][0] = cbx[s_][1] = T(0); cby[s_][0] = cby[s_][1] = T(0); }
     unsigned int nbad = 0;
 
     for (int r = rlo; r <= rhi; ++r) {
       // ---- primitives of plane r-1 (O2): needs bx(i+1), by(j+1) of plane r-1 and bz of plane r
       if (r - 1 >= rlo) {
-        const T* hy = RH(r - 1);
         const T* bb = RB(r - 1);
         const T* bzu = RB(r) + 2 * RA;
+        T* const qw = Qs(r - 1);
 #pragma unroll
-        for (int s = 0; s < C::PASS1; ++s) {
-          const int pos = tp + s * NP;
-          const int pr = pos / C::W1, pc = pos - pr * C::W1;
-          if (pos < C::N1) {
-            const int o = pr * PW + pc, ob = pr * BWX + pc + 2;
-            const T rho = hy[ob], ir = num<T>::rcp(rho);
-            const T u = hy[RA + ob] * ir, v = hy[2 * RA + ob] * ir, w = hy[3 * RA + ob] * ir;
-            const T bz0 = bb[2 * RA + ob];
-            const T bcx = h * (bb[ob] + bb[ob + 1]);
-            const T bcy = h * (bb[RA + ob] + bb[RA + ob + BWX]);
-            const T bcz = h * (bz0 + bzu[ob]);
-            const T pr_ = (gamma - T(1)) * (hy[4 * RA + ob] - h * rho * (u * u + v * v + w * w) - h * (bcx * bcx + bcy * bcy + bcz * bcz));
-            T* q = Qs(r - 1, 0) + o;
-            q[0] = rho; q[PA] = u; q[2 * PA] = v; q[3 * PA] = w; q[4 * PA] = pr_; q[5 * PA] = bcx; q[6 * PA] = bcy; q[7 * PA] = bcz;
-            const int ci = pc - 2, cj = pr - 2;   // tile-relative cell
-            if (ci >= 0 && ci < tw && cj >= 0 && cj < th && r - 1 >= za && r - 1 < zb &&
-                !(rho > T(0) && pr_ > T(0) && rho < T(INFINITY) && pr_ < T(INFINITY)))
-              ++nbad;
+        for (int s_ = 0; s_ < C::PASS1; ++s_) {
+          // a warp runs the body whole or not at all: lanes past the last task repeat it (same
+          // values to the same addresses), so no lane leaves its warp before the next barrier
+          if ((tp & ~31) + s_ * NP < C::NT1) {
+            const bool mine = tp + s_ * NP < C::NT1;
+            const int task = mine ? tp + s_ * NP : C::NT1 - 1;
+            const int pr = task / NS, st = task - pr * NS + 1;
+            const int o = pr * BWX + 2 * st;
+            const V2<T> rho = ld2(RHs + o), mx = ld2(RHs + RA + o), my = ld2(RHs + 2 * RA + o), mz = ld2(RHs + 3 * RA + o);
+            const V2<T> en = ld2(RHs + 4 * RA + o);
+            const V2<T> bx = ld2(bb + o);
+            const T bx2 = bb[o + 2];
+            const V2<T> by = ld2(bb + RA + o), byn = ld2(bb + RA + o + BWX);
+            const V2<T> bz = ld2(bb + 2 * RA + o), bzn = ld2(bzu + o);
+            T pv[2][8];
+            auto prim = [&](int e, T rh, T m0, T m1, T m2, T E, T bxa, T bxb, T bya, T byb, T bza, T bzb) {
+              const T ir = num<T>::rcp(rh);
+              const T u = m0 * ir, v = m1 * ir, w = m2 * ir;
+              const T bcx = h * (bxa + bxb), bcy = h * (bya + byb), bcz = h * (bza + bzb);
+              const T pr_ = gm1 * (E - h * rh * (u * u + v * v + w * w) - h * (bcx * bcx + bcy * bcy + bcz * bcz));
+              pv[e][0] = rh; pv[e][1] = u; pv[e][2] = v; pv[e][3] = w; pv[e][4] = pr_; pv[e][5] = bcx; pv[e][6] = bcy; pv[e][7] = bcz;
+              const int ci = 2 * st + e - 4, cj = pr - 2;   // tile-relative cell
+              if (mine && ci >= 0 && ci < tw && cj >= 0 && cj < th && r - 1 >= za && r - 1 < zb &&
+                  !(rh > T(0) && pr_ > T(0) && rh < T(INFINITY) && pr_ < T(INFINITY)))
+                ++nbad;
+            };
+            prim(0, rho.a, mx.a, my.a, mz.a, en.a, bx.a, bx.b, by.a, byn.a, bz.a, bzn.a);
+            prim(1, rho.b, mx.b, my.b, mz.b, en.b, bx.b, bx2, by.b, byn.b, bz.b, bzn.b);
+#pragma unroll
+            for (int f = 0; f < 8; ++f) st2(qw + f * RA + o, pv[0][f], pv[1][f]);
           }
         }
       }
       nb_sync(NB_P, NP);
-      // every P thread is past iteration r-1: the slots of hydro plane r-1 and field plane r-3 are free
-      if (r + 1 <= rhi) issue(r + 1);
+      // every P thread is past the primitives of plane r-1: the hydro slot and the field slot of plane r-3 are free
+      if (r + 1 <= rhi) issue(r, r + 1, true);
 
       // ---- edge EMFs of plane r-1 (O4a: Eq. 7-11 and cyclic images)
       if (r - 2 >= rlo) {
         const T* b1 = RB(r - 1);
         const T* b2 = RB(r - 2);
+        const T *q1 = Qs(r - 1), *q2 = Qs(r - 2);
+        T* const ew = Es(r - 1);
 #pragma unroll
-        for (int s = 0; s < C::PASS2; ++s) {
-          const int pos = tp + s * NP;
-          const int pr = pos / C::W2 + 1, pc = pos - (pr - 1) * C::W2 + 1;
-          if (pos < C::N2) {
-            const int o = pr * PW + pc, ob = pr * BWX + pc + 2;
-            const T *u1 = Qs(r - 1, 1) + o, *v1 = Qs(r - 1, 2) + o, *w1 = Qs(r - 1, 3) + o;
-            const T *u2 = Qs(r - 2, 1) + o, *v2 = Qs(r - 2, 2) + o, *w2 = Qs(r - 2, 3) + o;
-            const T *bx1 = b1 + ob, *by1 = b1 + RA + ob, *bz1 = b1 + 2 * RA + ob;
-            {  // ez over cells (i-1..i, j-1..j)
-              const T ub = q4 * (u1[0] + u1[-PW] + u1[-1] + u1[-PW - 1]);
-              const T vb = q4 * (v1[0] + v1[-PW] + v1[-1] + v1[-PW - 1]);
-              Es(r - 1, 2)[o] = ub * (h * (by1[0] + by1[-1])) - vb * (h * (bx1[0] + bx1[-BWX]));
-            }
-            {  // ex over (j-1..j, k-1..k)
-              const T vb = q4 * (v1[0] + v2[0] + v1[-PW] + v2[-PW]);
-              const T wb = q4 * (w1[0] + w2[0] + w1[-PW] + w2[-PW]);
-              Es(r - 1, 0)[o] = vb * (h * (bz1[0] + bz1[-BWX])) - wb * (h * (by1[0] + b2[RA + ob]));
-            }
-            {  // ey over (k-1..k, i-1..i)
-              const T wb = q4 * (w1[0] + w1[-1] + w2[0] + w2[-1]);
-              const T ub = q4 * (u1[0] + u1[-1] + u2[0] + u2[-1]);
-              Es(r - 1, 1)[o] = wb * (h * (bx1[0] + b2[ob])) - ub * (h * (bz1[0] + bz1[-1]));
-            }
+        for (int s_ = 0; s_ < C::PASS2; ++s_) {
+          if ((tp & ~31) + s_ * NP < C::NT2) {
+            const int task = min(tp + s_ * NP, C::NT2 - 1);
+            const int pr = task / NS + 1, st = task - (pr - 1) * NS + 1;
+            const int o = pr * BWX + 2 * st;
+            // columns -1, 0, 1 relative to the strip's first cell; rows 0 and -1; planes 1 (r-1) and 2 (r-2)
+            const T *u1 = q1 + RA + o, *v1 = q1 + 2 * RA + o, *w1 = q1 + 3 * RA + o;
+            const T *u2 = q2 + RA + o, *v2 = q2 + 2 * RA + o, *w2 = q2 + 3 * RA + o;
+            const T u1m = u1[-1], u1dm = u1[-BWX - 1];
+            const V2<T> u1c = ld2(u1), u1d = ld2(u1 - BWX);
+            const T v1m = v1[-1], v1dm = v1[-BWX - 1];
+            const V2<T> v1c = ld2(v1), v1d = ld2(v1 - BWX);
+            const T w1m = w1[-1];
+            const V2<T> w1c = ld2(w1), w1d = ld2(w1 - BWX);
+            const T u2m = u2[-1];
+            const V2<T> u2c = ld2(u2);
+            const V2<T> v2c = ld2(v2), v2d = ld2(v2 - BWX);
+            const T w2m = w2[-1];
+            const V2<T> w2c = ld2(w2), w2d = ld2(w2 - BWX);
+            const V2<T> bx1c = ld2(b1 + o), bx1d = ld2(b1 + o - BWX), bx2c = ld2(b2 + o);
+            const T by1m = b1[RA + o - 1];
+            const V2<T> by1c = ld2(b1 + RA + o), by2c = ld2(b2 + RA + o);
+            const T bz1m = b1[2 * RA + o - 1];
+            const V2<T> bz1c = ld2(b1 + 2 * RA + o), bz1d = ld2(b1 + 2 * RA + o - BWX);
+            // one position: own cell values X, west neighbour Xw (same row), row below Xd, its west Xdw
+            auto emfs = [&](T u, T uw, T ud, T udw, T v, T vw, T vd, T vdw, T w, T ww, T wd, T uu2, T uu2w, T vv2, T vv2d,
+                            T ww2, T ww2w, T ww2d, T bx, T bxd, T bxp, T by, T byw, T byp, T bz, T bzw, T bzd, T& ex, T& ey,
+                            T& ez) {
+              {  // ez over cells (i-1..i, j-1..j)
+                const T ub = q4 * (u + ud + uw + udw);
+                const T vb = q4 * (v + vd + vw + vdw);
+                ez = ub * (h * (by + byw)) - vb * (h * (bx + bxd));
+              }
+              {  // ex over (j-1..j, k-1..k)
+                const T vb = q4 * (v + vv2 + vd + vv2d);
+                const T wb = q4 * (w + ww2 + wd + ww2d);
+                ex = vb * (h * (bz + bzd)) - wb * (h * (by + byp));
+              }
+              {  // ey over (k-1..k, i-1..i)
+                const T wb = q4 * (w + ww + ww2 + ww2w);
+                const T ub = q4 * (u + uw + uu2 + uu2w);
+                ey = wb * (h * (bx + bxp)) - ub * (h * (bz + bzw));
+              }
+            };
+            T ex0, ey0, ez0, ex1, ey1, ez1;
+            emfs(u1c.a, u1m, u1d.a, u1dm, v1c.a, v1m, v1d.a, v1dm, w1c.a, w1m, w1d.a, u2c.a, u2m, v2c.a, v2d.a, w2c.a, w2m, w2d.a,
+                 bx1c.a, bx1d.a, bx2c.a, by1c.a, by1m, by2c.a, bz1c.a, bz1m, bz1d.a, ex0, ey0, ez0);
+            emfs(u1c.b, u1c.a, u1d.b, u1d.a, v1c.b, v1c.a, v1d.b, v1d.a, w1c.b, w1c.a, w1d.b, u2c.b, u2c.a, v2c.b, v2d.b, w2c.b, w2c.a,
+                 w2d.b, bx1c.b, bx1d.b, bx2c.b, by1c.b, by1c.a, by2c.b, bz1c.b, bz1c.a, bz1d.b, ex1, ey1, ez1);
+            st2(ew + o, ex0, ex1);
+            st2(ew + RA + o, ey0, ey1);
+            st2(ew + 2 * RA + o, ez0, ez1);
           }
         }
       }
@@ -273,72 +363,120 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         if (kd >= za + 1) nb_sync(NB_EMPTY + ((kd + 2) & 1), NALL);   // A and C are done with plane kd-2
         const T* b0 = RB(kd);
         const T* b1 = RB(kd + 1);
+        const T *qc = Qs(kd), *qm = Qs(kd - 1), *qp = Qs(kd + 1);
+        const T *e0 = Es(kd), *e1 = Es(kd + 1);
 #pragma unroll
-        for (int s = 0; s < C::PASS3; ++s) {
-          const int dcell = tp + s * NP;
-          if (dcell < DC) {
-            const int dr = dcell / DW, dcl = dcell - dr * DW;
-            const int o = (dr + 1) * PW + dcl + 1, ob = (dr + 1) * BWX + dcl + 3;
-            const T *bx = b0 + ob, *by = b0 + RA + ob, *bz = b0 + 2 * RA + ob;
-            const T bxc = bx[0], byc = by[0], bzc = bz[0];
-            const T bxu = b1[ob], byu = b1[RA + ob], bzu = b1[2 * RA + ob];   // raw fields one plane up
-            const T fwx = bxu - bxc, fwy = byu - byc;
+        for (int s_ = 0; s_ < C::PASS3; ++s_) {
+          if ((tp & ~31) + s_ * NP < C::NT3) {
+            const int task = min(tp + s_ * NP, C::NT3 - 1);
+            const int dr = task / NS, st = task - dr * NS + 1;
+            const int o = (dr + 1) * BWX + 2 * st;
+            const V2<T> bxc = ld2(b0 + o), byc = ld2(b0 + RA + o), bzc = ld2(b0 + 2 * RA + o);
+            const V2<T> bxu = ld2(b1 + o), byu = ld2(b1 + RA + o), bzu = ld2(b1 + 2 * RA + o);   // raw fields one plane up
+            const T fwx[2] = {bxu.a - bxc.a, bxu.b - bxc.b}, fwy[2] = {byu.a - byc.a, byu.b - byc.b};
             if (kd >= za - 1) {
-              const T* qc = Qs(kd, 0) + o;
-              const T* qm = Qs(kd - 1, 0) + o;
-              const T* qp = Qs(kd + 1, 0) + o;
-              T* D = Dw + dcell;
-              T c[8];
+              T* D = Dw + dr * DP + 2 * st;
+              T c[8][2];
 #pragma unroll
-              for (int f = 0; f < 8; ++f) c[f] = qc[f * PA];
+              for (int f = 0; f < 8; ++f) { const V2<T> v = ld2(qc + f * RA + o); c[f][0] = v.a; c[f][1] = v.b; }
               // slopes (O3) and the primitive half step (O4c), one direction at a time
-              const T rho = c[0], p_ = c[4], ir = num<T>::rcp(rho);
               const T lam[3] = {lx, ly, lz};
-              T rho_h = rho, p_h = p_, vh[3] = {c[1], c[2], c[3]};
+              T ir[2], rho_h[2], p_h[2], vh[3][2];
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                ir[e] = num<T>::rcp(c[0][e]); rho_h[e] = c[0][e]; p_h[e] = c[4][e];
+                vh[0][e] = c[1][e]; vh[1][e] = c[2][e]; vh[2][e] = c[3][e];
+              }
 #pragma unroll
               for (int d = 0; d < 3; ++d) {
-                T dq[8];
+                T dq[8][2];
 #pragma unroll
                 for (int f = 0; f < 8; ++f) {
-                  if (f == 5 + d) { dq[f] = T(0); continue; }
-                  const T lo = d == 0 ? qc[f * PA - 1] : (d == 1 ? qc[f * PA - PW] : qm[f * PA]);
-                  const T hi = d == 0 ? qc[f * PA + 1] : (d == 1 ? qc[f * PA + PW] : qp[f * PA]);
-                  dq[f] = limited_slope_k<LIM>(c[f] - lo, hi - c[f]);
-                  D[dq_slot(d, f) * DC] = dq[f];
+                  if (f == 5 + d) { dq[f][0] = dq[f][1] = T(0); continue; }
+                  const T* qf = qc + f * RA + o;
+                  if (d == 0) {
+                    const T lo = qf[-1], hi = qf[2];
+                    const T d0 = c[f][0] - lo, d1 = c[f][1] - c[f][0], d2 = hi - c[f][1];
+                    dq[f][0] = limited_slope_k<LIM>(d0, d1);
+                    dq[f][1] = limited_slope_k<LIM>(d1, d2);
+                  } else {
+                    const V2<T> lo = d == 1 ? ld2(qf - BWX) : ld2(qm + f * RA + o);
+                    const V2<T> hi = d == 1 ? ld2(qf + BWX) : ld2(qp + f * RA + o);
+                    dq[f][0] = limited_slope_k<LIM>(c[f][0] - lo.a, hi.a - c[f][0]);
+                    dq[f][1] = limited_slope_k<LIM>(c[f][1] - lo.b, hi.b - c[f][1]);
+                  }
+                  st2(D + dq_slot(d, f) * DCS, dq[f][0], dq[f][1]);
                 }
-                const int b = (d + 1) % 3, e = (d + 2) % 3;
-                const T ud = c[1 + d], dud = dq[1 + d];
-                rho_h -= lam[d] * (ud * dq[0] + rho * dud);
-                p_h -= lam[d] * (ud * dq[4] + gamma * p_ * dud);
+                const int b = (d + 1) % 3, eb = (d + 2) % 3;
 #pragma unroll
-                for (int a = 0; a < 3; ++a) vh[a] -= lam[d] * ud * dq[1 + a];
-                // -(1/rho) d_d (p + B_b^2/2 + B_e^2/2) acts on u_d;  +(B_d/rho) d_d B_a acts on u_a, a != d
-                vh[d] -= lam[d] * (dq[4] + c[5 + b] * dq[5 + b] + c[5 + e] * dq[5 + e]) * ir;
-                vh[b] += lam[d] * c[5 + d] * dq[5 + b] * ir;
-                vh[e] += lam[d] * c[5 + d] * dq[5 + e] * ir;
+                for (int e = 0; e < 2; ++e) {
+                  const T ud = c[1 + d][e], dud = dq[1 + d][e];
+                  rho_h[e] -= lam[d] * (ud * dq[0][e] + c[0][e] * dud);
+                  p_h[e] -= lam[d] * (ud * dq[4][e] + gamma * c[4][e] * dud);
+#pragma unroll
+                  for (int a = 0; a < 3; ++a) vh[a][e] -= lam[d] * ud * dq[1 + a][e];
+                  // -(1/rho) d_d (p + B_b^2/2 + B_e^2/2) acts on u_d;  +(B_d/rho) d_d B_a acts on u_a, a != d
+                  vh[d][e] -= lam[d] * (dq[4][e] + c[5 + b][e] * dq[5 + b][e] + c[5 + eb][e] * dq[5 + eb][e]) * ir[e];
+                  vh[b][e] += lam[d] * c[5 + d][e] * dq[5 + b][e] * ir[e];
+                  vh[eb][e] += lam[d] * c[5 + d][e] * dq[5 + eb][e] * ir[e];
+                }
               }
               // face-field transverse slopes: dy bx, dz bx, dx by, dz by, dx bz, dy bz
-              D[(D_DBF + 0) * DC] = limited_slope_k<LIM>(bxc - bx[-BWX], bx[BWX] - bxc);
-              D[(D_DBF + 1) * DC] = limited_slope_k<LIM>(cbx[s], fwx);
-              D[(D_DBF + 2) * DC] = limited_slope_k<LIM>(byc - by[-1], by[1] - byc);
-              D[(D_DBF + 3) * DC] = limited_slope_k<LIM>(cby[s], fwy);
-              D[(D_DBF + 4) * DC] = limited_slope_k<LIM>(bzc - bz[-1], bz[1] - bzc);
-              D[(D_DBF + 5) * DC] = limited_slope_k<LIM>(bzc - bz[-BWX], bz[BWX] - bzc);
-              // half-step faces (Eq. 12 with dt/2) of this cell and of its +x, +y, +z neighbours
-              const T *ex0 = Es(kd, 0) + o, *ey0 = Es(kd, 1) + o, *ez0 = Es(kd, 2) + o;
-              const T *ex1 = Es(kd + 1, 0) + o, *ey1 = Es(kd + 1, 1) + o;
-              const T bxh = bxc + (ly * (ez0[PW] - ez0[0]) - lz * (ey1[0] - ey0[0]));
-              const T bxh1 = bx[1] + (ly * (ez0[1 + PW] - ez0[1]) - lz * (ey1[1] - ey0[1]));
-              const T byh = byc + (lz * (ex1[0] - ex0[0]) - lx * (ez0[1] - ez0[0]));
-              const T byh1 = by[BWX] + (lz * (ex1[PW] - ex0[PW]) - lx * (ez0[PW + 1] - ez0[PW]));
-              const T bzh = bzc + (lx * (ey0[1] - ey0[0]) - ly * (ex0[PW] - ex0[0]));
-              const T bzh_up = bzu + (lx * (ey1[1] - ey1[0]) - ly * (ex1[PW] - ex1[0]));
-              D[(D_QH + 0) * DC] = rho_h; D[(D_QH + 1) * DC] = vh[0]; D[(D_QH + 2) * DC] = vh[1]; D[(D_QH + 3) * DC] = vh[2];
-              D[(D_QH + 4) * DC] = p_h;
-              D[(D_BCH + 0) * DC] = h * (bxh + bxh1); D[(D_BCH + 1) * DC] = h * (byh + byh1); D[(D_BCH + 2) * DC] = h * (bzh + bzh_up);
-              D[(D_BH + 0) * DC] = bxh; D[(D_BH + 1) * DC] = byh; D[(D_BH + 2) * DC] = bzh;
+              const T* bx = b0 + o;
+              const T* by = b0 + RA + o;
+              const T* bz = b0 + 2 * RA + o;
+              const V2<T> bxd = ld2(bx - BWX), bxn = ld2(bx + BWX);
+              const V2<T> byn = ld2(by + BWX);
+              const V2<T> bzd = ld2(bz - BWX), bzn = ld2(bz + BWX);
+              const T bx2 = bx[2], bym = by[-1], by2 = by[2], bzm = bz[-1], bz2 = bz[2];
+              st2(D + (D_DBF + 0) * DCS, limited_slope_k<LIM>(bxc.a - bxd.a, bxn.a - bxc.a), limited_slope_k<LIM>(bxc.b - bxd.b, bxn.b - bxc.b));
+              st2(D + (D_DBF + 1) * DCS, limited_slope_k<LIM>(cbx[s_][0], fwx[0]), limited_slope_k<LIM>(cbx[s_][1], fwx[1]));
+              {
+                const T d0 = byc.a - bym, d1 = byc.b - byc.a, d2 = by2 - byc.b;
+                st2(D + (D_DBF + 2) * DCS, limited_slope_k<LIM>(d0, d1), limited_slope_k<LIM>(d1, d2));
+              }
+              st2(D + (D_DBF + 3) * DCS, limited_slope_k<LIM>(cby[s_][0], fwy[0]), limited_slope_k<LIM>(cby[s_][1], fwy[1]));
+              {
+                const T d0 = bzc.a - bzm, d1 = bzc.b - bzc.a, d2 = bz2 - bzc.b;
+                st2(D + (D_DBF + 4) * DCS, limited_slope_k<LIM>(d0, d1), limited_slope_k<LIM>(d1, d2));
+              }
+              st2(D + (D_DBF + 5) * DCS, limited_slope_k<LIM>(bzc.a - bzd.a, bzn.a - bzc.a), limited_slope_k<LIM>(bzc.b - bzd.b, bzn.b - bzc.b));
+              // half-step faces (Eq. 12 with dt/2) of the two cells and of their +x, +y, +z neighbours:
+              // EMFs of planes kd (0) and kd+1 (1) at columns 0..2 and rows 0, +1
+              const T *ex0 = e0 + o, *ey0 = e0 + RA + o, *ez0 = e0 + 2 * RA + o;
+              const T *ex1 = e1 + o, *ey1 = e1 + RA + o;
+              const V2<T> ex0c = ld2(ex0), ex0n = ld2(ex0 + BWX), ex1c = ld2(ex1), ex1n = ld2(ex1 + BWX);
+              const V2<T> ey0c = ld2(ey0), ey1c = ld2(ey1);
+              const T ey02 = ey0[2], ey12 = ey1[2];
+              const V2<T> ez0c = ld2(ez0), ez0n = ld2(ez0 + BWX);
+              const T ez02 = ez0[2], ez0n2 = ez0[BWX + 2];
+              // bx at columns 0, 1, 2
+              const T bxh0 = bxc.a + (ly * (ez0n.a - ez0c.a) - lz * (ey1c.a - ey0c.a));
+              const T bxh1 = bxc.b + (ly * (ez0n.b - ez0c.b) - lz * (ey1c.b - ey0c.b));
+              const T bxh2 = bx2 + (ly * (ez0n2 - ez02) - lz * (ey12 - ey02));
+              // by at rows 0 and +1
+              const T byh0 = byc.a + (lz * (ex1c.a - ex0c.a) - lx * (ez0c.b - ez0c.a));
+              const T byh1 = byc.b + (lz * (ex1c.b - ex0c.b) - lx * (ez02 - ez0c.b));
+              const T byhn0 = byn.a + (lz * (ex1n.a - ex0n.a) - lx * (ez0n.b - ez0n.a));
+              const T byhn1 = byn.b + (lz * (ex1n.b - ex0n.b) - lx * (ez0n2 - ez0n.b));
+              // bz at planes kd and kd+1
+              const T bzh0 = bzc.a + (lx * (ey0c.b - ey0c.a) - ly * (ex0n.a - ex0c.a));
+              const T bzh1 = bzc.b + (lx * (ey02 - ey0c.b) - ly * (ex0n.b - ex0c.b));
+              const T bzhu0 = bzu.a + (lx * (ey1c.b - ey1c.a) - ly * (ex1n.a - ex1c.a));
+              const T bzhu1 = bzu.b + (lx * (ey12 - ey1c.b) - ly * (ex1n.b - ex1c.b));
+              st2(D + (D_QH + 0) * DCS, rho_h[0], rho_h[1]);
+              st2(D + (D_QH + 1) * DCS, vh[0][0], vh[0][1]);
+              st2(D + (D_QH + 2) * DCS, vh[1][0], vh[1][1]);
+              st2(D + (D_QH + 3) * DCS, vh[2][0], vh[2][1]);
+              st2(D + (D_QH + 4) * DCS, p_h[0], p_h[1]);
+              st2(D + (D_BCH + 0) * DCS, h * (bxh0 + bxh1), h * (bxh1 + bxh2));
+              st2(D + (D_BCH + 1) * DCS, h * (byh0 + byhn0), h * (byh1 + byhn1));
+              st2(D + (D_BCH + 2) * DCS, h * (bzh0 + bzhu0), h * (bzh1 + bzhu1));
+              st2(D + (D_BH + 0) * DCS, bxh0, bxh1);
+              st2(D + (D_BH + 1) * DCS, byh0, byh1);
+              st2(D + (D_BH + 2) * DCS, bzh0, bzh1);
             }
-            cbx[s] = fwx; cby[s] = fwy;
+            cbx[s_][0] = fwx[0]; cbx[s_][1] = fwx[1]; cby[s_][0] = fwy[0]; cby[s_][1] = fwy[1];
           }
         }
         if (kd >= za - 1) {
@@ -346,7 +484,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
           nb_arrive(NB_FULL + ((kd + 2) & 1), NALL);
         }
       }
-      cp_async_wait_all();   // own chunks of plane r+1 have landed ...
+      cp_async_wait_all();   // own chunks of hydro plane r and field plane r+1 have landed ...
       nb_sync(NB_P, NP);     // ... and everybody's; the rings are rewritten by the next iteration
     }
     if (nbad) atomicAdd(bad, (unsigned long long)nbad);
@@ -364,7 +502,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const bool cell = active && (fi < tw) && (fj < th);
   const bool xface = active && (fj < th) && (fi < tw || lastx);   // bx faces of the tile (closing face at the patch end)
   const bool yface = active && (fi < tw) && (fj < th || lasty);
-  const int own = (fj + 1) * DW + (fi + 1);
+  const int own = (fj + 1) * DP + (fi + 4);          // D cell of (fi, fj): row fj+1, column rc = fi+4
   const int fidx = min(fj, C::FH - 1) * FW + fi;
   const int tyn = colthr ? tr + 1 : tr + TX;              // thread that owns (fi, fj+1)
   const int txn = colthr ? tr : ((fi == TX - 1) ? C::CB + fj : tr + 1);   // thread that owns (fi+1, fj)
@@ -392,22 +530,22 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       State1D<T> Lz = {};
       Corner<T> xsw = {}, xse = {}, ysw = {}, ynw = {};
       T xAS = T(0), yBW = T(0);
-      if (doFz) Lz = face_state<T, DC, 2>(dp_, h);
+      if (doFz) Lz = face_state<T, DCS, 2>(dp_, h);
       if (doEx) {   // ex, in-plane (y,z): sw=(j-1,k-1) se=(j,k-1) nw=(j-1,k) ne=(j,k)
-        xsw = corner_state<T, DC, 0>(dp_ - DW, h, h);
-        xse = corner_state<T, DC, 0>(dp_, -h, h);
-        xAS = edge_field<T, DC, 1, 2>(dp_, h);
+        xsw = corner_state<T, DCS, 0>(dp_ - DP, h, h);
+        xse = corner_state<T, DCS, 0>(dp_, -h, h);
+        xAS = edge_field<T, DCS, 1, 2>(dp_, h);
       }
       if (doEy) {   // ey, in-plane (z,x): sw=(k-1,i-1) se=(k,i-1) nw=(k-1,i) ne=(k,i)
-        ysw = corner_state<T, DC, 1>(dp_ - 1, h, h);
-        ynw = corner_state<T, DC, 1>(dp_, h, -h);
-        yBW = edge_field<T, DC, 0, 2>(dp_, h);
+        ysw = corner_state<T, DCS, 1>(dp_ - 1, h, h);
+        ynw = corner_state<T, DCS, 1>(dp_, h, -h);
+        yBW = edge_field<T, DCS, 0, 2>(dp_, h);
       }
       if (k + 1 <= zb) nb_arrive(NB_EMPTY + ((k + 1) & 1), NALL);   // slot of plane k-1
 
       Flux5<T> cFz = {};
       T cex = T(0), cey = T(0);
-      if (doFz) cFz = riemann_flux_k<FS>(gamma, Lz, face_state<T, DC, 2>(dc_, -h), dc_[(D_BH + 2) * DC]);
+      if (doFz) cFz = riemann_flux_k<FS>(gamma, Lz, face_state<T, DCS, 2>(dc_, -h), dc_[(D_BH + 2) * DCS]);
       // The hydro part of plane k-1 only waits for this flux: finish it now (C is ahead, its
       // partial update is normally there already), so that the previous plane's flux is dead
       // while the two edge problems are solved.
@@ -426,11 +564,11 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       }
       pFz = cFz;
       if (doEx)
-        cex = emf_2d(gamma, solver, xsw, xse, corner_state<T, DC, 0>(dc_ - DW, h, -h), corner_state<T, DC, 0>(dc_, -h, -h),
-                     xAS, edge_field<T, DC, 1, 2>(dc_, -h), edge_field<T, DC, 2, 1>(dc_ - DW, h), edge_field<T, DC, 2, 1>(dc_, -h));
+        cex = emf_2d(gamma, solver, xsw, xse, corner_state<T, DCS, 0>(dc_ - DP, h, -h), corner_state<T, DCS, 0>(dc_, -h, -h),
+                     xAS, edge_field<T, DCS, 1, 2>(dc_, -h), edge_field<T, DCS, 2, 1>(dc_ - DP, h), edge_field<T, DCS, 2, 1>(dc_, -h));
       if (doEy)
-        cey = emf_2d(gamma, solver, ysw, corner_state<T, DC, 1>(dc_ - 1, -h, h), ynw, corner_state<T, DC, 1>(dc_, -h, -h),
-                     edge_field<T, DC, 2, 0>(dc_ - 1, h), edge_field<T, DC, 2, 0>(dc_, -h), yBW, edge_field<T, DC, 0, 2>(dc_, -h));
+        cey = emf_2d(gamma, solver, ysw, corner_state<T, DCS, 1>(dc_ - 1, -h, h), ynw, corner_state<T, DCS, 1>(dc_, -h, -h),
+                     edge_field<T, DCS, 2, 0>(dc_ - 1, h), edge_field<T, DCS, 2, 0>(dc_, -h), yBW, edge_field<T, DCS, 0, 2>(dc_, -h));
 
       XE[tr] = cex;
       XE[NR + tr] = cey;
@@ -470,13 +608,13 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         if (xface) un[5] = P.U[5 * fs + cu];
         if (yface) un[6] = P.U[6 * fs + cu];
         const T* dc_ = dslot(kd) + own;
-        if (doFx) Fx = riemann_flux_k<FS>(gamma, face_state<T, DC, 0>(dc_ - 1, h), face_state<T, DC, 0>(dc_, -h), dc_[(D_BH + 0) * DC]);
-        if (doFy) Fy = riemann_flux_k<FS>(gamma, face_state<T, DC, 1>(dc_ - DW, h), face_state<T, DC, 1>(dc_, -h), dc_[(D_BH + 1) * DC]);
+        if (doFx) Fx = riemann_flux_k<FS>(gamma, face_state<T, DCS, 0>(dc_ - 1, h), face_state<T, DCS, 0>(dc_, -h), dc_[(D_BH + 0) * DCS]);
+        if (doFy) Fy = riemann_flux_k<FS>(gamma, face_state<T, DCS, 1>(dc_ - DP, h), face_state<T, DCS, 1>(dc_, -h), dc_[(D_BH + 1) * DCS]);
         if (active)   // ez, in-plane (x,y): sw=(i-1,j-1) se=(i,j-1) nw=(i-1,j) ne=(i,j)
-          ez = emf_2d(gamma, solver, corner_state<T, DC, 2>(dc_ - DW - 1, h, h), corner_state<T, DC, 2>(dc_ - DW, -h, h),
-                      corner_state<T, DC, 2>(dc_ - 1, h, -h), corner_state<T, DC, 2>(dc_, -h, -h),
-                      edge_field<T, DC, 0, 1>(dc_ - DW, h), edge_field<T, DC, 0, 1>(dc_, -h),
-                      edge_field<T, DC, 1, 0>(dc_ - 1, h), edge_field<T, DC, 1, 0>(dc_, -h));
+          ez = emf_2d(gamma, solver, corner_state<T, DCS, 2>(dc_ - DP - 1, h, h), corner_state<T, DCS, 2>(dc_ - DP, -h, h),
+                      corner_state<T, DCS, 2>(dc_ - 1, h, -h), corner_state<T, DCS, 2>(dc_, -h, -h),
+                      edge_field<T, DCS, 0, 1>(dc_ - DP, h), edge_field<T, DCS, 0, 1>(dc_, -h),
+                      edge_field<T, DCS, 1, 0>(dc_ - 1, h), edge_field<T, DCS, 1, 0>(dc_, -h));
       }
       if (kd + 2 <= zb) nb_arrive(NB_EMPTY + ((kd + 2) & 1), NALL);   // done with plane kd
       if (!work) continue;

@@ -637,6 +637,9 @@ def test_config4_corner_4096_patches_of_64_cubed():
     spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "bench.py"))
     bench = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(bench)
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                       # earlier tests' buffers sit in torch's caching allocator
     free, _ = torch.cuda.mem_get_info()
     if free < 110 * 2 ** 30:
         pytest.skip("needs 2 x 46 GB of device memory")
