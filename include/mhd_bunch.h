@@ -231,9 +231,15 @@ int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
  *                          1 unless the bunch has fewer tiles than the device has SMs);
  *                          results do not depend on it, bit for bit.
  *   MHD_TUNE_PREDICT_TY    y-tile of the two-kernel path's predictor: 16, 8 or 4.
+ *   MHD_TUNE_FUSED_CFL     1: the one-pass step also reduces the CFL rates of the level it writes
+ *                          (in its epilogue, from registers), so that the next mhd_bunch_cfl_dt
+ *                          only runs the bunch-wide reduction instead of re-reading the state;
+ *                          0 (default): mhd_bunch_cfl_dt makes its own pass.  Same dt, bit for
+ *                          bit, either way (both evaluate one explicitly rounded function).
  * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
 #define MHD_TUNE_ONEPASS_ZSEG 1
 #define MHD_TUNE_PREDICT_TY   2
+#define MHD_TUNE_FUSED_CFL    3
 int mhd_bunch_set_tuning(mhd_bunch *b, int32_t key, int32_t value);
 
 /* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted

@@ -61,6 +61,12 @@ def _lib(key):
         lib.orc_step.argtypes = [C.POINTER(_Desc), rp, rp, C.c_double]
         lib.orc_stages.restype = None
         lib.orc_stages.argtypes = [C.POINTER(_Desc), rp, C.c_int32, C.c_double, rp]
+        lib.orc_local_ready.restype = C.c_int
+        lib.orc_local_ready.argtypes = [C.POINTER(_Desc), rp, rp, rp, rp, C.c_int32]
+        lib.orc_fill_guards_local.restype = None
+        lib.orc_fill_guards_local.argtypes = [C.POINTER(_Desc), rp, rp, rp, rp, rp, rp, C.c_int32]
+        lib.orc_step_local.restype = C.c_int
+        lib.orc_step_local.argtypes = [C.POINTER(_Desc), rp, rp, rp, rp, rp, rp, rp, C.c_int32, rp]
         real = C.c_float if key == "f32" else C.c_double
         lib.orc_limiter.restype = real
         lib.orc_limiter.argtypes = [C.c_int32, real, real]
@@ -127,6 +133,39 @@ class Oracle:
         out = np.zeros((NSTAGE,) + self.shape[2:], dtype=self.np_dtype)
         self.lib.orc_stages(C.byref(self.desc), _ptr(U), patch, dt, _ptr(out))
         return {k: out[a:b] for k, (a, b) in STAGE_SLICES.items()}
+
+    # ---- O10: local time steps (two slices per patch) -------------------------------------
+    def local_state(self, U, t0=0.0):
+        """Both slices = U at time t0: dict(S=[S0, S1], cur, t_old, t_new)."""
+        self._chk(U)
+        return {"S": [U.copy(), U.copy()], "cur": np.zeros(self.npatch, dtype=np.int32),
+                "t_old": np.full(self.npatch, t0), "t_new": np.full(self.npatch, t0)}
+
+    def local_ready(self, st, nbr, patches):
+        nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+        lst = np.ascontiguousarray(patches, dtype=np.int32)
+        return bool(self.lib.orc_local_ready(C.byref(self.desc), _ptr(nbr), _ptr(st["t_old"]), _ptr(st["t_new"]), _ptr(lst), len(lst)))
+
+    def fill_guards_local(self, st, nbr, p):
+        nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+        self.lib.orc_fill_guards_local(C.byref(self.desc), _ptr(nbr), _ptr(st["S"][0]), _ptr(st["S"][1]), _ptr(st["cur"]),
+                                       _ptr(st["t_old"]), _ptr(st["t_new"]), int(p))
+
+    def step_local(self, st, nbr, patches, dt):
+        """Advance the listed patches by their own dt (in place); False if one is not ready."""
+        nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+        lst = np.ascontiguousarray(patches, dtype=np.int32)
+        dts = np.ascontiguousarray(np.broadcast_to(np.asarray(dt, dtype=np.float64), lst.shape))
+        rc = self.lib.orc_step_local(C.byref(self.desc), _ptr(nbr), _ptr(st["S"][0]), _ptr(st["S"][1]), _ptr(st["cur"]),
+                                     _ptr(st["t_old"]), _ptr(st["t_new"]), _ptr(lst), len(lst), _ptr(dts))
+        return rc == 0
+
+    def local_newest(self, st):
+        """[8, npatch, ...]: the newer slice of every patch."""
+        out = np.empty_like(st["S"][0])
+        for p in range(self.npatch):
+            out[:, p] = st["S"][st["cur"][p]][:, p]
+        return out
 
     # interior view helper: [8, npatch, nz, ny, nx]
     def interior(self, U):

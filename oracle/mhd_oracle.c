@@ -679,3 +679,108 @@ double orc_cfl_dt(const orc_desc *d, const real *U, double courant, double *per_
   free(dts);
   return dtmin;
 }
+
+
+/* ------------------------------------------------- O10 local time steps -- */
+/* PAPER.md L122 (section 2.2): a patch holds several time slices and its own time and time
+ * step; L188, L200 (section 3.1): neighbouring patches sit at different times and ghost-zone
+ * values are interpolated.  Reading O10: two slices per patch, S[cur[p]] the newer
+ * one at time t_new[p], the other the older one at t_old[p]; guard values of a patch p are
+ * its neighbours' slices interpolated LINEARLY IN TIME to t_new[p].                          */
+static int times_equal(double a, double b) {
+  double s = fabs(a) > fabs(b) ? fabs(a) : fabs(b);
+  return fabs(a - b) <= 1e-12 * (s > 1.0 ? s : 1.0);
+}
+
+int orc_local_ready(const orc_desc *d, const int32_t *nbr, const double *t_old, const double *t_new,
+                    const int32_t *list, int32_t n) {
+  for (int i = 0; i < n; ++i) {
+    int p = list[i];
+    if (p < 0 || p >= d->npatch) return 0;
+    for (int c = 0; c < 27; ++c) {
+      int q = nbr[p * 27 + c];
+      if (q < 0 || q == p) continue;
+      int lo_ok = t_old[q] <= t_new[p] || times_equal(t_old[q], t_new[p]);
+      int hi_ok = t_new[p] <= t_new[q] || times_equal(t_new[p], t_new[q]);
+      if (!(lo_ok && hi_ok)) return 0;
+    }
+  }
+  return 1;
+}
+
+/* guard fill of the newer slice of patch p from its neighbours' two slices */
+void orc_fill_guards_local(const orc_desc *d, const int32_t *nbr, real *S0, real *S1, const int32_t *cur,
+                           const double *t_old, const double *t_new, int32_t p) {
+  geom G; mkgeom(d, &G);
+  real *S[2] = {S0, S1};
+  real *Up = S[cur[p]];
+  box all = mkbox(&G, G.g[0], G.g[0], G.g[1], G.g[1], G.g[2], G.g[2]);
+  BOXLOOP(all) {
+    int c[3] = {i, j, k}, o[3], src[3], clamp[3];
+    int guard = 0;
+    for (int a = 0; a < 3; ++a) {
+      o[a] = c[a] < 0 ? -1 : (c[a] >= G.n[a] ? 1 : 0);
+      if (o[a]) guard = 1;
+      src[a] = c[a] - o[a] * G.n[a];
+      clamp[a] = c[a] < 0 ? 0 : (c[a] >= G.n[a] ? G.n[a] - 1 : c[a]);
+    }
+    if (!guard) continue;
+    int q = nbr[p * 27 + (o[2] + 1) * 9 + (o[1] + 1) * 3 + (o[0] + 1)];
+    long dst = cidx(&G, i, j, k);
+    for (int f = 0; f < 8; ++f) {
+      long fo = (long)f * G.np * G.M;
+      if (q >= 0) {
+        long from = fo + (long)q * G.M + cidx(&G, src[0], src[1], src[2]);
+        real vnew = S[cur[q]][from];
+        real v = vnew;
+        if (!times_equal(t_new[p], t_new[q]) && !times_equal(t_new[q], t_old[q])) {
+          real vold = S[1 - cur[q]][from];
+          real w = (real)((t_new[p] - t_old[q]) / (t_new[q] - t_old[q]));
+          v = vold + w * (vnew - vold);
+        }
+        Up[fo + (long)p * G.M + dst] = v;
+      } else {
+        if (f >= 5) { /* the closing face keeps its evolved value (O8) */
+          int a = f - 5, b = (a + 1) % 3, e = (a + 2) % 3;
+          if (c[a] == G.n[a] && G.act[a] && o[b] == 0 && o[e] == 0) continue;
+        }
+        Up[fo + (long)p * G.M + dst] = Up[fo + (long)p * G.M + cidx(&G, clamp[0], clamp[1], clamp[2])];
+      }
+    }
+  }
+}
+
+/* One call advances the patches list[0..n) by their own dt[i]: (1) time-interpolated guard fill
+ * of the newer slice of every listed patch; (2) O2-O8 from the newer slice into the older one,
+ * which becomes the newer one (cur flips, t_old <- t_new, t_new += dt).  Readiness (the rule
+ * under which DISPATCH updates a task): t_old[q] <= t_new[p] <= t_new[q] for every neighbour q of
+ * a listed p, so that guard values are interpolated, never extrapolated; two listed neighbours
+ * are then at the same time and read only each other's newer slices, which this call does not
+ * write.  Returns 0, or -1 (nothing done) if a listed patch is not ready.                      */
+int orc_step_local(const orc_desc *d, const int32_t *nbr, real *S0, real *S1, int32_t *cur, double *t_old,
+                   double *t_new, const int32_t *list, int32_t n, const double *dt) {
+  if (!orc_local_ready(d, nbr, t_old, t_new, list, n)) return -1;
+  geom G; mkgeom(d, &G);
+  real *S[2] = {S0, S1};
+  for (int i = 0; i < n; ++i) orc_fill_guards_local(d, nbr, S0, S1, cur, t_old, t_new, list[i]);
+  real *buf = (real *)malloc(sizeof(real) * ORC_NSTAGE * G.M);
+  scratch Sc; scratch_bind(&Sc, buf, G.M);
+  for (int i = 0; i < n; ++i) {
+    int p = list[i];
+    const real *Up[8]; real *Un[8];
+    for (int f = 0; f < 8; ++f) {
+      Up[f] = S[cur[p]] + ((long)f * G.np + p) * G.M;
+      Un[f] = S[1 - cur[p]] + ((long)f * G.np + p) * G.M;
+    }
+    run_stages(&G, Up, (real)dt[i], &Sc);
+    update_patch(&G, Up, Un, (real)dt[i], &Sc);
+  }
+  free(buf);
+  for (int i = 0; i < n; ++i) {
+    int p = list[i];
+    cur[p] = 1 - cur[p];
+    t_old[p] = t_new[p];
+    t_new[p] += dt[i];
+  }
+  return 0;
+}

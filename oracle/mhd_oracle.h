@@ -75,6 +75,24 @@ void orc_step(const orc_desc *d, const real *U, real *Unew, double dt);
 /* the same stages for one patch, exporting every scratch array: out[ORC_NSTAGE][M]     */
 void orc_stages(const orc_desc *d, const real *U, int32_t patch, double dt, real *out);
 
+/* O10  local time steps with time-interpolated guard fill (patches hold several
+ *     time slices, their own time and time step; L188, L200: ghost zones of neighbours at other
+ *     times are interpolated).  S0, S1: two full bunch arrays; cur[p] = which of them holds the
+ *     newer slice of patch p (time t_new[p]); the other holds the older one (t_old[p]).
+ *     orc_step_local advances list[0..n) by dt[0..n): guard fill of each listed patch's newer
+ *     slice from its neighbours' slices, linearly interpolated in time to t_new[p]
+ *     (v_old + w (v_new - v_old), w = (t_new[p]-t_old[q])/(t_new[q]-t_old[q]); equal times: the newer
+ *     slice itself, bit for bit), then O2-O8 into the older slice, which becomes the newer one.
+ *     Returns -1 and changes nothing unless every neighbour q of every listed p has
+ *     t_old[q] <= t_new[p] <= t_new[q] (orc_local_ready).  Mass, momentum and energy are NOT
+ *     conserved across patches that step with different dt (no flux correction in the paper).   */
+int  orc_local_ready(const orc_desc *d, const int32_t *nbr, const double *t_old, const double *t_new,
+                     const int32_t *list, int32_t n);
+void orc_fill_guards_local(const orc_desc *d, const int32_t *nbr, real *S0, real *S1, const int32_t *cur,
+                           const double *t_old, const double *t_new, int32_t p);
+int  orc_step_local(const orc_desc *d, const int32_t *nbr, real *S0, real *S1, int32_t *cur, double *t_old,
+                    double *t_new, const int32_t *list, int32_t n, const double *dt);
+
 /* pointwise pieces, exported for the pins */
 real orc_limiter(int32_t kind, real a, real b);                               /* O3 */
 void orc_hlld(double gamma, const real L[7], const real R[7], real bn, real F[7]); /* O6 */

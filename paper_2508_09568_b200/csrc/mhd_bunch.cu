@@ -60,7 +60,10 @@ struct mhd_bunch {
   int chunk_s;         // patches per sub-bunch of the staged path
   // carved from the workspace head
   int* d_nbr;
-  unsigned long long* d_rate;  // [npatch]
+  unsigned long long* d_rate;  // [npatch] per-patch CFL rate maxima (bit patterns) of the stand-alone pass
+  unsigned long long* d_rate_next;  // [npatch] the same for the level a one-pass step is writing (its epilogue)
+  bool rate_valid;             // d_rate_next holds the rates of the CURRENT level (set by a one-pass step that
+                               // covered the bunch; cleared when the caller may have written the buffer)
   unsigned long long* d_bad;   // [1]
   double* d_dt;                // [2]: cfl result, step dt
   char* d_scratch;
@@ -97,6 +100,7 @@ struct mhd_bunch {
   bool all_nbr;        // no -1 entry in the neighbour table
   bool nbr_consistent; // the table composes like translations (see table_is_consistent)
   int tune_zseg;       // MHD_TUNE_ONEPASS_ZSEG: 0 = automatic
+  bool fused_cfl;      // MHD_TUNE_FUSED_CFL: the one-pass step reduces the new level's CFL rates in its epilogue
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
   std::vector<Ev>* events;
@@ -183,7 +187,7 @@ int build_geom(const mhd_bunch_desc* d, Geom* G) {
 }
 
 size_t head_bytes(int np) {
-  return align_up(sizeof(int) * 27 * (size_t)np, 256) + align_up(sizeof(unsigned long long) * (size_t)np, 256) + 256 + 256;
+  return align_up(sizeof(int) * 27 * (size_t)np, 256) + 2 * align_up(sizeof(unsigned long long) * (size_t)np, 256) + 256 + 256;
 }
 DGeom make_dgeom(const Geom& G, size_t esz, int chunk) {
   DGeom D;
@@ -272,6 +276,14 @@ template <typename T>
 int launch_cfl(mhd_bunch* b, double courant, void* dt_dev, void* dt_patch) {
   const Geom& G = b->G;
   Params<T> P = make_params<T>(b, 0, G.np);
+  if (b->rate_valid) {
+    // the one-pass step that produced this level reduced the rates in its epilogue (same function,
+    // same bits as k_cfl): only the bunch-wide reduction is left
+    LaunchScope ls(b, KC_MISC);
+    k_cfl_final<<<1, 256, 0, b->stream>>>(b->d_rate_next, G.np, courant, b->d_dt, (double*)dt_dev, (double*)dt_patch);
+    CUDA_TRY(cudaGetLastError());
+    return MHD_OK;
+  }
   { LaunchScope ls(b, KC_MISC); k_zero_u64<<<blocks_for(G.np, 256), 256, 0, b->stream>>>(b->d_rate, G.np); }
   const long long per = (long long)G.n[0] * G.n[1] * G.n[2];
 #ifndef CFL_CPT
@@ -312,14 +324,17 @@ template <> struct OnePassLaunch<float> {
   static int launch(mhd_bunch* b, const double* dtp, int p0, int npl, bool attr_only = false) {
     using Cfg = OneCfg<float, TX, TY, OneTile::NPW>;
     const Geom& G = b->G;
-    // limiter and flux solver are compile-time parameters of the kernel
-    auto kern = G.flux_solver == 1
-                    ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 1> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 1>)
-                    : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, 0> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, 0>);
     if (attr_only) {   // called once from create, on the handle's device (the attribute is per device)
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       return MHD_OK;
     }
+    // the limiter and the CFL epilogue are compile-time parameters of the kernel
+    auto kern = b->fused_cfl
+                    ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, true> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>)
+                    : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, false> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>);
     Params<float> P = make_params<float>(b, p0, npl);
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
     // fewer tiles than SMs: cut the columns into z segments of at least 8 planes so that the
@@ -335,7 +350,7 @@ template <> struct OnePassLaunch<float> {
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
-      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, xt, zseg);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, b->d_rate_next, xt, zseg);
     }
     CUDA_TRY(cudaGetLastError());
     return MHD_OK;
@@ -352,6 +367,7 @@ template <> struct OnePassLaunch<float> {
     if (last) {
       b->cur = 1 - b->cur;
       b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
+      b->rate_valid = b->fused_cfl;   // every patch went through the epilogue since the last k_set_dt
     }
     return MHD_OK;
   }
@@ -436,6 +452,7 @@ int launch_step(mhd_bunch* b) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
   const int path = effective_path(b);
+  b->rate_valid = false;     // set again below if the one-pass kernel (whose epilogue reduces the CFL rates) runs
   if (path == MHD_PATH_ONEPASS && b->gather_ok) return OnePassLaunch<T>::run(b, dtp);
   if (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) {
     // halos come through the neighbour table if the fill was deferred, from the shell otherwise
@@ -596,6 +613,8 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   char* p = b->ws;
   b->d_nbr = (int*)p;                 p += align_up(sizeof(int) * 27 * (size_t)desc->npatch, 256);
   b->d_rate = (unsigned long long*)p; p += align_up(sizeof(unsigned long long) * (size_t)desc->npatch, 256);
+  b->d_rate_next = (unsigned long long*)p; p += align_up(sizeof(unsigned long long) * (size_t)desc->npatch, 256);
+  b->rate_valid = false;
   b->d_bad = (unsigned long long*)p;  p += 256;
   b->d_dt = (double*)p;               p += 256;
   b->d_scratch = p;
@@ -644,6 +663,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->gather_ok = b->gather_ok && b->nbr_consistent;
   b->gather2_ok = b->fused_ok && b->nbr_consistent;
   b->tune_zseg = 0;
+  b->fused_cfl = false;
   b->hs = nullptr;
   b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
   if (!b->h_nbr) { delete b->events; delete b; return MHD_ENOMEM; }
@@ -704,14 +724,14 @@ static int step_common(mhd_bunch* b) {
 int mhd_bunch_step(mhd_bunch* b, double dt) {
   ENTER(b);
   if (!(dt > 0.0) || !isfinite(dt)) return MHD_EINVAL;
-  { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0); }
+  { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0, b->d_rate_next, b->G.np); }
   return step_common(b);
 }
 
 int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
   ENTER(b);
   if (!dt_dev || !(dt_max >= 0.0)) return MHD_EINVAL;
-  { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, (const double*)dt_dev, 0.0, dt_max); }
+  { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, (const double*)dt_dev, 0.0, dt_max, b->d_rate_next, b->G.np); }
   return step_common(b);
 }
 
@@ -721,6 +741,7 @@ int mhd_bunch_current(mhd_bunch* b, void** state) {
   const int rc = materialise_guards(b);   // the caller is about to look at the buffer
   if (rc != MHD_OK) return rc;
   b->closing_ok = false;                  // ... and may write it
+  b->rate_valid = false;
   *state = b->state[b->cur];
   return MHD_OK;
 }
@@ -757,6 +778,12 @@ int mhd_bunch_set_tuning(mhd_bunch* b, int32_t key, int32_t value) {
   if (value < 0) return MHD_EINVAL;
   if (key == MHD_TUNE_ONEPASS_ZSEG) {
     b->tune_zseg = value;
+    return MHD_OK;
+  }
+  if (key == MHD_TUNE_FUSED_CFL) {
+    if (value > 1 || !b->onepass_ok) return MHD_EINVAL;
+    b->fused_cfl = value == 1;
+    b->rate_valid = false;
     return MHD_OK;
   }
   if (key == MHD_TUNE_PREDICT_TY) {
@@ -834,6 +861,7 @@ int mhd_bunch_upload(mhd_bunch* b, const void* host_state) {
   ENTER(b);
   b->guards_stale = false;   // the whole buffer, guard shell included, is replaced
   b->closing_ok = false;
+  b->rate_valid = false;
   CUDA_TRY(cudaMemcpyAsync(b->state[b->cur], host_state, b->lay.state_bytes, cudaMemcpyHostToDevice, b->stream));
   return MHD_OK;
 }
@@ -1117,6 +1145,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
   }
   b->closing_ok = false;
   b->guards_stale = false;
+  b->rate_valid = false;
 
   const bool overlap_up = pipelined && have_dt;   // steps start while later chunks still upload
   if (!overlap_up) {
@@ -1128,7 +1157,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
     }
   }
   { LaunchScope ls(b, KC_MISC);
-    k_set_dt<<<1, 1, 0, b->stream>>>(b->d_dt + 1, have_dt ? nullptr : b->d_dt, dt, 0.0); }
+    k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, have_dt ? nullptr : b->d_dt, dt, 0.0, b->d_rate_next, b->G.np); }
 
   // ---- steps, and the way back: interiors of the new level -> staging -> host --------
   void* const next = b->state[1 - b->cur];
@@ -1161,6 +1190,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
     b->cur = 1 - b->cur;
     b->guards_stale = true;   // the new level's shell is owed (deferred fill), its closing faces are current
     b->closing_ok = true;
+    b->rate_valid = onepass && b->fused_cfl;  // every chunk went through the one-pass epilogue since k_set_dt
   } else {
     if ((rc = step_common(b)) != MHD_OK) return rc;
     CUDA_TRY(cudaEventRecord(h->ev_all_steps, b->stream));

@@ -23,6 +23,10 @@ template <> struct num<float> {
   static __device__ __forceinline__ float rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
   static __device__ __forceinline__ float rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
   static __device__ __forceinline__ float div(float a, float b) { return a * rcp(b); }
+  // single correctly rounded operations the compiler never fuses or reorders
+  static __device__ __forceinline__ float xmul(float a, float b) { return __fmul_rn(a, b); }
+  static __device__ __forceinline__ float xadd(float a, float b) { return __fadd_rn(a, b); }
+  static __device__ __forceinline__ float xfma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 };
 template <> struct num<double> {
   static __device__ __forceinline__ double eps() { return DBL_EPSILON; }
@@ -51,6 +55,9 @@ template <> struct num<double> {
     return fma(x, fma(e, e, e), x);                    // x (1 + e + e^2)
   }
   static __device__ __forceinline__ double div(double a, double b) { return a * rcp(b); }
+  static __device__ __forceinline__ double xmul(double a, double b) { return __dmul_rn(a, b); }
+  static __device__ __forceinline__ double xadd(double a, double b) { return __dadd_rn(a, b); }
+  static __device__ __forceinline__ double xfma(double a, double b, double c) { return __fma_rn(a, b, c); }
 };
 
 // ---- slope limiter: 0 at extrema; minmod (1) or monotonised central (2) -------------
@@ -84,6 +91,35 @@ __device__ __forceinline__ T fast_speed2(T gp, T b2, T bn2, T irho) {   // c_f^2
 template <typename T>
 __device__ __forceinline__ T fast_speed(T gp, T b2, T bn2, T irho) {
   return num<T>::sqrt(fast_speed2(gp, b2, bn2, irho));
+}
+
+// ---- CFL rate of a cell (O9): sum over active d of (|u_d| + c_f,d)/dx_d ----
+// From the conserved values and the six face fields of the cell.  Written with explicitly rounded
+// operations in a fixed order, so that every kernel that evaluates it (the stand-alone k_cfl and the
+// epilogue of the one-pass step) gets the same bits from the same inputs.  NaN -> +inf (dt = 0).
+template <typename T>
+__device__ __forceinline__ T cfl_rate(T gamma, T idx0, T idx1, T idx2, bool a0, bool a1, bool a2, T rho, T mx, T my, T mz,
+                                      T en, T bxl, T bxu, T byl, T byu, T bzl, T bzu) {
+  using N = num<T>;
+  const T h = T(0.5);
+  const T ir = N::rcp(rho);
+  const T u = N::xmul(mx, ir), v = N::xmul(my, ir), w = N::xmul(mz, ir);
+  const T bx = N::xmul(h, N::xadd(bxl, bxu)), by = N::xmul(h, N::xadd(byl, byu)), bz = N::xmul(h, N::xadd(bzl, bzu));
+  const T bx2 = N::xmul(bx, bx), by2 = N::xmul(by, by), bz2 = N::xmul(bz, bz);
+  const T b2 = N::xadd(N::xadd(bx2, by2), bz2);
+  const T v2 = N::xfma(w, w, N::xfma(v, v, N::xmul(u, u)));
+  const T pr = N::xmul(gamma - T(1), N::xadd(N::xfma(-N::xmul(h, rho), v2, en), -N::xmul(h, b2)));
+  const T gp = N::xmul(gamma, pr);
+  const T s = N::xadd(gp, b2), s2 = N::xmul(s, s), g4 = N::xmul(T(4), gp);
+  auto cf = [&](T bn2) {
+    const T disc = N::max(N::xfma(-g4, bn2, s2), T(0));
+    return N::sqrt(N::xmul(N::xmul(h, N::xadd(s, N::sqrt(disc))), ir));
+  };
+  T rate = T(0);
+  if (a0) rate = N::xfma(N::xadd(N::abs(u), cf(bx2)), idx0, rate);
+  if (a1) rate = N::xfma(N::xadd(N::abs(v), cf(by2)), idx1, rate);
+  if (a2) rate = N::xfma(N::xadd(N::abs(w), cf(bz2)), idx2, rate);
+  return rate == rate ? rate : T(INFINITY);
 }
 
 // primitive state seen by a 1D Riemann problem: normal velocity u, transverse (v,w),

@@ -33,20 +33,24 @@
 namespace mhd {
 
 // Named barriers.  bar.sync / bar.arrive are the .aligned forms: they ASSERT that the whole warp
-// executes them together, and ptxas uses that assertion -- it may place the reconvergence point of
-// a preceding divergent `if` after the barrier and drop a __syncwarp() in front of it as redundant,
-// so that a warp whose lanes took different sides arrives twice (seen in SASS; the barrier count
-// then drifts and the CTA hangs).  Hence: the non-aligned forms, which assert nothing, behind a
-// __syncwarp() that makes the warp whole; and the predictor passes keep their lanes together
-// (tasks are clamped, not skipped, inside a partly filled warp).  Every call site is reached by
-// all non-exited lanes of its warp.
-__device__ __forceinline__ void nb_sync(int id, int n) {
-  __syncwarp();
-  asm volatile("barrier.sync %0, %1;" ::"r"(id), "r"(n) : "memory");
+// executes them together, and ptxas uses that assertion -- seen in SASS: it merged the convergence
+// region of a lane-divergent `if` with the enclosing one whose end lay after a bar.arrive, and
+// dropped the __syncwarp() in front of it as redundant; the warp then arrived twice, the barrier
+// count drifted and the CTA hung.  (The non-aligned barrier.sync / barrier.arrive are safe but make
+// the kernel 5 % slower.)  The rules that keep the aligned forms sound here:
+//   * a barrier is never nested in an `if`: conditional ones are PREDICATED instructions
+//     (nb_sync_if / nb_arrive_if) at the top level of the role's plane loop, so no convergence
+//     region can span them;
+//   * the predictor passes keep the lanes of a warp together (tasks are clamped, not skipped);
+//   * tests/test_abi_cpu.py disassembles the library and fails if a named barrier lies inside any
+//     convergence region (BSSY ... BSYNC).
+__device__ __forceinline__ void nb_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void nb_sync_if(bool c, int id, int n) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %0, 0;\n\t@p bar.sync %1, %2;\n\t}" ::"r"((int)c), "r"(id), "r"(n) : "memory");
 }
-__device__ __forceinline__ void nb_arrive(int id, int n) {
-  __syncwarp();
-  asm volatile("barrier.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
+__device__ __forceinline__ void nb_arrive_if(bool c, int id, int n) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %0, 0;\n\t@p bar.arrive %1, %2;\n\t}" ::"r"((int)c), "r"(id), "r"(n) : "memory");
 }
 // 16-byte asynchronous copy global -> shared (L2 only), and the wait for all of a thread's copies
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
@@ -101,8 +105,8 @@ template <typename T, int TX, int TY, int NPW> struct OneCfg {
   static constexpr size_t o_d = o_rawb + 4 * rawb_slot;                // [2][38][DCS]
   static constexpr size_t o_q = o_d + al(sizeof(T) * 2 * D_COUNT * DCS);  // [3][8][RA]
   static constexpr size_t o_e = o_q + al(sizeof(T) * 3 * 8 * RA);      // [2][3][RA]
-  static constexpr size_t o_pu = o_e + al(sizeof(T) * 2 * 3 * RA);     // [7][FA]   C -> A partial update
-  static constexpr size_t o_xe = o_pu + al(sizeof(T) * 7 * FA);        // [2][NR]   A: ex, ey of the neighbours
+  static constexpr size_t o_pu = o_e + al(sizeof(T) * 2 * 3 * RA);     // [8][FA]   C -> A partial update; A -> C new values (CFL)
+  static constexpr size_t o_xe = o_pu + al(sizeof(T) * 8 * FA);        // [2][NR]   A: ex, ey of the neighbours
   static constexpr size_t o_xy = o_xe + al(sizeof(T) * 2 * NR);        // [6][NR]   C: +y exchange
   static constexpr size_t o_xc = o_xy + al(sizeof(T) * 6 * NR);        // [6][32]   C: closing column -> column TX-1
   static constexpr size_t o_nb = o_xc + al(sizeof(T) * 6 * 32);        // [27] source patch per neighbour class
@@ -153,10 +157,12 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
   return c[(D_BH + X) * DCS] + s * c[dbf_slot(X, ALONG) * DCS];
 }
 
-template <typename T, int TX, int TY, int NPW, int LIM, int FS>
+// LIM: limiter (1 minmod, 2 monotonised central), fixed at compile time; CFLE: reduce the CFL rates
+// of the new level in the epilogue (role C), so that mhd_bunch_cfl_dt has nothing left to read
+template <typename T, int TX, int TY, int NPW, int LIM, bool CFLE>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
-               unsigned long long* __restrict__ bad, int xtiles, int zseg) {
+               unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int zseg) {
   using C = OneCfg<T, TX, TY, NPW>;
   constexpr int PH = C::PH, BWX = C::BWX, RA = C::RA, DP = C::DP, DCS = C::DCS;
   constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL, NS = C::NS;
@@ -358,9 +364,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 
       // ---- D data of plane kd = r-2 -> shared slot
       const int kd = r - 2;
+      nb_sync_if(kd >= rlo && kd >= za + 1, NB_EMPTY + ((kd + 2) & 1), NALL);   // A and C are done with plane kd-2
       if (kd >= rlo) {
         T* const Dw = dslot(kd);
-        if (kd >= za + 1) nb_sync(NB_EMPTY + ((kd + 2) & 1), NALL);   // A and C are done with plane kd-2
         const T* b0 = RB(kd);
         const T* b1 = RB(kd + 1);
         const T *qc = Qs(kd), *qm = Qs(kd - 1), *qp = Qs(kd + 1);
@@ -479,11 +485,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
             cbx[s_][0] = fwx[0]; cbx[s_][1] = fwx[1]; cby[s_][0] = fwy[0]; cby[s_][1] = fwy[1];
           }
         }
-        if (kd >= za - 1) {
-          __threadfence_block();
-          nb_arrive(NB_FULL + ((kd + 2) & 1), NALL);
-        }
       }
+      __threadfence_block();
+      nb_arrive_if(kd >= rlo && kd >= za - 1, NB_FULL + ((kd + 2) & 1), NALL);
       cp_async_wait_all();   // own chunks of hydro plane r and field plane r+1 have landed ...
       nb_sync(NB_P, NP);     // ... and everybody's; the rings are rewritten by the next iteration
     }
@@ -502,6 +506,9 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const bool cell = active && (fi < tw) && (fj < th);
   const bool xface = active && (fj < th) && (fi < tw || lastx);   // bx faces of the tile (closing face at the patch end)
   const bool yface = active && (fi < tw) && (fj < th || lasty);
+  // the new face fields are also FORMED (not stored) on the tile's upper sides inside the patch: the
+  // CFL rate of the last column / row of cells needs both faces of every cell
+  const bool xcomp = active && (fj < th), ycomp = active && (fi < tw);
   const int own = (fj + 1) * DP + (fi + 4);          // D cell of (fi, fj): row fj+1, column rc = fi+4
   const int fidx = min(fj, C::FH - 1) * FW + fi;
   const int tyn = colthr ? tr + 1 : tr + TX;              // thread that owns (fi, fj+1)
@@ -510,7 +517,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const long long ubase = (long long)(P.p0 + pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
                           (long long)(y0 + fj + G.g[1]) * G.pitch + (long long)G.g[2] * plane;
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
-  const int solver = G.emf_solver;
+  const int solver = G.emf_solver, FS = G.flux_solver;
 
   if (roleA) {
     // ------------------------------------------------------------- role A -----------
@@ -519,6 +526,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
     const bool doEy = active && (fj < th);      // ey(i..i+1, j): bx faces and b_z
     Flux5<T> pFz = {};
     T pex = T(0), pey = T(0);
+    T bzlo = T(0);                              // new b_z on the lower face of the plane below
     nb_sync(NB_FULL + ((za + 1) & 1), NALL);    // plane za-1
     for (int k = za; k <= zb; ++k) {
       nb_sync(NB_FULL + ((k + 2) & 1), NALL);   // plane k
@@ -541,25 +549,29 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
         ynw = corner_state<T, DCS, 1>(dp_, h, -h);
         yBW = edge_field<T, DCS, 0, 2>(dp_, h);
       }
-      if (k + 1 <= zb) nb_arrive(NB_EMPTY + ((k + 1) & 1), NALL);   // slot of plane k-1
+      nb_arrive_if(k + 1 <= zb, NB_EMPTY + ((k + 1) & 1), NALL);   // slot of plane k-1
 
       Flux5<T> cFz = {};
       T cex = T(0), cey = T(0);
-      if (doFz) cFz = riemann_flux_k<FS>(gamma, Lz, face_state<T, DCS, 2>(dc_, -h), dc_[(D_BH + 2) * DCS]);
+      if (doFz) cFz = riemann_flux(FS, gamma, Lz, face_state<T, DCS, 2>(dc_, -h), dc_[(D_BH + 2) * DCS]);
       // The hydro part of plane k-1 only waits for this flux: finish it now (C is ahead, its
       // partial update is normally there already), so that the previous plane's flux is dead
       // while the two edge problems are solved.
       const long long cu = ubase + (long long)(k - 1) * plane;
-      const T* pu = PU + fidx;
-      if (k >= za + 1) {
-        nb_sync(NB_PUF, 2 * NR);
-        if (cell) {
-          // O8: (U - dt*dFx/dx - dt*dFy/dy) - dt*dFz/dz; z-face frame (mu,mv,mw) = (mz,mx,my)
-          P.Un[cu] = pu[0] - cz * (cFz.d - pFz.d);
-          P.Un[fs + cu] = pu[FA] - cz * (cFz.mv - pFz.mv);
-          P.Un[2 * fs + cu] = pu[2 * FA] - cz * (cFz.mw - pFz.mw);
-          P.Un[3 * fs + cu] = pu[3 * FA] - cz * (cFz.mu - pFz.mu);
-          P.Un[4 * fs + cu] = pu[4 * FA] - cz * (cFz.e - pFz.e);
+      T* pu = PU + fidx;
+      nb_sync_if(k >= za + 1, NB_PUF, 2 * NR);
+      {
+        if (k >= za + 1 && cell) {
+          // O8: (U - dt*dFx/dx - dt*dFy/dy) - dt*dFz/dz; z-face frame (mu,mv,mw) = (mz,mx,my).
+          // The new values also replace the partial ones in this thread's own PU entries: role C
+          // picks them up after NB_PUE for the CFL rate of the new level.
+          const T n0 = pu[0] - cz * (cFz.d - pFz.d);
+          const T n1 = pu[FA] - cz * (cFz.mv - pFz.mv);
+          const T n2 = pu[2 * FA] - cz * (cFz.mw - pFz.mw);
+          const T n3 = pu[3 * FA] - cz * (cFz.mu - pFz.mu);
+          const T n4 = pu[4 * FA] - cz * (cFz.e - pFz.e);
+          P.Un[cu] = n0; P.Un[fs + cu] = n1; P.Un[2 * fs + cu] = n2; P.Un[3 * fs + cu] = n3; P.Un[4 * fs + cu] = n4;
+          if (CFLE) { pu[0] = n0; pu[FA] = n1; pu[2 * FA] = n2; pu[3 * FA] = n3; pu[4 * FA] = n4; }
         }
       }
       pFz = cFz;
@@ -576,12 +588,26 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       const T yex = XE[tyn], xey = XE[NR + txn];
       // b_z on the lower z-face of plane k (k = nz: closing face) -- Eq. 12
       // (face zb belongs to the next segment unless it is the patch's closing face)
-      if (cell && (k < zb || zb == nz)) P.Un[7 * fs + ubase + (long long)k * plane] = u7 + (cx * (xey - cey) - cy * (yex - cex));
+      const T bzn = u7 + (cx * (xey - cey) - cy * (yex - cex));
+      if (cell && (k < zb || zb == nz)) P.Un[7 * fs + ubase + (long long)k * plane] = bzn;
       if (k >= za + 1) {
-        if (xface) P.Un[5 * fs + cu] = pu[5 * FA] - cz * (cey - pey);
-        if (yface) P.Un[6 * fs + cu] = pu[6 * FA] + cz * (cex - pex);
-        if (k <= zb - 1) nb_arrive(NB_PUE, 2 * NR);
+        // new b_x, b_y of plane k-1; with the cell-centred new b_z they join the new hydro values in
+        // the PU entries (every face of the tile, also those another tile stores)
+        if (CFLE ? xcomp : xface) {
+          const T bxn = pu[5 * FA] - cz * (cey - pey);
+          if (xface) P.Un[5 * fs + cu] = bxn;
+          if (CFLE) pu[5 * FA] = bxn;
+        }
+        if (CFLE ? ycomp : yface) {
+          const T byn = pu[6 * FA] + cz * (cex - pex);
+          if (yface) P.Un[6 * fs + cu] = byn;
+          if (CFLE) pu[6 * FA] = byn;
+        }
+        if (CFLE && cell) pu[7 * FA] = num<T>::xmul(h, num<T>::xadd(bzlo, bzn));
       }
+      if (CFLE) __threadfence_block();
+      nb_arrive_if(k >= za + 1, NB_PUE, 2 * NR);
+      bzlo = bzn;
       pex = cex; pey = cey;
     }
     return;
@@ -591,6 +617,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   {
     const bool doFx = active && (fj < th);
     const bool doFy = active && (fi < tw);
+    T rmax = T(0);                              // largest CFL rate of the own cells (new level)
     for (int kd = za - 1; kd <= zb; ++kd) {
       nb_sync(NB_FULL + ((kd + 2) & 1), NALL);
       const bool work = (kd >= za) && (kd <= zb - 1);
@@ -605,57 +632,87 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 #pragma unroll
           for (int f = 0; f < 5; ++f) un[f] = P.U[f * fs + cu];
         }
-        if (xface) un[5] = P.U[5 * fs + cu];
-        if (yface) un[6] = P.U[6 * fs + cu];
+        if (CFLE ? xcomp : xface) un[5] = P.U[5 * fs + cu];
+        if (CFLE ? ycomp : yface) un[6] = P.U[6 * fs + cu];
         const T* dc_ = dslot(kd) + own;
-        if (doFx) Fx = riemann_flux_k<FS>(gamma, face_state<T, DCS, 0>(dc_ - 1, h), face_state<T, DCS, 0>(dc_, -h), dc_[(D_BH + 0) * DCS]);
-        if (doFy) Fy = riemann_flux_k<FS>(gamma, face_state<T, DCS, 1>(dc_ - DP, h), face_state<T, DCS, 1>(dc_, -h), dc_[(D_BH + 1) * DCS]);
+        if (doFx) Fx = riemann_flux(FS, gamma, face_state<T, DCS, 0>(dc_ - 1, h), face_state<T, DCS, 0>(dc_, -h), dc_[(D_BH + 0) * DCS]);
+        if (doFy) Fy = riemann_flux(FS, gamma, face_state<T, DCS, 1>(dc_ - DP, h), face_state<T, DCS, 1>(dc_, -h), dc_[(D_BH + 1) * DCS]);
         if (active)   // ez, in-plane (x,y): sw=(i-1,j-1) se=(i,j-1) nw=(i-1,j) ne=(i,j)
           ez = emf_2d(gamma, solver, corner_state<T, DCS, 2>(dc_ - DP - 1, h, h), corner_state<T, DCS, 2>(dc_ - DP, -h, h),
                       corner_state<T, DCS, 2>(dc_ - 1, h, -h), corner_state<T, DCS, 2>(dc_, -h, -h),
                       edge_field<T, DCS, 0, 1>(dc_ - DP, h), edge_field<T, DCS, 0, 1>(dc_, -h),
                       edge_field<T, DCS, 1, 0>(dc_ - 1, h), edge_field<T, DCS, 1, 0>(dc_, -h));
       }
-      if (kd + 2 <= zb) nb_arrive(NB_EMPTY + ((kd + 2) & 1), NALL);   // done with plane kd
-      if (!work) continue;
+      nb_arrive_if(kd + 2 <= zb, NB_EMPTY + ((kd + 2) & 1), NALL);   // done with plane kd
 
       // neighbours: +x by warp shuffle (the closing column hands its values over through XC),
       // +y through XY
-      XY[tr] = Fy.d; XY[NR + tr] = Fy.mu; XY[2 * NR + tr] = Fy.mv; XY[3 * NR + tr] = Fy.mw; XY[4 * NR + tr] = Fy.e;
-      XY[5 * NR + tr] = ez;
-      if (colthr) {
-        XC[fj] = Fx.d; XC[32 + fj] = Fx.mu; XC[2 * 32 + fj] = Fx.mv; XC[3 * 32 + fj] = Fx.mw; XC[4 * 32 + fj] = Fx.e;
-        XC[5 * 32 + fj] = ez;
+      if (work) {
+        XY[tr] = Fy.d; XY[NR + tr] = Fy.mu; XY[2 * NR + tr] = Fy.mv; XY[3 * NR + tr] = Fy.mw; XY[4 * NR + tr] = Fy.e;
+        XY[5 * NR + tr] = ez;
+        if (colthr) {
+          XC[fj] = Fx.d; XC[32 + fj] = Fx.mu; XC[2 * 32 + fj] = Fx.mv; XC[3 * 32 + fj] = Fx.mw; XC[4 * 32 + fj] = Fx.e;
+          XC[5 * 32 + fj] = ez;
+        }
       }
-      nb_sync(NB_C, NR);
-      Flux5<T> xF, yF;
-      xF.d = __shfl_down_sync(0xffffffffu, Fx.d, 1);   xF.mu = __shfl_down_sync(0xffffffffu, Fx.mu, 1);
-      xF.mv = __shfl_down_sync(0xffffffffu, Fx.mv, 1); xF.mw = __shfl_down_sync(0xffffffffu, Fx.mw, 1);
-      xF.e = __shfl_down_sync(0xffffffffu, Fx.e, 1);
-      T xez = __shfl_down_sync(0xffffffffu, ez, 1);
-      if (!colthr && fi == TX - 1) {
-        const int cj = min(fj, 31);
-        xF.d = XC[cj]; xF.mu = XC[32 + cj]; xF.mv = XC[2 * 32 + cj]; xF.mw = XC[3 * 32 + cj]; xF.e = XC[4 * 32 + cj];
-        xez = XC[5 * 32 + cj];
-      }
-      const int ty_ = min(tyn, NR - 1);
-      yF.d = XY[ty_]; yF.mu = XY[NR + ty_]; yF.mv = XY[2 * NR + ty_]; yF.mw = XY[3 * NR + ty_]; yF.e = XY[4 * NR + ty_];
-      const T yez = XY[5 * NR + ty_];
-
-      if (kd >= za + 1) nb_sync(NB_PUE, 2 * NR);   // A has consumed the previous plane
+      // A has consumed the previous plane's partial update and left the NEW values of that plane
+      // in the PU entries: take the ten a cell's CFL rate needs before the entries are rewritten
+      const bool newvals = kd >= za + 1;
+      nb_sync_if(newvals, NB_PUE, 2 * NR);
       T* pu = PU + fidx;
-      if (cell) {
-        // momentum components by solver frame: x-face (mu,mv,mw)=(mx,my,mz); y-face (mu,mv,mw)=(my,mz,mx)
-        pu[0] = un[0] - cx * (xF.d - Fx.d) - cy * (yF.d - Fy.d);
-        pu[FA] = un[1] - cx * (xF.mu - Fx.mu) - cy * (yF.mw - Fy.mw);
-        pu[2 * FA] = un[2] - cx * (xF.mv - Fx.mv) - cy * (yF.mu - Fy.mu);
-        pu[3 * FA] = un[3] - cx * (xF.mw - Fx.mw) - cy * (yF.mv - Fy.mv);
-        pu[4 * FA] = un[4] - cx * (xF.e - Fx.e) - cy * (yF.e - Fy.e);
+      T nv[10];
+#pragma unroll
+      for (int f = 0; f < 10; ++f) nv[f] = T(1);
+      if (CFLE && newvals && cell) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) nv[f] = pu[f * FA];
+        nv[5] = pu[5 * FA]; nv[6] = pu[5 * FA + 1];          // new b_x on both x-faces of the cell
+        nv[7] = pu[6 * FA]; nv[8] = pu[6 * FA + FW];         // new b_y on both y-faces
+        nv[9] = pu[7 * FA];                                  // cell-centred new b_z
       }
-      if (xface) pu[5 * FA] = un[5] + cy * (yez - ez);
-      if (yface) pu[6 * FA] = un[6] - cx * (xez - ez);
+      nb_sync(NB_C, NR);      // every C thread has its XY/XC values out and its new values in
+      if (work) {
+        Flux5<T> xF, yF;
+        xF.d = __shfl_down_sync(0xffffffffu, Fx.d, 1);   xF.mu = __shfl_down_sync(0xffffffffu, Fx.mu, 1);
+        xF.mv = __shfl_down_sync(0xffffffffu, Fx.mv, 1); xF.mw = __shfl_down_sync(0xffffffffu, Fx.mw, 1);
+        xF.e = __shfl_down_sync(0xffffffffu, Fx.e, 1);
+        T xez = __shfl_down_sync(0xffffffffu, ez, 1);
+        if (!colthr && fi == TX - 1) {
+          const int cj = min(fj, 31);
+          xF.d = XC[cj]; xF.mu = XC[32 + cj]; xF.mv = XC[2 * 32 + cj]; xF.mw = XC[3 * 32 + cj]; xF.e = XC[4 * 32 + cj];
+          xez = XC[5 * 32 + cj];
+        }
+        const int ty_ = min(tyn, NR - 1);
+        yF.d = XY[ty_]; yF.mu = XY[NR + ty_]; yF.mv = XY[2 * NR + ty_]; yF.mw = XY[3 * NR + ty_]; yF.e = XY[4 * NR + ty_];
+        const T yez = XY[5 * NR + ty_];
+        if (cell) {
+          // momentum components by solver frame: x-face (mu,mv,mw)=(mx,my,mz); y-face (mu,mv,mw)=(my,mz,mx)
+          pu[0] = un[0] - cx * (xF.d - Fx.d) - cy * (yF.d - Fy.d);
+          pu[FA] = un[1] - cx * (xF.mu - Fx.mu) - cy * (yF.mw - Fy.mw);
+          pu[2 * FA] = un[2] - cx * (xF.mv - Fx.mv) - cy * (yF.mu - Fy.mu);
+          pu[3 * FA] = un[3] - cx * (xF.mw - Fx.mw) - cy * (yF.mv - Fy.mv);
+          pu[4 * FA] = un[4] - cx * (xF.e - Fx.e) - cy * (yF.e - Fy.e);
+        }
+        if (CFLE ? xcomp : xface) pu[5 * FA] = un[5] + cy * (yez - ez);
+        if (CFLE ? ycomp : yface) pu[6 * FA] = un[6] - cx * (xez - ez);
+      }
       __threadfence_block();
-      nb_arrive(NB_PUF, 2 * NR);
+      nb_arrive_if(work, NB_PUF, 2 * NR);
+      // CFL rate of the NEW level in cell (fi, fj, kd-1) (O9), off A's critical path:
+      // the step's epilogue replaces a separate pass over the state the step has just written
+      if (CFLE && newvals && cell) {
+        const T rate = cfl_rate<T>(gamma, P.idx[0], P.idx[1], P.idx[2], true, true, true, nv[0], nv[1], nv[2], nv[3], nv[4],
+                                   nv[5], nv[6], nv[7], nv[8], nv[9], nv[9]);
+        rmax = num<T>::max(rmax, rate);
+      }
+    }
+    // per-patch maximum: warp shuffle, then one integer atomicMax per warp on the bit pattern
+    // (positive doubles order like their bits: deterministic, no floating-point atomics)
+    if (CFLE) {
+      double rd = (double)rmax;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) rd = fmax(rd, __shfl_xor_sync(0xffffffffu, rd, o));
+      if ((t & 31) == 0) atomicMax(&rate_next[P.p0 + pl], enc_max(rd));
     }
   }
 }

@@ -138,21 +138,11 @@ __global__ void __launch_bounds__(256) k_cfl(Params<T> P, unsigned long long* __
     const long long c = (long long)p * G.ps + G.lead + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch +
                         (long long)(k + G.g[2]) * G.pitch * G.m[1];
     const T* U = P.U;
-    const T rho = U[c], irho = num<T>::rcp(rho);
-    const T u = U[G.fs + c] * irho, v = U[2 * G.fs + c] * irho, w = U[3 * G.fs + c] * irho;
-    const T bx = T(0.5) * (U[5 * G.fs + c] + U[5 * G.fs + c + G.s[0]]);
-    const T by = T(0.5) * (U[6 * G.fs + c] + U[6 * G.fs + c + G.s[1]]);
-    const T bz = T(0.5) * (U[7 * G.fs + c] + U[7 * G.fs + c + G.s[2]]);
-    const T b2 = bx * bx + by * by + bz * bz;
-    const T pr = (P.gamma - T(1)) * (U[4 * G.fs + c] - T(0.5) * rho * (u * u + v * v + w * w) - T(0.5) * b2);
-    const T gp = P.gamma * pr;
-    T rate = T(0);
-    if (G.act[0]) rate += (num<T>::abs(u) + fast_speed(gp, b2, bx * bx, irho)) * P.idx[0];
-    if (G.act[1]) rate += (num<T>::abs(v) + fast_speed(gp, b2, by * by, irho)) * P.idx[1];
-    if (G.act[2]) rate += (num<T>::abs(w) + fast_speed(gp, b2, bz * bz, irho)) * P.idx[2];
-    double rd = (double)rate;
-    if (!(rd == rd)) rd = INFINITY;  // a NaN cell forces dt = 0 rather than being ignored
-    rmax = fmax(rmax, rd);
+    const T rate = cfl_rate<T>(P.gamma, P.idx[0], P.idx[1], P.idx[2], G.act[0] != 0, G.act[1] != 0, G.act[2] != 0, U[c],
+                               U[G.fs + c], U[2 * G.fs + c], U[3 * G.fs + c], U[4 * G.fs + c], U[5 * G.fs + c],
+                               U[5 * G.fs + c + G.s[0]], U[6 * G.fs + c], U[6 * G.fs + c + G.s[1]], U[7 * G.fs + c],
+                               U[7 * G.fs + c + G.s[2]]);   // a NaN cell comes back as +inf: dt = 0 rather than being ignored
+    rmax = fmax(rmax, (double)rate);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
@@ -212,11 +202,17 @@ __global__ void __launch_bounds__(256) k_fma_peak(T* out, int iters, T a, T b) {
   if (s == T(-1)) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true: keeps the chains alive
 }
 
-// dt for a step, on the device: either the host value or min(*dt_dev, dt_max)
-__global__ void k_set_dt(double* dst, const double* src, double host_dt, double dt_max) {
-  double dt = src ? *src : host_dt;
-  if (dt_max > 0.0 && dt > dt_max) dt = dt_max;
-  *dst = dt;
+// dt for a step, on the device: either the host value or min(*dt_dev, dt_max).  The same launch
+// clears the per-patch rate maxima the step's epilogue is about to accumulate for the new level.
+__global__ void __launch_bounds__(256) k_set_dt(double* dst, const double* src, double host_dt, double dt_max,
+                                                unsigned long long* __restrict__ rate_next, int np) {
+  if (threadIdx.x == 0) {
+    double dt = src ? *src : host_dt;
+    if (dt_max > 0.0 && dt > dt_max) dt = dt_max;
+    *dst = dt;
+  }
+  if (rate_next)
+    for (int p = threadIdx.x; p < np; p += blockDim.x) rate_next[p] = 0ull;
 }
 
 // ------------------------------------------------------------------- step stages ----

@@ -112,3 +112,35 @@ def test_product_package_does_not_import_the_oracle():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert "oracle" not in open(os.path.join(root, f)).read().replace("the CPU oracle", "").replace("CPU oracle's", ""), f
+
+
+def test_no_named_barrier_inside_a_convergence_region():
+    """The one-pass kernel's named barriers are the .aligned forms, which ptxas takes as a promise
+    that the warp is whole; it once merged the convergence region of a divergent `if` with an outer
+    one that ended after a bar.arrive, so that a warp arrived twice and the CTA hung (see
+    onepass_kernel.cuh).  The source now keeps every barrier at the top level of its loop; this
+    disassembles the built library and checks the result: no BAR.SYNC / BAR.ARV with a non-zero id
+    (named barrier) may lie inside a BSSY ... BSYNC region that holds a lane-predicated forward
+    branch before it."""
+    import re
+    import subprocess
+    txt = subprocess.run(["cuobjdump", "-sass", B._build.TARGET], capture_output=True, text=True, check=True).stdout
+    checked = 0
+    for f in re.split(r"\n\s*Function : ", txt)[1:]:
+        name = f.split("\n", 1)[0].strip()
+        if "k_step_onepass" not in name:
+            continue
+        ins = [(int(m.group(1), 16), m.group(2).strip())
+               for m in (re.match(r"\s*/\*([0-9a-f]{4,6})\*/\s+(.*?);", l) for l in f.splitlines()) if m]
+        regions = [(a, int(m.group(1), 16)) for a, x in ins
+                   for m in [re.match(r"(?:@!?U?P\d+\s+)?BSSY(?:\.\w+)*\s+B\d+,\s*0x([0-9a-f]+)", x)] if m]
+        bars = [(a, x) for a, x in ins if re.search(r"\bBAR\.(SYNC|ARV)", x) and not re.search(r"BAR\.SYNC(\.\w+)*\s+0x0\s*$", x)]
+        assert len(bars) >= 10, name
+        for a, x in bars:
+            for s, e in regions:
+                if s < a < e:
+                    inside = [(ba, bx) for ba, bx in ins if s < ba < a and re.match(r"@!?P\d+\s+BRA\b", bx)
+                              and ba < int(re.search(r"0x([0-9a-f]+)", bx).group(1), 16) <= e]
+                    assert not inside, (name, hex(a), x, [(hex(p), q) for p, q in inside[:3]])
+        checked += 1
+    assert checked >= 8

@@ -672,3 +672,38 @@ def test_config4_corner_4096_patches_of_64_cubed():
         for p in same[1:].tolist():
             assert torch.equal(v[:, p][(slice(None),) + I], first), (q, p)
     b.close()
+
+
+# ------------------------------------------------ CFL reduction in the step's epilogue -------
+@pytest.mark.parametrize("name", ["turb16", "turb_ragged", "turb_self", "turb_nx10", "turb_nx38", "turb_thin"])
+def test_fused_cfl_epilogue_is_bitwise_the_standalone_reduction(name):
+    """The one-pass step reduces the CFL rates of the level it writes in its epilogue (SURVEY 8d);
+    mhd_bunch_cfl_dt then only runs the bunch-wide reduction.  The step it returns, and the per-patch
+    steps, must equal those of the stand-alone pass over the stored state bit for bit (both evaluate
+    the same explicitly rounded function), and the oracle's within the CFL tolerance."""
+    w = small_workloads("f32")[name]
+    b = make_gpu(w, "f32")
+    assert b.path == "onepass"
+    b.set_tuning("fused_cfl", 1)
+    o = make_oracle(w)
+    for _ in range(3):
+        b.fill_guards(); dt = b.cfl_dt(0.4, sync=True); b.step(dt)
+    b.fill_guards()
+    l0 = b.launches
+    dt_f = b.cfl_dt(0.4, sync=True, per_patch=True)
+    n_f, pp_f = b.launches - l0, b.dt_patch.cpu().numpy().copy()
+    U = b.download().astype(np.float64)          # looking at the buffer: the library must fall back to the full pass
+    b.fill_guards()
+    l0 = b.launches
+    dt_s = b.cfl_dt(0.4, sync=True, per_patch=True)
+    n_s, pp_s = b.launches - l0, b.dt_patch.cpu().numpy().copy()
+    assert n_f == 1 and n_s == 3, (n_f, n_s)
+    assert dt_f == dt_s and np.array_equal(pp_f, pp_s)
+    dt_o, pp_o = o.cfl_dt(o.fill_guards(U, w.nbr), 0.4, per_patch=True)
+    assert abs(dt_f - dt_o) <= 2e-6 * dt_o and np.all(np.abs(pp_f - pp_o) <= 2e-6 * pp_o)
+    # the state itself does not depend on the epilogue: a handle without it, same steps, same bits
+    c = make_gpu(w, "f32")
+    for _ in range(3):
+        c.fill_guards(); dt = c.cfl_dt(0.4, sync=True); c.step(dt)
+    assert np.array_equal(masked(c.download(), w.n), masked(U.astype(np.float32), w.n))
+    b.close(); c.close()
