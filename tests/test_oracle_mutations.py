@@ -3,7 +3,7 @@
 Every entry of MUTANTS is a plausible mistake -- a swapped weight, a dropped term, a wrong sign,
 index or metric factor -- applied as an exact text substitution to a COPY of oracle/mhd_oracle.c in
 a temporary directory.  The copy is compiled and the pin suites (tests/test_oracle_pointwise.py,
-test_oracle_stages.py, test_oracle_scheme.py) are run against it in a subprocess
+test_oracle_stages.py, test_oracle_scheme.py, test_oracle_local.py) are run against it in a subprocess
 (MHD_ORACLE_LIBDIR, see oracle/__init__.py).  A mutant that passes every pin is a hole in the
 pins, and this test fails.  The unmutated copy must pass (the harness itself is sound) and every
 substitution must match exactly once (the list follows the source).
@@ -17,7 +17,8 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, "oracle", "mhd_oracle.c")
-PINS = ["tests/test_oracle_pointwise.py", "tests/test_oracle_stages.py", "tests/test_oracle_scheme.py"]
+PINS = ["tests/test_oracle_pointwise.py", "tests/test_oracle_stages.py", "tests/test_oracle_scheme.py",
+        "tests/test_oracle_local.py"]
 
 # name: (old text, new text, pin files to try first)
 MUTANTS = {
@@ -100,6 +101,19 @@ MUTANTS = {
         "                                        - (S->emf[b][c + s[e]] - S->emf[b][c]) / G->dx[e]);",
         "Un[5 + a][c] = Up[5 + a][c] + dt * ((S->emf[e][c + s[b]] - S->emf[e][c]) / G->dx[e]\n"
         "                                        - (S->emf[b][c + s[e]] - S->emf[b][c]) / G->dx[b]);", PINS[1:]),
+    # ---- O10, local time steps -------------------------------------------------------------
+    "O10: interpolation weight measured from the wrong slice": (
+        "real w = (real)((t_new[p] - t_old[q]) / (t_new[q] - t_old[q]));",
+        "real w = (real)((t_new[q] - t_new[p]) / (t_new[q] - t_old[q]));", PINS[3:]),
+    "O10: interpolation to the patch's OLD time": (
+        "real w = (real)((t_new[p] - t_old[q]) / (t_new[q] - t_old[q]));",
+        "real w = (real)((t_old[p] - t_old[q]) / (t_new[q] - t_old[q]));", PINS[3:]),
+    "O10: no interpolation (newer slice always)": (
+        "v = vold + w * (vnew - vold);", "v = vnew;", PINS[3:]),
+    "O10: readiness accepts a patch that is ahead of a neighbour": (
+        "int hi_ok = t_new[p] <= t_new[q] || times_equal(t_new[p], t_new[q]);", "int hi_ok = 1;", PINS[3:]),
+    "O10: the step writes the newer slice instead of the older": (
+        "Un[f] = S[1 - cur[p]] + ((long)f * G.np + p) * G.M;", "Un[f] = S[cur[p]] + ((long)f * G.np + p) * G.M;", PINS[3:]),
     "O9: CFL sum over directions replaced by the last term": (
         "rate += (R_FABS(vel[a]) + cf) / G.dx[a];", "rate = (R_FABS(vel[a]) + cf) / G.dx[a];", PINS[1:2]),
 }
