@@ -187,6 +187,38 @@ int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t chunk_pa
                             int32_t *nchunk_out, int32_t *up_order, int32_t *ready, int32_t *step_order, int32_t cap,
                             double *makespan);
 
+/* Local time steps (a patch holds several time slices, its
+ * own time and its own time step; L188, L200: ghost zones of neighbours that sit at other times are
+ * interpolated).  The two state buffers become two TIME SLICES per patch: slot[p] says which buffer
+ * holds the newer slice of patch p (time t_new[p]), the other one holds the older (t_old[p]).
+ *
+ *   mhd_bunch_local_begin  both slices of every patch := the current level, all times = t0.
+ *   mhd_bunch_step_local   patches: HOST int32[n], distinct; dt: HOST double[n], > 0.  For every
+ *                          listed patch p: the guard shell of its newer slice is filled from its
+ *                          neighbours' slices LINEARLY INTERPOLATED IN TIME to t_new[p]
+ *                          (v_old + w (v_new - v_old), w = (t_new[p] - t_old[q]) / (t_new[q] - t_old[q]);
+ *                          a neighbour at the patch's own time contributes its newer slice bit for
+ *                          bit; -1 neighbours: zero gradient as in mhd_bunch_fill_guards), then the
+ *                          patch is advanced by its own dt into its older slice, which becomes the
+ *                          newer one.  One set of launches covers the whole list whatever its size.
+ *                          MHD_ESTATE unless every neighbour q of every listed p satisfies
+ *                          t_old[q] <= t_new[p] <= t_new[q] (values are interpolated, never
+ *                          extrapolated -- the rule under which DISPATCH updates a task); nothing is
+ *                          changed then.  With one dt and every patch listed this is the global
+ *                          step, bit for bit.  Totals are not conserved across patches that step
+ *                          with different dt (the paper describes no flux correction).
+ *   mhd_bunch_cfl_local    HOST out double[npatch]: the CFL step of each patch's newer slice;
+ *                          synchronises.
+ *   mhd_bunch_local_state  HOST out (each nullable) t_old, t_new: double[npatch]; slot: int32[npatch]
+ *                          (0: state_a, 1: state_b holds the newer slice).
+ *   mhd_bunch_local_end    all patches must be at one time (else MHD_ESTATE): their newer slices are
+ *                          gathered into the current level and the handle is back in global mode.  */
+int mhd_bunch_local_begin(mhd_bunch *b, double t0);
+int mhd_bunch_step_local(mhd_bunch *b, const int32_t *patches, int32_t n, const double *dt);
+int mhd_bunch_cfl_local(mhd_bunch *b, double courant, double *dt_patch);
+int mhd_bunch_local_state(mhd_bunch *b, double *t_old, double *t_new, int32_t *slot);
+int mhd_bunch_local_end(mhd_bunch *b);
+
 /* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
  * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
  * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to

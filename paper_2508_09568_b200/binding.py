@@ -23,6 +23,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_set_tuning", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
     "mhd_bunch_host_query", "mhd_bunch_host_attach", "mhd_bunch_step_host", "mhd_bunch_host_detach",
     "mhd_bunch_host_schedule",
+    "mhd_bunch_local_begin", "mhd_bunch_step_local", "mhd_bunch_cfl_local", "mhd_bunch_local_state", "mhd_bunch_local_end",
 ]
 
 
@@ -83,6 +84,11 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_step_host.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.mhd_bunch_host_detach.argtypes = [vp]
     lib.mhd_bunch_host_schedule.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, i32, C.POINTER(dbl)]
+    lib.mhd_bunch_local_begin.argtypes = [vp, dbl]
+    lib.mhd_bunch_step_local.argtypes = [vp, vp, i32, vp]
+    lib.mhd_bunch_cfl_local.argtypes = [vp, dbl, vp]
+    lib.mhd_bunch_local_state.argtypes = [vp, vp, vp, vp]
+    lib.mhd_bunch_local_end.argtypes = [vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
     lib.mhd_bunch_last_cuda_error.restype = C.c_char_p
@@ -248,6 +254,45 @@ class MhdBunch:
         _check(self.lib.mhd_bunch_step_host(self.h, host_in.data_ptr(), host_out.data_ptr(), dt, courant,
                                             C.byref(used), C.byref(nxt)), "mhd_bunch_step_host")
         return used.value, nxt.value
+
+    # ---- local time steps (include/mhd_bunch.h: mhd_bunch_local_*) --------------------------
+    def local_begin(self, t0=0.0):
+        _check(self.lib.mhd_bunch_local_begin(self.h, t0), "mhd_bunch_local_begin")
+
+    def step_local(self, patches, dt):
+        """Advance the listed patches by their own dt; returns False if one of them is not ready."""
+        lst = np.ascontiguousarray(patches, dtype=np.int32)
+        dts = np.ascontiguousarray(np.broadcast_to(np.asarray(dt, dtype=np.float64), lst.shape))
+        rc = self.lib.mhd_bunch_step_local(self.h, lst.ctypes.data_as(C.c_void_p), len(lst), dts.ctypes.data_as(C.c_void_p))
+        if rc == -4:
+            return False
+        _check(rc, "mhd_bunch_step_local")
+        return True
+
+    def cfl_local(self, courant):
+        out = np.zeros(self.npatch, dtype=np.float64)
+        _check(self.lib.mhd_bunch_cfl_local(self.h, courant, out.ctypes.data_as(C.c_void_p)), "mhd_bunch_cfl_local")
+        return out
+
+    def local_state(self):
+        t0, t1 = np.zeros(self.npatch), np.zeros(self.npatch)
+        slot = np.zeros(self.npatch, dtype=np.int32)
+        _check(self.lib.mhd_bunch_local_state(self.h, t0.ctypes.data_as(C.c_void_p), t1.ctypes.data_as(C.c_void_p),
+                                              slot.ctypes.data_as(C.c_void_p)), "mhd_bunch_local_state")
+        return t0, t1, slot
+
+    def local_newest(self):
+        """Dense numpy [8, npatch, mz, my, mx]: the newer slice of every patch."""
+        _, _, slot = self.local_state()
+        self.stream.synchronize()
+        both = [self.view(i).contiguous().cpu().numpy() for i in (0, 1)]
+        out = both[0].copy()
+        for p in np.nonzero(slot == 1)[0]:
+            out[:, p] = both[1][:, p]
+        return out
+
+    def local_end(self):
+        _check(self.lib.mhd_bunch_local_end(self.h), "mhd_bunch_local_end")
 
     def status(self):
         v = C.c_int64(0)

@@ -94,6 +94,12 @@ template <typename T> struct Params {
   long long wfs;   // elements per scratch array (= chunk*ps)
   int p0, npl;     // first patch and number of patches of this chunk
   T gamma, dx[3], idx[3];
+  // Local time steps (mhd_bunch_step_local): the launch covers a LIST of patches, each with its
+  // own dt; null for the ordinary launches over the patch range [p0, p0+npl) with one dt.
+  const int* plist;       // DEVICE, [npl]: patch of local index pl
+  const double* dtlist;   // DEVICE, [npl]: its time step
+  __device__ __forceinline__ int patch(int pl) const { return plist ? plist[pl] : p0 + pl; }
+  __device__ __forceinline__ T dt_of(int pl, const double* __restrict__ dtp) const { return (T)(dtlist ? dtlist[pl] : *dtp); }
 };
 
 

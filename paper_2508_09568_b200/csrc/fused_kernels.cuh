@@ -146,7 +146,7 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   const int o = pr * PW + pc;
   const bool rowok = inpos && (j + G.g[1] >= 0) && (j + G.g[1] < G.m[1]);
   const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1], fs = G.fs;
-  const long long cbase = (long long)(P.p0 + pl) * G.ps + G.lead + (i + G.g[0]) + (long long)(j + G.g[1]) * pitch +
+  const long long cbase = (long long)P.patch(pl) * G.ps + G.lead + (i + G.g[0]) + (long long)(j + G.g[1]) * pitch +
                           (long long)G.g[2] * plane;
   // GATHER mode (guard fill O1 folded into the loads, as in the one-pass kernel): a position
   // outside the patch reads the image cell of the neighbour of class (ox,oy,oz) through the
@@ -156,14 +156,14 @@ k_predict_fused(Params<T> P, const double* __restrict__ dtp, unsigned long long*
   if (gather && rowok) {
     const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0), oy = j < 0 ? -1 : (j >= ny ? 1 : 0);
     const long long inner = G.lead + (i - ox * nx + G.g[0]) + (long long)(j - oy * ny + G.g[1]) * pitch + (long long)G.g[2] * plane;
-    const int* tb = nbr + (long long)(P.p0 + pl) * 27 + (oy + 1) * 3 + (ox + 1);
+    const int* tb = nbr + (long long)P.patch(pl) * 27 + (oy + 1) * 3 + (ox + 1);
     cbm = (long long)tb[0] * G.ps + inner + (long long)nz * plane;
     cb0 = (long long)tb[9] * G.ps + inner;
     cbp = (long long)tb[18] * G.ps + inner - (long long)nz * plane;
   }
   auto at = [&](int rr) { return (rr < 0 ? cbm : (rr >= nz ? cbp : cb0)) + (long long)rr * plane; };
   const T h = T(0.5), q4 = T(0.25);
-  const T dt = (T)(*dtp), hdt = h * dt;
+  const T dt = P.dt_of(pl, dtp), hdt = h * dt;
   const T lx = hdt * P.idx[0], ly = hdt * P.idx[1], lz = hdt * P.idx[2];
   const int lim = G.limiter;
 
@@ -369,7 +369,7 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
   const bool active = (fi <= tw) && (fj <= th) && (colthr ? fj < C::FH : t < TXM * C::FH);
   const int ty = colthr ? t + 1 : t + TXM;              // thread that owns (fi, fj+1)
   const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1];
-  const T dt = (T)(*dtp);
+  const T dt = P.dt_of(pl, dtp);
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
   const T gamma = P.gamma;
   const int solver = G.emf_solver, fsolver = G.flux_solver;
@@ -398,7 +398,7 @@ k_riemann_update(Params<T> P, const __grid_constant__ CUtensorMap tmap, const do
   // own cell inside the tile: row fj+1, column fi+1
   const int own = (fj + 1) * DW + (fi + 1);
   // state offset of cell (x0+fi, y0+fj, k=0)
-  const long long ubase = (long long)(P.p0 + pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
+  const long long ubase = (long long)P.patch(pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
                           (long long)(y0 + fj + G.g[1]) * pitch + (long long)G.g[2] * plane;
   const bool cell = (fi < tw) && (fj < th);
   const bool lastx = (x0 + tw == nx), lasty = (y0 + th == ny);

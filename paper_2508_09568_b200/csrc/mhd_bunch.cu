@@ -98,6 +98,20 @@ struct mhd_bunch {
   HostStream* hs;
   std::vector<int>* h_nbr;   // HOST copy of the neighbour table (schedules of the host-streaming path)
   bool all_nbr;        // no -1 entry in the neighbour table
+  // local time steps (mhd_bunch_local_begin / mhd_bunch_step_local): per-patch times and slots on the
+  // host, small device tables carved from the workspace head
+  struct Local {
+    bool active;
+    std::vector<double> t_old, t_new;
+    std::vector<int> slot;                 // which state buffer holds the newer slice of a patch
+  };
+  Local* loc;
+  int* d_slot;         // [npatch]
+  int* d_plist;        // [npatch]
+  double* d_dtlist;    // [npatch]
+  double* d_wtab;      // [npatch][27]
+  // overrides make_params applies while a list of patches is stepped
+  const int* ov_plist; const double* ov_dtlist; int ov_side;
   bool nbr_consistent; // the table composes like translations (see table_is_consistent)
   int tune_zseg;       // MHD_TUNE_ONEPASS_ZSEG: 0 = automatic
   bool fused_cfl;      // MHD_TUNE_FUSED_CFL: the one-pass step reduces the new level's CFL rates in its epilogue
@@ -187,7 +201,9 @@ int build_geom(const mhd_bunch_desc* d, Geom* G) {
 }
 
 size_t head_bytes(int np) {
-  return align_up(sizeof(int) * 27 * (size_t)np, 256) + 2 * align_up(sizeof(unsigned long long) * (size_t)np, 256) + 256 + 256;
+  return align_up(sizeof(int) * 27 * (size_t)np, 256) + 2 * align_up(sizeof(unsigned long long) * (size_t)np, 256) + 256 + 256 +
+         2 * align_up(sizeof(int) * (size_t)np, 256) + align_up(sizeof(double) * (size_t)np, 256) +
+         align_up(sizeof(double) * 27 * (size_t)np, 256);
 }
 DGeom make_dgeom(const Geom& G, size_t esz, int chunk) {
   DGeom D;
@@ -226,6 +242,14 @@ Params<T> make_params(const mhd_bunch* b, int p0, int npl) {
   P.D = (T*)b->d_dblock;
   P.p0 = p0;
   P.npl = npl;
+  P.plist = nullptr;
+  P.dtlist = nullptr;
+  if (b->ov_plist) {   // a list of patches with their own time steps (local time stepping)
+    P.plist = b->ov_plist + p0;
+    P.dtlist = b->ov_dtlist + p0;
+    P.U = (const T*)b->state[b->ov_side];
+    P.Un = (T*)b->state[1 - b->ov_side];
+  }
   P.gamma = (T)b->desc.gamma;
   for (int a = 0; a < 3; ++a) {
     P.dx[a] = (T)b->desc.dx[a];
@@ -350,7 +374,7 @@ template <> struct OnePassLaunch<float> {
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
-      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, b->gather_ok ? 1 : 0, dtp, b->d_bad, b->d_rate_next, xt, zseg);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, (b->gather_ok && !b->ov_plist) ? 1 : 0, dtp, b->d_bad, b->d_rate_next, xt, zseg);
     }
     CUDA_TRY(cudaGetLastError());
     return MHD_OK;
@@ -408,6 +432,13 @@ bool table_is_consistent(const int32_t* nb, int np) {
   return true;
 }
 
+// the global-step entry points are closed while the handle is in local-time-step mode (the two
+// buffers are then time slices per patch, not levels n and n+1 of the whole bunch)
+#define NOT_LOCAL(b)                                               \
+  do {                                                             \
+    if ((b)->loc && (b)->loc->active) return MHD_ESTATE;           \
+  } while (0)
+
 // every launching entry point runs on the handle's device, whatever the caller's current one is
 #define ENTER(b)                                                   \
   do {                                                             \
@@ -447,35 +478,14 @@ int launch_fused_range(mhd_bunch* b, int q0, int nq) {
   return MHD_OK;
 }
 
+// staged path on patches [q0, q0+nq) (or on that many entries of a patch list): one kernel per stage
 template <typename T>
-int launch_step(mhd_bunch* b) {
+int launch_staged_range(mhd_bunch* b, int q0, int nq) {
   const Geom& G = b->G;
   const double* dtp = b->d_dt + 1;
-  const int path = effective_path(b);
-  b->rate_valid = false;     // set again below if the one-pass kernel (whose epilogue reduces the CFL rates) runs
-  if (path == MHD_PATH_ONEPASS && b->gather_ok) return OnePassLaunch<T>::run(b, dtp);
-  if (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) {
-    // halos come through the neighbour table if the fill was deferred, from the shell otherwise
-    const int rc = launch_fused_range<T>(b, 0, G.np);
-    if (rc != MHD_OK) return rc;
-    b->cur = 1 - b->cur;
-    b->guards_stale = false;
-    return MHD_OK;
-  }
-  {  // every other route reads the guard shell from HBM
-    const int rc = materialise_guards(b);
-    if (rc != MHD_OK) return rc;
-  }
-  if (path == MHD_PATH_ONEPASS) return OnePassLaunch<T>::run(b, dtp);
-  if (path == MHD_PATH_TWO_KERNEL) {
-    const int rc = launch_fused_range<T>(b, 0, G.np);
-    if (rc != MHD_OK) return rc;
-    b->cur = 1 - b->cur;
-    return MHD_OK;
-  }
   const int ch = b->chunk_s;
-  for (int p0 = 0; p0 < G.np; p0 += ch) {
-    const int npl = (G.np - p0 < ch) ? G.np - p0 : ch;
+  for (int p0 = q0; p0 < q0 + nq; p0 += ch) {
+    const int npl = (q0 + nq - p0 < ch) ? q0 + nq - p0 : ch;
     Params<T> P = make_params<T>(b, p0, npl);
     cudaStream_t st = b->stream;
     {
@@ -516,6 +526,40 @@ int launch_step(mhd_bunch* b) {
       LaunchScope ls(b, KC_UPDATE);
       k_update<T><<<blocks_for(B.cells * npl, 256), 256, 0, st>>>(P, B, dtp);
     }
+  }
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
+
+template <typename T>
+int launch_step(mhd_bunch* b) {
+  const Geom& G = b->G;
+  const double* dtp = b->d_dt + 1;
+  const int path = effective_path(b);
+  b->rate_valid = false;     // set again below if the one-pass kernel (whose epilogue reduces the CFL rates) runs
+  if (path == MHD_PATH_ONEPASS && b->gather_ok) return OnePassLaunch<T>::run(b, dtp);
+  if (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) {
+    // halos come through the neighbour table if the fill was deferred, from the shell otherwise
+    const int rc = launch_fused_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
+    b->cur = 1 - b->cur;
+    b->guards_stale = false;
+    return MHD_OK;
+  }
+  {  // every other route reads the guard shell from HBM
+    const int rc = materialise_guards(b);
+    if (rc != MHD_OK) return rc;
+  }
+  if (path == MHD_PATH_ONEPASS) return OnePassLaunch<T>::run(b, dtp);
+  if (path == MHD_PATH_TWO_KERNEL) {
+    const int rc = launch_fused_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
+    b->cur = 1 - b->cur;
+    return MHD_OK;
+  }
+  {
+    const int rc = launch_staged_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
   }
   CUDA_TRY(cudaGetLastError());
   b->cur = 1 - b->cur;
@@ -617,6 +661,12 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->rate_valid = false;
   b->d_bad = (unsigned long long*)p;  p += 256;
   b->d_dt = (double*)p;               p += 256;
+  b->d_slot = (int*)p;                p += align_up(sizeof(int) * (size_t)desc->npatch, 256);
+  b->d_plist = (int*)p;               p += align_up(sizeof(int) * (size_t)desc->npatch, 256);
+  b->d_dtlist = (double*)p;           p += align_up(sizeof(double) * (size_t)desc->npatch, 256);
+  b->d_wtab = (double*)p;             p += align_up(sizeof(double) * 27 * (size_t)desc->npatch, 256);
+  b->loc = nullptr;
+  b->ov_plist = nullptr; b->ov_dtlist = nullptr; b->ov_side = 0;
   b->d_scratch = p;
   const size_t avail = workspace_bytes - (size_t)(p - b->ws);
   {
@@ -685,6 +735,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
 
 int mhd_bunch_fill_guards(mhd_bunch* b) {
   ENTER(b);
+  NOT_LOCAL(b);
   if (step_gathers(b)) {
     // deferred: the one-pass step reads halos from the neighbours' interiors, so only the
     // closing faces are brought up to date now; the rest of the shell is written if and when
@@ -706,6 +757,7 @@ int mhd_bunch_sync_guards(mhd_bunch* b) {
 
 int mhd_bunch_cfl_dt(mhd_bunch* b, double courant, double* dt_host, void* dt_dev, void* dt_per_patch_dev) {
   ENTER(b);
+  NOT_LOCAL(b);
   if (!(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
   const int rc = b->desc.dtype == MHD_F64 ? launch_cfl<double>(b, courant, dt_dev, dt_per_patch_dev)
                                            : launch_cfl<float>(b, courant, dt_dev, dt_per_patch_dev);
@@ -723,6 +775,7 @@ static int step_common(mhd_bunch* b) {
 
 int mhd_bunch_step(mhd_bunch* b, double dt) {
   ENTER(b);
+  NOT_LOCAL(b);
   if (!(dt > 0.0) || !isfinite(dt)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0, b->d_rate_next, b->G.np); }
   return step_common(b);
@@ -730,6 +783,7 @@ int mhd_bunch_step(mhd_bunch* b, double dt) {
 
 int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
   ENTER(b);
+  NOT_LOCAL(b);
   if (!dt_dev || !(dt_max >= 0.0)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, (const double*)dt_dev, 0.0, dt_max, b->d_rate_next, b->G.np); }
   return step_common(b);
@@ -1102,6 +1156,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
 int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant,
                         double* dt_used, double* dt_next) {
   ENTER(b);
+  NOT_LOCAL(b);
   const int rc = step_host_impl(b, host_in, host_out, dt, courant, dt_used, dt_next);
   if (rc != MHD_OK && b->hs) {
     // copies into / out of the caller's host buffers may still be in flight: drain them before
@@ -1222,6 +1277,193 @@ int mhd_bunch_host_detach(mhd_bunch* b) {
 
 }  // extern "C"
 
+// ------------------------------------------------------- local time steps ----
+namespace {
+
+bool times_equal(double a, double b) {
+  const double s = fmax(fabs(a), fabs(b));
+  return fabs(a - b) <= 1e-12 * (s > 1.0 ? s : 1.0);
+}
+
+// steps the patches d_plist[0..n) (all with their newer slice in buffer `side`) by d_dtlist
+template <typename T>
+int launch_step_list(mhd_bunch* b, int off, int n, int side) {
+  b->ov_plist = b->d_plist + off;
+  b->ov_dtlist = b->d_dtlist + off;
+  b->ov_side = side;
+  const int path = effective_path(b);
+  int rc;
+  if (path == MHD_PATH_ONEPASS) rc = OnePassLaunch<T>::run(b, b->d_dt + 1, 0, n, false);
+  else if (path == MHD_PATH_TWO_KERNEL) rc = launch_fused_range<T>(b, 0, n);
+  else rc = launch_staged_range<T>(b, 0, n);
+  b->ov_plist = nullptr;
+  b->ov_dtlist = nullptr;
+  return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mhd_bunch_local_begin(mhd_bunch* b, double t0) {
+  ENTER(b);
+  if (!isfinite(t0)) return MHD_EINVAL;
+  int rc = materialise_guards(b);
+  if (rc != MHD_OK) return rc;
+  if (!b->loc) {
+    b->loc = new (std::nothrow) mhd_bunch::Local();
+    if (!b->loc) return MHD_ENOMEM;
+  }
+  // both slices = the current level
+  CUDA_TRY(cudaMemcpyAsync(b->state[1 - b->cur], b->state[b->cur], b->lay.state_bytes, cudaMemcpyDeviceToDevice, b->stream));
+  b->loc->active = true;
+  b->loc->t_old.assign(b->G.np, t0);
+  b->loc->t_new.assign(b->G.np, t0);
+  b->loc->slot.assign(b->G.np, b->cur);
+  b->rate_valid = false;
+  b->closing_ok = false;
+  return MHD_OK;
+}
+
+int mhd_bunch_local_state(mhd_bunch* b, double* t_old, double* t_new, int32_t* slot) {
+  if (!b || !b->loc || !b->loc->active) return MHD_ESTATE;
+  for (int p = 0; p < b->G.np; ++p) {
+    if (t_old) t_old[p] = b->loc->t_old[p];
+    if (t_new) t_new[p] = b->loc->t_new[p];
+    if (slot) slot[p] = b->loc->slot[p];
+  }
+  return MHD_OK;
+}
+
+int mhd_bunch_step_local(mhd_bunch* b, const int32_t* patches, int32_t n, const double* dt) {
+  ENTER(b);
+  if (!b->loc || !b->loc->active) return MHD_ESTATE;
+  if (!patches || !dt || n < 1 || n > b->G.np) return MHD_EINVAL;
+  mhd_bunch::Local& L = *b->loc;
+  const int np = b->G.np;
+  const std::vector<int>& nb = *b->h_nbr;
+  std::vector<char> seen(np, 0);
+  for (int i = 0; i < n; ++i) {
+    const int p = patches[i];
+    if (p < 0 || p >= np || seen[p] || !(dt[i] > 0.0) || !isfinite(dt[i])) return MHD_EINVAL;
+    seen[p] = 1;
+  }
+  // readiness: guard values are interpolated, never extrapolated (the rule under which DISPATCH
+  // updates a task): t_old[q] <= t_new[p] <= t_new[q] for every neighbour q of a listed patch
+  for (int i = 0; i < n; ++i) {
+    const int p = patches[i];
+    for (int c = 0; c < 27; ++c) {
+      const int q = nb[(size_t)p * 27 + c];
+      if (q < 0 || q == p) continue;
+      const bool lo = L.t_old[q] <= L.t_new[p] || times_equal(L.t_old[q], L.t_new[p]);
+      const bool hi = L.t_new[p] <= L.t_new[q] || times_equal(L.t_new[p], L.t_new[q]);
+      if (!(lo && hi)) return MHD_ESTATE;
+    }
+  }
+  // lists grouped by the buffer that holds the newer slice (one set of launches per group), with
+  // the interpolation weights of every (listed patch, neighbour class)
+  std::vector<int> plist;
+  std::vector<double> dtl, wt;
+  plist.reserve(n); dtl.reserve(n); wt.reserve((size_t)n * 27);
+  int count[2] = {0, 0};
+  for (int side = 0; side < 2; ++side)
+    for (int i = 0; i < n; ++i) {
+      const int p = patches[i];
+      if (L.slot[p] != side) continue;
+      ++count[side];
+      plist.push_back(p);
+      dtl.push_back(dt[i]);
+      for (int c = 0; c < 27; ++c) {
+        const int q = nb[(size_t)p * 27 + c];
+        double w = 1.0;
+        if (q >= 0 && !times_equal(L.t_new[p], L.t_new[q]) && !times_equal(L.t_new[q], L.t_old[q]))
+          w = (L.t_new[p] - L.t_old[q]) / (L.t_new[q] - L.t_old[q]);
+        wt.push_back(w);
+      }
+    }
+  CUDA_TRY(cudaMemcpyAsync(b->d_slot, L.slot.data(), sizeof(int) * np, cudaMemcpyHostToDevice, b->stream));
+  CUDA_TRY(cudaMemcpyAsync(b->d_plist, plist.data(), sizeof(int) * n, cudaMemcpyHostToDevice, b->stream));
+  CUDA_TRY(cudaMemcpyAsync(b->d_dtlist, dtl.data(), sizeof(double) * n, cudaMemcpyHostToDevice, b->stream));
+  CUDA_TRY(cudaMemcpyAsync(b->d_wtab, wt.data(), sizeof(double) * 27 * n, cudaMemcpyHostToDevice, b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));      // the host vectors go out of scope
+  const bool f64 = b->desc.dtype == MHD_F64;
+  {
+    const FillMap M = make_fill_map(b->G);
+    const long long tot = (long long)M.start[6] * n;
+    if (tot > 0) {
+      LaunchScope ls(b, KC_FILL);
+      if (f64) k_fill_guards_local<double><<<blocks_for(tot, 256), 256, 0, b->stream>>>(b->G, M, (double*)b->state[0], (double*)b->state[1], b->d_nbr, b->d_slot, b->d_plist, b->d_wtab, n);
+      else k_fill_guards_local<float><<<blocks_for(tot, 256), 256, 0, b->stream>>>(b->G, M, (float*)b->state[0], (float*)b->state[1], b->d_nbr, b->d_slot, b->d_plist, b->d_wtab, n);
+    }
+    CUDA_TRY(cudaGetLastError());
+  }
+  b->guards_stale = false;
+  b->rate_valid = false;
+  int off = 0;
+  for (int side = 0; side < 2; ++side) {
+    if (count[side] == 0) continue;
+    const int rc = f64 ? launch_step_list<double>(b, off, count[side], side) : launch_step_list<float>(b, off, count[side], side);
+    if (rc != MHD_OK) return rc;
+    off += count[side];
+  }
+  for (int i = 0; i < n; ++i) {
+    const int p = patches[i];
+    L.slot[p] = 1 - L.slot[p];
+    L.t_old[p] = L.t_new[p];
+    L.t_new[p] += dt[i];
+  }
+  return MHD_OK;
+}
+
+int mhd_bunch_cfl_local(mhd_bunch* b, double courant, double* dt_patch) {
+  ENTER(b);
+  if (!b->loc || !b->loc->active) return MHD_ESTATE;
+  if (!dt_patch || !(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
+  const int np = b->G.np;
+  // one pass per buffer; a patch's step comes from the buffer that holds its newer slice
+  std::vector<unsigned long long> r[2];
+  const int cur = b->cur;
+  for (int side = 0; side < 2; ++side) {
+    b->cur = side;
+    b->rate_valid = false;
+    const int rc = b->desc.dtype == MHD_F64 ? launch_cfl<double>(b, courant, nullptr, nullptr) : launch_cfl<float>(b, courant, nullptr, nullptr);
+    b->cur = cur;
+    if (rc != MHD_OK) return rc;
+    r[side].resize(np);
+    CUDA_TRY(cudaMemcpyAsync(r[side].data(), b->d_rate, sizeof(unsigned long long) * np, cudaMemcpyDeviceToHost, b->stream));
+    CUDA_TRY(cudaStreamSynchronize(b->stream));
+  }
+  for (int p = 0; p < np; ++p) {
+    double rate;
+    const unsigned long long bits = r[b->loc->slot[p]][p];
+    memcpy(&rate, &bits, sizeof(rate));
+    dt_patch[p] = courant / rate;
+  }
+  return MHD_OK;
+}
+
+int mhd_bunch_local_end(mhd_bunch* b) {
+  ENTER(b);
+  if (!b->loc || !b->loc->active) return MHD_ESTATE;
+  mhd_bunch::Local& L = *b->loc;
+  for (int p = 1; p < b->G.np; ++p)
+    if (!times_equal(L.t_new[p], L.t_new[0])) return MHD_ESTATE;      // the bunch is not at one time
+  // bring every newer slice into the current buffer (per patch and field: a strided device copy)
+  const size_t pb = (size_t)b->G.ps * b->esz, fb = (size_t)b->G.fs * b->esz;
+  for (int p = 0; p < b->G.np; ++p) {
+    if (L.slot[p] == b->cur) continue;
+    CUDA_TRY(cudaMemcpy2DAsync((char*)b->state[b->cur] + (size_t)p * pb, fb, (char*)b->state[1 - b->cur] + (size_t)p * pb, fb, pb, 8,
+                               cudaMemcpyDeviceToDevice, b->stream));
+  }
+  L.active = false;
+  b->guards_stale = false;
+  b->closing_ok = false;
+  b->rate_valid = false;
+  return MHD_OK;
+}
+
+}  // extern "C"
+
 extern "C" {
 
 int mhd_bunch_destroy(mhd_bunch* b) {
@@ -1229,6 +1471,7 @@ int mhd_bunch_destroy(mhd_bunch* b) {
   cudaStreamSynchronize(b->stream);
   drain_events(b, false);
   hs_release(b);
+  delete b->loc;
   delete b->h_nbr;
   delete b->events;
   delete b;

@@ -190,12 +190,12 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const bool lastx = (x0 + tw == nx), lasty = (y0 + th == ny);
   const int t = threadIdx.x;
   const T h = T(0.5);
-  const T dt = (T)(*dtp);
+  const T dt = P.dt_of(pl, dtp);
   const T gamma = P.gamma;
 
   // source patch of each of the 27 neighbour classes: the neighbour table in gather mode,
   // the patch itself (whose guard cells are then read) otherwise
-  if (t < 27) NBS[t] = gather ? nbr[(long long)(P.p0 + pl) * 27 + t] : P.p0 + pl;
+  if (t < 27) NBS[t] = gather ? nbr[(long long)P.patch(pl) * 27 + t] : P.patch(pl);
   __syncthreads();
 
   auto dslot = [&](int plane) { return Dm + (size_t)((plane + 2) & 1) * (D_COUNT * DCS); };
@@ -514,7 +514,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const int tyn = colthr ? tr + 1 : tr + TX;              // thread that owns (fi, fj+1)
   const int txn = colthr ? tr : ((fi == TX - 1) ? C::CB + fj : tr + 1);   // thread that owns (fi+1, fj)
   const long long plane = (long long)G.pitch * G.m[1], fs = G.fs;
-  const long long ubase = (long long)(P.p0 + pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
+  const long long ubase = (long long)P.patch(pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
                           (long long)(y0 + fj + G.g[1]) * G.pitch + (long long)G.g[2] * plane;
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
   const int solver = G.emf_solver, FS = G.flux_solver;
@@ -712,7 +712,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
       double rd = (double)rmax;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) rd = fmax(rd, __shfl_xor_sync(0xffffffffu, rd, o));
-      if ((t & 31) == 0) atomicMax(&rate_next[P.p0 + pl], enc_max(rd));
+      if ((t & 31) == 0) atomicMax(&rate_next[P.patch(pl)], enc_max(rd));
     }
   }
 }

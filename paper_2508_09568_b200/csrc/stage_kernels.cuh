@@ -89,6 +89,76 @@ __global__ void __launch_bounds__(256) k_fill_guards(Geom G, FillMap M, T* __res
   }
 }
 
+// O10, local time steps: guard fill of the NEWER slice of each listed
+// patch from its neighbours' two slices, linearly interpolated in time to the patch's own time.
+// S0/S1: the two state buffers; slot[q]: which of them holds the newer slice of patch q;
+// wtab[i][class]: weight of the newer slice for listed patch i and neighbour class (1: take the
+// newer slice itself, bit for bit -- equal times).  Same thread-to-guard-cell map as k_fill_guards.
+template <typename T>
+__global__ void __launch_bounds__(256) k_fill_guards_local(Geom G, FillMap M, T* __restrict__ S0, T* __restrict__ S1,
+                                                           const int* __restrict__ nbr, const int* __restrict__ slot,
+                                                           const int* __restrict__ plist, const double* __restrict__ wtab,
+                                                           int nlist) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int per = M.start[6];
+  if (t >= (long long)per * nlist) return;
+  const int il = (int)(t / per);
+  const int p = plist[il];
+  int r = (int)(t - (long long)il * per);
+  int st = 0, l0 = M.lo[0][0], l1 = M.lo[0][1], l2 = M.lo[0][2], e0 = M.ext[0][0], e1 = M.ext[0][1];
+#pragma unroll
+  for (int q = 1; q < 6; ++q) {
+    if (r >= M.start[q]) { st = M.start[q]; l0 = M.lo[q][0]; l1 = M.lo[q][1]; l2 = M.lo[q][2]; e0 = M.ext[q][0]; e1 = M.ext[q][1]; }
+  }
+  r -= st;
+  const int exy = e0 * e1;
+  const int kk = r / exy; r -= kk * exy;
+  const int jj = r / e0;
+  const int ii = r - jj * e0;
+  const int c[3] = {l0 + ii, l1 + jj, l2 + kk};
+  int o[3], src[3], cl[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    o[d] = c[d] < 0 ? -1 : (c[d] >= G.n[d] ? 1 : 0);
+    src[d] = c[d] - o[d] * G.n[d];
+    cl[d] = min(max(c[d], 0), G.n[d] - 1);
+  }
+  const int cls = (o[2] + 1) * 9 + (o[1] + 1) * 3 + (o[0] + 1);
+  const int q = nbr[p * 27 + cls];
+  const long long pitch = G.pitch, plane = (long long)G.pitch * G.m[1];
+  T* const mine = slot[p] ? S1 : S0;
+  const long long dst = (long long)p * G.ps + G.lead + (c[0] + G.g[0]) + (c[1] + G.g[1]) * pitch + (c[2] + G.g[2]) * plane;
+  if (q >= 0) {
+    const long long from = (long long)q * G.ps + G.lead + (src[0] + G.g[0]) + (src[1] + G.g[1]) * pitch + (src[2] + G.g[2]) * plane;
+    const T* const qn = slot[q] ? S1 : S0;
+    const T* const qo = slot[q] ? S0 : S1;
+    const double w = wtab[il * 27 + cls];
+    T v[8];
+#pragma unroll
+    for (int f = 0; f < 8; ++f) v[f] = qn[f * G.fs + from];
+    if (w != 1.0) {   // never touches the older slice of a neighbour at the patch's own time (it may be written by this call's steps)
+      const T wt = (T)w;
+#pragma unroll
+      for (int f = 0; f < 8; ++f) {
+        const T vo = qo[f * G.fs + from];
+        v[f] = vo + wt * (v[f] - vo);
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < 8; ++f) mine[f * G.fs + dst] = v[f];
+  } else {
+    const long long from = (long long)p * G.ps + G.lead + (cl[0] + G.g[0]) + (cl[1] + G.g[1]) * pitch + (cl[2] + G.g[2]) * plane;
+#pragma unroll
+    for (int f = 0; f < 8; ++f) {
+      if (f >= 5) {  // the closing face keeps its evolved value (O8)
+        const int a = f - 5, b = (a + 1) % 3, e = (a + 2) % 3;
+        if (G.act[a] && c[a] == G.n[a] && o[b] == 0 && o[e] == 0) continue;
+      }
+      mine[f * G.fs + dst] = mine[f * G.fs + from];
+    }
+  }
+}
+
 // The closing faces alone (O8: face n_a of the normal field b_a sits in the first high guard
 // slot): the neighbour's face 0 overwrites it, an outflow side keeps the evolved value.
 // This is the only part of the guard shell that cfl_dt and the one-pass kernel's update read
@@ -222,7 +292,7 @@ __global__ void __launch_bounds__(256) k_prim(Params<T> P, Box B, unsigned long 
   const Geom& G = P.G;
   int pl, i, j, k; long long c;
   if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
   const T* U = P.U;
   const T rho = U[cu], irho = num<T>::rcp(rho);
   const T u = U[G.fs + cu] * irho, v = U[2 * G.fs + cu] * irho, w = U[3 * G.fs + cu] * irho;
@@ -244,7 +314,7 @@ __global__ void __launch_bounds__(256) k_emf0(Params<T> P, Box B) {
   const Geom& G = P.G;
   int pl, i, j, k; long long c;
   if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
   const long long sx = G.s[0], sy = G.s[1], sz = G.s[2];
   const T* u = P.W + (W_Q + 1) * P.wfs + cw;
   const T* v = P.W + (W_Q + 2) * P.wfs + cw;
@@ -277,8 +347,8 @@ __global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const doubl
   const Geom& G = P.G;
   int pl, i, j, k; long long c;
   if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c;
-  const T dt = (T)(*dtp);
+  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
+  const T dt = P.dt_of(pl, dtp);
   const T hdt = T(0.5) * dt;
   const long long wfs = P.wfs;
   const int cc[3] = {i, j, k};
@@ -437,8 +507,8 @@ __global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double
   const Geom& G = P.G;
   int pl, i, j, k; long long c;
   if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)(P.p0 + pl) * G.ps + c, cw = (long long)pl * G.ps + c, wfs = P.wfs;
-  const T dt = (T)(*dtp);
+  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c, wfs = P.wfs;
+  const T dt = P.dt_of(pl, dtp);
   const int cc[3] = {i, j, k};
   if (inside(G, i, j, k, 0, 0)) {
 #pragma unroll
