@@ -187,6 +187,39 @@ int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t chunk_pa
                             int32_t *nchunk_out, int32_t *up_order, int32_t *ready, int32_t *step_order, int32_t cap,
                             double *makespan);
 
+/* Ring mode: a host-resident bunch LARGER than the device buffers (PAPER.md
+ * L164: bunches filled round-robin with several in flight; L243-247: asynchronous staging).  The
+ * handle is created for a WINDOW of patches (its npatch, its two state buffers); the bunch itself --
+ * `npatch` patches with their own neighbour table, compact host layout as for mhd_bunch_step_host --
+ * streams through the window in chunks of `chunk_patches` consecutive patches: the window holds
+ * R = (handle npatch) / chunk_patches chunk slots.  Chunks are stepped in order; before a chunk is
+ * stepped every chunk that holds one of its neighbours is resident in some slot (the kernels read
+ * halos through a neighbour table rewritten in slot numbers), a chunk nobody needs any more gives up
+ * its slot to the next upload, and results leave through the second buffer's slots -- uploads,
+ * kernels and downloads overlap as in mhd_bunch_step_host.  Chunks that are needed again after they
+ * were evicted (the first ones of a periodic bunch) are uploaded twice.
+ *
+ *   mhd_bunch_ring_plan    HOST only: the schedule for a table, a chunk size and R slots: number of
+ *                          chunks, number of uploads, and (nullable, capacity `cap`) per upload the
+ *                          chunk, its slot and the step it precedes, per step the slot of the chunk
+ *                          stepped.  MHD_ENOMEM if some chunk's neighbourhood does not fit in R slots.
+ *   mhd_bunch_ring_attach  nbr: HOST int32[npatch][27], no -1 entries, translation-consistent (see
+ *                          mhd_bunch_create); staging_dev: DEVICE, caller-owned, 16-byte aligned,
+ *                          >= 2 * 8 * chunk_patches * n_x n_y n_z * sizeof(real) bytes.  Needs the
+ *                          one-pass step (float32, three active dimensions, n_x a multiple of 4):
+ *                          MHD_EINVAL otherwise.
+ *   mhd_bunch_step_ring    host_in / host_out: HOST (pinned for overlap), distinct, compact layout
+ *                          of the WHOLE bunch; dt > 0; HOST out, nullable: *dt_next = CFL step of the
+ *                          new level (from the step's own epilogue).  Synchronises.  Results are bit
+ *                          for bit those of the resident step.
+ *   mhd_bunch_ring_detach  releases the streams; the handle is a plain window-sized bunch again.   */
+int mhd_bunch_ring_plan(const int32_t *nbr, int32_t npatch, int32_t chunk_patches, int32_t ring_chunks, int32_t *nchunk,
+                        int32_t *nupload, int32_t *up_chunk, int32_t *up_slot, int32_t *up_step, int32_t *step_slot, int32_t cap);
+int mhd_bunch_ring_attach(mhd_bunch *b, const int32_t *nbr, int32_t npatch, int32_t chunk_patches, void *staging_dev,
+                          size_t staging_bytes);
+int mhd_bunch_step_ring(mhd_bunch *b, const void *host_in, void *host_out, double dt, double courant, double *dt_next);
+int mhd_bunch_ring_detach(mhd_bunch *b);
+
 /* Local time steps (a patch holds several time slices, its
  * own time and its own time step; L188, L200: ghost zones of neighbours that sit at other times are
  * interpolated).  The two state buffers become two TIME SLICES per patch: slot[p] says which buffer

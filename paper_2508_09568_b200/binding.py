@@ -23,6 +23,7 @@ ABI_SYMBOLS = [
     "mhd_bunch_chunk", "mhd_bunch_sync_guards", "mhd_bunch_set_path", "mhd_bunch_get_path", "mhd_bunch_set_tuning", "mhd_bunch_measure_alu_peak", "mhd_bunch_destroy", "mhd_bunch_strerror", "mhd_bunch_last_cuda_error",
     "mhd_bunch_host_query", "mhd_bunch_host_attach", "mhd_bunch_step_host", "mhd_bunch_host_detach",
     "mhd_bunch_host_schedule",
+    "mhd_bunch_ring_plan", "mhd_bunch_ring_attach", "mhd_bunch_step_ring", "mhd_bunch_ring_detach",
     "mhd_bunch_local_begin", "mhd_bunch_step_local", "mhd_bunch_cfl_local", "mhd_bunch_local_state", "mhd_bunch_local_end",
 ]
 
@@ -84,6 +85,10 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_step_host.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.mhd_bunch_host_detach.argtypes = [vp]
     lib.mhd_bunch_host_schedule.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, i32, C.POINTER(dbl)]
+    lib.mhd_bunch_ring_plan.argtypes = [vp, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, vp, i32]
+    lib.mhd_bunch_ring_attach.argtypes = [vp, vp, i32, i32, vp, C.c_size_t]
+    lib.mhd_bunch_step_ring.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl)]
+    lib.mhd_bunch_ring_detach.argtypes = [vp]
     lib.mhd_bunch_local_begin.argtypes = [vp, dbl]
     lib.mhd_bunch_step_local.argtypes = [vp, vp, i32, vp]
     lib.mhd_bunch_cfl_local.argtypes = [vp, dbl, vp]
@@ -147,6 +152,25 @@ def host_schedule(nbr, chunk_patches=0):
     n = nchunk.value
     return {"chunk": chunk.value, "nchunk": n, "up_order": up[:n].copy(), "ready": ready[:n].copy(),
             "step_order": order[:n].copy(), "makespan": span.value}
+
+
+def ring_plan(nbr, chunk_patches, ring_chunks):
+    """Schedule of a ring step (host only): dict(nchunk, up_chunk, up_slot, up_step, step_slot) or
+    None if a chunk's neighbourhood does not fit in `ring_chunks` slots."""
+    nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+    npatch = nbr.shape[0]
+    nchunk, nup = C.c_int32(0), C.c_int32(0)
+    cap = 4 * npatch + 8
+    a, b_, c_, d_ = (np.zeros(cap, dtype=np.int32) for _ in range(4))
+    rc = load_library().mhd_bunch_ring_plan(nbr.ctypes.data_as(C.c_void_p), npatch, chunk_patches, ring_chunks, C.byref(nchunk),
+                                            C.byref(nup), a.ctypes.data_as(C.c_void_p), b_.ctypes.data_as(C.c_void_p),
+                                            c_.ctypes.data_as(C.c_void_p), d_.ctypes.data_as(C.c_void_p), cap)
+    if rc == -2:
+        return None
+    _check(rc, "mhd_bunch_ring_plan")
+    n = nup.value
+    return {"nchunk": nchunk.value, "up_chunk": a[:n].copy(), "up_slot": b_[:n].copy(), "up_step": c_[:n].copy(),
+            "step_slot": d_[:nchunk.value].copy()}
 
 
 class MhdBunch:
@@ -254,6 +278,24 @@ class MhdBunch:
         _check(self.lib.mhd_bunch_step_host(self.h, host_in.data_ptr(), host_out.data_ptr(), dt, courant,
                                             C.byref(used), C.byref(nxt)), "mhd_bunch_step_host")
         return used.value, nxt.value
+
+    # ---- ring mode: a host bunch larger than the device buffers (mhd_bunch_ring_*) ------------
+    def ring_attach(self, nbr_big, chunk_patches):
+        nbr_big = np.ascontiguousarray(nbr_big, dtype=np.int32)
+        esz = 4 if self.tdtype == self.torch.float32 else 8
+        nbytes = 2 * ((8 * chunk_patches * self.n[0] * self.n[1] * self.n[2] * esz + 255) // 256 * 256)
+        self.ring_staging = self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+        _check(self.lib.mhd_bunch_ring_attach(self.h, nbr_big.ctypes.data_as(C.c_void_p), nbr_big.shape[0], chunk_patches,
+                                              self.ring_staging.data_ptr(), nbytes), "mhd_bunch_ring_attach")
+
+    def step_ring(self, host_in, host_out, dt, courant=0.4):
+        nxt = C.c_double(0.0)
+        _check(self.lib.mhd_bunch_step_ring(self.h, host_in.data_ptr(), host_out.data_ptr(), dt, courant, C.byref(nxt)),
+               "mhd_bunch_step_ring")
+        return nxt.value
+
+    def ring_detach(self):
+        _check(self.lib.mhd_bunch_ring_detach(self.h), "mhd_bunch_ring_detach")
 
     # ---- local time steps (include/mhd_bunch.h: mhd_bunch_local_*) --------------------------
     def local_begin(self, t0=0.0):

@@ -96,6 +96,19 @@ struct mhd_bunch {
     std::vector<int> up_order, step_order, ready;   // ready[c]: upload position after which chunk c may step
   };
   HostStream* hs;
+  // ring mode (mhd_bunch_ring_attach / mhd_bunch_step_ring): the handle's buffers are a window of
+  // chunk slots through which a host-resident bunch LARGER than the buffers streams
+  struct Ring {
+    int NP, chunk, nchunk, nslot;                 // host bunch, patches per chunk, chunks, chunk slots of the window
+    std::vector<int> up_chunk, up_slot, up_step, up_wait;   // planned uploads: chunk, slot, before which step, and the
+                                                            // last step that read the slot's previous occupant (-1: none)
+    std::vector<int> slot_of_step;                // slot in which chunk c sits when it is stepped
+    std::vector<int> rows;                        // [NP][27] neighbour table in SLOT space (patch ids of the window)
+    char* stage_up; char* stage_dn;
+    cudaStream_t s_up, s_dn;
+    std::vector<cudaEvent_t> ev_up, ev_step, ev_dn;   // per upload, per step, per slot
+  };
+  Ring* ring;
   std::vector<int>* h_nbr;   // HOST copy of the neighbour table (schedules of the host-streaming path)
   bool all_nbr;        // no -1 entry in the neighbour table
   // local time steps (mhd_bunch_local_begin / mhd_bunch_step_local): per-patch times and slots on the
@@ -715,6 +728,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->tune_zseg = 0;
   b->fused_cfl = false;
   b->hs = nullptr;
+  b->ring = nullptr;
   b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
   if (!b->h_nbr) { delete b->events; delete b; return MHD_ENOMEM; }
   b->guards_stale = false;
@@ -1000,10 +1014,10 @@ int launch_pack(mhd_bunch* b, cudaStream_t st, void* state, char* stage, int p0,
 }
 
 // one strided copy per chunk: rows = the eight fields, host[f][p0 .. p0+npl) <-> stage[f][0 .. npl)
-int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device) {
+int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device, int host_np = -1) {
   const size_t per = (size_t)b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
   char* h = host + (size_t)p0 * per;
-  const size_t hp = (size_t)b->G.np * per, dp = (size_t)npl * per;
+  const size_t hp = (size_t)(host_np < 0 ? b->G.np : host_np) * per, dp = (size_t)npl * per;
   if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, hp, dp, 8, cudaMemcpyHostToDevice, st));
   else CUDA_TRY(cudaMemcpy2DAsync(h, hp, stage, dp, dp, 8, cudaMemcpyDeviceToHost, st));
   return MHD_OK;
@@ -1277,6 +1291,258 @@ int mhd_bunch_host_detach(mhd_bunch* b) {
 
 }  // extern "C"
 
+// ------------------------------------------------------------------ ring mode ----
+namespace {
+
+// Plan of one ring step for a host bunch of NP patches cut into chunks of `chunk` consecutive
+// patches, stepped in order 0..C-1 through a window of R chunk slots.  need(c) = chunks that hold a
+// neighbour of a patch of c (c included); before step c every chunk of need(c) must be resident.  A
+// missing chunk goes into a free slot, else into the slot of a resident chunk that step c does not
+// need and whose next use lies farthest ahead (it is uploaded again later if it is needed again:
+// the first chunks of a periodic bunch are).  Returns false if need(c) does not fit in R slots.
+struct RingPlan {
+  int C;
+  std::vector<int> up_chunk, up_slot, up_step, up_wait, slot_of_step;
+  std::vector<std::vector<int>> need;
+};
+bool ring_plan(const int* nb, int NP, int chunk, int R, RingPlan* pl) {
+  const int C = (NP + chunk - 1) / chunk;
+  pl->C = C;
+  pl->need.assign(C, {});
+  for (int c = 0; c < C; ++c) {
+    std::vector<char> m(C, 0);
+    m[c] = 1;
+    for (int p = c * chunk; p < std::min(NP, (c + 1) * chunk); ++p)
+      for (int k = 0; k < 27; ++k) {
+        const int q = nb[(size_t)p * 27 + k];
+        if (q >= 0) m[q / chunk] = 1;
+      }
+    for (int x = 0; x < C; ++x) if (m[x]) pl->need[c].push_back(x);
+    if ((int)pl->need[c].size() > R) return false;
+  }
+  std::vector<int> slot_chunk(R, -1), where(C, -1), last_read(R, -1);
+  pl->slot_of_step.assign(C, -1);
+  for (int c = 0; c < C; ++c) {
+    std::vector<char> needed(C, 0);
+    for (int x : pl->need[c]) needed[x] = 1;
+    for (int x : pl->need[c]) {
+      if (where[x] >= 0) continue;
+      int s = -1;
+      for (int r = 0; r < R && s < 0; ++r) if (slot_chunk[r] < 0) s = r;
+      if (s < 0) {
+        int best = -1;
+        for (int r = 0; r < R; ++r) {
+          const int e = slot_chunk[r];
+          if (needed[e]) continue;
+          int next = C + 1;                                   // next step that needs e
+          for (int t = c + 1; t < C && next > C; ++t)
+            for (int y : pl->need[t]) if (y == e) { next = t; break; }
+          if (next > best) { best = next; s = r; }
+        }
+        if (s < 0) return false;
+        where[slot_chunk[s]] = -1;
+      }
+      pl->up_chunk.push_back(x); pl->up_slot.push_back(s); pl->up_step.push_back(c); pl->up_wait.push_back(last_read[s]);
+      slot_chunk[s] = x; where[x] = s;
+    }
+    for (int x : pl->need[c]) last_read[where[x]] = c;
+    pl->slot_of_step[c] = where[c];
+  }
+  return true;
+}
+
+void ring_release(mhd_bunch* b) {
+  mhd_bunch::Ring* r = b->ring;
+  if (!r) return;
+  if (r->s_up) cudaStreamSynchronize(r->s_up);
+  if (r->s_dn) cudaStreamSynchronize(r->s_dn);
+  for (auto* v : {&r->ev_up, &r->ev_step, &r->ev_dn})
+    for (cudaEvent_t e : *v) if (e) cudaEventDestroy(e);
+  if (r->s_up) cudaStreamDestroy(r->s_up);
+  if (r->s_dn) cudaStreamDestroy(r->s_dn);
+  delete r;
+  b->ring = nullptr;
+  // the window's own neighbour table goes back on the device
+  cudaMemcpyAsync(b->d_nbr, b->h_nbr->data(), sizeof(int) * 27 * (size_t)b->G.np, cudaMemcpyHostToDevice, b->stream);
+  cudaStreamSynchronize(b->stream);
+}
+
+}  // namespace
+
+extern "C" {
+
+int mhd_bunch_ring_plan(const int32_t* nbr, int32_t npatch, int32_t chunk_patches, int32_t ring_chunks, int32_t* nchunk,
+                        int32_t* nupload, int32_t* up_chunk, int32_t* up_slot, int32_t* up_step, int32_t* step_slot, int32_t cap) {
+  if (!nbr || npatch < 1 || chunk_patches < 1 || ring_chunks < 1 || !nchunk || !nupload) return MHD_EINVAL;
+  for (long long c = 0; c < 27ll * npatch; ++c)
+    if (nbr[c] < -1 || nbr[c] >= npatch) return MHD_EINVAL;
+  RingPlan pl;
+  if (!ring_plan(nbr, npatch, chunk_patches, ring_chunks, &pl)) return MHD_ENOMEM;
+  *nchunk = pl.C;
+  *nupload = (int)pl.up_chunk.size();
+  if (up_chunk || up_slot || up_step) {
+    if (cap < *nupload) return MHD_ENOMEM;
+    for (int u = 0; u < *nupload; ++u) {
+      if (up_chunk) up_chunk[u] = pl.up_chunk[u];
+      if (up_slot) up_slot[u] = pl.up_slot[u];
+      if (up_step) up_step[u] = pl.up_step[u];
+    }
+  }
+  if (step_slot) {
+    if (cap < pl.C) return MHD_ENOMEM;
+    for (int c = 0; c < pl.C; ++c) step_slot[c] = pl.slot_of_step[c];
+  }
+  return MHD_OK;
+}
+
+int mhd_bunch_ring_attach(mhd_bunch* b, const int32_t* nbr, int32_t npatch, int32_t chunk_patches, void* staging_dev,
+                          size_t staging_bytes) {
+  ENTER(b);
+  NOT_LOCAL(b);
+  if (!nbr || npatch < 1 || chunk_patches < 1 || !staging_dev || ((uintptr_t)staging_dev & 15)) return MHD_EINVAL;
+  if (!b->onepass_ok || b->G.n[0] % (int)(16 / b->esz) != 0) return MHD_EINVAL;     // the step must gather its halos
+  for (long long c = 0; c < 27ll * npatch; ++c)
+    if (nbr[c] < 0 || nbr[c] >= npatch) return MHD_EINVAL;                          // no outflow sides (compact host layout)
+  if (!table_is_consistent(nbr, npatch)) return MHD_EINVAL;
+  const int R = b->G.np / chunk_patches;
+  if (R < 1) return MHD_ENOMEM;
+  if (staging_bytes < 2 * hs_chunk_bytes(b, chunk_patches)) return MHD_ENOMEM;
+  RingPlan pl;
+  if (!ring_plan(nbr, npatch, chunk_patches, R, &pl)) return MHD_ENOMEM;
+  hs_release(b);
+  ring_release(b);
+  mhd_bunch::Ring* r = new (std::nothrow) mhd_bunch::Ring();
+  if (!r) return MHD_ENOMEM;
+  r->s_up = r->s_dn = nullptr;
+  b->ring = r;
+  struct Guard { mhd_bunch* b; bool ok; ~Guard() { if (!ok) ring_release(b); } } guard{b, false};
+  r->NP = npatch; r->chunk = chunk_patches; r->nchunk = pl.C; r->nslot = R;
+  r->up_chunk = pl.up_chunk; r->up_slot = pl.up_slot; r->up_step = pl.up_step; r->up_wait = pl.up_wait;
+  r->slot_of_step = pl.slot_of_step;
+  r->stage_up = (char*)staging_dev;
+  r->stage_dn = (char*)staging_dev + hs_chunk_bytes(b, chunk_patches);
+  // neighbour rows in slot space: when chunk c is stepped, chunk x of need(c) sits in the slot the
+  // plan put it in at that time -- replay the plan
+  r->rows.assign((size_t)npatch * 27, 0);
+  {
+    std::vector<int> where(pl.C, -1), slot_chunk(R, -1);
+    size_t u = 0;
+    for (int c = 0; c < pl.C; ++c) {
+      for (; u < pl.up_chunk.size() && pl.up_step[u] == c; ++u) {
+        if (slot_chunk[pl.up_slot[u]] >= 0) where[slot_chunk[pl.up_slot[u]]] = -1;
+        slot_chunk[pl.up_slot[u]] = pl.up_chunk[u];
+        where[pl.up_chunk[u]] = pl.up_slot[u];
+      }
+      for (int p = c * chunk_patches; p < std::min(npatch, (c + 1) * chunk_patches); ++p)
+        for (int k = 0; k < 27; ++k) {
+          const int q = nbr[(size_t)p * 27 + k], cq = q / chunk_patches;
+          r->rows[(size_t)p * 27 + k] = where[cq] * chunk_patches + (q - cq * chunk_patches);
+        }
+    }
+  }
+  CUDA_TRY(cudaStreamCreateWithFlags(&r->s_up, cudaStreamNonBlocking));
+  CUDA_TRY(cudaStreamCreateWithFlags(&r->s_dn, cudaStreamNonBlocking));
+  r->ev_up.assign(pl.up_chunk.size(), nullptr);
+  r->ev_step.assign(pl.C, nullptr);
+  r->ev_dn.assign(R, nullptr);
+  for (auto* v : {&r->ev_up, &r->ev_step, &r->ev_dn})
+    for (cudaEvent_t& e : *v) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  guard.ok = true;
+  return MHD_OK;
+}
+
+static int step_ring_body(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant, double* dt_next) {
+  mhd_bunch::Ring* r = b->ring;
+  const Geom& G = b->G;
+  const int C = r->nchunk;
+  { LaunchScope ls(b, KC_MISC);
+    k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0, b->d_rate_next, G.np); }
+  cudaEvent_t ev_begin = r->ev_step[C - 1];      // free at this point: marks "everything enqueued so far"
+  CUDA_TRY(cudaEventRecord(ev_begin, b->stream));
+  CUDA_TRY(cudaStreamWaitEvent(r->s_up, ev_begin, 0));
+  CUDA_TRY(cudaStreamWaitEvent(r->s_dn, ev_begin, 0));
+  void* const cur = b->state[b->cur];
+  void* const next = b->state[1 - b->cur];
+  std::vector<char> dn_pending(r->nslot, 0);
+  size_t u = 0;
+  for (int c = 0; c < C; ++c) {
+    for (; u < r->up_chunk.size() && r->up_step[u] == c; ++u) {
+      const int x = r->up_chunk[u], s = r->up_slot[u];
+      const int hp0 = x * r->chunk, npl = std::min(r->chunk, r->NP - hp0);
+      if (r->up_wait[u] >= 0) CUDA_TRY(cudaStreamWaitEvent(r->s_up, r->ev_step[r->up_wait[u]], 0));   // readers of the slot are done
+      int e = hs_copy(b, r->s_up, r->stage_up, (char*)const_cast<void*>(host_in), hp0, npl, true, r->NP);
+      if (e != MHD_OK) return e;
+      e = launch_pack<float, false>(b, r->s_up, cur, r->stage_up, s * r->chunk, npl);   // into the slot's patches
+      if (e != MHD_OK) return e;
+      CUDA_TRY(cudaEventRecord(r->ev_up[u], r->s_up));
+    }
+    const int s = r->slot_of_step[c], p0 = s * r->chunk, hp0 = c * r->chunk, npl = std::min(r->chunk, r->NP - hp0);
+    if (u > 0) CUDA_TRY(cudaStreamWaitEvent(b->stream, r->ev_up[u - 1], 0));     // uploads are in order: the latest covers all
+    CUDA_TRY(cudaMemcpyAsync(b->d_nbr + (size_t)p0 * 27, r->rows.data() + (size_t)hp0 * 27, sizeof(int) * 27 * npl,
+                             cudaMemcpyHostToDevice, b->stream));
+    {
+      const int e = launch_sync_closing<float>(b, p0, npl);
+      if (e != MHD_OK) return e;
+    }
+    if (dn_pending[s]) CUDA_TRY(cudaStreamWaitEvent(b->stream, r->ev_dn[s], 0));   // the slot's previous result has left
+    b->guards_stale = true;
+    {
+      const int e = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, false);
+      if (e != MHD_OK) return e;
+    }
+    CUDA_TRY(cudaEventRecord(r->ev_step[c], b->stream));
+    CUDA_TRY(cudaStreamWaitEvent(r->s_dn, r->ev_step[c], 0));
+    {
+      int e = launch_pack<float, true>(b, r->s_dn, next, r->stage_dn, p0, npl);
+      if (e != MHD_OK) return e;
+      e = hs_copy(b, r->s_dn, r->stage_dn, (char*)host_out, hp0, npl, false, r->NP);
+      if (e != MHD_OK) return e;
+    }
+    CUDA_TRY(cudaEventRecord(r->ev_dn[s], r->s_dn));
+    dn_pending[s] = 1;
+  }
+  { LaunchScope ls(b, KC_MISC);
+    k_cfl_final<<<1, 256, 0, b->stream>>>(b->d_rate_next, G.np, courant, b->d_dt, nullptr, nullptr); }
+  double dts = 0.0;
+  CUDA_TRY(cudaMemcpyAsync(&dts, b->d_dt, sizeof(double), cudaMemcpyDeviceToHost, b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));
+  CUDA_TRY(cudaStreamSynchronize(r->s_dn));
+  CUDA_TRY(cudaStreamSynchronize(r->s_up));
+  if (dt_next) *dt_next = dts;
+  return MHD_OK;
+}
+
+int mhd_bunch_step_ring(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant, double* dt_next) {
+  ENTER(b);
+  mhd_bunch::Ring* r = b->ring;
+  if (!r) return MHD_ESTATE;
+  if (!host_in || !host_out || host_in == host_out) return MHD_EINVAL;
+  if (!(dt > 0.0) || !isfinite(dt) || !(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
+  const bool fused_saved = b->fused_cfl, gather_saved = b->gather_ok;
+  b->fused_cfl = true;        // the CFL rates of the new level come out of the step's epilogue, slot by slot
+  b->gather_ok = true;        // halos through the (slot-space) neighbour rows
+  const int rc = step_ring_body(b, host_in, host_out, dt, courant, dt_next);
+  if (rc != MHD_OK) {
+    cudaStreamSynchronize(b->stream);
+    cudaStreamSynchronize(r->s_up);
+    cudaStreamSynchronize(r->s_dn);
+  }
+  b->fused_cfl = fused_saved;
+  b->gather_ok = gather_saved;
+  b->guards_stale = false;
+  b->closing_ok = false;
+  b->rate_valid = false;
+  return rc;
+}
+
+int mhd_bunch_ring_detach(mhd_bunch* b) {
+  ENTER(b);
+  ring_release(b);
+  return MHD_OK;
+}
+
+}  // extern "C"
+
 // ------------------------------------------------------- local time steps ----
 namespace {
 
@@ -1471,6 +1737,7 @@ int mhd_bunch_destroy(mhd_bunch* b) {
   cudaStreamSynchronize(b->stream);
   drain_events(b, false);
   hs_release(b);
+  ring_release(b);
   delete b->loc;
   delete b->h_nbr;
   delete b->events;

@@ -141,3 +141,59 @@ def test_host_stream_schedule_and_rejections():
     with pytest.raises(RuntimeError):
         b.step_host(t, t, dt=0.1)
     b.close()
+
+
+# ------------------------------------------------- ring mode: bunch larger than the buffers ----
+@pytest.mark.parametrize("shape", ["slabs16_R3", "slabs16_R5", "cube64_R3", "ragged_chunks"])
+def test_ring_step_equals_resident_step_bitwise(shape):
+    """a host-resident bunch streams through device
+    buffers that hold only a WINDOW of it (a ring of chunk slots deliberately smaller than the bunch;
+    halos are read through a neighbour table rewritten in slot numbers, the first chunks are uploaded
+    a second time for the last ones).  Three chained steps, each bit for bit the resident step of the
+    same kernel (the ring always runs the variant with the CFL epilogue, so the resident handle is
+    switched to it too), with the same dt sequence from that epilogue."""
+    import torch
+    from paper_2508_09568_b200.binding import MhdBunch
+    w, chunk, R = {"slabs16_R3": (lambda: W.turbulence(N=(32, 32, 128), n=16, dtype=np.float32), 4, 3),
+                   "slabs16_R5": (lambda: W.turbulence(N=(32, 32, 128), n=16, dtype=np.float32), 4, 5),
+                   "cube64_R3": (lambda: W.turbulence(N=128, n=32, dtype=np.float32, config=2), 16, 3),
+                   "ragged_chunks": (lambda: W.turbulence(N=(48, 32, 160), n=16, dtype=np.float32), 7, 6)}[shape]
+    w = w()
+    assert R * chunk < w.npatch
+    ref = make_gpu(w, "f32")                                   # the whole bunch resident
+    ref.set_tuning("fused_cfl", 1)
+    win = MhdBunch(w.n, R * chunk, W.neighbour_table((R * chunk, 1, 1), (True, True, True)), w.gamma, w.dx, dtype="f32")
+    win.ring_attach(w.nbr, chunk)
+    hin = pinned(W.to_compact(w.U, w.n))
+    hout = torch.empty_like(hin).pin_memory()
+    ref.fill_guards()
+    dt = ref.cfl_dt(0.4, sync=True)
+    for _ in range(3):
+        ref.fill_guards()
+        ref.step(dt)
+        dt_next = win.step_ring(hin, hout, dt, 0.4)
+        want = W.to_compact(ref.download(), w.n)
+        assert np.array_equal(hout.numpy(), want)
+        ref.fill_guards()
+        dt = ref.cfl_dt(0.4, sync=True)
+        assert dt_next == dt
+        hin, hout = hout, hin
+    assert win.status() == 0
+    win.ring_detach()
+    ref.close(); win.close()
+
+
+def test_ring_attach_rejections():
+    from paper_2508_09568_b200.binding import MhdBunch
+    w = W.turbulence(N=(32, 32, 64), n=16, dtype=np.float32)
+    win = MhdBunch(w.n, 8, W.neighbour_table((8, 1, 1), (True, True, True)), w.gamma, w.dx, dtype="f32")
+    with pytest.raises(RuntimeError):
+        win.ring_attach(w.nbr, 4)                              # two slots cannot hold a slab and both neighbours
+    bad = w.nbr.copy(); bad[3, 0] = -1
+    with pytest.raises(RuntimeError):
+        win.ring_attach(bad, 2)
+    w64 = MhdBunch(w.n, 12, W.neighbour_table((12, 1, 1), (True, True, True)), w.gamma, w.dx, dtype="f64")
+    with pytest.raises(RuntimeError):
+        w64.ring_attach(w.nbr, 4)                              # needs the one-pass step
+    assert win.lib.mhd_bunch_step_ring(win.h, None, None, 1e-3, 0.4, None) == -4
+    win.close(); w64.close()

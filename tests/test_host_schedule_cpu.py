@@ -83,3 +83,44 @@ def test_schedule_rejects_bad_tables():
     assert lib.mhd_bunch_host_schedule(nbr.ctypes.data_as(C.c_void_p), 8, 1, C.byref(a), C.byref(b_),
                                        up.ctypes.data_as(C.c_void_p), None, None, 1, None) == -2       # capacity too small
     assert lib.mhd_bunch_host_schedule(None, 8, 1, C.byref(a), C.byref(b_), None, None, None, 0, None) == -1
+
+
+# ---------------------------------------------------------------- ring mode: the planner ----
+def _need(nbr, chunk):
+    C = (len(nbr) + chunk - 1) // chunk
+    return [sorted({q // chunk for p in range(c * chunk, min(len(nbr), (c + 1) * chunk)) for q in nbr[p] if q >= 0} | {c})
+            for c in range(C)]
+
+
+@pytest.mark.parametrize("P,chunk,R", [((2, 2, 8), 4, 3), ((2, 2, 8), 4, 5), ((4, 4, 4), 16, 3), ((4, 4, 4), 8, 6), ((8, 8, 8), 64, 4),
+                                       ((3, 2, 5), 6, 3), ((2, 2, 2), 8, 1), ((4, 4, 4), 5, 13)])
+def test_ring_plan_keeps_every_needed_chunk_resident_and_never_overfills(P, chunk, R):
+    """mhd_bunch_ring_plan replayed on the host: before step c every chunk holding a neighbour of chunk
+    c sits in a slot, no slot holds two chunks, a chunk is only evicted when the step at hand does not
+    need it, and a periodic stack of slabs costs exactly two uploads more than it has slabs."""
+    nbr = W.neighbour_table(P, (True, True, True))
+    pl = B.ring_plan(nbr, chunk, R)
+    need = _need(nbr, chunk)
+    assert pl is not None and pl["nchunk"] == len(need)
+    slot_chunk, u = {}, 0
+    for c in range(pl["nchunk"]):
+        while u < len(pl["up_chunk"]) and pl["up_step"][u] == c:
+            s, x = int(pl["up_slot"][u]), int(pl["up_chunk"][u])
+            assert 0 <= s < R and x in need[c] and x not in slot_chunk.values()
+            assert slot_chunk.get(s) not in need[c]               # never evicts what the step needs
+            slot_chunk[s] = x
+            u += 1
+        resident = set(slot_chunk.values())
+        assert set(need[c]) <= resident and len(slot_chunk) <= R
+        assert slot_chunk[int(pl["step_slot"][c])] == c
+    assert u == len(pl["up_chunk"])
+    if P == (2, 2, 8) and R == 3:
+        assert len(pl["up_chunk"]) == 8 + 2                        # slabs 7 and 0 come twice
+    if R >= pl["nchunk"]:
+        assert len(pl["up_chunk"]) == pl["nchunk"]                 # everything fits: one upload each
+
+
+def test_ring_plan_refuses_a_window_that_cannot_hold_a_neighbourhood():
+    nbr = W.neighbour_table((2, 2, 8), (True, True, True))
+    assert B.ring_plan(nbr, 4, 2) is None                          # a slab needs itself and both neighbours
+    assert B.ring_plan(nbr, 4, 3) is not None
