@@ -187,12 +187,16 @@ def measure(name, args, local, world, rank, field_cache, headline):
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, device=local)
     b.load(w.U if dtype == "f64" else w.U.astype(np.float32))
     b.set_path(args.path)
+    if args.fused_cfl and b.path == "onepass":
+        b.set_tuning("fused_cfl", 1)
     stream = b.stream
     courant = 0.4
     steps = args.steps if headline else max(3, min(args.steps, args.sub_steps))
 
     def one_step():
         b.fill_guards()
+        if args.explicit_fill:
+            b.sync_guards()        # write the guard shell to HBM every step (k_fill_guards), as a caller that reads it would
         b.cfl_dt(courant, sync=False)
         b.step_dev()
 
@@ -431,6 +435,10 @@ def main():
     ap.add_argument("--host-chunk", type=int, default=0, help="patches per chunk of the host-streaming path (0: library default)")
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "two_kernel", "onepass"],
                     help="which CUDA implementation of the step runs (include/mhd_bunch.h, MHD_PATH_*)")
+    ap.add_argument("--explicit-fill", action="store_true",
+                    help="materialise the guard shell in HBM every step (the fill is otherwise folded into the step's halo loads)")
+    ap.add_argument("--fused-cfl", type=int, default=0, choices=[0, 1],
+                    help="one-pass step: reduce the new level's CFL rates in the step's epilogue (MHD_TUNE_FUSED_CFL)")
     ap.add_argument("--sizes", default="16,24,32,64", help="c4: patch sizes")
     ap.add_argument("--bunches", default="1,8,64,512,4096", help="c4: bunch sizes")
     args = ap.parse_args()

@@ -200,9 +200,19 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
 
   auto dslot = [&](int plane) { return Dm + (size_t)((plane + 2) & 1) * (D_COUNT * DCS); };
 
-  if (t >= 2 * NR) {
+  // Warp ids decide issue priority on an SM sub-partition (the higher id wins a tie), so the order of
+  // the roles in the thread index is a tuning knob: ROLE_ORDER 0 = A, C, P (P highest), 1 = P, C, A,
+  // 2 = C, P, A, 3 = P, A, C, 4 = C, A, P, 5 = A, P, C
+#ifndef ONEPASS_ROLE_ORDER
+#define ONEPASS_ROLE_ORDER 0
+#endif
+  constexpr int RO = ONEPASS_ROLE_ORDER;
+  constexpr int P0 = (RO == 0 || RO == 4) ? 2 * NR : ((RO == 1 || RO == 3) ? 0 : NR);
+  constexpr int A0 = (RO == 0 || RO == 5) ? 0 : ((RO == 1 || RO == 2) ? NP + NR : ((RO == 3) ? NP : NR));
+  constexpr int C0 = (RO == 2 || RO == 4) ? 0 : ((RO == 0) ? NR : ((RO == 1) ? NP : ((RO == 3) ? NP + NR : NR + NP)));
+  if (t >= P0 && t < P0 + NP) {
     // =============================================================== role P ==========
-    const int tp = t - 2 * NR;
+    const int tp = t - P0;
     const T q4 = T(0.25), hdt = h * dt;
     const T lx = hdt * P.idx[0], ly = hdt * P.idx[1], lz = hdt * P.idx[2];
     const T gm1 = gamma - T(1);
@@ -496,8 +506,8 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   }
 
   // =========================================================== roles A and C ==========
-  const bool roleA = t < NR;
-  const int tr = roleA ? t : t - NR;
+  const bool roleA = t >= A0 && t < A0 + NR;
+  const int tr = roleA ? t - A0 : t - C0;
   const bool colthr = tr >= C::CB;                        // closing-column warp
   const int fj = colthr ? tr - C::CB : tr / TX;
   const int fi = colthr ? TX : tr - fj * TX;
