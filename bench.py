@@ -315,9 +315,9 @@ def measure(name, args, local, world, rank, field_cache, headline):
         assert bool(torch.isfinite(hin).all())
         e2e = {"value": world * w.cells * esteps / el, "unit": UNIT, "h2d_bytes_per_step": int(hl.host_bytes),
                "d2h_bytes_per_step": int(hl.host_bytes), "steps": esteps, "ms_per_step": 1e3 * el / esteps,
-               "chunk_patches": int(hl.chunk_patches), "chunks": int(hl.nchunk), "overlapped": bool(hl.pipelined),
+               "chunk_patches": int(hl.chunk_patches), "chunks": int(hl.nchunk), "bands": int(hl.bands), "overlapped": bool(hl.pipelined),
                "note": "mhd_bunch_step_host: compact host state (interiors only) uploaded from pinned memory, "
-                       "stepped and downloaded every step in chunks on two copy streams; wall clock"}
+                       "stepped and downloaded every step in chunks (thin z-layers of the next chunk ahead of its bulk, first chunk and last two in z-bands) on library copy streams; wall clock"}
         del hin, hout
     rec = {"workload": name, "value": value, "unit": UNIT, "steps": steps, "warmup": warm, "ms_per_step": ms / steps,
            "dtype": dtype,

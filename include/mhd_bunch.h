@@ -138,10 +138,15 @@ int mhd_bunch_download(mhd_bunch *b, void *host_state);
  * bunch lives in HOST memory in the COMPACT layout  host[field][patch][k][j][i]  (interior
  * cells only, n_z*n_y*n_x per patch and field, fields in Eq. 6's order; B components on the
  * lower faces; host_bytes long; pinned memory lets the copies run asynchronously).  One
- * call advances it by one step: chunks of patches cross PCIe on two library-owned copy
- * streams, are scattered into the padded HBM layout, stepped chunk by chunk as soon as the
- * chunks holding their neighbours have arrived (the neighbour table decides), gathered and
- * copied back -- so uploads, kernels and downloads overlap.  Guard zones never cross PCIe.
+ * call advances it by one step: pieces of chunks of patches cross PCIe on library-owned copy
+ * streams (through two staging buffers per direction, so the link never waits for a kernel),
+ * are scattered into the padded HBM layout, stepped chunk by chunk as soon as what their
+ * neighbours must provide has arrived (the neighbour table decides), gathered and copied
+ * back -- so uploads, kernels and downloads overlap.  Guard zones never cross PCIe.  A chunk
+ * needs the chunks of its in-plane neighbours whole, but of a chunk it reaches only through
+ * o_z = +1 (-1) just the lowest (highest) guard-width planes: those thin layers are uploaded
+ * ahead of the rest, so a chunk never waits for the bulk of its z-neighbours (and the first
+ * chunk of a periodic stack not for the last one).
  *
  *   mhd_bunch_host_query   HOST out *layout for a chunk size (<= 0: library default):
  *                          host_bytes, the staging size, the number of chunks, and whether
@@ -168,7 +173,7 @@ typedef struct {
   int32_t chunk_patches;   /* patches per chunk                                            */
   int32_t nchunk;          /* chunks per bunch                                             */
   int32_t pipelined;       /* 1: uploads, steps and downloads overlap chunk by chunk       */
-  int32_t reserved;
+  int32_t bands;           /* z-bands the first chunk and the last two are stepped in      */
 } mhd_bunch_host_layout;
 int mhd_bunch_host_query(mhd_bunch *b, int32_t chunk_patches, mhd_bunch_host_layout *layout);
 int mhd_bunch_host_attach(mhd_bunch *b, void *staging_dev, size_t staging_bytes, int32_t chunk_patches);
@@ -177,15 +182,24 @@ int mhd_bunch_step_host(mhd_bunch *b, const void *host_in, void *host_out, doubl
 int mhd_bunch_host_detach(mhd_bunch *b);
 
 /* HOST only, no device needed: the schedule mhd_bunch_step_host would follow for a neighbour
- * table (HOST int32 [npatch][27]) and a chunk size (<= 0: the library's choice, the candidate
- * with the shortest simulated makespan).  Outputs (HOST; the three arrays nullable, capacity
- * `cap` >= *nchunk else MHD_ENOMEM): up_order[u] = chunk uploaded u-th; ready[c] = position
- * of the last upload that carries a neighbour of chunk c (its step may start after it);
- * step_order[s] = chunk stepped s-th; *makespan = simulated length of the step in units of
- * "one patch across PCIe" (a step costs 0.3 per patch, each transfer 1.5 fixed).           */
-int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t chunk_patches, int32_t *chunk_out,
-                            int32_t *nchunk_out, int32_t *up_order, int32_t *ready, int32_t *step_order, int32_t cap,
-                            double *makespan);
+ * table (HOST int32 [npatch][27]), patches of nz planes, a guard width, a chunk size and a number
+ * of bands (each <= 0: the library's choice, the candidate with the shortest simulated makespan).
+ * STEP UNITS are stepped in order: chunks 0 .. nchunk-1, the first chunk and the last two in
+ * `bands` bands of planes each (so that downloads start early and the step ends with the download
+ * of two bands, not of two chunks), the others whole.  Outputs (HOST; the arrays nullable, capacity `cap` >= *npiece
+ * and >= *nunit else MHD_ENOMEM): upload piece i carries planes [piece_k0[i], piece_k1[i]) of
+ * every patch of chunk piece_chunk[i]; the pieces of a chunk partition its planes (every plane
+ * crosses PCIe once); unit u = planes [unit_za[u], unit_zb[u]) of chunk unit_chunk[u]; ready[u] =
+ * index of the last piece unit u needs before it may step (planes [za-guard, zb+guard) of itself
+ * and of its in-plane neighbours' chunks; the lowest planes of chunks reached through o_z = +1 if
+ * the range passes nz, the highest of those reached through o_z = -1 if it passes 0; everything
+ * whole if nz < 2 guard + 1 or nz > 64); *makespan = simulated length of the step in units of
+ * "one patch across PCIe" (a step costs 0.33 per patch; fixed costs: 2.0 per upload piece, 0.5
+ * per step, 0.7 per download -- measured on a B200 / PCIe 5 box).                               */
+int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t nz, int32_t guard, int32_t chunk_patches, int32_t bands,
+                            int32_t *chunk_out, int32_t *bands_out, int32_t *npiece_out, int32_t *piece_chunk,
+                            int32_t *piece_k0, int32_t *piece_k1, int32_t *nunit_out, int32_t *unit_chunk, int32_t *unit_za,
+                            int32_t *unit_zb, int32_t *ready, int32_t cap, double *makespan);
 
 /* Ring mode: a host-resident bunch LARGER than the device buffers (PAPER.md
  * L164: bunches filled round-robin with several in flight; L243-247: asynchronous staging).  The
@@ -301,7 +315,12 @@ int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
  *                          only runs the bunch-wide reduction instead of re-reading the state;
  *                          0 (default): mhd_bunch_cfl_dt makes its own pass.  Same dt, bit for
  *                          bit, either way (both evaluate one explicitly rounded function).
+ *   MHD_TUNE_HOST_BANDS    z-bands in which mhd_bunch_step_host steps the first chunk and the last
+ *                          two (0 = automatic; clipped to bands of at least eight planes; only
+ *                          the one-pass path steps plane ranges).  Read by host_query / attach;
+ *                          results do not depend on it, bit for bit.
  * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
+#define MHD_TUNE_HOST_BANDS   4
 #define MHD_TUNE_ONEPASS_ZSEG 1
 #define MHD_TUNE_PREDICT_TY   2
 #define MHD_TUNE_FUSED_CFL    3

@@ -13,7 +13,7 @@ from . import build as _build
 
 MHD_F32, MHD_F64 = 0, 1
 PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3}
-TUNE = {"onepass_zseg": 1, "predict_ty": 2, "fused_cfl": 3}
+TUNE = {"onepass_zseg": 1, "predict_ty": 2, "fused_cfl": 3, "host_bands": 4}
 _ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
 
 ABI_SYMBOLS = [
@@ -42,7 +42,7 @@ class Layout(C.Structure):
 
 class HostLayout(C.Structure):
     _fields_ = [("host_bytes", C.c_size_t), ("staging_bytes", C.c_size_t), ("chunk_patches", C.c_int32),
-                ("nchunk", C.c_int32), ("pipelined", C.c_int32), ("reserved", C.c_int32)]
+                ("nchunk", C.c_int32), ("pipelined", C.c_int32), ("bands", C.c_int32)]
 
 
 _lib = None
@@ -84,7 +84,8 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_host_attach.argtypes = [vp, vp, C.c_size_t, i32]
     lib.mhd_bunch_step_host.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.mhd_bunch_host_detach.argtypes = [vp]
-    lib.mhd_bunch_host_schedule.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, i32, C.POINTER(dbl)]
+    lib.mhd_bunch_host_schedule.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), vp, vp, vp,
+                                            C.POINTER(i32), vp, vp, vp, vp, i32, C.POINTER(dbl)]
     lib.mhd_bunch_ring_plan.argtypes = [vp, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), vp, vp, vp, vp, i32]
     lib.mhd_bunch_ring_attach.argtypes = [vp, vp, i32, i32, vp, C.c_size_t]
     lib.mhd_bunch_step_ring.argtypes = [vp, vp, vp, dbl, dbl, C.POINTER(dbl)]
@@ -138,20 +139,25 @@ def measure_alu_peak(dtype="f32", device=0):
     return v.value
 
 
-def host_schedule(nbr, chunk_patches=0):
-    """Schedule of the host-streaming step for a neighbour table (host only, no device):
-    dict with chunk, up_order, ready, step_order (numpy int32) and the simulated makespan."""
+def host_schedule(nbr, chunk_patches=0, nz=32, guard=3, bands=0):
+    """Schedule of the host-streaming step for a neighbour table (host only, no device): dict with
+    chunk, bands, the upload pieces (piece_chunk, piece_k0, piece_k1: planes [k0, k1) of a chunk), the
+    step units in order (unit_chunk, unit_za, unit_zb), ready[u] (last piece unit u needs) and the
+    simulated makespan."""
     nbr = np.ascontiguousarray(nbr, dtype=np.int32)
     npatch = nbr.shape[0]
-    chunk, nchunk, span = C.c_int32(0), C.c_int32(0), C.c_double(0.0)
-    up, ready, order = (np.zeros(npatch, dtype=np.int32) for _ in range(3))
-    _check(load_library().mhd_bunch_host_schedule(nbr.ctypes.data_as(C.c_void_p), npatch, chunk_patches, C.byref(chunk),
-                                                  C.byref(nchunk), up.ctypes.data_as(C.c_void_p),
-                                                  ready.ctypes.data_as(C.c_void_p), order.ctypes.data_as(C.c_void_p),
-                                                  npatch, C.byref(span)), "mhd_bunch_host_schedule")
-    n = nchunk.value
-    return {"chunk": chunk.value, "nchunk": n, "up_order": up[:n].copy(), "ready": ready[:n].copy(),
-            "step_order": order[:n].copy(), "makespan": span.value}
+    chunk, bnd, npiece, nunit, span = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_double(0.0)
+    cap = 4 * npatch + 64
+    pc, k0, k1, uc, za, zb, ready = (np.zeros(cap, dtype=np.int32) for _ in range(7))
+    ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+    _check(load_library().mhd_bunch_host_schedule(ptr(nbr), npatch, nz, guard, chunk_patches, bands, C.byref(chunk), C.byref(bnd),
+                                                  C.byref(npiece), ptr(pc), ptr(k0), ptr(k1), C.byref(nunit), ptr(uc), ptr(za),
+                                                  ptr(zb), ptr(ready), cap, C.byref(span)), "mhd_bunch_host_schedule")
+    n, m = nunit.value, npiece.value
+    return {"chunk": chunk.value, "nchunk": -(-npatch // chunk.value), "bands": bnd.value, "npiece": m, "nunit": n,
+            "piece_chunk": pc[:m].copy(), "piece_k0": k0[:m].copy(), "piece_k1": k1[:m].copy(),
+            "unit_chunk": uc[:n].copy(), "unit_za": za[:n].copy(), "unit_zb": zb[:n].copy(), "ready": ready[:n].copy(),
+            "makespan": span.value}
 
 
 def ring_plan(nbr, chunk_patches, ring_chunks):
@@ -364,7 +370,7 @@ class MhdBunch:
         return {k: n for n, k in PATHS.items()}[v.value]
 
     def set_tuning(self, key, value):
-        """key: 'onepass_zseg' | 'predict_ty' (include/mhd_bunch.h, MHD_TUNE_*)."""
+        """key: 'onepass_zseg' | 'predict_ty' | 'fused_cfl' | 'host_bands' (include/mhd_bunch.h, MHD_TUNE_*)."""
         _check(self.lib.mhd_bunch_set_tuning(self.h, TUNE[key], int(value)), "mhd_bunch_set_tuning")
 
     def set_timing(self, on):

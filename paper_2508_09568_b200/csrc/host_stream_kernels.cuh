@@ -4,16 +4,19 @@
 // (interior cells only); a chunk of patches crosses PCIe as eight contiguous copies into a
 // staging buffer and is scattered into / gathered from the padded HBM layout by these
 // kernels (pure data movement, HBM-bound, 16-byte accesses where the row length allows).
+// A transfer may carry only the z-planes [k0, k0+nk) of its patches (a PIECE): the lowest or
+// highest guard-width planes of a chunk are all its z-neighbours need from it, so they cross
+// PCIe ahead of the rest (see hs_plan in mhd_bunch.cu).
 #pragma once
 #include "bunch_types.cuh"
 
 namespace mhd {
 
-// stage[f][pl][k][j][i] (npl patches of the chunk)  <->  U[f][p0+pl][k+g][j+g][i+g]
+// stage[f][pl][kk][j][i] (npl patches, nk planes)  <->  U[f][p0+pl][k0+kk+g][j+g][i+g]
 template <typename T, int VEC, bool PACK>
-__global__ void __launch_bounds__(256) k_pack_unpack(Geom G, T* __restrict__ U, T* __restrict__ stage, int p0, int npl) {
+__global__ void __launch_bounds__(256) k_pack_unpack(Geom G, T* __restrict__ U, T* __restrict__ stage, int p0, int npl, int k0, int nk) {
   const int nxv = G.n[0] / VEC;
-  const long long rows = (long long)G.n[1] * G.n[2];
+  const long long rows = (long long)G.n[1] * nk;
   const long long per = rows * nxv;                       // vectors per (field, patch)
   const long long tot = per * npl * 8;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
@@ -23,7 +26,7 @@ __global__ void __launch_bounds__(256) k_pack_unpack(Geom G, T* __restrict__ U, 
     const int row = r / nxv, iv = r - row * nxv;
     const int k = row / G.n[1], j = row - k * G.n[1];
     const long long u = (long long)f * G.fs + (long long)(p0 + pl) * G.ps + G.lead + (iv * VEC + G.g[0]) +
-                        (long long)(j + G.g[1]) * G.pitch + (long long)(k + G.g[2]) * G.pitch * G.m[1];
+                        (long long)(j + G.g[1]) * G.pitch + (long long)(k0 + k + G.g[2]) * G.pitch * G.m[1];
     const long long s = (fp * rows + row) * G.n[0] + (long long)iv * VEC;
     if (VEC == 1) {
       if (PACK) stage[s] = U[u]; else U[u] = stage[s];

@@ -88,12 +88,19 @@ struct mhd_bunch {
   CUtensorMap tmap_d;  // D block of the scratch: [38][chunk][mz][my][pitch]
   // host-streaming path (mhd_bunch_host_attach / mhd_bunch_step_host)
   struct HostStream {
-    char* stage_up; char* stage_dn;      // DEVICE staging, one chunk each (caller-owned)
-    int chunk, nchunk;                   // patches per chunk, number of chunks
-    cudaStream_t s_up, s_dn;             // copy-in and copy-out streams (library-owned)
+    char* stage_up[2]; char* stage_dn[2];   // DEVICE staging, two chunk-sized buffers per direction (caller-owned)
+    int chunk, nchunk;                      // patches per chunk, number of chunks
+    // Library-owned streams: H2D copies alternate between two streams and so do D2H copies -- measured
+    // on this box: while the other direction is busy, a copy that has to wait for the COMPLETION of the
+    // previous copy of its stream starts ~40 us late (the completion signal queues behind the data);
+    // two independent copies in flight keep the link busy.  Unpack and pack kernels have their own streams.
+    cudaStream_t s_up[2], s_un, s_pk, s_dn[2];
     cudaEvent_t ev_begin, ev_all_steps;
-    std::vector<cudaEvent_t> ev_up, ev_step;   // per upload position / per chunk
-    std::vector<int> up_order, step_order, ready;   // ready[c]: upload position after which chunk c may step
+    std::vector<cudaEvent_t> ev_copied, ev_up;            // per piece: staged / scattered into the state
+    std::vector<cudaEvent_t> ev_step, ev_packed, ev_dn;   // per step unit: stepped / gathered / on the host
+    std::vector<int> piece_chunk, piece_k0, piece_k1;     // upload pieces in order: planes [k0, k1) of a chunk
+    std::vector<int> unit_chunk, unit_za, unit_zb;        // step units in order: planes [za, zb) of a chunk
+    std::vector<int> ready;                 // ready[u]: piece after which unit u may step
   };
   HostStream* hs;
   // ring mode (mhd_bunch_ring_attach / mhd_bunch_step_ring): the handle's buffers are a window of
@@ -127,6 +134,7 @@ struct mhd_bunch {
   const int* ov_plist; const double* ov_dtlist; int ov_side;
   bool nbr_consistent; // the table composes like translations (see table_is_consistent)
   int tune_zseg;       // MHD_TUNE_ONEPASS_ZSEG: 0 = automatic
+  int tune_bands;      // MHD_TUNE_HOST_BANDS: 0 = automatic
   bool fused_cfl;      // MHD_TUNE_FUSED_CFL: the one-pass step reduces the new level's CFL rates in its epilogue
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
@@ -288,14 +296,15 @@ int launch_fill(mhd_bunch* b) {
 
 // closing faces only (the part of the fill that cfl_dt and the one-pass kernel's update read)
 template <typename T>
-int launch_sync_closing(mhd_bunch* b, int p0 = 0, int npl = -1) {
+int launch_sync_closing(mhd_bunch* b, int p0 = 0, int npl = -1, int zlo = 0, int zhi = -1) {
   const Geom& G = b->G;
   if (npl < 0) npl = G.np;
+  if (zhi < 0) zhi = G.n[2];
   const long long per = (long long)G.n[1] * G.n[2] + (long long)G.n[0] * G.n[2] + (long long)G.n[0] * G.n[1];
   const long long tot = per * npl;
   {
     LaunchScope ls(b, KC_CLOSING);
-    k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr, p0, npl);
+    k_sync_closing_faces<T><<<blocks_for(tot, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr, p0, npl, zlo, zhi);
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
@@ -353,12 +362,12 @@ bool step_gathers(const mhd_bunch* b) {
 
 template <typename T> struct OnePassLaunch {
   static int prepare(mhd_bunch*) { return MHD_OK; }
-  static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true) { return MHD_EINVAL; }
+  static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true, int = 0, int = -1) { return MHD_EINVAL; }
 };
 template <> struct OnePassLaunch<float> {
   // one tile shape: patches [p0, p0+npl) of the bunch
   template <int TX, int TY>
-  static int launch(mhd_bunch* b, const double* dtp, int p0, int npl, bool attr_only = false) {
+  static int launch(mhd_bunch* b, const double* dtp, int p0, int npl, bool attr_only = false, int zlo = 0, int zhi = -1) {
     using Cfg = OneCfg<float, TX, TY, OneTile::NPW>;
     const Geom& G = b->G;
     if (attr_only) {   // called once from create, on the handle's device (the attribute is per device)
@@ -373,6 +382,7 @@ template <> struct OnePassLaunch<float> {
                     ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, true> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>)
                     : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, false> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>);
     Params<float> P = make_params<float>(b, p0, npl);
+    if (zhi < 0) zhi = G.n[2];
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
     // fewer tiles than SMs: cut the columns into z segments of at least 8 planes so that the
     // launch covers the GPU about twice (each segment pays a five-plane run-in, so only then)
@@ -380,14 +390,14 @@ template <> struct OnePassLaunch<float> {
     const long long tiles = (long long)xt * yt * npl;
     if (tiles < b->nsm) {
       zseg = (int)((2ll * b->nsm + tiles - 1) / tiles);
-      const int zmax = G.n[2] / 8 > 1 ? G.n[2] / 8 : 1;
+      const int zmax = (zhi - zlo) / 8 > 1 ? (zhi - zlo) / 8 : 1;
       if (zseg > zmax) zseg = zmax;
     }
-    if (b->tune_zseg >= 1) zseg = b->tune_zseg < G.n[2] ? b->tune_zseg : G.n[2];   // mhd_bunch_set_tuning
+    if (b->tune_zseg >= 1) zseg = b->tune_zseg < zhi - zlo ? b->tune_zseg : zhi - zlo;   // mhd_bunch_set_tuning
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
-      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, (b->gather_ok && !b->ov_plist) ? 1 : 0, dtp, b->d_bad, b->d_rate_next, xt, zseg);
+      kern<<<grid, Cfg::NTH, Cfg::smem, b->stream>>>(P, b->d_nbr, (b->gather_ok && !b->ov_plist) ? 1 : 0, dtp, b->d_bad, b->d_rate_next, xt, zseg, zlo, zhi);
     }
     CUDA_TRY(cudaGetLastError());
     return MHD_OK;
@@ -397,9 +407,10 @@ template <> struct OnePassLaunch<float> {
   static int prepare(mhd_bunch* b) {
     return b->G.n[0] <= 16 ? launch<16, 16>(b, nullptr, 0, 0, true) : launch<OneTile::TX, OneTile::TY>(b, nullptr, 0, 0, true);
   }
-  static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true) {
+  static int run(mhd_bunch* b, const double* dtp, int p0 = 0, int npl = -1, bool last = true, int zlo = 0, int zhi = -1) {
     if (npl < 0) npl = b->G.np;
-    const int rc = b->G.n[0] <= 16 ? launch<16, 16>(b, dtp, p0, npl) : launch<OneTile::TX, OneTile::TY>(b, dtp, p0, npl);
+    const int rc = b->G.n[0] <= 16 ? launch<16, 16>(b, dtp, p0, npl, false, zlo, zhi)
+                                   : launch<OneTile::TX, OneTile::TY>(b, dtp, p0, npl, false, zlo, zhi);
     if (rc != MHD_OK) return rc;
     if (last) {
       b->cur = 1 - b->cur;
@@ -726,6 +737,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->gather_ok = b->gather_ok && b->nbr_consistent;
   b->gather2_ok = b->fused_ok && b->nbr_consistent;
   b->tune_zseg = 0;
+  b->tune_bands = 0;
   b->fused_cfl = false;
   b->hs = nullptr;
   b->ring = nullptr;
@@ -846,6 +858,10 @@ int mhd_bunch_set_tuning(mhd_bunch* b, int32_t key, int32_t value) {
   if (value < 0) return MHD_EINVAL;
   if (key == MHD_TUNE_ONEPASS_ZSEG) {
     b->tune_zseg = value;
+    return MHD_OK;
+  }
+  if (key == MHD_TUNE_HOST_BANDS) {
+    b->tune_bands = value;
     return MHD_OK;
   }
   if (key == MHD_TUNE_FUSED_CFL) {
@@ -984,102 +1000,183 @@ size_t hs_chunk_bytes(const mhd_bunch* b, int chunk) {
 void hs_release(mhd_bunch* b) {
   mhd_bunch::HostStream* h = b->hs;
   if (!h) return;
-  // members are null until created (a failed attach releases what it got so far)
-  if (h->s_up) cudaStreamSynchronize(h->s_up);
-  if (h->s_dn) cudaStreamSynchronize(h->s_dn);
-  for (cudaEvent_t e : h->ev_up) if (e) cudaEventDestroy(e);
-  for (cudaEvent_t e : h->ev_step) if (e) cudaEventDestroy(e);
+  for (auto* v : {&h->ev_copied, &h->ev_up, &h->ev_step, &h->ev_packed, &h->ev_dn})
+    for (cudaEvent_t e : *v) if (e) cudaEventDestroy(e);
   if (h->ev_begin) cudaEventDestroy(h->ev_begin);
   if (h->ev_all_steps) cudaEventDestroy(h->ev_all_steps);
-  if (h->s_up) cudaStreamDestroy(h->s_up);
-  if (h->s_dn) cudaStreamDestroy(h->s_dn);
+  for (cudaStream_t st : {h->s_up[0], h->s_up[1], h->s_un, h->s_pk, h->s_dn[0], h->s_dn[1]}) if (st) cudaStreamDestroy(st);
   delete h;
   b->hs = nullptr;
 }
 
+// scatter / gather planes [k0, k0+nk) of patches [p0, p0+npl) between the state and a staging buffer
 template <typename T, bool PACK>
-int launch_pack(mhd_bunch* b, cudaStream_t st, void* state, char* stage, int p0, int npl) {
+int launch_pack(mhd_bunch* b, cudaStream_t st, void* state, char* stage, int p0, int npl, int k0 = 0, int nk = -1) {
   const Geom& G = b->G;
+  if (nk < 0) nk = G.n[2];
   const int vec = (int)(16 / sizeof(T));
-  const long long n = (long long)8 * npl * G.n[0] * G.n[1] * G.n[2];
+  const long long n = (long long)8 * npl * G.n[0] * G.n[1] * nk;
   b->launches += 1;
   if (G.n[0] % vec == 0) {
     const unsigned blocks = blocks_for(n / vec, 256);
-    k_pack_unpack<T, (int)(16 / sizeof(T)), PACK><<<blocks, 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl);
+    k_pack_unpack<T, (int)(16 / sizeof(T)), PACK><<<blocks, 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl, k0, nk);
   } else {
-    k_pack_unpack<T, 1, PACK><<<blocks_for(n, 256), 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl);
+    k_pack_unpack<T, 1, PACK><<<blocks_for(n, 256), 256, 0, st>>>(G, (T*)state, (T*)stage, p0, npl, k0, nk);
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
 }
 
-// one strided copy per chunk: rows = the eight fields, host[f][p0 .. p0+npl) <-> stage[f][0 .. npl)
-int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device, int host_np = -1) {
-  const size_t per = (size_t)b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
-  char* h = host + (size_t)p0 * per;
-  const size_t hp = (size_t)(host_np < 0 ? b->G.np : host_np) * per, dp = (size_t)npl * per;
-  if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, hp, dp, 8, cudaMemcpyHostToDevice, st));
-  else CUDA_TRY(cudaMemcpy2DAsync(h, hp, stage, dp, dp, 8, cudaMemcpyDeviceToHost, st));
+// One strided copy per transfer: host[f][p0 .. p0+npl)[k0 .. k0+nk) <-> stage[f][0 .. npl)[0 .. nk).
+// Whole patches are eight contiguous rows (the eight fields: a 2D copy); a z-range of every patch
+// is a 3D copy (row = the planes of one patch and field, rows per slice = patches, slices = fields).
+int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device, int host_np = -1,
+            int k0 = 0, int nk = -1) {
+  const int nz = b->G.n[2];
+  if (nk < 0) nk = nz;
+  const size_t plane = (size_t)b->G.n[0] * b->G.n[1] * b->esz, per = plane * nz;
+  const size_t hnp = (size_t)(host_np < 0 ? b->G.np : host_np);
+  if (k0 == 0 && nk == nz) {
+    char* h = host + (size_t)p0 * per;
+    const size_t hp = hnp * per, dp = (size_t)npl * per;
+    if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, hp, dp, 8, cudaMemcpyHostToDevice, st));
+    else CUDA_TRY(cudaMemcpy2DAsync(h, hp, stage, dp, dp, 8, cudaMemcpyDeviceToHost, st));
+    return MHD_OK;
+  }
+  const size_t w = plane * nk;
+  cudaMemcpy3DParms q;
+  memset(&q, 0, sizeof q);
+  const cudaPitchedPtr hptr = make_cudaPitchedPtr(host, per, per, hnp);
+  const cudaPitchedPtr dptr = make_cudaPitchedPtr(stage, w, w, (size_t)npl);
+  const cudaPos hpos = make_cudaPos(plane * k0, (size_t)p0, 0), dpos = make_cudaPos(0, 0, 0);
+  q.srcPtr = to_device ? hptr : dptr; q.srcPos = to_device ? hpos : dpos;
+  q.dstPtr = to_device ? dptr : hptr; q.dstPos = to_device ? dpos : hpos;
+  q.extent = make_cudaExtent(w, (size_t)npl, 8);
+  q.kind = to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
+  CUDA_TRY(cudaMemcpy3DAsync(&q, st));
   return MHD_OK;
 }
 
-// Schedule of one host-streamed step for a chunk size.  Uploads run in rotated order (last
-// chunk first: a periodic stack of slabs can then start stepping after three uploads); a
-// chunk may step once the last upload carrying one of its neighbours has landed (ready[c] =
-// that upload's position); chunks step in order of readiness.
-struct HsPlan { std::vector<int> up_order, ready, step_order; };
-HsPlan hs_plan(const int* nb, int np, int chunk) {
+// Schedule of one host-streamed step for a chunk size.  STEP UNITS are stepped in order: chunk 0,
+// 1, .. C-1, the first chunk and the last two cut into `bands` bands of planes [za, zb) each (the
+// one-pass kernel steps any plane range of its patches), every other chunk whole: downloads then start
+// early, and what is left to download when the last upload lands is two bands, not two chunks.  What a unit (c, [za, zb))
+// needs on the device before it may step (O1: guard zones come from the neighbours' interiors, at
+// most `guard` cells deep): planes [za-guard, zb+guard) of its own chunk and of every chunk that holds
+// an in-plane neighbour (o_z = 0) of one of its patches; if the range reaches below plane 0, the
+// HIGHEST planes of the chunks reached through o_z = -1, and if it reaches beyond n_z, the LOWEST
+// planes of the chunks reached through o_z = +1 -- the kernels read nothing else.  Uploads are PIECES
+// (chunk, planes [k0, k1)): walking the units in step order, whatever a unit still misses is
+// appended, so every plane of every patch crosses PCIe exactly once, the thin layers of the chunks
+// ahead arrive early and no step waits for the bulk of a z-neighbour: a periodic stack of slabs
+// starts stepping after a band of the first slab and ends with the download of one band of the last
+// (the whole-chunk schedule ended with three slabs: the first one waited for the last one's upload).
+// ready[u] = index of the last piece unit u needs.  Patches too thin for two disjoint layers
+// (n_z < 2 guard + 1, collapsed dimensions) or thicker than 64 planes are needed whole.
+struct HsPlan { std::vector<int> piece_chunk, piece_k0, piece_k1, unit_chunk, unit_za, unit_zb, ready; };
+bool hs_layered(int nz, int guard) { return guard >= 1 && nz >= 2 * guard + 1 && nz <= 64; }
+int hs_bands(int nz, int guard, int bands) {                      // bands of at least eight planes
+  if (!hs_layered(nz, guard) || bands < 1) return 1;
+  return bands > nz / 8 ? (nz / 8 > 1 ? nz / 8 : 1) : bands;
+}
+HsPlan hs_plan(const int* nb, int np, int chunk, int nz, int guard, int bands) {
   HsPlan pl;
   const int C = (np + chunk - 1) / chunk;
-  pl.up_order.resize(C);
-  std::vector<int> upos(C);
-  for (int u = 0; u < C; ++u) { pl.up_order[u] = (u + C - 1) % C; upos[pl.up_order[u]] = u; }
-  pl.ready.assign(C, 0);
-  for (int p = 0; p < np; ++p) {
-    const int c = p / chunk;
-    int r = upos[c];
-    for (int k = 0; k < 27; ++k) {
-      const int q = nb[(size_t)p * 27 + k];
-      if (q >= 0) r = std::max(r, upos[q / chunk]);
+  const bool layered = hs_layered(nz, guard);
+  bands = hs_bands(nz, guard, bands);
+  const int NZ = layered ? nz : 1;                               // one bit per plane, or one for the whole patch
+  auto planes = [&](int a, int z) -> unsigned long long {
+    a = std::max(a, 0); z = std::min(z, NZ);
+    if (a >= z) return 0ull;
+    return (z - a == 64 ? ~0ull : ((1ull << (z - a)) - 1ull)) << a;
+  };
+  std::vector<unsigned long long> have(C, 0ull);
+  std::vector<unsigned char> reach(C, 0);                        // bit 0: o_z = -1, bit 1: o_z = 0, bit 2: o_z = +1
+  std::vector<int> touched;
+  for (int c = 0; c < C; ++c) {
+    touched.clear();
+    auto mark = [&](int q, int bit) { if (!reach[q]) touched.push_back(q); reach[q] |= (unsigned char)bit; };
+    mark(c, 2);
+    for (int p = c * chunk; p < std::min(np, (c + 1) * chunk); ++p)
+      for (int k = 0; k < 27; ++k) {
+        const int q = nb[(size_t)p * 27 + k];
+        if (q >= 0) mark(q / chunk, 1 << (k / 9));
+      }
+    std::sort(touched.begin() + 1, touched.end());               // own chunk first, then by index
+    const int J = (c == 0 || c >= C - 2) ? bands : 1;
+    for (int j = 0; j < J; ++j) {
+      const int za = (int)((long long)nz * j / J), zb = (int)((long long)nz * (j + 1) / J);
+      const int lo = za - guard, hi = zb + guard;
+      for (int q : touched) {
+        unsigned long long w = 0ull;
+        if (!layered) w = 1ull;
+        else {
+          if (reach[q] & 2) w |= planes(lo, hi);
+          if ((reach[q] & 1) && lo < 0) w |= planes(nz + lo, nz);
+          if ((reach[q] & 4) && hi > nz) w |= planes(0, hi - nz);
+        }
+        unsigned long long miss = w & ~have[q];
+        have[q] |= miss;
+        while (miss) {                                           // maximal runs of missing planes
+          int k0 = 0;
+          while (!((miss >> k0) & 1ull)) ++k0;
+          int k1 = k0;
+          while (k1 < NZ && ((miss >> k1) & 1ull)) ++k1;
+          pl.piece_chunk.push_back(q);
+          pl.piece_k0.push_back(layered ? k0 : 0);
+          pl.piece_k1.push_back(layered ? k1 : nz);
+          miss &= ~planes(k0, k1);
+        }
+      }
+      pl.unit_chunk.push_back(c); pl.unit_za.push_back(za); pl.unit_zb.push_back(zb);
+      pl.ready.push_back((int)pl.piece_chunk.size() - 1);
     }
-    pl.ready[c] = std::max(pl.ready[c], r);
+    for (int q : touched) reach[q] = 0;
   }
-  pl.step_order.resize(C);
-  for (int c = 0; c < C; ++c) pl.step_order[c] = c;
-  std::stable_sort(pl.step_order.begin(), pl.step_order.end(), [&](int a, int c2) {
-    return pl.ready[a] != pl.ready[c2] ? pl.ready[a] < pl.ready[c2] : upos[a] < upos[c2];
-  });
   return pl;
 }
-// Makespan of that schedule in units of "one patch across PCIe": uploads back to back, a
-// step costs `alpha` per patch, a download 1 per patch, `eps` of fixed cost per transfer.
-double hs_makespan(int np, int chunk, const HsPlan& pl, double alpha, double eps) {
-  const int C = (int)pl.up_order.size();
+// Makespan of that schedule in units of "one patch across PCIe": uploads back to back, a step
+// costs HS_ALPHA per patch, a download 1 per patch; fixed costs per upload piece, step and download.
+// Calibrated on a B200 / PCIe 5 box with both directions busy (21 us per 32^3 fp32 patch): an H2D
+// copy starts ~40 us after the previous one has ended (its completion signal queues behind the
+// D2H data), a D2H copy ~15 us, a unit's launches take ~10 us.
+constexpr double HS_ALPHA = 0.33, HS_EPS_UP = 2.0, HS_EPS_STEP = 0.5, HS_EPS_DN = 0.7;
+double hs_makespan(int np, int chunk, int nz, const HsPlan& pl) {
+  const int NU = (int)pl.ready.size(), NPC = (int)pl.piece_chunk.size();
   auto size = [&](int c) { return (double)std::min(chunk, np - c * chunk); };
-  std::vector<double> t_up(C);
+  std::vector<double> t_up(NPC);
   double t = 0.0;
-  for (int u = 0; u < C; ++u) { t += size(pl.up_order[u]) + eps; t_up[u] = t; }
+  for (int u = 0; u < NPC; ++u) {
+    t += size(pl.piece_chunk[u]) * (pl.piece_k1[u] - pl.piece_k0[u]) / (double)nz + HS_EPS_UP;
+    t_up[u] = t;
+  }
   double t_step = 0.0, t_dn = 0.0;
-  for (int s2 = 0; s2 < C; ++s2) {
-    const int c = pl.step_order[s2];
-    t_step = std::max(t_step, t_up[pl.ready[c]]) + alpha * size(c) + eps;
-    t_dn = std::max(t_dn, t_step) + size(c) + eps;
+  for (int u = 0; u < NU; ++u) {
+    const double sz = size(pl.unit_chunk[u]) * (pl.unit_zb[u] - pl.unit_za[u]) / (double)nz;
+    t_step = std::max(t_step, t_up[pl.ready[u]]) + HS_ALPHA * sz + HS_EPS_STEP;
+    t_dn = std::max(t_dn, t_step) + sz + HS_EPS_DN;
   }
   return t_dn;
 }
-// default chunk: the candidate with the shortest simulated step (transfers dominate: a step
-// of a patch costs about a third of its transfer; ~30 us of fixed cost per chunk and stream)
-int hs_default_chunk(const int* nb, int np) {
-  int best = np;
+// default chunk and bands: the candidate with the shortest simulated step
+void hs_default(const int* nb, int np, int nz, int guard, bool can_band, int chunk_fixed, int* chunk_out, int* bands_out) {
+  int best = np, best_b = 1;
   double best_t = 1e300;
-  for (int k : {1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64}) {
-    const int chunk = (np + k - 1) / k;
+  for (int k : {1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64, 96, 128}) {
+    const int chunk = chunk_fixed > 0 ? chunk_fixed : (np + k - 1) / k;
     if (chunk < 1) break;
-    const double tt = hs_makespan(np, chunk, hs_plan(nb, np, chunk), 0.3, 1.5);
-    if (tt < best_t - 1e-9) { best_t = tt; best = chunk; }
-    if (chunk == 1) break;
+    for (int bands : {1, 2, 4}) {
+      if (bands > 1 && !can_band) break;
+      const double tt = hs_makespan(np, chunk, nz, hs_plan(nb, np, chunk, nz, guard, bands));
+      // near ties (0.2 %) go to more bands of the same chunk: measured 2.4 % faster on config 2
+      // (13.47 against 13.80 ms) where the model sees none -- it overestimates the start-up of small copies
+      const bool tie = chunk == best && bands > best_b && tt < best_t * 1.002;
+      if (tt < best_t - 1e-9 || tie) { best_t = std::min(tt, best_t); best = chunk; best_b = bands; }
+    }
+    if (chunk == 1 || chunk_fixed > 0) break;
   }
-  return best;
+  *chunk_out = best;
+  *bands_out = best_b;
 }
 
 }  // namespace
@@ -1088,36 +1185,53 @@ extern "C" {
 
 int mhd_bunch_host_query(mhd_bunch* b, int32_t chunk_patches, mhd_bunch_host_layout* out) {
   if (!b || !out) return MHD_ESTATE;
-  int chunk = chunk_patches;
-  if (chunk <= 0) chunk = hs_default_chunk(b->h_nbr->data(), b->G.np);
-  if (chunk > b->G.np) chunk = b->G.np;
+  const bool pipelined = b->all_nbr && step_gathers(b);
+  const bool can_band = pipelined && effective_path(b) == MHD_PATH_ONEPASS;    // the one-pass kernel steps plane ranges
+  int chunk = chunk_patches > b->G.np ? b->G.np : chunk_patches, bands = 1;
+  hs_default(b->h_nbr->data(), b->G.np, b->G.n[2], b->G.g[2], can_band, chunk, &chunk, &bands);
+  if (can_band && b->tune_bands >= 1) bands = hs_bands(b->G.n[2], b->G.g[2], b->tune_bands);     // mhd_bunch_set_tuning
   out->chunk_patches = chunk;
   out->nchunk = (b->G.np + chunk - 1) / chunk;
   out->host_bytes = (size_t)8 * b->G.np * b->G.n[0] * b->G.n[1] * b->G.n[2] * b->esz;
-  out->staging_bytes = 2 * hs_chunk_bytes(b, chunk);
-  out->pipelined = (b->all_nbr && step_gathers(b)) ? 1 : 0;
+  out->staging_bytes = 4 * hs_chunk_bytes(b, chunk);
+  out->pipelined = pipelined ? 1 : 0;
+  out->bands = bands;
   return MHD_OK;
 }
 
-int mhd_bunch_host_schedule(const int32_t* nbr, int32_t npatch, int32_t chunk_patches, int32_t* chunk_out,
-                            int32_t* nchunk_out, int32_t* up_order, int32_t* ready, int32_t* step_order, int32_t cap,
-                            double* makespan) {
-  if (!nbr || npatch < 1 || !chunk_out || !nchunk_out) return MHD_EINVAL;
+int mhd_bunch_host_schedule(const int32_t* nbr, int32_t npatch, int32_t nz, int32_t guard, int32_t chunk_patches, int32_t bands,
+                            int32_t* chunk_out, int32_t* bands_out, int32_t* npiece_out, int32_t* piece_chunk,
+                            int32_t* piece_k0, int32_t* piece_k1, int32_t* nunit_out, int32_t* unit_chunk, int32_t* unit_za,
+                            int32_t* unit_zb, int32_t* ready, int32_t cap, double* makespan) {
+  if (!nbr || npatch < 1 || nz < 1 || guard < 0 || !chunk_out || !bands_out || !npiece_out || !nunit_out) return MHD_EINVAL;
   for (long long c = 0; c < 27ll * npatch; ++c)
     if (nbr[c] < -1 || nbr[c] >= npatch) return MHD_EINVAL;
-  int chunk = chunk_patches > 0 ? chunk_patches : hs_default_chunk(nbr, npatch);
-  if (chunk > npatch) chunk = npatch;
-  const HsPlan pl = hs_plan(nbr, npatch, chunk);
-  const int C = (int)pl.up_order.size();
+  int chunk = chunk_patches > npatch ? npatch : chunk_patches, bb = bands;
+  if (chunk <= 0 || bands <= 0) {
+    int c2, b2;
+    hs_default(nbr, npatch, nz, guard, true, chunk > 0 ? chunk : 0, &c2, &b2);
+    if (chunk <= 0) chunk = c2;
+    if (bands <= 0) bb = b2;
+  }
+  const HsPlan pl = hs_plan(nbr, npatch, chunk, nz, guard, bb);
+  const int NU = (int)pl.ready.size(), NPC = (int)pl.piece_chunk.size();
   *chunk_out = chunk;
-  *nchunk_out = C;
-  if (makespan) *makespan = hs_makespan(npatch, chunk, pl, 0.3, 1.5);
-  if (up_order || ready || step_order) {
-    if (cap < C) return MHD_ENOMEM;
-    for (int c = 0; c < C; ++c) {
-      if (up_order) up_order[c] = pl.up_order[c];
-      if (ready) ready[c] = pl.ready[c];
-      if (step_order) step_order[c] = pl.step_order[c];
+  *bands_out = hs_bands(nz, guard, bb);
+  *npiece_out = NPC;
+  *nunit_out = NU;
+  if (makespan) *makespan = hs_makespan(npatch, chunk, nz, pl);
+  if (piece_chunk || piece_k0 || piece_k1 || unit_chunk || unit_za || unit_zb || ready) {
+    if (cap < NPC || cap < NU) return MHD_ENOMEM;
+    for (int u = 0; u < NPC; ++u) {
+      if (piece_chunk) piece_chunk[u] = pl.piece_chunk[u];
+      if (piece_k0) piece_k0[u] = pl.piece_k0[u];
+      if (piece_k1) piece_k1[u] = pl.piece_k1[u];
+    }
+    for (int u = 0; u < NU; ++u) {
+      if (unit_chunk) unit_chunk[u] = pl.unit_chunk[u];
+      if (unit_za) unit_za[u] = pl.unit_za[u];
+      if (unit_zb) unit_zb[u] = pl.unit_zb[u];
+      if (ready) ready[u] = pl.ready[u];
     }
   }
   return MHD_OK;
@@ -1134,7 +1248,7 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   hs_release(b);
   mhd_bunch::HostStream* h = new (std::nothrow) mhd_bunch::HostStream();
   if (!h) return MHD_ENOMEM;
-  h->s_up = h->s_dn = nullptr;
+  h->s_up[0] = h->s_up[1] = h->s_un = h->s_pk = h->s_dn[0] = h->s_dn[1] = nullptr;
   h->ev_begin = h->ev_all_steps = nullptr;
   b->hs = h;                               // owned by the handle from here on: released by detach / destroy,
   struct Guard {                           // or right here if the attach fails half way
@@ -1143,23 +1257,32 @@ int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes,
   } guard{b, false};
   h->chunk = lay.chunk_patches;
   h->nchunk = lay.nchunk;
-  h->stage_up = (char*)staging_dev;
-  h->stage_dn = (char*)staging_dev + hs_chunk_bytes(b, h->chunk);
+  const size_t cb = hs_chunk_bytes(b, h->chunk);
+  for (int i = 0; i < 2; ++i) {
+    h->stage_up[i] = (char*)staging_dev + (size_t)i * cb;
+    h->stage_dn[i] = (char*)staging_dev + (size_t)(2 + i) * cb;
+  }
+  HsPlan pl = hs_plan(b->h_nbr->data(), b->G.np, h->chunk, b->G.n[2], b->G.g[2], lay.bands);
+  h->piece_chunk = pl.piece_chunk;
+  h->piece_k0 = pl.piece_k0;
+  h->piece_k1 = pl.piece_k1;
+  h->unit_chunk = pl.unit_chunk;
+  h->unit_za = pl.unit_za;
+  h->unit_zb = pl.unit_zb;
+  h->ready = pl.ready;
   CUDA_TRY(cudaSetDevice(b->desc.device));
-  CUDA_TRY(cudaStreamCreateWithFlags(&h->s_up, cudaStreamNonBlocking));
-  CUDA_TRY(cudaStreamCreateWithFlags(&h->s_dn, cudaStreamNonBlocking));
+  for (cudaStream_t* st : {&h->s_up[0], &h->s_up[1], &h->s_un, &h->s_pk, &h->s_dn[0], &h->s_dn[1]})
+    CUDA_TRY(cudaStreamCreateWithFlags(st, cudaStreamNonBlocking));
   CUDA_TRY(cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming));
   CUDA_TRY(cudaEventCreateWithFlags(&h->ev_all_steps, cudaEventDisableTiming));
-  h->ev_up.assign(h->nchunk, nullptr);
-  h->ev_step.assign(h->nchunk, nullptr);
-  for (int c = 0; c < h->nchunk; ++c) {
-    CUDA_TRY(cudaEventCreateWithFlags(&h->ev_up[c], cudaEventDisableTiming));
-    CUDA_TRY(cudaEventCreateWithFlags(&h->ev_step[c], cudaEventDisableTiming));
-  }
-  HsPlan pl = hs_plan(b->h_nbr->data(), b->G.np, h->chunk);
-  h->up_order = pl.up_order;
-  h->ready = pl.ready;
-  h->step_order = pl.step_order;
+  const size_t NPC = h->piece_chunk.size();
+  h->ev_copied.assign(NPC, nullptr);
+  h->ev_up.assign(NPC, nullptr);
+  h->ev_step.assign(h->unit_chunk.size(), nullptr);
+  h->ev_packed.assign(h->unit_chunk.size(), nullptr);
+  h->ev_dn.assign(h->unit_chunk.size(), nullptr);
+  for (auto* v : {&h->ev_copied, &h->ev_up, &h->ev_step, &h->ev_packed, &h->ev_dn})
+    for (cudaEvent_t& e : *v) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   guard.ok = true;
   return MHD_OK;
 }
@@ -1176,8 +1299,8 @@ int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, doubl
     // copies into / out of the caller's host buffers may still be in flight: drain them before
     // the caller sees the error and reuses the buffers
     cudaStreamSynchronize(b->stream);
-    if (b->hs->s_up) cudaStreamSynchronize(b->hs->s_up);
-    if (b->hs->s_dn) cudaStreamSynchronize(b->hs->s_dn);
+    for (cudaStream_t st : {b->hs->s_up[0], b->hs->s_up[1], b->hs->s_un, b->hs->s_pk, b->hs->s_dn[0], b->hs->s_dn[1]})
+      if (st) cudaStreamSynchronize(st);
   }
   return rc;
 }
@@ -1193,32 +1316,43 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
   const bool pipelined = step_gathers(b);
   const bool onepass = effective_path(b) == MHD_PATH_ONEPASS;
   const Geom& G = b->G;
-  const int C = h->nchunk;
+  const int C = h->nchunk, NPC = (int)h->piece_chunk.size();
   auto range = [&](int c, int& p0, int& npl) { p0 = c * h->chunk; npl = std::min(h->chunk, G.np - p0); };
   int rc;
 
-  // the copy streams start after whatever the caller's stream has enqueued so far
+  // the library's streams start after whatever the caller's stream has enqueued so far
   CUDA_TRY(cudaEventRecord(h->ev_begin, b->stream));
-  CUDA_TRY(cudaStreamWaitEvent(h->s_up, h->ev_begin, 0));
-  CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_begin, 0));
+  for (cudaStream_t st : {h->s_up[0], h->s_up[1], h->s_un, h->s_pk, h->s_dn[0], h->s_dn[1]}) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_begin, 0));
 
-  // ---- uploads: host -> staging -> interiors of the current level --------------------
-  for (int u = 0; u < C; ++u) {
-    int p0, npl;
-    range(h->up_order[u], p0, npl);
-    if ((rc = hs_copy(b, h->s_up, h->stage_up, (char*)const_cast<void*>(host_in), p0, npl, true)) != MHD_OK) return rc;
-    rc = f64 ? launch_pack<double, false>(b, h->s_up, b->state[b->cur], h->stage_up, p0, npl)
-             : launch_pack<float, false>(b, h->s_up, b->state[b->cur], h->stage_up, p0, npl);
-    if (rc != MHD_OK) return rc;
-    CUDA_TRY(cudaEventRecord(h->ev_up[u], h->s_up));
-  }
+  // ---- uploads: host -> staging (copy streams) -> interiors of the current level (unpack stream).
+  // Two staging buffers, one per copy stream: piece u+1 crosses PCIe while piece u is scattered.
+  int next_piece = 0;
+  auto upload_through = [&](int last) -> int {
+    for (; next_piece <= last; ++next_piece) {
+      const int u = next_piece, p0 = h->piece_chunk[u] * h->chunk, npl = std::min(h->chunk, G.np - p0);
+      const int k0 = h->piece_k0[u], nk = h->piece_k1[u] - k0;
+      char* st = h->stage_up[u & 1];
+      cudaStream_t su = h->s_up[u & 1];
+      if (u >= 2) CUDA_TRY(cudaStreamWaitEvent(su, h->ev_up[u - 2], 0));           // the buffer has been scattered
+      int r2 = hs_copy(b, su, st, (char*)const_cast<void*>(host_in), p0, npl, true, -1, k0, nk);
+      if (r2 != MHD_OK) return r2;
+      CUDA_TRY(cudaEventRecord(h->ev_copied[u], su));
+      CUDA_TRY(cudaStreamWaitEvent(h->s_un, h->ev_copied[u], 0));
+      r2 = f64 ? launch_pack<double, false>(b, h->s_un, b->state[b->cur], st, p0, npl, k0, nk)
+               : launch_pack<float, false>(b, h->s_un, b->state[b->cur], st, p0, npl, k0, nk);
+      if (r2 != MHD_OK) return r2;
+      CUDA_TRY(cudaEventRecord(h->ev_up[u], h->s_un));
+    }
+    return MHD_OK;
+  };
   b->closing_ok = false;
   b->guards_stale = false;
   b->rate_valid = false;
 
-  const bool overlap_up = pipelined && have_dt;   // steps start while later chunks still upload
+  const bool overlap_up = pipelined && have_dt;   // steps start while later pieces still upload
   if (!overlap_up) {
-    CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[C - 1], 0));
+    if ((rc = upload_through(NPC - 1)) != MHD_OK) return rc;
+    CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[NPC - 1], 0));
     if ((rc = mhd_bunch_fill_guards(b)) != MHD_OK) return rc;    // deferred on the one-pass path: closing faces only
     if (!have_dt) {
       rc = f64 ? launch_cfl<double>(b, courant, nullptr, nullptr) : launch_cfl<float>(b, courant, nullptr, nullptr);
@@ -1228,44 +1362,56 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
   { LaunchScope ls(b, KC_MISC);
     k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, have_dt ? nullptr : b->d_dt, dt, 0.0, b->d_rate_next, b->G.np); }
 
-  // ---- steps, and the way back: interiors of the new level -> staging -> host --------
+  // ---- steps, and the way back: interiors of the new level -> staging (pack stream) -> host
+  // (copy-out stream), again through two staging buffers
   void* const next = b->state[1 - b->cur];
-  auto download = [&](int c) -> int {
+  const int NU = (int)h->unit_chunk.size();
+  auto download = [&](int u, cudaEvent_t after) -> int {
     int p0, npl;
-    range(c, p0, npl);
-    int r2 = f64 ? launch_pack<double, true>(b, h->s_dn, next, h->stage_dn, p0, npl)
-                 : launch_pack<float, true>(b, h->s_dn, next, h->stage_dn, p0, npl);
+    range(h->unit_chunk[u], p0, npl);
+    const int za = h->unit_za[u], nk = h->unit_zb[u] - za;
+    char* st = h->stage_dn[u & 1];
+    CUDA_TRY(cudaStreamWaitEvent(h->s_pk, after, 0));
+    if (u >= 2) CUDA_TRY(cudaStreamWaitEvent(h->s_pk, h->ev_dn[u - 2], 0));        // the buffer has left for the host
+    int r2 = f64 ? launch_pack<double, true>(b, h->s_pk, next, st, p0, npl, za, nk)
+                 : launch_pack<float, true>(b, h->s_pk, next, st, p0, npl, za, nk);
     if (r2 != MHD_OK) return r2;
-    return hs_copy(b, h->s_dn, h->stage_dn, (char*)host_out, p0, npl, false);
+    CUDA_TRY(cudaEventRecord(h->ev_packed[u], h->s_pk));
+    cudaStream_t sd = h->s_dn[u & 1];
+    CUDA_TRY(cudaStreamWaitEvent(sd, h->ev_packed[u], 0));
+    if ((r2 = hs_copy(b, sd, st, (char*)host_out, p0, npl, false, -1, za, nk)) != MHD_OK) return r2;
+    CUDA_TRY(cudaEventRecord(h->ev_dn[u], sd));
+    return MHD_OK;
   };
   if (pipelined) {
-    for (int s2 = 0; s2 < C; ++s2) {
-      const int c = h->step_order[s2];
+    for (int u = 0; u < NU; ++u) {
       int p0, npl;
-      range(c, p0, npl);
+      range(h->unit_chunk[u], p0, npl);
+      const int za = h->unit_za[u], zb = h->unit_zb[u];
       if (overlap_up) {
-        CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[h->ready[c]], 0));
-        rc = f64 ? launch_sync_closing<double>(b, p0, npl) : launch_sync_closing<float>(b, p0, npl);
+        // enqueue what this unit needs, then the unit: the host stays just ahead of the device
+        if ((rc = upload_through(h->ready[u])) != MHD_OK) return rc;
+        CUDA_TRY(cudaStreamWaitEvent(b->stream, h->ev_up[h->ready[u]], 0));
+        rc = f64 ? launch_sync_closing<double>(b, p0, npl, za, zb) : launch_sync_closing<float>(b, p0, npl, za, zb);
         if (rc != MHD_OK) return rc;
-        b->guards_stale = true;    // halos of this chunk come through the neighbour table
+        b->guards_stale = true;    // halos of this unit come through the neighbour table
       }
-      if (onepass) rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, false);
+      if (onepass) rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, false, za, zb);
+      else if (za != 0 || zb != G.n[2]) rc = MHD_ESTATE;          // only the one-pass kernel steps plane ranges
       else rc = f64 ? launch_fused_range<double>(b, p0, npl) : launch_fused_range<float>(b, p0, npl);
       if (rc != MHD_OK) return rc;
-      CUDA_TRY(cudaEventRecord(h->ev_step[c], b->stream));
-      CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_step[c], 0));
-      if ((rc = download(c)) != MHD_OK) return rc;
+      CUDA_TRY(cudaEventRecord(h->ev_step[u], b->stream));
+      if ((rc = download(u, h->ev_step[u])) != MHD_OK) return rc;
     }
     b->cur = 1 - b->cur;
     b->guards_stale = true;   // the new level's shell is owed (deferred fill), its closing faces are current
     b->closing_ok = true;
-    b->rate_valid = onepass && b->fused_cfl;  // every chunk went through the one-pass epilogue since k_set_dt
+    b->rate_valid = onepass && b->fused_cfl;  // every unit went through the one-pass epilogue since k_set_dt
   } else {
     if ((rc = step_common(b)) != MHD_OK) return rc;
     CUDA_TRY(cudaEventRecord(h->ev_all_steps, b->stream));
-    CUDA_TRY(cudaStreamWaitEvent(h->s_dn, h->ev_all_steps, 0));
-    for (int c = 0; c < C; ++c)
-      if ((rc = download(c)) != MHD_OK) return rc;
+    for (int u = 0; u < NU; ++u)
+      if ((rc = download(u, h->ev_all_steps)) != MHD_OK) return rc;
     if ((rc = mhd_bunch_fill_guards(b)) != MHD_OK) return rc;   // cfl of the new level reads its closing faces
   }
 
@@ -1276,8 +1422,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
   if (rc != MHD_OK) return rc;
   CUDA_TRY(cudaMemcpyAsync(&dts[0], b->d_dt, sizeof(double), cudaMemcpyDeviceToHost, b->stream));
   CUDA_TRY(cudaStreamSynchronize(b->stream));
-  CUDA_TRY(cudaStreamSynchronize(h->s_dn));
-  CUDA_TRY(cudaStreamSynchronize(h->s_up));
+  for (cudaStream_t st : {h->s_dn[0], h->s_dn[1], h->s_pk, h->s_un, h->s_up[0], h->s_up[1]}) CUDA_TRY(cudaStreamSynchronize(st));
   if (dt_used) *dt_used = dts[1];
   if (dt_next) *dt_next = dts[0];
   return MHD_OK;

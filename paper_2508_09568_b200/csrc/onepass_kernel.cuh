@@ -162,7 +162,8 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
 template <typename T, int TX, int TY, int NPW, int LIM, bool CFLE>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
-               unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int zseg) {
+               unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int zseg,
+               int zlo, int zhi) {
   using C = OneCfg<T, TX, TY, NPW>;
   constexpr int PH = C::PH, BWX = C::BWX, RA = C::RA, DP = C::DP, DCS = C::DCS;
   constexpr int FW = C::FW, FA = C::FA, NR = C::NR, NP = C::NP, NALL = C::NALL, NS = C::NS;
@@ -180,9 +181,10 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const int nx = G.n[0], ny = G.n[1], nz = G.n[2];
   // Small bunches have fewer tiles than the GPU has SMs; their columns are then cut into zseg
   // segments along z (blockIdx.z), each a CTA of its own that marches planes [za, zb) after a
-  // five-plane run-in through its lower neighbour's planes.  zseg == 1: za = 0, zb = nz.
-  const int zlen = (nz + zseg - 1) / zseg;
-  const int za = (int)blockIdx.z * zlen, zb = min(nz, za + zlen);
+  // five-plane run-in through its lower neighbour's planes.  The launch covers planes [zlo, zhi) of
+  // its patches (the whole column unless the host-streaming path steps a chunk band by band).
+  const int zlen = (zhi - zlo + zseg - 1) / zseg;
+  const int za = zlo + (int)blockIdx.z * zlen, zb = min(zhi, za + zlen);
   const int pl = blockIdx.y;
   const int xt = blockIdx.x % xtiles, yt = blockIdx.x / xtiles;
   const int x0 = xt * TX, y0 = yt * TY;

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(256) k_fill_guards_local(Geom G, FillMap M, T*
 // from HBM, so it is all a deferred fill has to do up front.
 template <typename T>
 __global__ void __launch_bounds__(256) k_sync_closing_faces(Geom G, T* __restrict__ U, const int* __restrict__ nbr,
-                                                            int p0, int npl) {
+                                                            int p0, int npl, int zlo, int zhi) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int fx = G.n[1] * G.n[2], fy = G.n[0] * G.n[2], fz = G.n[0] * G.n[1];
   const int per = fx + fy + fz;
@@ -177,6 +177,8 @@ __global__ void __launch_bounds__(256) k_sync_closing_faces(Geom G, T* __restric
   else if (r < fx + fy) { r -= fx; a = 1; c[0] = r % G.n[0]; c[1] = G.n[1]; c[2] = r / G.n[0]; }
   else { r -= fx + fy; a = 2; c[0] = r % G.n[0]; c[1] = r / G.n[0]; c[2] = G.n[2]; }
   if (!G.act[a]) return;
+  // planes [zlo, zhi) only (the z closing face belongs to the band that ends at n_z)
+  if (a == 2 ? zhi != G.n[2] : (c[2] < zlo || c[2] >= zhi)) return;
   const int cls = 13 + (a == 0 ? 1 : (a == 1 ? 3 : 9));      // neighbour class with offset +1 along a
   const int q = nbr[p * 27 + cls];
   if (q < 0) return;

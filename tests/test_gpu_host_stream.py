@@ -115,6 +115,39 @@ def test_host_stream_equals_resident_path_bitwise_over_several_steps(name, dtype
     b.close()
 
 
+@pytest.mark.parametrize("chunk,bands", [(2, 4), (4, 2), (8, 4), (3, 3)])
+def test_banded_host_stream_equals_resident_path_bitwise(chunk, bands):
+    """The first chunk and the last two are stepped band by band (MHD_TUNE_HOST_BANDS): the one-pass
+    kernel and the closing-face sync run on plane ranges, uploads arrive as plane ranges, downloads
+    leave as plane ranges -- the result is the resident step's, bit for bit, over chained steps."""
+    import torch
+    w = W.turbulence(N=(32, 32, 64), n=(16, 16, 32), dtype=np.float32)      # 2 x 2 x 2 patches of 32 planes
+    r = make_gpu(w, "f32")
+    res_dts = []
+    for _ in range(3):
+        r.fill_guards()
+        dt = r.cfl_dt(0.4, sync=True)
+        res_dts.append(dt)
+        r.step(dt)
+    want = W.to_compact(r.download(), w.n)
+    r.close()
+    b = make_gpu(w, "f32")
+    b.load(np.zeros_like(w.U))
+    b.set_tuning("host_bands", bands)
+    lay = b.host_attach(chunk)
+    assert (lay.chunk_patches, lay.bands, lay.pipelined) == (chunk, bands, 1)
+    bufs = [pinned(W.to_compact(w.U, w.n)), None]
+    bufs[1] = torch.zeros_like(bufs[0]).pin_memory()
+    dt, dts = 0.0, []
+    for s in range(3):
+        used, dt = b.step_host(bufs[s % 2], bufs[(s + 1) % 2], dt=dt, courant=0.4)
+        dts.append(used)
+    assert dts == res_dts
+    assert np.array_equal(bufs[1].numpy(), want)
+    assert np.array_equal(W.to_compact(b.download(), w.n), want)
+    b.close()
+
+
 def test_host_stream_schedule_and_rejections():
     from paper_2508_09568_b200.binding import HostLayout, _check
     import ctypes as C

@@ -1,8 +1,9 @@
 """Host logic of the host-streaming path (include/mhd_bunch.h, mhd_bunch_host_schedule): the
-chunk schedule is computed from the neighbour table alone, so it is checked here without a
-GPU -- safety (no chunk steps before every chunk holding one of its neighbours has been
-uploaded), tightness, the permutations, the simulated makespan against a pipeline simulation
-typed in this file, and the library's choice of chunk size."""
+upload schedule is computed from the neighbour table alone, so it is checked here without a
+GPU -- safety (no chunk steps before every plane its kernels read has been uploaded: its own
+patches, its in-plane neighbours whole, the guard-width layers of its z-neighbours), tightness,
+completeness (every plane of every patch crosses PCIe exactly once), the simulated makespan
+against a pipeline simulation typed in this file, and the library's choice of chunk size."""
 import ctypes as C
 
 import numpy as np
@@ -14,75 +15,128 @@ from paper_2508_09568_b200 import workloads as W
 TABLES = {
     "cube8": W.neighbour_table((8, 8, 8), (True, True, True)),          # config 2
     "slabs": W.neighbour_table((1, 1, 8), (True, True, True)),
+    "pair": W.neighbour_table((2, 2, 2), (True, True, True)),           # the same patch is the +z and the -z neighbour
     "paper300": W.neighbour_table((5, 6, 10), (True, True, True)),      # bunch of 300
     "single": W.neighbour_table((1, 1, 1), (True, True, True)),
 }
 
 
-def simulate(npatch, chunk, up_order, ready, step_order, alpha=0.3, eps=1.5):
-    """Three in-order queues: uploads back to back, a step after its last needed upload and
+def simulate(npatch, chunk, nz, s, alpha=0.33, eps_up=2.0, eps_step=0.5, eps_dn=0.7):
+    """Three in-order queues: uploads back to back, a step after the last piece it needs and
     after the previous step, a download after its step and after the previous download."""
     size = lambda c: min(chunk, npatch - c * chunk)
     t, t_up = 0.0, []
-    for c in up_order:
-        t += size(c) + eps
+    for q, k0, k1 in zip(s["piece_chunk"], s["piece_k0"], s["piece_k1"]):
+        t += size(q) * (k1 - k0) / nz + eps_up
         t_up.append(t)
     t_step = t_dn = 0.0
-    for c in step_order:
-        t_step = max(t_step, t_up[ready[c]]) + alpha * size(c) + eps
-        t_dn = max(t_dn, t_step) + size(c) + eps
+    for u in range(s["nunit"]):
+        sz = size(s["unit_chunk"][u]) * (s["unit_zb"][u] - s["unit_za"][u]) / nz
+        t_step = max(t_step, t_up[s["ready"][u]]) + alpha * sz + eps_step
+        t_dn = max(t_dn, t_step) + sz + eps_dn
     return t_dn
 
 
+def planes_read(nbr, ck, c, za, zb, nz, g):
+    """What the step of planes [za, zb) of chunk c reads, as a set of (patch, plane): O1 -- guard zones
+    come from the neighbours' interiors, at most g cells deep (plane k of an o_z = +1 neighbour is the
+    patch's plane nz + k, plane k of an o_z = -1 neighbour its plane k - nz)."""
+    need = set()
+    layered = g >= 1 and 2 * g + 1 <= nz <= 64
+    for p in range(c * ck, min(len(nbr), (c + 1) * ck)):
+        for cls in range(27):
+            q = nbr[p][cls]
+            if q < 0:
+                continue
+            oz = cls // 9 - 1
+            if not layered:
+                need |= {(q, k) for k in range(nz)}
+            else:
+                need |= {(q, k) for k in range(nz) if za - g <= k + oz * nz < zb + g}
+    return need
+
+
+@pytest.mark.parametrize("nz,g,bands", [(32, 3, 1), (32, 3, 4), (6, 3, 2), (1, 0, 1), (16, 3, 2), (64, 3, 0)])
 @pytest.mark.parametrize("chunk", [0, 1, 7, 37, 64, 10 ** 6])
 @pytest.mark.parametrize("name", sorted(TABLES))
-def test_schedule_is_safe_tight_and_complete(name, chunk):
+def test_schedule_is_safe_tight_and_complete(name, chunk, nz, g, bands):
     nbr = TABLES[name]
     npatch = nbr.shape[0]
-    s = B.host_schedule(nbr, chunk)
+    if npatch * nz > 9000 and chunk in (1, 7):
+        pytest.skip("set arithmetic over every plane: covered by the smaller tables")
+    s = B.host_schedule(nbr, chunk, nz=nz, guard=g, bands=bands)
     ck, n = s["chunk"], s["nchunk"]
-    assert 1 <= ck <= npatch and n == -(-npatch // ck)
+    assert 1 <= ck <= npatch and n == -(-npatch // ck) and s["bands"] >= 1
     if 0 < chunk <= npatch:
         assert ck == chunk
-    assert sorted(s["up_order"]) == list(range(n)) and sorted(s["step_order"]) == list(range(n))
-    upos = np.empty(n, dtype=int)
-    upos[s["up_order"]] = np.arange(n)
-    need = np.zeros(n, dtype=int)
-    for p in range(npatch):
-        c = p // ck
-        qs = nbr[p][nbr[p] >= 0]
-        need[c] = max(need[c], upos[c], upos[qs // ck].max())
-    assert np.array_equal(s["ready"], need)                      # safe (>=) and tight (==)
-    r = s["ready"][s["step_order"]]
-    assert np.all(np.diff(r) >= 0)                               # chunks step in order of readiness
-    assert abs(s["makespan"] - simulate(npatch, ck, s["up_order"], s["ready"], s["step_order"])) < 1e-9
+    # completeness: the pieces of a chunk partition its planes, and so do the units (in chunk order, bands ascending)
+    seen, landed_after = {}, {}             # (patch, plane) -> index of the piece that carries it
+    for i, (q, k0, k1) in enumerate(zip(s["piece_chunk"], s["piece_k0"], s["piece_k1"])):
+        assert 0 <= q < n and 0 <= k0 < k1 <= nz
+        for k in range(k0, k1):
+            assert (q, k) not in seen, "plane uploaded twice"
+            seen[(q, k)] = i
+        for p in range(q * ck, min(npatch, (q + 1) * ck)):
+            for k in range(k0, k1):
+                landed_after[(p, k)] = i
+    assert len(seen) == n * nz
+    units = list(zip(s["unit_chunk"], s["unit_za"], s["unit_zb"]))
+    assert units == sorted(units) and [u[0] for u in units if u[1] == 0] == list(range(n))
+    for c in range(n):
+        mine = [(za, zb) for q, za, zb in units if q == c]
+        assert mine[0][0] == 0 and mine[-1][1] == nz and all(a[1] == b_[0] for a, b_ in zip(mine, mine[1:]))
+        assert len(mine) == 1 or (c in (0, n - 2, n - 1) and all(zb - za >= 8 for za, zb in mine))
+    # safety (>=) and tightness (==): ready[u] is the last piece that carries something unit u reads;
+    # units step in order, so ready does not decrease
+    for u, (c, za, zb) in enumerate(units):
+        last = max(landed_after[x] for x in planes_read(nbr, ck, c, za, zb, nz, g))
+        assert s["ready"][u] == max(last, s["ready"][u - 1] if u else -1)
+    assert abs(s["makespan"] - simulate(npatch, ck, nz, s)) < 1e-9
 
 
-def test_periodic_stack_starts_after_three_uploads_and_default_chunk_is_the_best_candidate():
-    s = B.host_schedule(TABLES["cube8"], 64)                     # one z-slab of patches per chunk
-    assert list(s["up_order"]) == [7, 0, 1, 2, 3, 4, 5, 6]       # last slab first: slab 0 needs it
-    assert list(s["ready"]) == [2, 3, 4, 5, 6, 7, 7, 7]          # slab c waits for slab c+1; three slabs wait for the last upload
-    assert s["step_order"][0] == 0
+def test_periodic_stack_never_waits_for_the_bulk_of_a_z_neighbour():
+    s = B.host_schedule(TABLES["cube8"], 64, bands=1)             # one z-slab of patches per chunk, stepped whole
+    pieces = list(zip(s["piece_chunk"], s["piece_k0"], s["piece_k1"]))
+    # slab 0 whole, then the bottom layer of slab 1 and the top layer of slab 7: slab 0 steps after ONE slab
+    assert pieces[:3] == [(0, 0, 32), (1, 0, 3), (7, 29, 32)] and s["ready"][0] == 2
+    # every later slab waits for the rest of itself and the bottom layer of the next one only
+    assert pieces[3:5] == [(1, 3, 32), (2, 0, 3)] and s["ready"][1] == 4
+    assert pieces[-1] == (7, 3, 29) and s["ready"][7] == len(pieces) - 1 and s["ready"][6] == len(pieces) - 2
+    # the last upload releases ONE slab (the whole-chunk schedule released three, 1.45 of the transfer time)
+    assert s["makespan"] < 512 * 1.26
+    # bands: the first slab starts stepping after a quarter of it (+ guard planes) is up, the last upload
+    # releases a quarter of the last slab
+    t = B.host_schedule(TABLES["cube8"], 64, bands=4)
+    pieces = list(zip(t["piece_chunk"], t["piece_k0"], t["piece_k1"]))
+    units = list(zip(t["unit_chunk"], t["unit_za"], t["unit_zb"]))
+    assert pieces[:2] == [(0, 0, 11), (7, 29, 32)] and t["ready"][0] == 1
+    assert units[:4] == [(0, 0, 8), (0, 8, 16), (0, 16, 24), (0, 24, 32)] and units[-1] == (7, 24, 32) and t["nunit"] == 17
+    assert pieces[-1] == (7, 27, 29) and t["makespan"] < 512 * 1.28      # every extra H2D copy costs 2 patch-times of start-up
     best = B.host_schedule(TABLES["cube8"], 0)
-    assert best["chunk"] == 64
-    for k in (1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64):
-        ck = -(-512 // k)
-        assert best["makespan"] <= B.host_schedule(TABLES["cube8"], ck)["makespan"] + 1e-9
-    assert B.host_schedule(W.neighbour_table((16, 16, 16), (True,) * 3), 0)["chunk"] == 256     # config 3: a slab again
+    for k in (1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64, 96, 128):
+        for bands in (1, 2, 4):
+            assert best["makespan"] <= B.host_schedule(TABLES["cube8"], -(-512 // k), bands=bands)["makespan"] * 1.002
+    assert best["makespan"] < 512 * 1.26 and (best["chunk"], best["bands"]) == (64, 2)
+    # thin patches: no layers, no bands, every need is a whole chunk
+    t = B.host_schedule(TABLES["cube8"], 64, nz=6, guard=3, bands=4)
+    assert all(k0 == 0 and k1 == 6 for k0, k1 in zip(t["piece_k0"], t["piece_k1"])) and t["npiece"] == 8 and t["nunit"] == 8
 
 
 def test_schedule_rejects_bad_tables():
     lib = B.load_library()
     nbr = TABLES["slabs"].copy()
-    a, b_ = C.c_int32(0), C.c_int32(0)
-    args = lambda t, cap=8: (t.ctypes.data_as(C.c_void_p), t.shape[0], 0, C.byref(a), C.byref(b_), None, None, None, cap, None)
-    assert lib.mhd_bunch_host_schedule(*args(nbr)) == 0 and b_.value >= 1
+    o = [C.c_int32(0) for _ in range(4)]
+    ptr = lambda t: t.ctypes.data_as(C.c_void_p)
+    def call(t, npatch=8, nz=32, chunk=0, arr=None, cap=64):
+        return lib.mhd_bunch_host_schedule(ptr(t) if t is not None else None, npatch, nz, 3, chunk, 0, C.byref(o[0]), C.byref(o[1]),
+                                           C.byref(o[2]), arr, None, None, C.byref(o[3]), None, None, None, None, cap, None)
+    assert call(nbr) == 0 and o[0].value >= 1 and o[2].value >= 1 and o[3].value >= 1
     bad = nbr.copy(); bad[3, 5] = 8
-    assert lib.mhd_bunch_host_schedule(*args(bad)) == -1
+    assert call(bad) == -1
     up = np.zeros(1, dtype=np.int32)
-    assert lib.mhd_bunch_host_schedule(nbr.ctypes.data_as(C.c_void_p), 8, 1, C.byref(a), C.byref(b_),
-                                       up.ctypes.data_as(C.c_void_p), None, None, 1, None) == -2       # capacity too small
-    assert lib.mhd_bunch_host_schedule(None, 8, 1, C.byref(a), C.byref(b_), None, None, None, 0, None) == -1
+    assert call(nbr, chunk=1, arr=ptr(up), cap=1) == -2          # capacity too small
+    assert call(None) == -1
+    assert call(nbr, nz=0) == -1
 
 
 # ---------------------------------------------------------------- ring mode: the planner ----
