@@ -289,9 +289,12 @@ int mhd_bunch_status(mhd_bunch *b, int64_t *bad_cells);
 /* Number of kernel launches issued so far through this handle (for bench.py).           */
 int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 
-/* The step has three CUDA implementations, all on the GPU:
+/* The step has four CUDA implementations, all on the GPU:
  *   MHD_PATH_ONEPASS     the whole step in one kernel, nothing intermediate in HBM (three
  *                        active dimensions, float32): the default where it applies;
+ *   MHD_PATH_TILE2D      the whole step of a two-dimensional bunch (n_z = 1, x and y active) in
+ *                        one kernel on shared-memory tiles, any type: the default there (the
+ *                        staged path's stage functions on a tile: same result to rounding);
  *   MHD_PATH_TWO_KERNEL  predictor kernel + Riemann/update kernel with one scratch block in
  *                        HBM (three active dimensions, any type);
  *   MHD_PATH_STAGED      one kernel per stage of PAPER.md section 2.1.4 (general: collapsed
@@ -302,6 +305,7 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 #define MHD_PATH_STAGED      1
 #define MHD_PATH_TWO_KERNEL  2
 #define MHD_PATH_ONEPASS     3
+#define MHD_PATH_TILE2D      4
 int mhd_bunch_set_path(mhd_bunch *b, int32_t path);
 int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
 

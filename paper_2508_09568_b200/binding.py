@@ -12,7 +12,7 @@ import numpy as np
 from . import build as _build
 
 MHD_F32, MHD_F64 = 0, 1
-PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3}
+PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3, "tile2d": 4}
 TUNE = {"onepass_zseg": 1, "predict_ty": 2, "fused_cfl": 3, "host_bands": 4}
 _ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
 

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 TARGET = os.path.join(HERE, "libmhd_bunch.so")
 SOURCES = [os.path.join(CSRC, "mhd_bunch.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mhd_math.cuh", "bunch_types.cuh", "stage_kernels.cuh", "fused_kernels.cuh", "onepass_kernel.cuh", "tma_utils.cuh", "host_stream_kernels.cuh")] + \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mhd_math.cuh", "bunch_types.cuh", "stage_kernels.cuh", "fused_kernels.cuh", "onepass_kernel.cuh", "tile_kernel.cuh", "tma_utils.cuh", "host_stream_kernels.cuh")] + \
     [os.path.join(os.path.dirname(HERE), "include", "mhd_bunch.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

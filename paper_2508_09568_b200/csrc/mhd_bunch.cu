@@ -12,6 +12,7 @@
 #include "stage_kernels.cuh"
 #include "fused_kernels.cuh"
 #include "onepass_kernel.cuh"
+#include "tile_kernel.cuh"
 #include "host_stream_kernels.cuh"
 
 #include <cuda_runtime.h>
@@ -74,6 +75,7 @@ struct mhd_bunch {
   int path;            // MHD_PATH_*: 0 = automatic choice
   int nsm;             // multiprocessors of the device
   bool onepass_ok;     // three active dimensions, fp32
+  bool tile2d_ok;      // x and y active, z collapsed: the whole step in one kernel on shared-memory tiles
   bool gather_ok;      // the one-pass kernel can read halos from the neighbours' interiors: every
                        // neighbour exists (no outflow side) and n_x is a whole number of 16-byte chunks
   bool gather2_ok;     // the two-kernel path can do the same (predictor loads through the neighbour table)
@@ -144,10 +146,10 @@ struct mhd_bunch {
 };
 
 enum KClass : int { KC_FILL = 0, KC_CFL, KC_PRIM, KC_EMF0, KC_PREDICT, KC_FLUX, KC_EMF, KC_UPDATE, KC_MISC, KC_RIEMANN, KC_ONEPASS,
-                    KC_CLOSING, KC_COUNT };
+                    KC_CLOSING, KC_TILE2D, KC_COUNT };
 static const char* const kclass_names[KC_COUNT] = {"fill_guards", "cfl", "prim", "emf0", "predict", "hlld_flux",
                                                    "emf_2d", "update", "misc", "riemann_update", "step_onepass",
-                                                   "sync_closing_faces"};
+                                                   "sync_closing_faces", "step_tile2d"};
 
 // brackets one launch with events when timing is on
 struct LaunchScope {
@@ -348,6 +350,7 @@ int launch_cfl(mhd_bunch* b, double courant, void* dt_dev, void* dt_patch) {
 // which implementation of the step runs: MHD_PATH_ONEPASS, MHD_PATH_TWO_KERNEL or MHD_PATH_STAGED
 int effective_path(const mhd_bunch* b) {
   if (b->path == MHD_PATH_STAGED) return MHD_PATH_STAGED;
+  if (b->tile2d_ok && (b->path == MHD_PATH_AUTO || b->path == MHD_PATH_TILE2D)) return MHD_PATH_TILE2D;
   if (b->path == MHD_PATH_TWO_KERNEL) return b->fused_ok ? MHD_PATH_TWO_KERNEL : MHD_PATH_STAGED;
   if (b->onepass_ok) return MHD_PATH_ONEPASS;           // automatic, or asked for
   return b->fused_ok ? MHD_PATH_TWO_KERNEL : MHD_PATH_STAGED;
@@ -420,6 +423,31 @@ template <> struct OnePassLaunch<float> {
     return MHD_OK;
   }
 };
+
+// 2D bunches: one kernel, every stage on a shared-memory tile (tile_kernel.cuh).  fp32 32 x 16 tiles,
+// fp64 32 x 8 (the tile with its halo and 50 arrays has to fit in 227 KB).
+template <typename T> struct Tile2D { static constexpr int TX = 32, TY = sizeof(T) == 4 ? 16 : 8; };
+template <typename T>
+int prepare_tile2d() {
+  using C = TileCfg<T, Tile2D<T>::TX, Tile2D<T>::TY>;
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
+  return MHD_OK;
+}
+template <typename T>
+int launch_tile2d(mhd_bunch* b, int p0, int npl) {
+  constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY;
+  using C = TileCfg<T, TX, TY>;
+  const Geom& G = b->G;
+  Params<T> P = make_params<T>(b, p0, npl);
+  const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
+  dim3 grid((unsigned)(xt * yt), (unsigned)npl, 1);
+  {
+    LaunchScope ls(b, KC_TILE2D);
+    k_step_tile2d<T, TX, TY><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_dt + 1, b->d_bad, xt);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
 
 // dynamic shared memory opt-in of the fused kernels: per device, so done once per handle in create
 template <typename T>
@@ -582,7 +610,7 @@ int launch_step(mhd_bunch* b) {
     return MHD_OK;
   }
   {
-    const int rc = launch_staged_range<T>(b, 0, G.np);
+    const int rc = path == MHD_PATH_TILE2D ? launch_tile2d<T>(b, 0, G.np) : launch_staged_range<T>(b, 0, G.np);
     if (rc != MHD_OK) return rc;
   }
   CUDA_TRY(cudaGetLastError());
@@ -727,6 +755,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
                                         b->DG.ps, b->DG.fs, bx, by, W_DCOUNT);
   }
   b->onepass_ok = all_active(b->G) && desc->dtype == MHD_F32;
+  b->tile2d_ok = b->G.act[0] && b->G.act[1] && !b->G.act[2];
   b->nsm = 148;
   cudaDeviceGetAttribute(&b->nsm, cudaDevAttrMultiProcessorCount, desc->device);
   b->gather_ok = b->onepass_ok && b->G.n[0] % (int)(16 / b->esz) == 0;
@@ -753,6 +782,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
     int ra = MHD_OK;
     if (b->fused_ok) ra = desc->dtype == MHD_F64 ? prepare_fused<double>() : prepare_fused<float>();
     if (ra == MHD_OK && b->onepass_ok) ra = OnePassLaunch<float>::prepare(b);
+    if (ra == MHD_OK && b->tile2d_ok) ra = desc->dtype == MHD_F64 ? prepare_tile2d<double>() : prepare_tile2d<float>();
     if (ra != MHD_OK) { delete b->h_nbr; delete b->events; delete b; return ra; }
   }
   *out = b;
@@ -844,8 +874,9 @@ int mhd_bunch_launch_count(mhd_bunch* b, int64_t* launches) {
 
 int mhd_bunch_set_path(mhd_bunch* b, int32_t path) {
   ENTER(b);
-  if (path < MHD_PATH_AUTO || path > MHD_PATH_ONEPASS) return MHD_EINVAL;
+  if (path < MHD_PATH_AUTO || path > MHD_PATH_TILE2D) return MHD_EINVAL;
   if (path == MHD_PATH_ONEPASS && !b->onepass_ok) return MHD_EINVAL;
+  if (path == MHD_PATH_TILE2D && !b->tile2d_ok) return MHD_EINVAL;
   if (path == MHD_PATH_TWO_KERNEL && !b->fused_ok) return MHD_EINVAL;
   const int rc = materialise_guards(b);   // the other paths read the guard shell from HBM
   if (rc != MHD_OK) return rc;
@@ -1706,6 +1737,7 @@ int launch_step_list(mhd_bunch* b, int off, int n, int side) {
   int rc;
   if (path == MHD_PATH_ONEPASS) rc = OnePassLaunch<T>::run(b, b->d_dt + 1, 0, n, false);
   else if (path == MHD_PATH_TWO_KERNEL) rc = launch_fused_range<T>(b, 0, n);
+  else if (path == MHD_PATH_TILE2D) rc = launch_tile2d<T>(b, 0, n);
   else rc = launch_staged_range<T>(b, 0, n);
   b->ov_plist = nullptr;
   b->ov_dtlist = nullptr;

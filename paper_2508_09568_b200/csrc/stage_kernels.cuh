@@ -288,76 +288,81 @@ __global__ void __launch_bounds__(256) k_set_dt(double* dst, const double* src, 
 }
 
 // ------------------------------------------------------------------- step stages ----
+// The body of every stage is a device function over an ACCESSOR x that says where the stage finds the
+// state and the scratch arrays at "its" cell: HbmAcc = the bunch's arrays in HBM (the staged kernels
+// below: one kernel per stage), TileAcc (tile_kernel.cuh) = a tile held in shared memory (all stages
+// in one kernel).  x.u(f): field f of U^n, x.w(a): scratch array a, x.un(f): field f of U^{n+1} (always
+// HBM), each a pointer AT the cell; x.s(d): element step for +1 along d (0 if collapsed).  Both paths
+// therefore evaluate the same expressions in the same order (results agree to rounding: the compiler
+// may contract multiply-adds differently in the two instantiations).
+template <typename T> struct HbmAcc {
+  const T* U; T* Un; T* W;
+  long long ufs, wfs, cu, cw;
+  long long st[3];
+  __device__ __forceinline__ HbmAcc(const Params<T>& P, int pl, long long c)
+      : U(P.U), Un(P.Un), W(P.W), ufs(P.G.fs), wfs(P.wfs), cu((long long)P.patch(pl) * P.G.ps + c), cw((long long)pl * P.G.ps + c) {
+    st[0] = P.G.s[0]; st[1] = P.G.s[1]; st[2] = P.G.s[2];
+  }
+  __device__ __forceinline__ const T* u(int f) const { return U + f * ufs + cu; }
+  __device__ __forceinline__ T* un(int f) const { return Un + f * ufs + cu; }
+  __device__ __forceinline__ T* w(int a) const { return W + a * wfs + cw; }
+  __device__ __forceinline__ long long s(int d) const { return st[d]; }
+};
+
 // O2 (EOS L68): primitives on cells [-2, n+1]
-template <typename T>
-__global__ void __launch_bounds__(256) k_prim(Params<T> P, Box B, unsigned long long* __restrict__ bad) {
+template <typename T, typename X>
+__device__ __forceinline__ void st_prim(const Params<T>& P, const X& x, int i, int j, int k, unsigned long long* __restrict__ bad) {
   const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
-  const T* U = P.U;
-  const T rho = U[cu], irho = num<T>::rcp(rho);
-  const T u = U[G.fs + cu] * irho, v = U[2 * G.fs + cu] * irho, w = U[3 * G.fs + cu] * irho;
-  const T bx = T(0.5) * (U[5 * G.fs + cu] + U[5 * G.fs + cu + G.s[0]]);
-  const T by = T(0.5) * (U[6 * G.fs + cu] + U[6 * G.fs + cu + G.s[1]]);
-  const T bz = T(0.5) * (U[7 * G.fs + cu] + U[7 * G.fs + cu + G.s[2]]);
+  const T rho = x.u(0)[0], irho = num<T>::rcp(rho);
+  const T u = x.u(1)[0] * irho, v = x.u(2)[0] * irho, w = x.u(3)[0] * irho;
+  const T bx = T(0.5) * (x.u(5)[0] + x.u(5)[x.s(0)]);
+  const T by = T(0.5) * (x.u(6)[0] + x.u(6)[x.s(1)]);
+  const T bz = T(0.5) * (x.u(7)[0] + x.u(7)[x.s(2)]);
   const T pr = (P.gamma - T(1)) *
-               (U[4 * G.fs + cu] - T(0.5) * rho * (u * u + v * v + w * w) - T(0.5) * (bx * bx + by * by + bz * bz));
-  T* q = P.W + W_Q * P.wfs + cw;
-  q[0] = rho; q[P.wfs] = u; q[2 * P.wfs] = v; q[3 * P.wfs] = w; q[4 * P.wfs] = pr;
-  q[5 * P.wfs] = bx; q[6 * P.wfs] = by; q[7 * P.wfs] = bz;
+               (x.u(4)[0] - T(0.5) * rho * (u * u + v * v + w * w) - T(0.5) * (bx * bx + by * by + bz * bz));
+  x.w(W_Q + 0)[0] = rho; x.w(W_Q + 1)[0] = u; x.w(W_Q + 2)[0] = v; x.w(W_Q + 3)[0] = w; x.w(W_Q + 4)[0] = pr;
+  x.w(W_Q + 5)[0] = bx; x.w(W_Q + 6)[0] = by; x.w(W_Q + 7)[0] = bz;
   if (inside(G, i, j, k, 0, 0) && !(rho > T(0) && pr > T(0) && rho < T(INFINITY) && pr < T(INFINITY)))
     atomicAdd(bad, 1ull);
 }
 
 // O4a: Eq. 7-11 and cyclic images, edges [-1, n+1]
-template <typename T>
-__global__ void __launch_bounds__(256) k_emf0(Params<T> P, Box B) {
-  const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
-  const long long sx = G.s[0], sy = G.s[1], sz = G.s[2];
-  const T* u = P.W + (W_Q + 1) * P.wfs + cw;
-  const T* v = P.W + (W_Q + 2) * P.wfs + cw;
-  const T* w = P.W + (W_Q + 3) * P.wfs + cw;
-  const T* bx = P.U + 5 * G.fs + cu;
-  const T* by = P.U + 6 * G.fs + cu;
-  const T* bz = P.U + 7 * G.fs + cu;
+template <typename T, typename X>
+__device__ __forceinline__ void st_emf0(const Params<T>& P, const X& x) {
+  const long long sx = x.s(0), sy = x.s(1), sz = x.s(2);
+  const T* u = x.w(W_Q + 1);
+  const T* v = x.w(W_Q + 2);
+  const T* w = x.w(W_Q + 3);
+  const T* bx = x.u(5);
+  const T* by = x.u(6);
+  const T* bz = x.u(7);
   const T q4 = T(0.25), h = T(0.5);
-  T* e0 = P.W + W_E0 * P.wfs + cw;
   {  // ez = <u><By> - <v><Bx> over cells (i-1..i, j-1..j)
     const T ub = q4 * (u[0] + u[-sy] + u[-sx] + u[-sx - sy]);
     const T vb = q4 * (v[0] + v[-sy] + v[-sx] + v[-sx - sy]);
-    e0[2 * P.wfs] = ub * (h * (by[0] + by[-sx])) - vb * (h * (bx[0] + bx[-sy]));
+    x.w(W_E0 + 2)[0] = ub * (h * (by[0] + by[-sx])) - vb * (h * (bx[0] + bx[-sy]));
   }
   {  // ex = <v><Bz> - <w><By> over (j-1..j, k-1..k)
     const T vb = q4 * (v[0] + v[-sz] + v[-sy] + v[-sy - sz]);
     const T wb = q4 * (w[0] + w[-sz] + w[-sy] + w[-sy - sz]);
-    e0[0] = vb * (h * (bz[0] + bz[-sy])) - wb * (h * (by[0] + by[-sz]));
+    x.w(W_E0 + 0)[0] = vb * (h * (bz[0] + bz[-sy])) - wb * (h * (by[0] + by[-sz]));
   }
   {  // ey = <w><Bx> - <u><Bz> over (k-1..k, i-1..i)
     const T wb = q4 * (w[0] + w[-sx] + w[-sz] + w[-sz - sx]);
     const T ub = q4 * (u[0] + u[-sx] + u[-sz] + u[-sz - sx]);
-    e0[P.wfs] = wb * (h * (bx[0] + bx[-sz])) - ub * (h * (bz[0] + bz[-sx]));
+    x.w(W_E0 + 1)[0] = wb * (h * (bx[0] + bx[-sz])) - ub * (h * (bz[0] + bz[-sx]));
   }
 }
 
 // O3 + O4b + O4c: limited slopes and the half-step predictor
-template <typename T>
-__global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const double* __restrict__ dtp) {
+template <typename T, typename X>
+__device__ __forceinline__ void st_predict(const Params<T>& P, const X& x, int i, int j, int k, T dt) {
   const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c;
-  const T dt = P.dt_of(pl, dtp);
   const T hdt = T(0.5) * dt;
-  const long long wfs = P.wfs;
   const int cc[3] = {i, j, k};
 
   // half-step face fields: Eq. 12 with dt/2
   {
-    const T* e0 = P.W + W_E0 * wfs + cw;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       const int b = (a + 1) % 3, e = (a + 2) % 3;
@@ -367,20 +372,19 @@ __global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const doubl
       for (int d = 0; d < 3; ++d)
         if (G.act[d]) ok = ok && (d == a ? true : cc[d] <= G.n[d]);
       if (!ok) continue;
-      const T* Ee = e0 + e * wfs;
-      const T* Eb = e0 + b * wfs;
+      const T* Ee = x.w(W_E0 + e);
+      const T* Eb = x.w(W_E0 + b);
       T curl = T(0);  // differences along a collapsed dimension vanish identically
-      if (G.act[b]) curl += (Ee[G.s[b]] - Ee[0]) * P.idx[b];
-      if (G.act[e]) curl -= (Eb[G.s[e]] - Eb[0]) * P.idx[e];
-      P.W[(W_BH + a) * wfs + cw] = P.U[(5 + a) * G.fs + cu] + hdt * curl;
+      if (G.act[b]) curl += (Ee[x.s(b)] - Ee[0]) * P.idx[b];
+      if (G.act[e]) curl -= (Eb[x.s(e)] - Eb[0]) * P.idx[e];
+      x.w(W_BH + a)[0] = x.u(5 + a)[0] + hdt * curl;
     }
   }
   if (!inside(G, i, j, k, 1, 1)) return;
 
-  const T* q = P.W + W_Q * wfs + cw;
   T qc[8];
 #pragma unroll
-  for (int f = 0; f < 8; ++f) qc[f] = q[f * wfs];
+  for (int f = 0; f < 8; ++f) qc[f] = x.w(W_Q + f)[0];
   T dq[3][8];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
@@ -388,10 +392,10 @@ __global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const doubl
     for (int f = 0; f < 8; ++f) {
       T s = T(0);
       if (G.act[d] && f != 5 + d) {
-        const T* qf = q + f * wfs;
-        s = limited_slope(G.limiter, qc[f] - qf[-G.s[d]], qf[G.s[d]] - qc[f]);
+        const T* qf = x.w(W_Q + f);
+        s = limited_slope(G.limiter, qc[f] - qf[-x.s(d)], qf[x.s(d)] - qc[f]);
       }
-      if (f != 5 + d) P.W[(W_DQ + d * 8 + f) * wfs + cw] = s;  // the normal-field slot is never read
+      if (f != 5 + d) x.w(W_DQ + d * 8 + f)[0] = s;  // the normal-field slot is never read
       dq[d][f] = s;
     }
   }
@@ -402,10 +406,10 @@ __global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const doubl
       if (t == a) continue;
       T s = T(0);
       if (G.act[t]) {
-        const T* bf = P.U + (5 + a) * G.fs + cu;
-        s = limited_slope(G.limiter, bf[0] - bf[-G.s[t]], bf[G.s[t]] - bf[0]);
+        const T* bf = x.u(5 + a);
+        s = limited_slope(G.limiter, bf[0] - bf[-x.s(t)], bf[x.s(t)] - bf[0]);
       }
-      P.W[(W_DBF + dbf_index(a, t)) * wfs + cw] = s;
+      x.w(W_DBF + dbf_index(a, t))[0] = s;
     }
   }
   // primitive half step
@@ -429,100 +433,83 @@ __global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const doubl
     const T tens = lam[b] * qc[5 + b] * dq[b][5 + a] + lam[e] * qc[5 + e] * dq[e][5 + a];
     vh[a] += (tens - press) * irho;
   }
-  T* qh = P.W + W_QH * wfs + cw;
-  qh[0] = rho_h; qh[wfs] = vh[0]; qh[2 * wfs] = vh[1]; qh[3 * wfs] = vh[2]; qh[4 * wfs] = p_h;
+  x.w(W_QH + 0)[0] = rho_h; x.w(W_QH + 1)[0] = vh[0]; x.w(W_QH + 2)[0] = vh[1]; x.w(W_QH + 3)[0] = vh[2]; x.w(W_QH + 4)[0] = p_h;
 }
 
 // O5 + O6: face states and HLLD flux through the lower face along D
-template <typename T, int D>
-__global__ void __launch_bounds__(256) k_flux(Params<T> P, Box B) {
+template <typename T, int D, typename X>
+__device__ __forceinline__ void st_flux(const Params<T>& P, const X& x) {
   const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cw = (long long)pl * G.ps + c, wfs = P.wfs;
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  const long long sd = G.s[D];
-  const T* qh = P.W + W_QH * wfs + cw;
-  const T* dq = P.W + (W_DQ + D * 8) * wfs + cw;
-  const T* bh = P.W + W_BH * wfs + cw;
+  const long long sd = x.s(D);
   const T h = T(0.5);
   State1D<T> L, R;
   // left state: upper face of cell c - e_D; right state: lower face of cell c
-  L.rho = qh[-sd] + h * dq[-sd];                               R.rho = qh[0] - h * dq[0];
-  L.u = qh[(1 + D) * wfs - sd] + h * dq[(1 + D) * wfs - sd];   R.u = qh[(1 + D) * wfs] - h * dq[(1 + D) * wfs];
-  L.v = qh[(1 + T1) * wfs - sd] + h * dq[(1 + T1) * wfs - sd]; R.v = qh[(1 + T1) * wfs] - h * dq[(1 + T1) * wfs];
-  L.w = qh[(1 + T2) * wfs - sd] + h * dq[(1 + T2) * wfs - sd]; R.w = qh[(1 + T2) * wfs] - h * dq[(1 + T2) * wfs];
-  L.p = qh[4 * wfs - sd] + h * dq[4 * wfs - sd];               R.p = qh[4 * wfs] - h * dq[4 * wfs];
+  L.rho = x.w(W_QH)[-sd] + h * x.w(W_DQ + D * 8)[-sd];                   R.rho = x.w(W_QH)[0] - h * x.w(W_DQ + D * 8)[0];
+  L.u = x.w(W_QH + 1 + D)[-sd] + h * x.w(W_DQ + D * 8 + 1 + D)[-sd];     R.u = x.w(W_QH + 1 + D)[0] - h * x.w(W_DQ + D * 8 + 1 + D)[0];
+  L.v = x.w(W_QH + 1 + T1)[-sd] + h * x.w(W_DQ + D * 8 + 1 + T1)[-sd];   R.v = x.w(W_QH + 1 + T1)[0] - h * x.w(W_DQ + D * 8 + 1 + T1)[0];
+  L.w = x.w(W_QH + 1 + T2)[-sd] + h * x.w(W_DQ + D * 8 + 1 + T2)[-sd];   R.w = x.w(W_QH + 1 + T2)[0] - h * x.w(W_DQ + D * 8 + 1 + T2)[0];
+  L.p = x.w(W_QH + 4)[-sd] + h * x.w(W_DQ + D * 8 + 4)[-sd];             R.p = x.w(W_QH + 4)[0] - h * x.w(W_DQ + D * 8 + 4)[0];
   // half-step centred transverse fields = mean of the two half-step faces
-  const T* b1 = bh + T1 * wfs;
-  const T* b2 = bh + T2 * wfs;
-  L.by = h * (b1[-sd] + b1[-sd + G.s[T1]]) + h * dq[(5 + T1) * wfs - sd];
-  R.by = h * (b1[0] + b1[G.s[T1]]) - h * dq[(5 + T1) * wfs];
-  L.bz = h * (b2[-sd] + b2[-sd + G.s[T2]]) + h * dq[(5 + T2) * wfs - sd];
-  R.bz = h * (b2[0] + b2[G.s[T2]]) - h * dq[(5 + T2) * wfs];
-  const Flux5<T> F = riemann_flux(G.flux_solver, P.gamma, L, R, bh[D * wfs]);
-  T* fl = P.W + (W_FLUX + D * 5) * wfs + cw;
-  fl[0] = F.d; fl[(1 + D) * wfs] = F.mu; fl[(1 + T1) * wfs] = F.mv; fl[(1 + T2) * wfs] = F.mw; fl[4 * wfs] = F.e;
+  const T* b1 = x.w(W_BH + T1);
+  const T* b2 = x.w(W_BH + T2);
+  L.by = h * (b1[-sd] + b1[-sd + x.s(T1)]) + h * x.w(W_DQ + D * 8 + 5 + T1)[-sd];
+  R.by = h * (b1[0] + b1[x.s(T1)]) - h * x.w(W_DQ + D * 8 + 5 + T1)[0];
+  L.bz = h * (b2[-sd] + b2[-sd + x.s(T2)]) + h * x.w(W_DQ + D * 8 + 5 + T2)[-sd];
+  R.bz = h * (b2[0] + b2[x.s(T2)]) - h * x.w(W_DQ + D * 8 + 5 + T2)[0];
+  const Flux5<T> F = riemann_flux(G.flux_solver, P.gamma, L, R, x.w(W_BH + D)[0]);
+  x.w(W_FLUX + D * 5)[0] = F.d; x.w(W_FLUX + D * 5 + 1 + D)[0] = F.mu; x.w(W_FLUX + D * 5 + 1 + T1)[0] = F.mv;
+  x.w(W_FLUX + D * 5 + 1 + T2)[0] = F.mw; x.w(W_FLUX + D * 5 + 4)[0] = F.e;
 }
 
 // O5 + O7: corner states and the 2D Riemann problem at the edge along E
-template <typename T, int E>
-__global__ void __launch_bounds__(128) k_emf(Params<T> P, Box B) {
+template <typename T, int E, typename X>
+__device__ __forceinline__ void st_emf(const Params<T>& P, const X& x) {
   const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cw = (long long)pl * G.ps + c, wfs = P.wfs;
   constexpr int A = (E + 1) % 3, Bd = (E + 2) % 3;
-  const long long sa = G.s[A], sb = G.s[Bd], se = G.s[E];
-  const T* qh = P.W + W_QH * wfs + cw;
-  const T* da = P.W + (W_DQ + A * 8) * wfs + cw;
-  const T* db = P.W + (W_DQ + Bd * 8) * wfs + cw;
-  const T* bh = P.W + W_BH * wfs + cw;
+  const long long sa = x.s(A), sb = x.s(Bd), se = x.s(E);
   const T h = T(0.5);
   // corner of cell at offset o seen with signs (sga, sgb)
   auto corner = [&](long long o, T sga, T sgb) {
     Corner<T> q;
-    q.rho = qh[o] + sga * h * da[o] + sgb * h * db[o];
-    q.ua = qh[(1 + A) * wfs + o] + sga * h * da[(1 + A) * wfs + o] + sgb * h * db[(1 + A) * wfs + o];
-    q.ub = qh[(1 + Bd) * wfs + o] + sga * h * da[(1 + Bd) * wfs + o] + sgb * h * db[(1 + Bd) * wfs + o];
-    q.p = qh[4 * wfs + o] + sga * h * da[4 * wfs + o] + sgb * h * db[4 * wfs + o];
-    const T* be = bh + E * wfs + o;
-    q.be = h * (be[0] + be[se]) + sga * h * da[(5 + E) * wfs + o] + sgb * h * db[(5 + E) * wfs + o];
+    q.rho = x.w(W_QH)[o] + sga * h * x.w(W_DQ + A * 8)[o] + sgb * h * x.w(W_DQ + Bd * 8)[o];
+    q.ua = x.w(W_QH + 1 + A)[o] + sga * h * x.w(W_DQ + A * 8 + 1 + A)[o] + sgb * h * x.w(W_DQ + Bd * 8 + 1 + A)[o];
+    q.ub = x.w(W_QH + 1 + Bd)[o] + sga * h * x.w(W_DQ + A * 8 + 1 + Bd)[o] + sgb * h * x.w(W_DQ + Bd * 8 + 1 + Bd)[o];
+    q.p = x.w(W_QH + 4)[o] + sga * h * x.w(W_DQ + A * 8 + 4)[o] + sgb * h * x.w(W_DQ + Bd * 8 + 4)[o];
+    const T* be = x.w(W_BH + E) + o;
+    q.be = h * (be[0] + be[se]) + sga * h * x.w(W_DQ + A * 8 + 5 + E)[o] + sgb * h * x.w(W_DQ + Bd * 8 + 5 + E)[o];
     return q;
   };
   // SW = RT of cell (a-1,b-1), SE = LT of (a,b-1), NW = RB of (a-1,b), NE = LB of (a,b)
   const Corner<T> sw = corner(-sa - sb, T(1), T(1)), se_ = corner(-sb, T(-1), T(1));
   const Corner<T> nw = corner(-sa, T(1), T(-1)), ne = corner(0, T(-1), T(-1));
-  const T* dba = P.W + (W_DBF + dbf_index(A, Bd)) * wfs + cw;  // slope of b_A along B
-  const T* dbb = P.W + (W_DBF + dbf_index(Bd, A)) * wfs + cw;  // slope of b_B along A
-  const T* ba = bh + A * wfs;
-  const T* bb = bh + Bd * wfs;
+  const T* dba = x.w(W_DBF + dbf_index(A, Bd));  // slope of b_A along B
+  const T* dbb = x.w(W_DBF + dbf_index(Bd, A));  // slope of b_B along A
+  const T* ba = x.w(W_BH + A);
+  const T* bb = x.w(W_BH + Bd);
   const T AS = ba[-sb] + h * dba[-sb], AN = ba[0] - h * dba[0];
   const T BW = bb[-sa] + h * dbb[-sa], BE = bb[0] - h * dbb[0];
-  P.W[(W_EMF + E) * wfs + cw] = emf_2d(P.gamma, G.emf_solver, sw, se_, nw, ne, AS, AN, BW, BE);
+  x.w(W_EMF + E)[0] = emf_2d(P.gamma, G.emf_solver, sw, se_, nw, ne, AS, AN, BW, BE);
 }
 
 // O8: conservative update + constrained transport with the metric factor of each term
-// (Eq. 12; L154)
-template <typename T>
-__global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double* __restrict__ dtp) {
+// (Eq. 12; L154).  xlim/ylim: faces up to n along x/y are written (a tile that does
+// not end its patch leaves its last column/row of faces to the next tile: pass n-1 there)
+template <typename T, typename X>
+__device__ __forceinline__ void st_update(const Params<T>& P, const X& x, int i, int j, int k, T dt) {
   const Geom& G = P.G;
-  int pl, i, j, k; long long c;
-  if (!decode(G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  const long long cu = (long long)P.patch(pl) * G.ps + c, cw = (long long)pl * G.ps + c, wfs = P.wfs;
-  const T dt = P.dt_of(pl, dtp);
   const int cc[3] = {i, j, k};
   if (inside(G, i, j, k, 0, 0)) {
 #pragma unroll
     for (int f = 0; f < 5; ++f) {
-      T v = P.U[f * G.fs + cu];
+      T v = x.u(f)[0];
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         if (!G.act[d]) continue;
-        const T* fl = P.W + (W_FLUX + d * 5 + f) * wfs + cw;
-        v -= dt * P.idx[d] * (fl[G.s[d]] - fl[0]);
+        const T* fl = x.w(W_FLUX + d * 5 + f);
+        v -= dt * P.idx[d] * (fl[x.s(d)] - fl[0]);
       }
-      P.Un[f * G.fs + cu] = v;
+      x.un(f)[0] = v;
     }
   }
 #pragma unroll
@@ -534,14 +521,51 @@ __global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double
     for (int d = 0; d < 3; ++d)
       if (G.act[d] && d != a) ok = ok && cc[d] < G.n[d];
     if (!ok) continue;
-    const T* Ee = P.W + (W_EMF + e) * wfs + cw;
-    const T* Eb = P.W + (W_EMF + b) * wfs + cw;
+    const T* Ee = x.w(W_EMF + e);
+    const T* Eb = x.w(W_EMF + b);
     T curl = T(0);
-    if (G.act[b]) curl += (Ee[G.s[b]] - Ee[0]) * P.idx[b];
-    if (G.act[e]) curl -= (Eb[G.s[e]] - Eb[0]) * P.idx[e];
-    P.Un[(5 + a) * G.fs + cu] = P.U[(5 + a) * G.fs + cu] + dt * curl;
+    if (G.act[b]) curl += (Ee[x.s(b)] - Ee[0]) * P.idx[b];
+    if (G.act[e]) curl -= (Eb[x.s(e)] - Eb[0]) * P.idx[e];
+    x.un(5 + a)[0] = x.u(5 + a)[0] + dt * curl;
   }
 }
 
+// ---- the staged kernels: one stage each, arrays in HBM ----
+template <typename T>
+__global__ void __launch_bounds__(256) k_prim(Params<T> P, Box B, unsigned long long* __restrict__ bad) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_prim<T>(P, HbmAcc<T>(P, pl, c), i, j, k, bad);
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_emf0(Params<T> P, Box B) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_emf0<T>(P, HbmAcc<T>(P, pl, c));
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_predict(Params<T> P, Box B, const double* __restrict__ dtp) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_predict<T>(P, HbmAcc<T>(P, pl, c), i, j, k, P.dt_of(pl, dtp));
+}
+template <typename T, int D>
+__global__ void __launch_bounds__(256) k_flux(Params<T> P, Box B) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_flux<T, D>(P, HbmAcc<T>(P, pl, c));
+}
+template <typename T, int E>
+__global__ void __launch_bounds__(128) k_emf(Params<T> P, Box B) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_emf<T, E>(P, HbmAcc<T>(P, pl, c));
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double* __restrict__ dtp) {
+  int pl, i, j, k; long long c;
+  if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
+  st_update<T>(P, HbmAcc<T>(P, pl, c), i, j, k, P.dt_of(pl, dtp));
+}
 
 }  // namespace mhd

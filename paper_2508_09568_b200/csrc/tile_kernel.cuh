@@ -1,0 +1,152 @@
+// tile_kernel.cuh -- the whole step of a TWO-DIMENSIONAL bunch (n_z = 1: BASELINE.json config 1, the
+// paper's Orszag-Tang runs) in ONE kernel: every stage of PAPER.md section 2.1.4
+// (L108-116) runs on a tile held in shared memory, so U^n is read once (with its halo) and U^{n+1}
+// written once; nothing intermediate touches HBM and one launch replaces the staged path's eleven.
+//
+// The stages are the SAME device functions the staged kernels run (stage_kernels.cuh: st_prim,
+// st_emf0, st_predict, st_flux, st_emf, st_update), fed through an accessor that points into the
+// tile instead of the HBM scratch, so the results are the staged path's to rounding (the compiler may
+// contract multiply-adds differently in the two instantiations).
+//
+// A CTA owns a TX x TY tile of one patch.  Tile arrays have rows of TP = TX + 6 cells and TH = TY + 6
+// rows: cell (i, j) of the patch sits at column i - x0 + 3, row j - y0 + 3 (guard width 3, PAPER.md
+// L212).  42 scratch arrays + the 8 raw fields: the scratch map of bunch_types.cuh with the arrays
+// that are dead by then reused (the fluxes and the final EMFs take the place of the primitives and
+// the time-n EMFs) and every slope along the collapsed z direction (all zero) in ONE array.
+#pragma once
+#include "bunch_types.cuh"
+#include "mhd_math.cuh"
+#include "stage_kernels.cuh"
+
+namespace mhd {
+
+// scratch array of bunch_types.cuh -> slot of the tile (z collapsed)
+__host__ __device__ constexpr int tile_slot(int a) {
+  return a < W_DQ ? a                                           // W_Q 0..7          -> 0..7
+       : a < W_DQ + 16 ? 21 + (a - W_DQ)                        // slopes along x, y -> 21..36
+       : a < W_DBF ? 41                                         // slopes along z    -> the zero array
+       : a < W_E0 ? ((a - W_DBF) == 0 ? 37 : ((a - W_DBF) == 2 ? 38 : ((a - W_DBF) == 4 ? 39 : ((a - W_DBF) == 5 ? 40 : 41))))
+       : a < W_BH ? 8 + (a - W_E0)                              // time-n EMFs       -> 8..10
+       : a < W_QH ? 13 + (a - W_BH)                             // half-step faces   -> 13..15
+       : a < W_FLUX ? 16 + (a - W_QH)                           // half-step hydro   -> 16..20
+       : a < W_FLUX + 10 ? (a - W_FLUX)                         // fluxes along x, y -> 0..9 (over the primitives)
+       : a < W_EMF ? 41                                         // fluxes along z: never touched
+       : 10 + (a - W_EMF);                                      // final EMFs        -> 10..12 (10 over the time-n e_z)
+}
+constexpr int TILE_SLOTS = 42;
+
+template <typename T, int TX, int TY> struct TileCfg {
+  static constexpr int TP = TX + 6, TH = TY + 6, AR = TP * TH;
+  static constexpr int NTH = sizeof(T) == 4 ? 512 : 384;
+  static constexpr size_t smem = sizeof(T) * (size_t)(8 + TILE_SLOTS) * AR;
+  static_assert(smem <= 227 * 1024, "shared memory of one CTA");
+};
+
+template <typename T, int AR, int TP> struct TileAcc {
+  const T* raw;   // [8][AR] at the cell
+  T* W;           // [TILE_SLOTS][AR] at the cell
+  T* Un;          // U^{n+1} in HBM at the cell
+  long long ufs;
+  __device__ __forceinline__ const T* u(int f) const { return raw + f * AR; }
+  __device__ __forceinline__ T* un(int f) const { return Un + f * ufs; }
+  __device__ __forceinline__ T* w(int a) const { return W + tile_slot(a) * AR; }
+  __device__ __forceinline__ long long s(int d) const { return d == 0 ? 1 : (d == 1 ? TP : 0); }
+};
+
+template <typename T, int TX, int TY>
+__global__ void __launch_bounds__(TileCfg<T, TX, TY>::NTH, 1)
+k_step_tile2d(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad, int xtiles) {
+  using C = TileCfg<T, TX, TY>;
+  constexpr int TP = C::TP, TH = C::TH, AR = C::AR, NTH = C::NTH;
+  extern __shared__ __align__(16) unsigned char tile_smem[];
+  T* const raw = reinterpret_cast<T*>(tile_smem);
+  T* const W = raw + 8 * AR;
+  const Geom& G = P.G;
+  const int nx = G.n[0], ny = G.n[1];
+  const int pl = blockIdx.y;
+  const int xt = blockIdx.x % xtiles, yt = blockIdx.x / xtiles;
+  const int x0 = xt * TX, y0 = yt * TY;
+  const int tw = min(TX, nx - x0), th = min(TY, ny - y0);
+  const bool lastx = x0 + tw == nx, lasty = y0 + th == ny;
+  const int t = threadIdx.x;
+  const T dt = P.dt_of(pl, dtp);
+  const long long pbase = (long long)P.patch(pl) * G.ps + G.lead;
+
+  // U^n of cells [x0-3, x0+tw+2] x [y0-3, y0+th+2] (guard cells filled: O1) -> raw tile
+  for (int idx = t; idx < AR; idx += NTH) {
+    const int lr = idx / TP, lc = idx - lr * TP;
+    const int i = x0 - 3 + lc, j = y0 - 3 + lr;
+    if (i <= nx + 2 && j <= ny + 2) {
+      const long long g = pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
+#pragma unroll
+      for (int f = 0; f < 8; ++f) raw[f * AR + idx] = P.U[f * G.fs + g];
+    }
+  }
+  __syncthreads();
+
+  // a stage over the cells [ilo, ihi] x [jlo, jhi] of the patch
+  auto acc = [&](int i, int j) {
+    const int o = (j - y0 + 3) * TP + (i - x0 + 3);
+    TileAcc<T, AR, TP> a;
+    a.raw = raw + o; a.W = W + o; a.ufs = G.fs;
+    a.Un = P.Un + pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
+    return a;
+  };
+#define TILE_FOR(ilo, ihi, jlo, jhi, BODY)                                   \
+  {                                                                          \
+    const int ni_ = (ihi) - (ilo) + 1, nj_ = (jhi) - (jlo) + 1;              \
+    for (int it_ = t; it_ < ni_ * nj_; it_ += NTH) {                         \
+      const int jj_ = it_ / ni_, i = (ilo) + it_ - jj_ * ni_, j = (jlo) + jj_; \
+      const TileAcc<T, AR, TP> x = acc(i, j);                                \
+      BODY;                                                                  \
+    }                                                                        \
+  }
+  // O2: primitives; only the tile's own cells count towards the bad-cell total
+  TILE_FOR(x0 - 2, x0 + tw + 1, y0 - 2, y0 + th + 1,
+           st_prim<T>(P, x, (i >= x0 && i < x0 + tw && j >= y0 && j < y0 + th) ? i : -1, j, 0, bad));
+  __syncthreads();
+  TILE_FOR(x0 - 1, x0 + tw + 1, y0 - 1, y0 + th + 1, st_emf0<T>(P, x));
+  __syncthreads();
+  TILE_FOR(x0 - 1, x0 + tw + 1, y0 - 1, y0 + th + 1, st_predict<T>(P, x, i, j, 0, dt));
+  __syncthreads();
+  // the five Riemann problems of the plane as one list of tasks: x and y faces, the three edges
+  {
+    const int n0 = (tw + 1) * th, n1 = tw * (th + 1), n2 = (tw + 1) * (th + 1);
+    const int tot = 2 * n0 + 2 * n1 + n2;
+    for (int it = t; it < tot; it += NTH) {
+      int r = it;
+      if (r < n0) {                      // x faces: i in [x0, x0+tw], j in [y0, y0+th-1]
+        const int jj = r / (tw + 1);
+        st_flux<T, 0>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
+        continue;
+      }
+      r -= n0;
+      if (r < n1) {                      // y faces
+        const int jj = r / tw;
+        st_flux<T, 1>(P, acc(x0 + r - jj * tw, y0 + jj));
+        continue;
+      }
+      r -= n1;
+      if (r < n1) {                      // x-directed edges: i in [x0, x0+tw-1], j in [y0, y0+th]
+        const int jj = r / tw;
+        st_emf<T, 0>(P, acc(x0 + r - jj * tw, y0 + jj));
+        continue;
+      }
+      r -= n1;
+      if (r < n0) {                      // y-directed edges: i in [x0, x0+tw], j in [y0, y0+th-1]
+        const int jj = r / (tw + 1);
+        st_emf<T, 1>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
+        continue;
+      }
+      r -= n0;
+      const int jj = r / (tw + 1);       // z-directed edges: every corner of the tile
+      st_emf<T, 2>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
+    }
+  }
+  __syncthreads();
+  // O8: the tile's cells and lower faces; the closing faces where the tile ends its patch
+  TILE_FOR(x0, x0 + tw - 1 + (lastx ? 1 : 0), y0, y0 + th - 1 + (lasty ? 1 : 0), st_update<T>(P, x, i, j, 0, dt));
+#undef TILE_FOR
+}
+
+}  // namespace mhd

@@ -1,0 +1,95 @@
+"""GPU parity of the one-kernel step of two-dimensional bunches (MHD_PATH_TILE2D, csrc/tile_kernel.cuh;
+BASELINE.json config 1 = the paper's Orszag-Tang runs): every stage of PAPER.md section
+2.1.4 on a shared-memory tile.  Checked against the CPU oracle and, bit for bit, against the staged path
+(the two run the same stage functions: they agree to rounding -- not always bit for bit, the compiler is free
+to contract multiply-adds differently in the two instantiations)."""
+import numpy as np
+import pytest
+
+from parity_util import TOL_STEP, assert_nstep_parity, assert_step_parity, make_gpu, make_oracle, masked, rel_err
+from paper_2508_09568_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+NPD = {"f32": np.float32, "f64": np.float64}
+
+
+def workloads_2d(dtype):
+    t = NPD[dtype]
+    w = {
+        "ot64": W.orszag_tang(64, 32, dtype=t),              # 2 x 2 patches of 32^2: whole tiles in x
+        "ot_ragged": W.orszag_tang(60, 20, dtype=t),         # 20^2 patches: ragged tiles in x and y
+        "ot_wide": W.orszag_tang(80, 40, dtype=t),           # 40^2 patches: two x-tiles, several y-tiles
+        "ot_tiny": W.orszag_tang(12, 3, dtype=t),            # n = guard width: the thinnest legal patch
+        "ot_self": W.orszag_tang(24, 24, dtype=t),           # one patch, its own neighbour
+    }
+    # a 2.5D state: out-of-plane velocity and field, so that e_x, e_y and the b_z update do work
+    rng = np.random.default_rng(7)
+    for k in ("ot64", "ot_ragged"):
+        u = w[k].U
+        u[3] += (0.3 * u[0] * (1 + 0.2 * rng.standard_normal(u[0].shape))).astype(t)      # m_z (zero in the guard shell)
+        u[7] += t(0.2)                                                                       # b_z
+        u[4] += (0.5 * u[3] ** 2 / np.where(u[0] > 0, u[0], 1) + 0.5 * 0.04).astype(t)
+    return w
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("limiter,emf_solver,flux_solver", [(1, 0, 0), (2, 1, 1)])
+@pytest.mark.parametrize("name", ["ot64", "ot_ragged", "ot_wide", "ot_tiny", "ot_self"])
+def test_tile2d_step_matches_oracle_and_the_staged_path(name, dtype, limiter, emf_solver, flux_solver):
+    w = workloads_2d(dtype)[name]
+    o = make_oracle(w, limiter, emf_solver, flux_solver=flux_solver)
+    outs = {}
+    for path in ("tile2d", "staged"):
+        b = make_gpu(w, dtype, limiter, emf_solver, path=path, flux_solver=flux_solver)
+        assert b.path == path
+        U = w.U.astype(np.float64)
+        for s in range(3):
+            U = o.fill_guards(U, w.nbr)
+            dt = o.cfl_dt(U, 0.4)
+            U = o.step(U, dt)
+            b.fill_guards()
+            b.step(dt)
+            if s == 0:
+                assert_step_parity(masked(b.download(), w.n), masked(U, w.n), dtype, (name, path))
+        outs[path] = b.download()
+        assert b.status() == 0
+        b.close()
+    got = outs["tile2d"]
+    assert rel_err(masked(got, w.n), masked(U, w.n)) <= TOL_STEP[dtype]
+    assert_nstep_parity(W.gather(got, w.n, w.P), W.gather(U, w.n, w.P), dtype, name)
+    close = {"f64": 1e-14, "f32": 2e-6}[dtype]
+    assert rel_err(masked(got, w.n), masked(outs["staged"], w.n).astype(np.float64)) <= close
+
+
+def test_tile2d_is_the_default_for_2d_bunches_and_one_launch():
+    w = W.orszag_tang(64, 32, dtype=np.float32)
+    b = make_gpu(w, "f32")
+    assert b.path == "tile2d"
+    b.fill_guards()
+    l0 = b.launches
+    b.step(1e-3)
+    assert b.launches - l0 == 2                 # k_set_dt + the step
+    with pytest.raises(RuntimeError):
+        make_gpu(W.turbulence(N=32, n=16, dtype=np.float32), "f32", path="tile2d")     # 3D: not applicable
+    b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_tile2d_with_outflow_sides(dtype):
+    """-1 neighbours: guard cells are zero-gradient copies (k_fill_guards) and a patch evolves its own
+    closing faces (O8)."""
+    w = W.orszag_tang(64, 32, dtype=NPD[dtype])
+    w.nbr = W.neighbour_table(w.P, (False, True, True))
+    o = make_oracle(w)
+    b = make_gpu(w, dtype)
+    U = w.U.astype(np.float64)
+    for _ in range(3):
+        U = o.fill_guards(U, w.nbr)
+        dt = o.cfl_dt(U, 0.4)
+        U = o.step(U, dt)
+        b.fill_guards()
+        b.step(dt)
+    got = b.download()
+    assert rel_err(masked(got, w.n), masked(U, w.n)) <= TOL_STEP[dtype]
+    assert b.status() == 0
+    b.close()
