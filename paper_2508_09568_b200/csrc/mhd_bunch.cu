@@ -76,6 +76,7 @@ struct mhd_bunch {
   int nsm;             // multiprocessors of the device
   bool onepass_ok;     // three active dimensions, fp32
   bool tile2d_ok;      // x and y active, z collapsed: the whole step in one kernel on shared-memory tiles
+  bool gather_t_ok;    // ... which may read its halos through the neighbour table (consistent table, no -1 side)
   bool gather_ok;      // the one-pass kernel can read halos from the neighbours' interiors: every
                        // neighbour exists (no outflow side) and n_x is a whole number of 16-byte chunks
   bool gather2_ok;     // the two-kernel path can do the same (predictor loads through the neighbour table)
@@ -360,7 +361,8 @@ int effective_path(const mhd_bunch* b) {
 // guard shell need not exist in HBM (deferred fill)
 bool step_gathers(const mhd_bunch* b) {
   const int path = effective_path(b);
-  return (path == MHD_PATH_ONEPASS && b->gather_ok) || (path == MHD_PATH_TWO_KERNEL && b->gather2_ok);
+  return (path == MHD_PATH_ONEPASS && b->gather_ok) || (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) ||
+         (path == MHD_PATH_TILE2D && b->gather_t_ok);
 }
 
 template <typename T> struct OnePassLaunch {
@@ -443,7 +445,8 @@ int launch_tile2d(mhd_bunch* b, int p0, int npl) {
   dim3 grid((unsigned)(xt * yt), (unsigned)npl, 1);
   {
     LaunchScope ls(b, KC_TILE2D);
-    k_step_tile2d<T, TX, TY><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_dt + 1, b->d_bad, xt);
+    k_step_tile2d<T, TX, TY><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, (b->gather_t_ok && !b->ov_plist) ? 1 : 0, b->d_dt + 1,
+                                                                  b->d_bad, xt);
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
@@ -593,6 +596,13 @@ int launch_step(mhd_bunch* b) {
   if (path == MHD_PATH_TWO_KERNEL && b->gather2_ok) {
     // halos come through the neighbour table if the fill was deferred, from the shell otherwise
     const int rc = launch_fused_range<T>(b, 0, G.np);
+    if (rc != MHD_OK) return rc;
+    b->cur = 1 - b->cur;
+    b->guards_stale = false;
+    return MHD_OK;
+  }
+  if (path == MHD_PATH_TILE2D && b->gather_t_ok) {
+    const int rc = launch_tile2d<T>(b, 0, G.np);
     if (rc != MHD_OK) return rc;
     b->cur = 1 - b->cur;
     b->guards_stale = false;
@@ -765,6 +775,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->nbr_consistent = b->all_nbr && table_is_consistent(nbr, desc->npatch);
   b->gather_ok = b->gather_ok && b->nbr_consistent;
   b->gather2_ok = b->fused_ok && b->nbr_consistent;
+  b->gather_t_ok = b->tile2d_ok && b->nbr_consistent;
   b->tune_zseg = 0;
   b->tune_bands = 0;
   b->fused_cfl = false;
@@ -1429,6 +1440,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
       }
       if (onepass) rc = OnePassLaunch<float>::run(b, b->d_dt + 1, p0, npl, false, za, zb);
       else if (za != 0 || zb != G.n[2]) rc = MHD_ESTATE;          // only the one-pass kernel steps plane ranges
+      else if (effective_path(b) == MHD_PATH_TILE2D) rc = f64 ? launch_tile2d<double>(b, p0, npl) : launch_tile2d<float>(b, p0, npl);
       else rc = f64 ? launch_fused_range<double>(b, p0, npl) : launch_fused_range<float>(b, p0, npl);
       if (rc != MHD_OK) return rc;
       CUDA_TRY(cudaEventRecord(h->ev_step[u], b->stream));

@@ -55,7 +55,8 @@ template <typename T, int AR, int TP> struct TileAcc {
 
 template <typename T, int TX, int TY>
 __global__ void __launch_bounds__(TileCfg<T, TX, TY>::NTH, 1)
-k_step_tile2d(Params<T> P, const double* __restrict__ dtp, unsigned long long* __restrict__ bad, int xtiles) {
+k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
+              unsigned long long* __restrict__ bad, int xtiles) {
   using C = TileCfg<T, TX, TY>;
   constexpr int TP = C::TP, TH = C::TH, AR = C::AR, NTH = C::NTH;
   extern __shared__ __align__(16) unsigned char tile_smem[];
@@ -72,12 +73,22 @@ k_step_tile2d(Params<T> P, const double* __restrict__ dtp, unsigned long long* _
   const T dt = P.dt_of(pl, dtp);
   const long long pbase = (long long)P.patch(pl) * G.ps + G.lead;
 
-  // U^n of cells [x0-3, x0+tw+2] x [y0-3, y0+th+2] (guard cells filled: O1) -> raw tile
+  // U^n of cells [x0-3, x0+tw+2] x [y0-3, y0+th+2] -> raw tile.  GATHER mode: a cell outside the patch is
+  // read from the interior of the neighbour of its class (guard fill O1 folded into the load: PAPER.md
+  // L124, L188, L241), so the guard shell in HBM is neither written nor read; otherwise the patch's own
+  // (already filled) guard cells are read.
   for (int idx = t; idx < AR; idx += NTH) {
     const int lr = idx / TP, lc = idx - lr * TP;
     const int i = x0 - 3 + lc, j = y0 - 3 + lr;
     if (i <= nx + 2 && j <= ny + 2) {
-      const long long g = pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
+      long long g = pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
+      if (gather) {
+        const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0), oy = j < 0 ? -1 : (j >= ny ? 1 : 0);
+        if (ox | oy) {
+          const int q = nbr[(long long)P.patch(pl) * 27 + 9 + (oy + 1) * 3 + (ox + 1)];
+          g = (long long)q * G.ps + G.lead + (i - ox * nx + G.g[0]) + (long long)(j - oy * ny + G.g[1]) * G.pitch;
+        }
+      }
 #pragma unroll
       for (int f = 0; f < 8; ++f) raw[f * AR + idx] = P.U[f * G.fs + g];
     }

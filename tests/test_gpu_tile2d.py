@@ -93,3 +93,33 @@ def test_tile2d_with_outflow_sides(dtype):
     assert rel_err(masked(got, w.n), masked(U, w.n)) <= TOL_STEP[dtype]
     assert b.status() == 0
     b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["ot64", "ot_ragged", "ot_self"])
+def test_tile2d_defers_the_fill_too(name, dtype):
+    """Periodic 2D bunches: the tile kernel reads its halo from the neighbours' interiors through the
+    neighbour table, so mhd_bunch_fill_guards launches nothing in the loop.  What a caller sees equals an
+    immediate fill (the shell after download, bit for bit against the oracle's fill), and steps with and
+    without the shell written first agree bit for bit."""
+    w = workloads_2d(dtype)[name]
+    o = make_oracle(w)
+    outs, launches = [], []
+    for force in (False, True):
+        b = make_gpu(w, dtype)
+        assert b.path == "tile2d"
+        l0 = b.launches
+        for _ in range(3):
+            b.fill_guards()
+            if force:
+                b.sync_guards()
+            b.cfl_dt(0.4, sync=False)
+            b.step_dev()
+        launches.append(b.launches - l0)
+        b.fill_guards()
+        outs.append(b.download())
+        b.close()
+    assert np.array_equal(outs[0], outs[1])
+    assert launches[0] < launches[1]                                   # no k_fill_guards in the deferred loop
+    ref = o.fill_guards(outs[0].astype(np.float64).copy(), w.nbr)
+    assert np.array_equal(outs[0].astype(np.float64), ref)
