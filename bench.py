@@ -62,6 +62,17 @@ def peaks():
 #        FMA = 2): whole step 3625.4, cfl 86; HLLD solve 392, HLLD-2D edge solve 453.
 STEP_FLOPS_32 = 3625.4
 CFL_FLOPS = 86.0
+STEP_FLOPS_2D, CFL_FLOPS_2D = 3088.2, 66.0     # `oracle/opcount 32 2d`: patches of 32 x 32 x 1 cells (no z face, three edges)
+# configs 0 and 1 of BASELINE.json: small bunches (256 and 65 536 cells) -- a step is a handful of launches and
+# the rate is set by launch latency, so these records carry the per-step time and the launch count, and an ALU
+# fraction only for the 2D tile kernel
+SMALL = {
+    "c0": ("sod", "f64", "config0: 1D Sod tube, 8 patches x 32 cells, fp64, outflow ends"),
+    "c1": ("ot", "f64", "config1: Orszag-Tang 256^2, 64 patches x 32^2, fp64, periodic"),
+    "c1f32": ("ot", "f32", "config1: Orszag-Tang 256^2, 64 patches x 32^2, fp32, periodic"),
+    "ot2048f64": ("ot2048", "f64", "Orszag-Tang 2048^2, 4096 patches x 32^2, fp64 (a 2D bunch large enough to fill the GPU)"),
+    "ot2048": ("ot2048", "f32", "Orszag-Tang 2048^2, 4096 patches x 32^2, fp32 (a 2D bunch large enough to fill the GPU)"),
+}
 
 
 def algorithmic_work(cls, n, ng=3):
@@ -333,6 +344,57 @@ def measure(name, args, local, world, rank, field_cache, headline):
     return rec
 
 
+def measure_small(name, args, local):
+    """Configs 0 and 1 (and a large 2D bunch): resident loop fill_guards -> cfl_dt -> step with CUDA events,
+    launches per step, per-class device times, and for 2D bunches the tile kernel's ALU fraction."""
+    import torch
+    from paper_2508_09568_b200.binding import MhdBunch, measure_alu_peak
+    kind, dtype, desc = SMALL[name]
+    npd = np.float32 if dtype == "f32" else np.float64
+    w = W.sod(256, 8, dtype=npd) if kind == "sod" else W.orszag_tang(2048 if kind == "ot2048" else 256, 32, dtype=npd)
+    b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, device=local)
+    b.load(w.U)
+
+    def one_step():
+        b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+    steps = 200 if w.cells < (1 << 20) else max(3, min(args.steps, args.sub_steps))
+    for _ in range(5):
+        one_step()
+    torch.cuda.synchronize()
+    l0 = b.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(b.stream):
+        ev0.record(b.stream)
+        for _ in range(steps):
+            one_step()
+        ev1.record(b.stream)
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / steps
+    launches = (b.launches - l0) / steps
+    b.set_timing(True)
+    for _ in range(10):
+        one_step()
+    kt = b.kernel_times()
+    b.set_timing(False)
+    classes = {k: {"ms_per_step": v[0] / 10, "launches_per_step": v[1] / 10} for k, v in kt.items()}
+    rec = {"workload": name, "dtype": dtype, "value": w.cells / (ms * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms,
+           "config": {"workload": desc, "patches": w.npatch, "patch": list(w.n), "guard": 3, "courant": 0.4, "step_path": b.path},
+           "gpu_launches_per_step": launches, "bad_cells": b.status(), "kernel_classes": classes,
+           "note": "events around every launch inflate the per-class times of kernels this short; ms_per_step is the untimed loop"}
+    if "step_tile2d" in classes:
+        tk = classes["step_tile2d"]["ms_per_step"]
+        alu_peak = measure_alu_peak(dtype, local)
+        rec["roofline"] = {"kernel": "step_tile2d", "bound": "alu", "achieved": STEP_FLOPS_2D * w.cells / (tk * 1e-3) / 1e12,
+                           "peak": alu_peak, "unit": "TFLOP/s", "frac": STEP_FLOPS_2D * w.cells / (tk * 1e-3) / 1e12 / alu_peak,
+                           "peak_source": "measured FMA chain (mhd_bunch_measure_alu_peak), FMA = 2 flops",
+                           "alg_flops_per_launch": STEP_FLOPS_2D * w.cells, "avg_launch_ms": tk, "traffic": None,
+                           "share_of_step": tk / sum(c["ms_per_step"] for c in classes.values())}
+    b.close()
+    del b
+    torch.cuda.empty_cache()
+    return rec
+
+
 # ---------------------------------------------------------------- config 4: the sweep ----
 ARRANGE = {1: (1, 1, 1), 8: (2, 2, 2), 64: (4, 4, 4), 300: (5, 6, 10), 512: (8, 8, 8), 4096: (16, 16, 16)}
 
@@ -425,8 +487,8 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS) + ["c4"])
-    ap.add_argument("--sub", default="c2f64,c3,c3f64",
+    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS) + sorted(SMALL) + ["c4"])
+    ap.add_argument("--sub", default="c2f64,c3,c3f64,c0,c1,c1f32,ot2048,ot2048f64",
                     help="sub-records added to the default (c2) line: comma list of workloads, or 'none'")
     ap.add_argument("--sub-steps", type=int, default=20, help="timed steps of each sub-record")
     ap.add_argument("--cpu-steps", type=int, default=20, help="oracle steps for the cpu_baseline legs")
@@ -488,12 +550,27 @@ def main():
             dist.destroy_process_group()
         return 0
 
+    if args.workload in SMALL:
+        if rank == 0:
+            r = measure_small(args.workload, args, local)
+            print(json.dumps({"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": 1, "steps": r["steps"], "warmup": 5,
+                              "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                              "dtype": r["dtype"], "data": "synthetic", "config": r["config"], "gpu_launches": r["gpu_launches_per_step"] * r["steps"],
+                              "roofline": r.get("roofline"), "kernel_classes": r["kernel_classes"], "note": r["note"]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
     field_cache = {}
     head = measure(args.workload, args, local, world, rank, field_cache, headline=True)
     subs = []
     if args.workload == "c2" and args.sub != "none":
         for name in [s for s in args.sub.split(",") if s]:
             try:
+                if name in SMALL:
+                    if rank == 0:
+                        subs.append(measure_small(name, args, local))
+                    continue
                 r = measure(name, args, local, world, rank, field_cache, headline=False)
                 subs.append({k: r[k] for k in ("workload", "dtype", "value", "unit", "steps", "ms_per_step", "config", "e2e",
                                                "gpu_launches", "bad_cells", "roofline", "step_roofline", "kernel_classes")})

@@ -2,7 +2,8 @@
 // Counts the floating-point operations the oracle performs, by compiling the very same
 // source (mhd_oracle.c) with `real` replaced by a counting type.  Used to state the
 // ALGORITHMIC flops per cell-update in DESIGN.md / bench.py's roofline; it is not part
-// of the product path.   g++ -O1 -std=c++17 oracle/opcount.cpp -o oracle/opcount && oracle/opcount
+// of the product path.   g++ -O1 -std=c++17 oracle/opcount.cpp -o oracle/opcount && oracle/opcount [n [2d]]
+// ("2d": patches of n x n x 1 cells, z collapsed -- the count behind the 2D tile kernel's roofline)
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -48,13 +49,15 @@ static void show(const char* name, Ops o, double per) {
 
 int main(int argc, char** argv) {
   const int n = argc > 1 ? std::atoi(argv[1]) : 32;
+  const bool two_d = argc > 2 && std::strcmp(argv[2], "2d") == 0;
   // a smooth, fully three-dimensional state on 2 patches of n^3 (values only matter
   // for which HLLD branch is taken; the count per call is branch-independent up to selects)
   orc_desc d;
   std::memset(&d, 0, sizeof d);
   d.n[0] = d.n[1] = d.n[2] = n; d.ng = 3; d.npatch = 2; d.limiter = 1; d.emf_solver = 0;
+  if (two_d) d.n[2] = 1;
   d.gamma = 5.0 / 3.0; d.dx[0] = d.dx[1] = d.dx[2] = 1.0 / (2 * n);
-  const long m = n + 6, M = m * m * m;
+  const long m = n + 6, M = m * m * (two_d ? 1 : m);
   std::vector<Counted> U(8 * 2 * M), V(8 * 2 * M);
   for (int f = 0; f < 8; ++f)
     for (long c = 0; c < 2 * M; ++c) {
@@ -62,7 +65,7 @@ int main(int argc, char** argv) {
       const double base[8] = {1.0, 0.3, -0.2, 0.1, 3.0, 0.1, 0.05, -0.07};
       U[f * 2 * M + c] = base[f] * (1.0 + 0.1 * std::sin(x + f));
     }
-  const double cells = 2.0 * n * n * n;
+  const double cells = 2.0 * n * n * (two_d ? 1 : n);
   Ops a = snap();
   orc_step(&d, U.data(), V.data(), 1e-3);
   Ops b = snap();
