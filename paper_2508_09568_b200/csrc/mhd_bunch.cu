@@ -287,6 +287,22 @@ inline unsigned blocks_for(long long threads, int bs) { return (unsigned)((threa
 template <typename T>
 int launch_fill(mhd_bunch* b) {
   const Geom& G = b->G;
+  const int vec = (int)(16 / sizeof(T));
+  // every neighbour present and rows made of whole 16-byte chunks: the chunked fill (aligned 16-byte
+  // accesses, x-guards included); otherwise cell by cell (zero-gradient sides, ragged rows)
+  const bool chunked = b->all_nbr && G.act[0] && G.n[0] % vec == 0 && (G.lead + G.g[0]) % vec == 0 && G.pitch % vec == 0 &&
+                       G.ps % vec == 0 && G.fs % vec == 0 && ((uintptr_t)b->state[b->cur] & 15) == 0;
+  if (chunked) {
+    const int cpr = G.pitch / vec, lg = (G.lead + G.g[0]) / vec, ni = G.n[0] / vec;
+    const long long per = (long long)(G.m[1] * G.m[2] - G.n[1] * G.n[2]) * cpr + (long long)G.n[1] * G.n[2] * (cpr - ni);
+    (void)lg;
+    if (per > 0) {
+      LaunchScope ls(b, KC_FILL);
+      k_fill_guards_vec<T><<<blocks_for(per * G.np, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return MHD_OK;
+  }
   const FillMap M = make_fill_map(G);
   const long long tot = (long long)M.start[6] * G.np;
   if (tot > 0) {

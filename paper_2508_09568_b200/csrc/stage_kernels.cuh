@@ -89,6 +89,63 @@ __global__ void __launch_bounds__(256) k_fill_guards(Geom G, FillMap M, T* __res
   }
 }
 
+// The same fill in 16-byte chunks, for bunches whose every neighbour exists (no zero-gradient side) and
+// whose rows are whole chunks (n_x a multiple of 16 / sizeof(T); lead pad + guard width = 4 elements).
+// A row of the padded patch is CPR chunks: LG chunks of low x-guards (with the lead pad), n_x / VEC
+// interior chunks, HG chunks of high x-guards (with the trailing pad).  Guard ROWS (y or z outside the
+// interior) are copied whole, chunk by chunk, from the row of the neighbour of class (o_x of the
+// chunk, o_y, o_z); interior rows only get their LG + HG guard chunks.  Every chunk of a destination
+// row comes from ONE chunk of a source row (the guard chunks of a row are the interior chunks at the
+// far / near end of the x-neighbour's row), so the x-guards -- 12-byte fragments that cost whole
+// sectors in the scalar kernel -- move as aligned 16-byte accesses like everything else.  Pad
+// elements receive copies of interior values nobody reads.  A thread moves one chunk of all 8 fields.
+template <typename T>
+__global__ void __launch_bounds__(256) k_fill_guards_vec(Geom G, T* __restrict__ U, const int* __restrict__ nbr) {
+  constexpr int VEC = 16 / sizeof(T);
+  using V = int4;
+  const int nx = G.n[0], ny = G.n[1], nz = G.n[2], g1 = G.g[1], g2 = G.g[2], my = G.m[1];
+  const int CPR = G.pitch / VEC, LG = (G.lead + G.g[0]) / VEC, NI = nx / VEC, HG = CPR - LG - NI;
+  const int nfull = my * G.m[2] - ny * nz;                 // guard rows of a patch
+  const int per = nfull * CPR + ny * nz * (LG + HG);
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long long)per * G.np) return;
+  const int p = (int)(t / per);
+  int r = (int)(t - (long long)p * per);
+  int jj, kk, c;                                           // padded row (jj, kk), chunk of the row
+  if (r < nfull * CPR) {
+    int fr = r / CPR;
+    c = r - fr * CPR;
+    if (fr < g2 * my) { kk = fr / my; jj = fr - kk * my; }
+    else if (fr < 2 * g2 * my) { fr -= g2 * my; kk = fr / my; jj = fr - kk * my; kk += g2 + nz; }
+    else {
+      fr -= 2 * g2 * my;
+      kk = fr / (2 * g1);
+      const int s_ = fr - kk * 2 * g1;
+      kk += g2;
+      jj = s_ < g1 ? s_ : ny + s_;
+    }
+  } else {
+    r -= nfull * CPR;
+    const int ir = r / (LG + HG), cc = r - ir * (LG + HG);
+    kk = g2 + ir / ny;
+    jj = g1 + ir - (ir / ny) * ny;
+    c = cc < LG ? cc : NI + cc;
+  }
+  const int j = jj - g1, k = kk - g2;
+  const int ox = c < LG ? -1 : (c >= LG + NI ? 1 : 0);
+  const int oy = j < 0 ? -1 : (j >= ny ? 1 : 0), oz = k < 0 ? -1 : (k >= nz ? 1 : 0);
+  const int q = nbr[p * 27 + (oz + 1) * 9 + (oy + 1) * 3 + (ox + 1)];
+  const long long plane = (long long)G.pitch * my;
+  const long long dst = (long long)p * G.ps + (long long)kk * plane + (long long)jj * G.pitch + (long long)c * VEC;
+  const long long from = (long long)q * G.ps + (long long)(kk - oz * nz) * plane + (long long)(jj - oy * ny) * G.pitch +
+                         (long long)(c - ox * NI) * VEC;
+  V v[8];
+#pragma unroll
+  for (int f = 0; f < 8; ++f) v[f] = *reinterpret_cast<const V*>(U + f * G.fs + from);
+#pragma unroll
+  for (int f = 0; f < 8; ++f) *reinterpret_cast<V*>(U + f * G.fs + dst) = v[f];
+}
+
 // O10, local time steps: guard fill of the NEWER slice of each listed
 // patch from its neighbours' two slices, linearly interpolated in time to the patch's own time.
 // S0/S1: the two state buffers; slot[q]: which of them holds the newer slice of patch q;
