@@ -37,7 +37,7 @@ constexpr int TILE_SLOTS = 42;
 
 template <typename T, int TX, int TY> struct TileCfg {
   static constexpr int TP = TX + 6, TH = TY + 6, AR = TP * TH;
-  static constexpr int NTH = sizeof(T) == 4 ? 512 : 384;
+  static constexpr int NTH = sizeof(T) == 4 ? 704 : 384;
   static constexpr size_t smem = sizeof(T) * (size_t)(8 + TILE_SLOTS) * AR;
   static_assert(smem <= 227 * 1024, "shared memory of one CTA");
 };
