@@ -387,7 +387,7 @@ def measure_small(name, args, local):
         rec["roofline"] = {"kernel": "step_tile2d", "bound": "alu", "achieved": STEP_FLOPS_2D * w.cells / (tk * 1e-3) / 1e12,
                            "peak": alu_peak, "unit": "TFLOP/s", "frac": STEP_FLOPS_2D * w.cells / (tk * 1e-3) / 1e12 / alu_peak,
                            "peak_source": "measured FMA chain (mhd_bunch_measure_alu_peak), FMA = 2 flops",
-                           "alg_flops_per_launch": STEP_FLOPS_2D * w.cells, "avg_launch_ms": tk, "traffic": None,
+                           "alg_flops_per_launch": STEP_FLOPS_2D * w.cells, "avg_launch_ms": tk, "traffic": ncu_traffic(name, "step_tile2d"), "traffic_source": TRAFFIC_FILE,
                            "share_of_step": tk / sum(c["ms_per_step"] for c in classes.values())}
     b.close()
     del b
