@@ -257,9 +257,10 @@ def test_3d_bunch_with_outflow_sides(sides, path, dtype):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_fused_tiles_cover_large_and_odd_patches(dtype):
-    """Patch sizes that need several (x,y) tiles of the fused kernel with ragged edges:
-    40 x 20 x 12 cells (x tiles 32+8, y tiles 8+8+4) and 64 x 8 x 8."""
-    for N, n in (((80, 40, 24), (40, 20, 12)), ((64, 16, 16), (64, 8, 8))):
+    """Patch sizes that need several (x,y) tiles of the fused kernels with ragged edges: 40 x 20 x 12
+    cells and 64 x 8 x 8; 24^3 (the paper's patch size), 24 x 40 x 12 and 48 x 24 x 10."""
+    for N, n in (((80, 40, 24), (40, 20, 12)), ((64, 16, 16), (64, 8, 8)), ((48, 48, 48), (24, 24, 24)),
+                 ((48, 40, 24), (24, 40, 12)), ((48, 48, 20), (48, 24, 10))):
         w = W.turbulence(N=N, n=n, dtype=NPD[dtype])
         o = make_oracle(w)
         U = o.fill_guards(w.U.astype(np.float64), w.nbr)
