@@ -448,11 +448,20 @@ template <typename T> struct Tile2D { static constexpr int TX = 32, TY = sizeof(
 template <typename T>
 int prepare_tile2d() {
   using C = TileCfg<T, Tile2D<T>::TX, Tile2D<T>::TY>;
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
   return MHD_OK;
 }
+// Small 2D bunches are bound by launch latency: there the tile kernel's CFL epilogue replaces two launches
+// of the next cfl_dt (config 1: 31 -> 24 us per step in fp32).  On bunches of many waves the stand-alone
+// pass is as cheap (fp64 2048^2: 2.08 against 2.14 ms per step), so the epilogue is used up to 8 waves.
+template <typename T> bool tile2d_wants_cfl(const mhd_bunch* b) {
+  const long long tiles = (long long)((b->G.n[0] + Tile2D<T>::TX - 1) / Tile2D<T>::TX) * ((b->G.n[1] + Tile2D<T>::TY - 1) / Tile2D<T>::TY) * b->G.np;
+  return tiles <= 8ll * b->nsm;
+}
+// cfle: the kernel also reduces the CFL rates of the level it writes into d_rate_next (cleared by k_set_dt)
 template <typename T>
-int launch_tile2d(mhd_bunch* b, int p0, int npl) {
+int launch_tile2d(mhd_bunch* b, int p0, int npl, bool cfle = false) {
   constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY;
   using C = TileCfg<T, TX, TY>;
   const Geom& G = b->G;
@@ -461,8 +470,9 @@ int launch_tile2d(mhd_bunch* b, int p0, int npl) {
   dim3 grid((unsigned)(xt * yt), (unsigned)npl, 1);
   {
     LaunchScope ls(b, KC_TILE2D);
-    k_step_tile2d<T, TX, TY><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, (b->gather_t_ok && !b->ov_plist) ? 1 : 0, b->d_dt + 1,
-                                                                  b->d_bad, xt);
+    const int gather = (b->gather_t_ok && !b->ov_plist) ? 1 : 0;
+    if (cfle) k_step_tile2d<T, TX, TY, true><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt);
+    else k_step_tile2d<T, TX, TY, false><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt);
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;
@@ -618,10 +628,12 @@ int launch_step(mhd_bunch* b) {
     return MHD_OK;
   }
   if (path == MHD_PATH_TILE2D && b->gather_t_ok) {
-    const int rc = launch_tile2d<T>(b, 0, G.np);
+    const bool cfle = tile2d_wants_cfl<T>(b);
+    const int rc = launch_tile2d<T>(b, 0, G.np, cfle);
     if (rc != MHD_OK) return rc;
     b->cur = 1 - b->cur;
     b->guards_stale = false;
+    b->rate_valid = cfle;      // every patch went through the tile kernel's CFL epilogue since the last k_set_dt
     return MHD_OK;
   }
   {  // every other route reads the guard shell from HBM
@@ -636,8 +648,10 @@ int launch_step(mhd_bunch* b) {
     return MHD_OK;
   }
   {
-    const int rc = path == MHD_PATH_TILE2D ? launch_tile2d<T>(b, 0, G.np) : launch_staged_range<T>(b, 0, G.np);
+    const bool cfle = path == MHD_PATH_TILE2D && tile2d_wants_cfl<T>(b);
+    const int rc = path == MHD_PATH_TILE2D ? launch_tile2d<T>(b, 0, G.np, cfle) : launch_staged_range<T>(b, 0, G.np);
     if (rc != MHD_OK) return rc;
+    b->rate_valid = cfle;
   }
   CUDA_TRY(cudaGetLastError());
   b->cur = 1 - b->cur;

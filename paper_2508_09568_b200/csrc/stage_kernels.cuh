@@ -362,6 +362,7 @@ template <typename T> struct HbmAcc {
   }
   __device__ __forceinline__ const T* u(int f) const { return U + f * ufs + cu; }
   __device__ __forceinline__ T* un(int f) const { return Un + f * ufs + cu; }
+  __device__ __forceinline__ T* keep(int f) const { return Un + f * ufs + cu; }     // (unused: KEEP is false here)
   __device__ __forceinline__ T* w(int a) const { return W + a * wfs + cw; }
   __device__ __forceinline__ long long s(int d) const { return st[d]; }
 };
@@ -550,13 +551,14 @@ __device__ __forceinline__ void st_emf(const Params<T>& P, const X& x) {
 }
 
 // O8: conservative update + constrained transport with the metric factor of each term
-// (Eq. 12; L154).  xlim/ylim: faces up to n along x/y are written (a tile that does
-// not end its patch leaves its last column/row of faces to the next tile: pass n-1 there)
-template <typename T, typename X>
-__device__ __forceinline__ void st_update(const Params<T>& P, const X& x, int i, int j, int k, T dt) {
+// (Eq. 12; L154).  what: bit 0 the hydro fields, bit 1+a the face field b_a; store:
+// write U^{n+1}; KEEP: also leave the new values in x.keep(f) (the tile kernel reduces the CFL rates of
+// the new level from them, and forms -- without storing -- the faces another tile owns).
+template <typename T, bool KEEP, typename X>
+__device__ __forceinline__ void st_update(const Params<T>& P, const X& x, int i, int j, int k, T dt, int what = 15, bool store = true) {
   const Geom& G = P.G;
   const int cc[3] = {i, j, k};
-  if (inside(G, i, j, k, 0, 0)) {
+  if ((what & 1) && inside(G, i, j, k, 0, 0)) {
 #pragma unroll
     for (int f = 0; f < 5; ++f) {
       T v = x.u(f)[0];
@@ -566,12 +568,14 @@ __device__ __forceinline__ void st_update(const Params<T>& P, const X& x, int i,
         const T* fl = x.w(W_FLUX + d * 5 + f);
         v -= dt * P.idx[d] * (fl[x.s(d)] - fl[0]);
       }
-      x.un(f)[0] = v;
+      if (store) x.un(f)[0] = v;
+      if (KEEP) x.keep(f)[0] = v;
     }
   }
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const int b = (a + 1) % 3, e = (a + 2) % 3;
+    if (!(what & (2 << a))) continue;
     // faces 0..n along a (n = closing face), interior transversally
     bool ok = true;
 #pragma unroll
@@ -583,7 +587,9 @@ __device__ __forceinline__ void st_update(const Params<T>& P, const X& x, int i,
     T curl = T(0);
     if (G.act[b]) curl += (Ee[x.s(b)] - Ee[0]) * P.idx[b];
     if (G.act[e]) curl -= (Eb[x.s(e)] - Eb[0]) * P.idx[e];
-    x.un(5 + a)[0] = x.u(5 + a)[0] + dt * curl;
+    const T v = x.u(5 + a)[0] + dt * curl;
+    if (store) x.un(5 + a)[0] = v;
+    if (KEEP) x.keep(5 + a)[0] = v;
   }
 }
 
@@ -622,7 +628,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) k_update(Params<T> P, Box B, const double* __restrict__ dtp) {
   int pl, i, j, k; long long c;
   if (!decode(P.G, B, P.npl, (long long)blockIdx.x * blockDim.x + threadIdx.x, pl, i, j, k, c)) return;
-  st_update<T>(P, HbmAcc<T>(P, pl, c), i, j, k, P.dt_of(pl, dtp));
+  st_update<T, false>(P, HbmAcc<T>(P, pl, c), i, j, k, P.dt_of(pl, dtp));
 }
 
 }  // namespace mhd

@@ -49,14 +49,20 @@ template <typename T, int AR, int TP> struct TileAcc {
   long long ufs;
   __device__ __forceinline__ const T* u(int f) const { return raw + f * AR; }
   __device__ __forceinline__ T* un(int f) const { return Un + f * ufs; }
+  __device__ __forceinline__ T* keep(int f) const { return const_cast<T*>(raw) + f * AR; }   // new value over the old one
   __device__ __forceinline__ T* w(int a) const { return W + tile_slot(a) * AR; }
   __device__ __forceinline__ long long s(int d) const { return d == 0 ? 1 : (d == 1 ? TP : 0); }
 };
 
-template <typename T, int TX, int TY>
+// CFLE: reduce the CFL rates of the NEW level in the kernel's epilogue (per-patch integer atomicMax on the
+// bit pattern, as k_cfl does), so that the next mhd_bunch_cfl_dt only runs the bunch-wide reduction: the
+// update leaves the new values in the raw tile (each thread over its own old values), the faces on the
+// tile's upper sides that another tile stores are formed without being stored, and cfl_rate -- the same
+// explicitly rounded function k_cfl evaluates -- gets the same inputs, hence the same bits.
+template <typename T, int TX, int TY, bool CFLE>
 __global__ void __launch_bounds__(TileCfg<T, TX, TY>::NTH, 1)
 k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
-              unsigned long long* __restrict__ bad, int xtiles) {
+              unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles) {
   using C = TileCfg<T, TX, TY>;
   constexpr int TP = C::TP, TH = C::TH, AR = C::AR, NTH = C::NTH;
   extern __shared__ __align__(16) unsigned char tile_smem[];
@@ -156,7 +162,25 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
   }
   __syncthreads();
   // O8: the tile's cells and lower faces; the closing faces where the tile ends its patch
-  TILE_FOR(x0, x0 + tw - 1 + (lastx ? 1 : 0), y0, y0 + th - 1 + (lasty ? 1 : 0), st_update<T>(P, x, i, j, 0, dt));
+  TILE_FOR(x0, x0 + tw - 1 + (lastx ? 1 : 0), y0, y0 + th - 1 + (lasty ? 1 : 0), (st_update<T, CFLE>(P, x, i, j, 0, dt)));
+  if (CFLE) {
+    // b_x on the tile's last column of faces and b_y on its last row, where the next tile stores them
+    if (!lastx) TILE_FOR(x0 + tw, x0 + tw, y0, y0 + th - 1, (st_update<T, true>(P, x, i, j, 0, dt, 2, false)));
+    if (!lasty) TILE_FOR(x0, x0 + tw - 1, y0 + th, y0 + th, (st_update<T, true>(P, x, i, j, 0, dt, 4, false)));
+    __syncthreads();
+    T rmax = T(0);
+    for (int it = t; it < tw * th; it += NTH) {
+      const int jj = it / tw;
+      const T* c = raw + (jj + 3) * TP + (it - jj * tw + 3);
+      const T rate = cfl_rate<T>(P.gamma, P.idx[0], P.idx[1], P.idx[2], true, true, false, c[0], c[AR], c[2 * AR], c[3 * AR], c[4 * AR],
+                                 c[5 * AR], c[5 * AR + 1], c[6 * AR], c[6 * AR + TP], c[7 * AR], c[7 * AR]);
+      rmax = num<T>::max(rmax, rate);
+    }
+    double rd = (double)rmax;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) rd = fmax(rd, __shfl_xor_sync(0xffffffffu, rd, o));
+    if ((t & 31) == 0 && rd > 0.0) atomicMax(&rate_next[P.patch(pl)], enc_max(rd));
+  }
 #undef TILE_FOR
 }
 

@@ -123,3 +123,29 @@ def test_tile2d_defers_the_fill_too(name, dtype):
     assert launches[0] < launches[1]                                   # no k_fill_guards in the deferred loop
     ref = o.fill_guards(outs[0].astype(np.float64).copy(), w.nbr)
     assert np.array_equal(outs[0].astype(np.float64), ref)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["ot64", "ot_ragged", "ot_wide"])
+def test_tile2d_cfl_epilogue_gives_the_standalone_pass_bit_for_bit(name, dtype):
+    """The tile kernel reduces the CFL rates of the level it writes (O9), so the next cfl_dt is
+    one small launch; the step it returns equals, bit for bit, the one k_cfl computes from the stored state."""
+    w = workloads_2d(dtype)[name]
+    b = make_gpu(w, dtype)
+    for _ in range(2):
+        b.fill_guards(); b.cfl_dt(0.4, sync=False); b.step_dev()
+    b.fill_guards()
+    l0 = b.launches
+    dt1 = b.cfl_dt(0.4, sync=True)
+    assert b.launches - l0 == 1                      # k_cfl_final only
+    U = b.download()
+    b.load(U)                                        # the caller wrote the buffer: the rates are no longer trusted
+    b.fill_guards()
+    l0 = b.launches
+    dt2 = b.cfl_dt(0.4, sync=True)
+    assert b.launches - l0 >= 3                      # zero, k_cfl, k_cfl_final
+    assert dt1 == dt2
+    o = make_oracle(w)
+    ref = o.cfl_dt(o.fill_guards(U.astype(np.float64), w.nbr), 0.4)
+    assert abs(dt1 - ref) <= (1e-13 if dtype == "f64" else 2e-6) * ref
+    b.close()
