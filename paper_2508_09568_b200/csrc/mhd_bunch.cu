@@ -445,34 +445,47 @@ template <> struct OnePassLaunch<float> {
 // 2D bunches: one kernel, every stage on a shared-memory tile (tile_kernel.cuh).  fp32 32 x 16 tiles,
 // fp64 32 x 8 (the tile with its halo and 50 arrays has to fit in 227 KB).
 template <typename T> struct Tile2D { static constexpr int TX = 32, TY = sizeof(T) == 4 ? 16 : 8; };
+// fp32: persistent CTAs with two raw buffers (the next tile is prefetched); fp64: one tile per CTA (a second raw
+// buffer does not fit beside the 42 scratch arrays of a 32 x 8 tile)
+template <typename T> struct Tile2DBuf { static constexpr int N = sizeof(T) == 4 ? 2 : 1; };
 template <typename T>
 int prepare_tile2d() {
-  using C = TileCfg<T, Tile2D<T>::TX, Tile2D<T>::TY>;
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, Tile2D<T>::TX, Tile2D<T>::TY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem));
+  constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY, NB = Tile2DBuf<T>::N;
+  using C1 = TileCfg<T, TX, TY, 1>;
+  using C2 = TileCfg<T, TX, TY, NB>;
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
   return MHD_OK;
 }
 // Small 2D bunches are bound by launch latency: there the tile kernel's CFL epilogue replaces two launches
 // of the next cfl_dt (config 1: 31 -> 24 us per step in fp32).  On bunches of many waves the stand-alone
 // pass is as cheap (fp64 2048^2: 2.08 against 2.14 ms per step), so the epilogue is used up to 8 waves.
-template <typename T> bool tile2d_wants_cfl(const mhd_bunch* b) {
-  const long long tiles = (long long)((b->G.n[0] + Tile2D<T>::TX - 1) / Tile2D<T>::TX) * ((b->G.n[1] + Tile2D<T>::TY - 1) / Tile2D<T>::TY) * b->G.np;
-  return tiles <= 8ll * b->nsm;
+template <typename T> long long tile2d_tiles(const mhd_bunch* b, int npl) {
+  return (long long)((b->G.n[0] + Tile2D<T>::TX - 1) / Tile2D<T>::TX) * ((b->G.n[1] + Tile2D<T>::TY - 1) / Tile2D<T>::TY) * npl;
 }
+template <typename T> bool tile2d_wants_cfl(const mhd_bunch* b) { return tile2d_tiles<T>(b, b->G.np) <= 8ll * b->nsm; }
 // cfle: the kernel also reduces the CFL rates of the level it writes into d_rate_next (cleared by k_set_dt)
 template <typename T>
 int launch_tile2d(mhd_bunch* b, int p0, int npl, bool cfle = false) {
-  constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY;
-  using C = TileCfg<T, TX, TY>;
+  constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY, NB = Tile2DBuf<T>::N;
   const Geom& G = b->G;
   Params<T> P = make_params<T>(b, p0, npl);
   const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
-  dim3 grid((unsigned)(xt * yt), (unsigned)npl, 1);
+  const long long tiles = tile2d_tiles<T>(b, npl);
+  const int gather = (b->gather_t_ok && !b->ov_plist) ? 1 : 0;
+  // more than two waves of tiles: persistent CTAs that prefetch (where a second raw buffer fits)
+  const bool persist = NB == 2 && !cfle && tiles > 2ll * b->nsm;
   {
     LaunchScope ls(b, KC_TILE2D);
-    const int gather = (b->gather_t_ok && !b->ov_plist) ? 1 : 0;
-    if (cfle) k_step_tile2d<T, TX, TY, true><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt);
-    else k_step_tile2d<T, TX, TY, false><<<grid, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt);
+    if (persist) {
+      using C = TileCfg<T, TX, TY, NB>;
+      k_step_tile2d<T, TX, TY, false, NB><<<(unsigned)b->nsm, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+    } else {
+      using C = TileCfg<T, TX, TY, 1>;
+      if (cfle) k_step_tile2d<T, TX, TY, true, 1><<<(unsigned)tiles, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+      else k_step_tile2d<T, TX, TY, false, 1><<<(unsigned)tiles, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+    }
   }
   CUDA_TRY(cudaGetLastError());
   return MHD_OK;

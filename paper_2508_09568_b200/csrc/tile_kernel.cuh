@@ -35,12 +35,22 @@ __host__ __device__ constexpr int tile_slot(int a) {
 }
 constexpr int TILE_SLOTS = 42;
 
-template <typename T, int TX, int TY> struct TileCfg {
+// NBUF raw-tile buffers: 1 = one tile per CTA, loaded with plain loads; 2 = PERSISTENT CTAs (one per SM) that
+// walk the tiles and fetch the next tile's U^n with asynchronous copies (cp.async) while the current one
+// is computed -- with one CTA per SM (shared memory) the load of a tile and the drain of its stores are
+// otherwise fully exposed (30 % of the kernel's stall samples on a 2048^2 bunch).
+template <typename T, int TX, int TY, int NBUF = 1> struct TileCfg {
   static constexpr int TP = TX + 6, TH = TY + 6, AR = TP * TH;
   static constexpr int NTH = sizeof(T) == 4 ? 704 : 384;
-  static constexpr size_t smem = sizeof(T) * (size_t)(8 + TILE_SLOTS) * AR;
+  static constexpr size_t smem = sizeof(T) * (size_t)(8 * NBUF + TILE_SLOTS) * AR;
   static_assert(smem <= 227 * 1024, "shared memory of one CTA");
 };
+__device__ __forceinline__ void tile_cp_async(float* dst, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void tile_cp_async(double* dst, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
 
 template <typename T, int AR, int TP> struct TileAcc {
   const T* raw;   // [8][AR] at the cell
@@ -59,47 +69,68 @@ template <typename T, int AR, int TP> struct TileAcc {
 // update leaves the new values in the raw tile (each thread over its own old values), the faces on the
 // tile's upper sides that another tile stores are formed without being stored, and cfl_rate -- the same
 // explicitly rounded function k_cfl evaluates -- gets the same inputs, hence the same bits.
-template <typename T, int TX, int TY, bool CFLE>
+template <typename T, int TX, int TY, bool CFLE, int NBUF>
 __global__ void __launch_bounds__(TileCfg<T, TX, TY>::NTH, 1)
 k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
-              unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles) {
-  using C = TileCfg<T, TX, TY>;
+              unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int ytiles) {
+  using C = TileCfg<T, TX, TY, NBUF>;
   constexpr int TP = C::TP, TH = C::TH, AR = C::AR, NTH = C::NTH;
   extern __shared__ __align__(16) unsigned char tile_smem[];
-  T* const raw = reinterpret_cast<T*>(tile_smem);
-  T* const W = raw + 8 * AR;
+  T* const raw_all = reinterpret_cast<T*>(tile_smem);
+  T* const W = raw_all + NBUF * 8 * AR;
   const Geom& G = P.G;
   const int nx = G.n[0], ny = G.n[1];
-  const int pl = blockIdx.y;
-  const int xt = blockIdx.x % xtiles, yt = blockIdx.x / xtiles;
+  const int t = threadIdx.x;
+  const int ntile = xtiles * ytiles * P.npl;
+
+  // U^n of cells [x0-3, x0+tw+2] x [y0-3, y0+th+2] of a tile -> a raw buffer.  GATHER mode: a cell outside the
+  // patch is read from the interior of the neighbour of its class (guard fill O1 folded into the load:
+  // PAPER.md L124, L188, L241), so the guard shell in HBM is neither written nor read; otherwise the patch's
+  // own (already filled) guard cells are read.
+  auto fetch = [&](int tile, T* dst) {
+    const int pl_ = tile / (xtiles * ytiles), rt = tile - pl_ * (xtiles * ytiles);
+    const int yt_ = rt / xtiles, xt_ = rt - yt_ * xtiles;
+    const int X0 = xt_ * TX, Y0 = yt_ * TY;
+    const long long pb = (long long)P.patch(pl_) * G.ps + G.lead;
+    for (int idx = t; idx < AR; idx += NTH) {
+      const int lr = idx / TP, lc = idx - lr * TP;
+      const int i = X0 - 3 + lc, j = Y0 - 3 + lr;
+      if (i <= nx + 2 && j <= ny + 2) {
+        long long g = pb + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
+        if (gather) {
+          const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0), oy = j < 0 ? -1 : (j >= ny ? 1 : 0);
+          if (ox | oy) {
+            const int q = nbr[(long long)P.patch(pl_) * 27 + 9 + (oy + 1) * 3 + (ox + 1)];
+            g = (long long)q * G.ps + G.lead + (i - ox * nx + G.g[0]) + (long long)(j - oy * ny + G.g[1]) * G.pitch;
+          }
+        }
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+          if (NBUF == 1) dst[f * AR + idx] = P.U[f * G.fs + g];
+          else tile_cp_async(dst + f * AR + idx, P.U + f * G.fs + g);
+        }
+      }
+    }
+  };
+  if (NBUF == 2 && (int)blockIdx.x < ntile) fetch(blockIdx.x, raw_all);
+
+  int nb = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, nb ^= (NBUF - 1)) {
+  T* const raw = raw_all + nb * 8 * AR;
+  const int pl = tile / (xtiles * ytiles), rt_ = tile - pl * (xtiles * ytiles);
+  const int yt = rt_ / xtiles, xt = rt_ - yt * xtiles;
   const int x0 = xt * TX, y0 = yt * TY;
   const int tw = min(TX, nx - x0), th = min(TY, ny - y0);
   const bool lastx = x0 + tw == nx, lasty = y0 + th == ny;
-  const int t = threadIdx.x;
   const T dt = P.dt_of(pl, dtp);
   const long long pbase = (long long)P.patch(pl) * G.ps + G.lead;
-
-  // U^n of cells [x0-3, x0+tw+2] x [y0-3, y0+th+2] -> raw tile.  GATHER mode: a cell outside the patch is
-  // read from the interior of the neighbour of its class (guard fill O1 folded into the load: PAPER.md
-  // L124, L188, L241), so the guard shell in HBM is neither written nor read; otherwise the patch's own
-  // (already filled) guard cells are read.
-  for (int idx = t; idx < AR; idx += NTH) {
-    const int lr = idx / TP, lc = idx - lr * TP;
-    const int i = x0 - 3 + lc, j = y0 - 3 + lr;
-    if (i <= nx + 2 && j <= ny + 2) {
-      long long g = pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
-      if (gather) {
-        const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0), oy = j < 0 ? -1 : (j >= ny ? 1 : 0);
-        if (ox | oy) {
-          const int q = nbr[(long long)P.patch(pl) * 27 + 9 + (oy + 1) * 3 + (ox + 1)];
-          g = (long long)q * G.ps + G.lead + (i - ox * nx + G.g[0]) + (long long)(j - oy * ny + G.g[1]) * G.pitch;
-        }
-      }
-#pragma unroll
-      for (int f = 0; f < 8; ++f) raw[f * AR + idx] = P.U[f * G.fs + g];
-    }
+  if (NBUF == 1) {
+    fetch(tile, raw);
+  } else {
+    asm volatile("cp.async.wait_all;" ::: "memory");
   }
-  __syncthreads();
+  __syncthreads();     // the tile has landed; every thread is done with the previous tile (its W arrays, its raw buffer)
+  if (NBUF == 2 && tile + (int)gridDim.x < ntile) fetch(tile + gridDim.x, raw_all + (nb ^ 1) * 8 * AR);
 
   // a stage over the cells [ilo, ihi] x [jlo, jhi] of the patch
   auto acc = [&](int i, int j) {
@@ -181,6 +212,7 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
     for (int o = 16; o > 0; o >>= 1) rd = fmax(rd, __shfl_xor_sync(0xffffffffu, rd, o));
     if ((t & 31) == 0 && rd > 0.0) atomicMax(&rate_next[P.patch(pl)], enc_max(rd));
   }
+  }   // tiles of this CTA
 #undef TILE_FOR
 }
 

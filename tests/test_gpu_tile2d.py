@@ -149,3 +149,37 @@ def test_tile2d_cfl_epilogue_gives_the_standalone_pass_bit_for_bit(name, dtype):
     ref = o.cfl_dt(o.fill_guards(U.astype(np.float64), w.nbr), 0.4)
     assert abs(dt1 - ref) <= (1e-13 if dtype == "f64" else 2e-6) * ref
     b.close()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("N,n", [(512, 32), (480, 20)])
+def test_tile2d_on_bunches_of_many_waves(N, n, dtype):
+    """More than two waves of tiles: in fp32 persistent CTAs walk the tiles and prefetch the next tile's U^n
+    with asynchronous copies while the current one is computed (two raw buffers); the CFL epilogue is off
+    beyond eight waves.  Two chained steps against the oracle, and the staged path to rounding."""
+    w = W.orszag_tang(N, n, dtype=NPD[dtype])
+    o = make_oracle(w)
+    U = w.U.astype(np.float64)
+    outs = {}
+    for path in ("tile2d", "staged"):
+        b = make_gpu(w, dtype, path=path)
+        V = U
+        for _ in range(2):
+            V = o.fill_guards(V, w.nbr) if path == "tile2d" else V
+            if path == "tile2d":
+                dt = o.cfl_dt(V, 0.4)
+                V = o.step(V, dt)
+                dts = outs.setdefault("dts", [])
+                dts.append(dt)
+            b.fill_guards()
+            b.step(outs["dts"][len(outs.get("n_" + path, []))])
+            outs.setdefault("n_" + path, []).append(1)
+        outs[path] = b.download()
+        if path == "tile2d":
+            ref = V
+        assert b.status() == 0
+        b.close()
+    assert rel_err(masked(outs["tile2d"], w.n), masked(ref, w.n)) <= TOL_STEP[dtype]
+    assert_nstep_parity(W.gather(outs["tile2d"], w.n, w.P), W.gather(ref, w.n, w.P), dtype, (N, n))
+    close = {"f64": 1e-14, "f32": 2e-6}[dtype]
+    assert rel_err(masked(outs["tile2d"], w.n), masked(outs["staged"], w.n).astype(np.float64)) <= close
