@@ -140,11 +140,23 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
     a.Un = P.Un + pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
     return a;
   };
+  // Task r of a w x h box -> (di, dj).  The first 32 columns go row by row, 32 tasks = one warp = one tile
+  // row (consecutive shared-memory words: no bank conflicts, also for the +-1 and +-TP neighbours); the
+  // remaining columns go column by column (stride TP = 38 words: 16 distinct banks before one repeats).
+  // Mapping tasks of a 33- to 36-wide box straight onto 38-word rows made 44 % of the kernel's shared-memory
+  // wavefronts bank-conflict replays.
+  auto task = [&](int r, int w, int h, int& di, int& dj) {
+    if (w <= 32) { dj = r / w; di = r - dj * w; }
+    else if (r < 32 * h) { dj = r >> 5; di = r & 31; }
+    else { r -= 32 * h; di = r / h; dj = r - di * h; di += 32; }
+  };
 #define TILE_FOR(ilo, ihi, jlo, jhi, BODY)                                   \
   {                                                                          \
     const int ni_ = (ihi) - (ilo) + 1, nj_ = (jhi) - (jlo) + 1;              \
     for (int it_ = t; it_ < ni_ * nj_; it_ += NTH) {                         \
-      const int jj_ = it_ / ni_, i = (ilo) + it_ - jj_ * ni_, j = (jlo) + jj_; \
+      int di_, dj_;                                                          \
+      task(it_, ni_, nj_, di_, dj_);                                         \
+      const int i = (ilo) + di_, j = (jlo) + dj_;                            \
       const TileAcc<T, AR, TP> x = acc(i, j);                                \
       BODY;                                                                  \
     }                                                                        \
@@ -157,38 +169,35 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
   __syncthreads();
   TILE_FOR(x0 - 1, x0 + tw + 1, y0 - 1, y0 + th + 1, st_predict<T>(P, x, i, j, 0, dt));
   __syncthreads();
-  // the five Riemann problems of the plane as one list of tasks: x and y faces, the three edges
+  // the five Riemann problems of the plane as ONE list of tasks over all threads: x faces (tw+1) x th, y faces
+  // tw x (th+1), x-directed edges tw x (th+1), y-directed edges (tw+1) x th, z-directed edges (tw+1) x (th+1).
+  // The row-by-row parts of all five come first (each a whole number of warps for a full tile), then their
+  // 33rd columns.
   {
-    const int n0 = (tw + 1) * th, n1 = tw * (th + 1), n2 = (tw + 1) * (th + 1);
-    const int tot = 2 * n0 + 2 * n1 + n2;
-    for (int it = t; it < tot; it += NTH) {
-      int r = it;
-      if (r < n0) {                      // x faces: i in [x0, x0+tw], j in [y0, y0+th-1]
-        const int jj = r / (tw + 1);
-        st_flux<T, 0>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
-        continue;
+    // (scalars, not arrays: nothing here may end up in local memory)
+    const int wA = tw + 1, wB = tw, hA = th, hB = th + 1;                       // widths / heights of the five boxes
+    const int m0 = min(wA, 32) * hA, m1 = min(wB, 32) * hB, m2 = m1, m3 = m0, m4 = min(wA, 32) * hB;
+    const int c0 = wA * hA - m0, c1 = wB * hB - m1, c2 = c1, c3 = c0, c4 = wA * hB - m4;
+    const int M1 = m0, M2 = M1 + m1, M3 = M2 + m2, M4 = M3 + m3, M5 = M4 + m4;
+    const int C1 = M5 + c0, C2 = C1 + c1, C3 = C2 + c2, C4 = C3 + c3, C5 = C4 + c4;
+    for (int it = t; it < C5; it += NTH) {
+      int q, r;
+      if (it < M5) {
+        q = (it >= M1) + (it >= M2) + (it >= M3) + (it >= M4);
+        r = it - (q == 0 ? 0 : (q == 1 ? M1 : (q == 2 ? M2 : (q == 3 ? M3 : M4))));
+      } else {
+        q = (it >= C1) + (it >= C2) + (it >= C3) + (it >= C4);
+        r = it - (q == 0 ? M5 : (q == 1 ? C1 : (q == 2 ? C2 : (q == 3 ? C3 : C4)))) + (q == 0 ? m0 : (q == 1 ? m1 : (q == 2 ? m2 : (q == 3 ? m3 : m4))));
       }
-      r -= n0;
-      if (r < n1) {                      // y faces
-        const int jj = r / tw;
-        st_flux<T, 1>(P, acc(x0 + r - jj * tw, y0 + jj));
-        continue;
-      }
-      r -= n1;
-      if (r < n1) {                      // x-directed edges: i in [x0, x0+tw-1], j in [y0, y0+th]
-        const int jj = r / tw;
-        st_emf<T, 0>(P, acc(x0 + r - jj * tw, y0 + jj));
-        continue;
-      }
-      r -= n1;
-      if (r < n0) {                      // y-directed edges: i in [x0, x0+tw], j in [y0, y0+th-1]
-        const int jj = r / (tw + 1);
-        st_emf<T, 1>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
-        continue;
-      }
-      r -= n0;
-      const int jj = r / (tw + 1);       // z-directed edges: every corner of the tile
-      st_emf<T, 2>(P, acc(x0 + r - jj * (tw + 1), y0 + jj));
+      const int bwq = (q == 1 || q == 2) ? wB : wA, bhq = (q == 0 || q == 3) ? hA : hB;
+      int di, dj;
+      task(r, bwq, bhq, di, dj);
+      const TileAcc<T, AR, TP> x = acc(x0 + di, y0 + dj);
+      if (q == 0) st_flux<T, 0>(P, x);
+      else if (q == 1) st_flux<T, 1>(P, x);
+      else if (q == 2) st_emf<T, 0>(P, x);
+      else if (q == 3) st_emf<T, 1>(P, x);
+      else st_emf<T, 2>(P, x);
     }
   }
   __syncthreads();
