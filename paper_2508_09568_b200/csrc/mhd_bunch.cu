@@ -453,9 +453,12 @@ int prepare_tile2d() {
   constexpr int TX = Tile2D<T>::TX, TY = Tile2D<T>::TY, NB = Tile2DBuf<T>::N;
   using C1 = TileCfg<T, TX, TY, 1>;
   using C2 = TileCfg<T, TX, TY, NB>;
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
-  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
   return MHD_OK;
 }
 // Small 2D bunches are bound by launch latency: there the tile kernel's CFL epilogue replaces two launches
@@ -478,13 +481,21 @@ int launch_tile2d(mhd_bunch* b, int p0, int npl, bool cfle = false) {
   const bool persist = NB == 2 && !cfle && tiles > 2ll * b->nsm;
   {
     LaunchScope ls(b, KC_TILE2D);
+    // the limiter is a compile-time parameter of the kernel
+    auto go = [&](auto kern, unsigned grid, int nth, size_t smem) {
+      kern<<<grid, nth, smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+    };
+    const bool mm = G.limiter == 1;
     if (persist) {
       using C = TileCfg<T, TX, TY, NB>;
-      k_step_tile2d<T, TX, TY, false, NB><<<(unsigned)b->nsm, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+      if (mm) go(k_step_tile2d<T, TX, TY, false, NB, 1>, (unsigned)b->nsm, C::NTH, C::smem);
+      else go(k_step_tile2d<T, TX, TY, false, NB, 2>, (unsigned)b->nsm, C::NTH, C::smem);
     } else {
       using C = TileCfg<T, TX, TY, 1>;
-      if (cfle) k_step_tile2d<T, TX, TY, true, 1><<<(unsigned)tiles, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
-      else k_step_tile2d<T, TX, TY, false, 1><<<(unsigned)tiles, C::NTH, C::smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
+      if (cfle && mm) go(k_step_tile2d<T, TX, TY, true, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
+      else if (cfle) go(k_step_tile2d<T, TX, TY, true, 1, 2>, (unsigned)tiles, C::NTH, C::smem);
+      else if (mm) go(k_step_tile2d<T, TX, TY, false, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
+      else go(k_step_tile2d<T, TX, TY, false, 1, 2>, (unsigned)tiles, C::NTH, C::smem);
     }
   }
   CUDA_TRY(cudaGetLastError());

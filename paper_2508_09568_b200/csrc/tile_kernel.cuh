@@ -52,7 +52,8 @@ __device__ __forceinline__ void tile_cp_async(double* dst, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
 
-template <typename T, int AR, int TP> struct TileAcc {
+template <typename T, int AR, int TP, int LIM> struct TileAcc {
+  static constexpr int lim_kind = LIM;
   const T* raw;   // [8][AR] at the cell
   T* W;           // [TILE_SLOTS][AR] at the cell
   T* Un;          // U^{n+1} in HBM at the cell
@@ -62,6 +63,7 @@ template <typename T, int AR, int TP> struct TileAcc {
   __device__ __forceinline__ T* keep(int f) const { return const_cast<T*>(raw) + f * AR; }   // new value over the old one
   __device__ __forceinline__ T* w(int a) const { return W + tile_slot(a) * AR; }
   __device__ __forceinline__ long long s(int d) const { return d == 0 ? 1 : (d == 1 ? TP : 0); }
+  __device__ __forceinline__ bool act(int d) const { return d < 2; }      // x, y active; z collapsed: folds at compile time
 };
 
 // CFLE: reduce the CFL rates of the NEW level in the kernel's epilogue (per-patch integer atomicMax on the
@@ -69,7 +71,7 @@ template <typename T, int AR, int TP> struct TileAcc {
 // update leaves the new values in the raw tile (each thread over its own old values), the faces on the
 // tile's upper sides that another tile stores are formed without being stored, and cfl_rate -- the same
 // explicitly rounded function k_cfl evaluates -- gets the same inputs, hence the same bits.
-template <typename T, int TX, int TY, bool CFLE, int NBUF>
+template <typename T, int TX, int TY, bool CFLE, int NBUF, int LIM>
 __global__ void __launch_bounds__(TileCfg<T, TX, TY>::NTH, 1)
 k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
               unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int ytiles) {
@@ -135,7 +137,7 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
   // a stage over the cells [ilo, ihi] x [jlo, jhi] of the patch
   auto acc = [&](int i, int j) {
     const int o = (j - y0 + 3) * TP + (i - x0 + 3);
-    TileAcc<T, AR, TP> a;
+    TileAcc<T, AR, TP, LIM> a;
     a.raw = raw + o; a.W = W + o; a.ufs = G.fs;
     a.Un = P.Un + pbase + (i + G.g[0]) + (long long)(j + G.g[1]) * G.pitch;
     return a;
@@ -157,7 +159,7 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
       int di_, dj_;                                                          \
       task(it_, ni_, nj_, di_, dj_);                                         \
       const int i = (ilo) + di_, j = (jlo) + dj_;                            \
-      const TileAcc<T, AR, TP> x = acc(i, j);                                \
+      const TileAcc<T, AR, TP, LIM> x = acc(i, j);                                \
       BODY;                                                                  \
     }                                                                        \
   }
@@ -192,7 +194,7 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
       const int bwq = (q == 1 || q == 2) ? wB : wA, bhq = (q == 0 || q == 3) ? hA : hB;
       int di, dj;
       task(r, bwq, bhq, di, dj);
-      const TileAcc<T, AR, TP> x = acc(x0 + di, y0 + dj);
+      const TileAcc<T, AR, TP, LIM> x = acc(x0 + di, y0 + dj);
       if (q == 0) st_flux<T, 0>(P, x);
       else if (q == 1) st_flux<T, 1>(P, x);
       else if (q == 2) st_emf<T, 0>(P, x);
