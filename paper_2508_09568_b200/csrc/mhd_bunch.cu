@@ -396,12 +396,16 @@ template <> struct OnePassLaunch<float> {
       CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
+      CUDA_TRY(cudaFuncSetAttribute(k_step_onepass<float, TX, TY, OneTile::NPW, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem));
       return MHD_OK;
     }
     // the limiter and the CFL epilogue are compile-time parameters of the kernel
     auto kern = b->fused_cfl
                     ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, true> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>)
                     : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, false> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>);
+    // the default scheme (minmod, HLLD, HLLD-2D) has an instantiation with the solvers fixed at compile time
+    if (!b->fused_cfl && G.limiter == 1 && G.emf_solver == 0 && G.flux_solver == 0)
+      kern = k_step_onepass<float, TX, TY, OneTile::NPW, 1, false, true>;
     Params<float> P = make_params<float>(b, p0, npl);
     if (zhi < 0) zhi = G.n[2];
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;

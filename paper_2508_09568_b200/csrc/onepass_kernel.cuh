@@ -159,7 +159,9 @@ __device__ __forceinline__ T edge_field(const T* __restrict__ c, T s) {
 
 // LIM: limiter (1 minmod, 2 monotonised central), fixed at compile time; CFLE: reduce the CFL rates
 // of the new level in the epilogue (role C), so that mhd_bunch_cfl_dt has nothing left to read
-template <typename T, int TX, int TY, int NPW, int LIM, bool CFLE>
+// DEFS: the default solvers (HLLD at faces, HLLD-2D at edges) fixed at compile time instead of read from the
+// descriptor (2 % faster; instantiated for the default limiter without the CFL epilogue only)
+template <typename T, int TX, int TY, int NPW, int LIM, bool CFLE, bool DEFS = false>
 __global__ void __launch_bounds__(OneCfg<T, TX, TY, NPW>::NTH, 1)
 k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
                unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next, int xtiles, int zseg,
@@ -529,7 +531,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   const long long ubase = (long long)P.patch(pl) * G.ps + G.lead + (x0 + fi + G.g[0]) +
                           (long long)(y0 + fj + G.g[1]) * G.pitch + (long long)G.g[2] * plane;
   const T cx = dt * P.idx[0], cy = dt * P.idx[1], cz = dt * P.idx[2];
-  const int solver = G.emf_solver, FS = G.flux_solver;
+  const int solver = DEFS ? 0 : G.emf_solver, FS = DEFS ? 0 : G.flux_solver;
 
   if (roleA) {
     // ------------------------------------------------------------- role A -----------
