@@ -463,6 +463,9 @@ int prepare_tile2d() {
   CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
   CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
   CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, 1, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, true, 1, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C1::smem));
+  CUDA_TRY(cudaFuncSetAttribute(k_step_tile2d<T, TX, TY, false, NB, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::smem));
   return MHD_OK;
 }
 // Small 2D bunches are bound by launch latency: there the tile kernel's CFL epilogue replaces two launches
@@ -489,16 +492,23 @@ int launch_tile2d(mhd_bunch* b, int p0, int npl, bool cfle = false) {
     auto go = [&](auto kern, unsigned grid, int nth, size_t smem) {
       kern<<<grid, nth, smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next, xt, yt);
     };
-    const bool mm = G.limiter == 1;
+    // limiter: a compile-time parameter (1 minmod, 2 monotonised central); -1 = the default scheme, minmod with the
+    // default solvers (HLLD, HLLD-2D) fixed at compile time as well
+    const int lim = G.limiter == 1 ? ((G.emf_solver == 0 && G.flux_solver == 0) ? -1 : 1) : 2;
     if (persist) {
       using C = TileCfg<T, TX, TY, NB>;
-      if (mm) go(k_step_tile2d<T, TX, TY, false, NB, 1>, (unsigned)b->nsm, C::NTH, C::smem);
+      if (lim < 0) go(k_step_tile2d<T, TX, TY, false, NB, -1>, (unsigned)b->nsm, C::NTH, C::smem);
+      else if (lim == 1) go(k_step_tile2d<T, TX, TY, false, NB, 1>, (unsigned)b->nsm, C::NTH, C::smem);
       else go(k_step_tile2d<T, TX, TY, false, NB, 2>, (unsigned)b->nsm, C::NTH, C::smem);
+    } else if (cfle) {
+      using C = TileCfg<T, TX, TY, 1>;
+      if (lim < 0) go(k_step_tile2d<T, TX, TY, true, 1, -1>, (unsigned)tiles, C::NTH, C::smem);
+      else if (lim == 1) go(k_step_tile2d<T, TX, TY, true, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
+      else go(k_step_tile2d<T, TX, TY, true, 1, 2>, (unsigned)tiles, C::NTH, C::smem);
     } else {
       using C = TileCfg<T, TX, TY, 1>;
-      if (cfle && mm) go(k_step_tile2d<T, TX, TY, true, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
-      else if (cfle) go(k_step_tile2d<T, TX, TY, true, 1, 2>, (unsigned)tiles, C::NTH, C::smem);
-      else if (mm) go(k_step_tile2d<T, TX, TY, false, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
+      if (lim < 0) go(k_step_tile2d<T, TX, TY, false, 1, -1>, (unsigned)tiles, C::NTH, C::smem);
+      else if (lim == 1) go(k_step_tile2d<T, TX, TY, false, 1, 1>, (unsigned)tiles, C::NTH, C::smem);
       else go(k_step_tile2d<T, TX, TY, false, 1, 2>, (unsigned)tiles, C::NTH, C::smem);
     }
   }

@@ -361,6 +361,7 @@ __device__ __forceinline__ T stage_slope(int kind, T a, T b) {
 }
 template <typename T> struct HbmAcc {
   static constexpr int lim_kind = 0;
+  static constexpr bool def_solvers = false;
   const T* U; T* Un; T* W;
   long long ufs, wfs, cu, cw;
   long long st[3];
@@ -526,7 +527,7 @@ __device__ __forceinline__ void st_flux(const Params<T>& P, const X& x) {
   R.by = h * (b1[0] + b1[x.s(T1)]) - h * x.w(W_DQ + D * 8 + 5 + T1)[0];
   L.bz = h * (b2[-sd] + b2[-sd + x.s(T2)]) + h * x.w(W_DQ + D * 8 + 5 + T2)[-sd];
   R.bz = h * (b2[0] + b2[x.s(T2)]) - h * x.w(W_DQ + D * 8 + 5 + T2)[0];
-  const Flux5<T> F = riemann_flux(G.flux_solver, P.gamma, L, R, x.w(W_BH + D)[0]);
+  const Flux5<T> F = riemann_flux(X::def_solvers ? 0 : G.flux_solver, P.gamma, L, R, x.w(W_BH + D)[0]);
   x.w(W_FLUX + D * 5)[0] = F.d; x.w(W_FLUX + D * 5 + 1 + D)[0] = F.mu; x.w(W_FLUX + D * 5 + 1 + T1)[0] = F.mv;
   x.w(W_FLUX + D * 5 + 1 + T2)[0] = F.mw; x.w(W_FLUX + D * 5 + 4)[0] = F.e;
 }
@@ -558,7 +559,7 @@ __device__ __forceinline__ void st_emf(const Params<T>& P, const X& x) {
   const T* bb = x.w(W_BH + Bd);
   const T AS = ba[-sb] + h * dba[-sb], AN = ba[0] - h * dba[0];
   const T BW = bb[-sa] + h * dbb[-sa], BE = bb[0] - h * dbb[0];
-  x.w(W_EMF + E)[0] = emf_2d(P.gamma, G.emf_solver, sw, se_, nw, ne, AS, AN, BW, BE);
+  x.w(W_EMF + E)[0] = emf_2d(P.gamma, X::def_solvers ? 0 : G.emf_solver, sw, se_, nw, ne, AS, AN, BW, BE);
 }
 
 // O8: conservative update + constrained transport with the metric factor of each term

@@ -53,7 +53,8 @@ __device__ __forceinline__ void tile_cp_async(double* dst, const double* src) {
 }
 
 template <typename T, int AR, int TP, int LIM> struct TileAcc {
-  static constexpr int lim_kind = LIM;
+  static constexpr int lim_kind = LIM < 0 ? 1 : LIM;
+  static constexpr bool def_solvers = LIM < 0;      // LIM = -1: minmod AND the default solvers (HLLD, HLLD-2D) at compile time
   const T* raw;   // [8][AR] at the cell
   T* W;           // [TILE_SLOTS][AR] at the cell
   T* Un;          // U^{n+1} in HBM at the cell
