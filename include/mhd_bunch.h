@@ -292,8 +292,9 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 /* The step has four CUDA implementations, all on the GPU:
  *   MHD_PATH_ONEPASS     the whole step in one kernel, nothing intermediate in HBM (three
  *                        active dimensions, float32): the default where it applies;
- *   MHD_PATH_TILE2D      the whole step of a two-dimensional bunch (n_z = 1, x and y active) in
- *                        one kernel on shared-memory tiles, any type: the default there (the
+ *   MHD_PATH_TILE2D      the whole step of a two-dimensional bunch (n_z = 1, x and y active) or of
+ *                        a one-dimensional one along x (n_y = n_z = 1) in one kernel on
+ *                        shared-memory tiles / rows, any type: the default there (the
  *                        staged path's stage functions on a tile: same result to rounding);
  *   MHD_PATH_TWO_KERNEL  predictor kernel + Riemann/update kernel with one scratch block in
  *                        HBM (three active dimensions, any type);

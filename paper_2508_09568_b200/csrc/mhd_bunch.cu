@@ -484,6 +484,19 @@ int launch_tile2d(mhd_bunch* b, int p0, int npl, bool cfle = false) {
   const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
   const long long tiles = tile2d_tiles<T>(b, npl);
   const int gather = (b->gather_t_ok && !b->ov_plist) ? 1 : 0;
+  if (!G.act[1]) {     // one-dimensional bunch along x: one small CTA per patch
+    const size_t smem = (size_t)75 * (G.n[0] + 6) * sizeof(T);
+    const int lim = G.limiter == 1 ? ((G.emf_solver == 0 && G.flux_solver == 0) ? -1 : 1) : 2;
+    LaunchScope ls(b, KC_TILE2D);
+    auto go1 = [&](auto kern) {
+      if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      kern<<<(unsigned)npl, 128, smem, b->stream>>>(P, b->d_nbr, gather, b->d_dt + 1, b->d_bad, b->d_rate_next);
+    };
+    if (cfle) { if (lim < 0) go1(k_step_line1d<T, true, -1>); else if (lim == 1) go1(k_step_line1d<T, true, 1>); else go1(k_step_line1d<T, true, 2>); }
+    else { if (lim < 0) go1(k_step_line1d<T, false, -1>); else if (lim == 1) go1(k_step_line1d<T, false, 1>); else go1(k_step_line1d<T, false, 2>); }
+    CUDA_TRY(cudaGetLastError());
+    return MHD_OK;
+  }
   // more than two waves of tiles: persistent CTAs that prefetch (where a second raw buffer fits)
   const bool persist = NB == 2 && !cfle && tiles > 2ll * b->nsm;
   {
@@ -833,7 +846,8 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
                                         b->DG.ps, b->DG.fs, bx, by, W_DCOUNT);
   }
   b->onepass_ok = all_active(b->G) && desc->dtype == MHD_F32;
-  b->tile2d_ok = b->G.act[0] && b->G.act[1] && !b->G.act[2];
+  // x and y active with z collapsed (tile kernel), or x alone (line kernel: the whole row of a patch in shared memory)
+  b->tile2d_ok = b->G.act[0] && !b->G.act[2] && (b->G.act[1] || (size_t)75 * (b->G.n[0] + 6) * b->esz <= (size_t)200 * 1024);
   b->nsm = 148;
   cudaDeviceGetAttribute(&b->nsm, cudaDevAttrMultiProcessorCount, desc->device);
   b->gather_ok = b->onepass_ok && b->G.n[0] % (int)(16 / b->esz) == 0;

@@ -228,4 +228,80 @@ k_step_tile2d(Params<T> P, const int* __restrict__ nbr, int gather, const double
 #undef TILE_FOR
 }
 
+// ---- one-dimensional bunches along x (n_y = n_z = 1: BASELINE.json config 0, the shock-tube runs of PAPER.md
+// L186): the same stages on the whole row of a patch, one small CTA per patch, one launch instead of twelve.
+// Every scratch array keeps its own slot (75 short rows).
+template <typename T, int LIM> struct LineAcc {
+  static constexpr int lim_kind = LIM < 0 ? 1 : LIM;
+  static constexpr bool def_solvers = LIM < 0;
+  const T* raw; T* W; T* Un;
+  long long ufs; int L;
+  __device__ __forceinline__ const T* u(int f) const { return raw + f * L; }
+  __device__ __forceinline__ T* un(int f) const { return Un + f * ufs; }
+  __device__ __forceinline__ T* keep(int f) const { return const_cast<T*>(raw) + f * L; }
+  __device__ __forceinline__ T* w(int a) const { return W + a * L; }
+  __device__ __forceinline__ long long s(int d) const { return d == 0 ? 1 : 0; }
+  __device__ __forceinline__ bool act(int d) const { return d == 0; }
+};
+
+template <typename T, bool CFLE, int LIM>
+__global__ void __launch_bounds__(128)
+k_step_line1d(Params<T> P, const int* __restrict__ nbr, int gather, const double* __restrict__ dtp,
+              unsigned long long* __restrict__ bad, unsigned long long* __restrict__ rate_next) {
+  extern __shared__ __align__(16) unsigned char tile_smem[];
+  const Geom& G = P.G;
+  const int nx = G.n[0], L = nx + 6, t = threadIdx.x, NTH = blockDim.x;
+  T* const raw = reinterpret_cast<T*>(tile_smem);
+  T* const W = raw + 8 * L;
+  const int pl = blockIdx.x;
+  const T dt = P.dt_of(pl, dtp);
+  const long long pbase = (long long)P.patch(pl) * G.ps + G.lead;
+  for (int idx = t; idx < L; idx += NTH) {
+    const int i = idx - 3;
+    long long g = pbase + (i + G.g[0]);
+    if (gather) {
+      const int ox = i < 0 ? -1 : (i >= nx ? 1 : 0);
+      if (ox) g = (long long)nbr[(long long)P.patch(pl) * 27 + 13 + ox] * G.ps + G.lead + (i - ox * nx + G.g[0]);
+    }
+#pragma unroll
+    for (int f = 0; f < 8; ++f) raw[f * L + idx] = P.U[f * G.fs + g];
+  }
+  __syncthreads();
+  auto acc = [&](int i) {
+    LineAcc<T, LIM> a;
+    a.raw = raw + i + 3; a.W = W + i + 3; a.ufs = G.fs; a.L = L;
+    a.Un = P.Un + pbase + (i + G.g[0]);
+    return a;
+  };
+  for (int i = -2 + t; i <= nx + 1; i += NTH) st_prim<T>(P, acc(i), (i >= 0 && i < nx) ? i : -1, 0, 0, bad);
+  __syncthreads();
+  for (int i = -1 + t; i <= nx + 1; i += NTH) st_emf0<T>(P, acc(i));
+  __syncthreads();
+  for (int i = -1 + t; i <= nx + 1; i += NTH) st_predict<T>(P, acc(i), i, 0, 0, dt);
+  __syncthreads();
+  // x faces and the y- and z-directed edges at the faces (the x-directed edge EMF only enters through differences
+  // that vanish)
+  for (int it = t; it < 3 * (nx + 1); it += NTH) {
+    const int q = it / (nx + 1), i = it - q * (nx + 1);
+    if (q == 0) st_flux<T, 0>(P, acc(i));
+    else if (q == 1) st_emf<T, 1>(P, acc(i));
+    else st_emf<T, 2>(P, acc(i));
+  }
+  __syncthreads();
+  for (int i = t; i <= nx; i += NTH) st_update<T, CFLE>(P, acc(i), i, 0, 0, dt);
+  if (CFLE) {
+    __syncthreads();
+    T rmax = T(0);
+    for (int i = t; i < nx; i += NTH) {
+      const T* c = raw + i + 3;
+      rmax = num<T>::max(rmax, cfl_rate<T>(P.gamma, P.idx[0], P.idx[1], P.idx[2], true, false, false, c[0], c[L], c[2 * L], c[3 * L],
+                                            c[4 * L], c[5 * L], c[5 * L + 1], c[6 * L], c[6 * L], c[7 * L], c[7 * L]));
+    }
+    double rd = (double)rmax;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) rd = fmax(rd, __shfl_xor_sync(0xffffffffu, rd, o));
+    if ((t & 31) == 0 && rd > 0.0) atomicMax(&rate_next[P.patch(pl)], enc_max(rd));
+  }
+}
+
 }  // namespace mhd

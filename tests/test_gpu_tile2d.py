@@ -183,3 +183,58 @@ def test_tile2d_on_bunches_of_many_waves(N, n, dtype):
     assert_nstep_parity(W.gather(outs["tile2d"], w.n, w.P), W.gather(ref, w.n, w.P), dtype, (N, n))
     close = {"f64": 1e-14, "f32": 2e-6}[dtype]
     assert rel_err(masked(outs["tile2d"], w.n), masked(outs["staged"], w.n).astype(np.float64)) <= close
+
+
+# ------------------------------------------------------------------ one-dimensional bunches along x ----
+def workloads_1d(dtype):
+    t = NPD[dtype]
+    return {
+        "sod": W.sod(256, 8, dtype=t),                                             # config 0: outflow ends
+        "tube": W.mhd_tube((1.0, 0.2, 0.3, -0.1, 1.0, 1.0, 0.4), (0.125, -0.1, -0.2, 0.25, 0.1, -1.0, 0.2), 0.75, 2.0,
+                           ncell=120, npatch=3, axis=0, dtype=t),                   # all seven waves, ragged n = 40
+        "alfven": W.alfven_wave(N=64, n=16, dtype=t),                               # periodic: halo gathered through the table
+        "alfven_self": W.alfven_wave(N=24, n=24, dtype=t),                          # one patch, its own neighbour
+    }
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("limiter,emf_solver,flux_solver", [(1, 0, 0), (2, 1, 1)])
+@pytest.mark.parametrize("name", ["sod", "tube", "alfven", "alfven_self"])
+def test_line_kernel_on_1d_bunches_matches_oracle_and_the_staged_path(name, dtype, limiter, emf_solver, flux_solver):
+    """1D bunches along x (config 0) step in one kernel too (k_step_line1d: the stages on the whole row of a patch);
+    three chained steps against the oracle, the staged path to rounding, the CFL step from the kernel's epilogue bit
+    for bit the stand-alone pass's."""
+    w = workloads_1d(dtype)[name]
+    o = make_oracle(w, limiter, emf_solver, flux_solver=flux_solver)
+    outs = {}
+    for path in ("tile2d", "staged"):
+        b = make_gpu(w, dtype, limiter, emf_solver, path=path, flux_solver=flux_solver)
+        assert b.path == path
+        U = w.U.astype(np.float64)
+        for s in range(3):
+            U = o.fill_guards(U, w.nbr)
+            dt = o.cfl_dt(U, 0.4)
+            U = o.step(U, dt)
+            b.fill_guards()
+            b.step(dt)
+        if path == "tile2d":
+            b.fill_guards()
+            dt1 = b.cfl_dt(0.4, sync=True)
+            V = b.download()
+            b.load(V)
+            b.fill_guards()
+            assert b.cfl_dt(0.4, sync=True) == dt1
+        outs[path] = b.download()
+        assert b.status() == 0
+        b.close()
+    got = outs["tile2d"]
+    assert rel_err(masked(got, w.n), masked(U, w.n)) <= TOL_STEP[dtype]
+    assert_nstep_parity(W.gather(got, w.n, w.P), W.gather(U, w.n, w.P), dtype, name)
+    close = {"f64": 1e-14, "f32": 2e-6}[dtype]
+    assert rel_err(masked(got, w.n), masked(outs["staged"], w.n).astype(np.float64)) <= close
+
+
+def test_1d_bunches_along_y_or_z_stay_on_the_staged_path():
+    b = make_gpu(W.sod(96, 3, dtype=np.float64, axis=1), "f64")
+    assert b.path == "staged"
+    b.close()
