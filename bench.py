@@ -381,7 +381,7 @@ def measure_small(name, args, local):
            "config": {"workload": desc, "patches": w.npatch, "patch": list(w.n), "guard": 3, "courant": 0.4, "step_path": b.path},
            "gpu_launches_per_step": launches, "bad_cells": b.status(), "kernel_classes": classes,
            "note": "events around every launch inflate the per-class times of kernels this short; ms_per_step is the untimed loop"}
-    if "step_tile2d" in classes:
+    if "step_tile2d" in classes and w.n[1] > 1:      # 2D bunches: the tile kernel against the flops counted in 2D
         tk = classes["step_tile2d"]["ms_per_step"]
         alu_peak = measure_alu_peak(dtype, local)
         rec["roofline"] = {"kernel": "step_tile2d", "bound": "alu", "achieved": STEP_FLOPS_2D * w.cells / (tk * 1e-3) / 1e12,
