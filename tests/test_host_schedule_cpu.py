@@ -94,6 +94,40 @@ def test_schedule_is_safe_tight_and_complete(name, chunk, nz, g, bands):
     assert abs(s["makespan"] - simulate(npatch, ck, nz, s)) < 1e-9
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_schedule_on_arbitrary_tables(seed):
+    """The planner assumes nothing about the arrangement: random tables (any patch may be anybody's neighbour in
+    any class, some entries -1), random chunk sizes, plane counts, guard widths and band counts -- the same three
+    properties must hold (every plane uploaded once, ready[] safe and tight, units partition their chunks)."""
+    rng = np.random.default_rng(1000 + seed)
+    npatch = int(rng.integers(1, 40))
+    nbr = rng.integers(-1, npatch, size=(npatch, 27)).astype(np.int32)
+    nbr[:, 13] = np.arange(npatch)
+    nz = int(rng.choice([1, 5, 7, 16, 33, 64, 70]))
+    g = int(rng.choice([0, 1, 3]))
+    chunk = int(rng.integers(1, npatch + 1))
+    bands = int(rng.integers(1, 6))
+    s = B.host_schedule(nbr, chunk, nz=nz, guard=g, bands=bands)
+    ck, n = s["chunk"], s["nchunk"]
+    landed_after, seen = {}, set()
+    for i, (q, k0, k1) in enumerate(zip(s["piece_chunk"], s["piece_k0"], s["piece_k1"])):
+        for k in range(k0, k1):
+            assert (q, k) not in seen
+            seen.add((q, k))
+            for p in range(q * ck, min(npatch, (q + 1) * ck)):
+                landed_after[(p, k)] = i
+    assert len(seen) == n * nz
+    units = list(zip(s["unit_chunk"], s["unit_za"], s["unit_zb"]))
+    assert units == sorted(units)
+    for c in range(n):
+        mine = [(za, zb) for q, za, zb in units if q == c]
+        assert mine[0][0] == 0 and mine[-1][1] == nz and all(a[1] == b_[0] for a, b_ in zip(mine, mine[1:]))
+    for u, (c, za, zb) in enumerate(units):
+        last = max(landed_after[x] for x in planes_read(nbr, ck, c, za, zb, nz, g))
+        assert s["ready"][u] == max(last, s["ready"][u - 1] if u else -1)
+    assert abs(s["makespan"] - simulate(npatch, ck, nz, s)) < 1e-9
+
+
 def test_periodic_stack_never_waits_for_the_bulk_of_a_z_neighbour():
     s = B.host_schedule(TABLES["cube8"], 64, bands=1)             # one z-slab of patches per chunk, stepped whole
     pieces = list(zip(s["piece_chunk"], s["piece_k0"], s["piece_k1"]))
