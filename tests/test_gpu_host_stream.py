@@ -20,7 +20,8 @@ def workloads(dtype):
         "turb_slabs": W.turbulence(N=(16, 16, 64), n=(16, 16, 8), dtype=t),   # 8 slabs stacked along z
         "turb_ragged": W.turbulence(N=(24, 20, 36), n=(12, 10, 9), dtype=t),
         "turb_self": W.turbulence(N=16, n=16, dtype=t),
-        "ot64": W.orszag_tang(64, 32, dtype=t),                               # 2D: general step path
+        "ot64": W.orszag_tang(64, 32, dtype=t),                               # 2D: tile kernel, whole-chunk units
+        "alfven1d": W.alfven_wave(N=64, n=16, dtype=t),                       # 1D along x: line kernel
     }
 
 
@@ -60,7 +61,7 @@ def test_step_host_on_the_other_step_paths(dtype, path):
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("chunk", [1, 3, 0])
 @pytest.mark.parametrize("given_dt", [True, False])
-@pytest.mark.parametrize("name", ["turb16", "turb_slabs", "turb_ragged", "turb_self", "ot64"])
+@pytest.mark.parametrize("name", ["turb16", "turb_slabs", "turb_ragged", "turb_self", "ot64", "alfven1d"])
 def test_step_host_matches_oracle(name, given_dt, chunk, dtype):
     import torch
     w = workloads(dtype)[name]
@@ -84,7 +85,7 @@ def test_step_host_matches_oracle(name, given_dt, chunk, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("name", ["turb16", "turb_slabs", "ot64"])
+@pytest.mark.parametrize("name", ["turb16", "turb_slabs", "ot64", "alfven1d"])
 def test_host_stream_equals_resident_path_bitwise_over_several_steps(name, dtype):
     """Three chained steps (dt_next of one call is the dt of the next) through host buffers
     against the resident loop fill_guards -> cfl_dt -> step of the same library."""
