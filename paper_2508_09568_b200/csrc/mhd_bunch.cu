@@ -409,14 +409,20 @@ template <> struct OnePassLaunch<float> {
     Params<float> P = make_params<float>(b, p0, npl);
     if (zhi < 0) zhi = G.n[2];
     const int xt = (G.n[0] + TX - 1) / TX, yt = (G.n[1] + TY - 1) / TY;
-    // fewer tiles than SMs: cut the columns into z segments of at least 8 planes so that the
-    // launch covers the GPU about twice (each segment pays a five-plane run-in, so only then)
+    // Small launches (fewer than four waves of tiles): the columns are cut into z segments, each a CTA that
+    // pays a five-plane run-in.  The cut minimises waves x (planes per segment + 5), segments of at least four
+    // planes -- a launch that leaves SMs idle is bound by the latency of one CTA's march (one 32^3 patch:
+    // 78 -> 56 us per step with 4-plane segments), a launch that already fills them only loses to the run-in.
     int zseg = 1;
     const long long tiles = (long long)xt * yt * npl;
-    if (tiles < b->nsm) {
-      zseg = (int)((2ll * b->nsm + tiles - 1) / tiles);
-      const int zmax = (zhi - zlo) / 8 > 1 ? (zhi - zlo) / 8 : 1;
-      if (zseg > zmax) zseg = zmax;
+    if (tiles < 4ll * b->nsm) {
+      const int nzr = zhi - zlo;
+      long long best = -1;
+      for (int z = 1; z <= (nzr / 4 > 1 ? nzr / 4 : 1); ++z) {
+        const long long waves = (tiles * z + b->nsm - 1) / b->nsm;
+        const long long cost = waves * ((nzr + z - 1) / z + 5);
+        if (best < 0 || cost < best) { best = cost; zseg = z; }
+      }
     }
     if (b->tune_zseg >= 1) zseg = b->tune_zseg < zhi - zlo ? b->tune_zseg : zhi - zlo;   // mhd_bunch_set_tuning
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
