@@ -298,7 +298,7 @@ int launch_fill(mhd_bunch* b) {
     (void)lg;
     if (per > 0) {
       LaunchScope ls(b, KC_FILL);
-      k_fill_guards_vec<T><<<blocks_for(per * G.np, 256), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr);
+      k_fill_guards_vec<T><<<dim3(blocks_for(per * G.np, 256), 8 / FillFpt<T>::N), 256, 0, b->stream>>>(G, (T*)b->state[b->cur], b->d_nbr);
     }
     CUDA_TRY(cudaGetLastError());
     return MHD_OK;
