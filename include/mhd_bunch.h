@@ -343,6 +343,52 @@ int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);
 
 int mhd_bunch_destroy(mhd_bunch *b);
 
+/* CFL time step WITHOUT a handle and WITHOUT a workspace (same quantity as mhd_bunch_cfl_dt:
+ * PAPER.md L122; O9).
+ *
+ * Who this is for.  Everything above needs device memory from the caller: a workspace handed
+ * to mhd_bunch_create, which somebody had to cudaMalloc.  Some callers cannot do that at the
+ * point where they need a time step:
+ *   - a task-update hook of a host framework (DISPATCH updates a patch from inside a worker
+ *     thread) that runs while other streams are busy: cudaMalloc and
+ *     cudaFree serialise the whole device, so one allocation there stalls every bunch in flight;
+ *   - an application that gave all of HBM to its own pool at start-up, where a late cudaMalloc
+ *     simply fails, and whose pool is not reachable from the place the call is made;
+ *   - code that is only handed a state pointer (a diagnostics or restart module checking the
+ *     time step of a dump it mapped) and owns no handle and no scratch at all.
+ * For them the per-patch rate maxima that the two-stage reduction needs between its kernels live
+ * in an array that is PART OF THE LIBRARY IMAGE: MHD_CFL_STATIC_MAX_PATCHES 8-byte slots
+ * (256 KiB), present on every GPU that loads libmhd_bunch.so, from load until the process ends,
+ * whether or not this call is ever made.  The call makes no cudaMalloc / cudaFree and uses no
+ * allocating library routine; it launches the same three kernels as mhd_bunch_cfl_dt and the
+ * results are the same bits.
+ *
+ *   desc             HOST.  n, ng, npatch, dtype, gamma, dx, device and stream are read (limiter
+ *                    and solver choices must be valid but play no part).
+ *                    npatch > MHD_CFL_STATIC_MAX_PATCHES -> MHD_ENOMEM, nothing is launched
+ *                    (mhd_bunch_last_cuda_error then says what the limit is).
+ *   state_dev        DEVICE const, the layout mhd_bunch_query returns for desc, 16-byte aligned,
+ *                    with the closing faces up to date (after mhd_bunch_fill_guards, or straight
+ *                    after a step: a rate reads the upper face of a cell).  Not modified.
+ *   dt_dev           DEVICE double*, required: receives courant / (largest rate of the bunch).
+ *   dt_per_patch_dev DEVICE double[npatch], nullable: per-patch steps.
+ * Only enqueues on desc.stream; read the outputs after synchronising it yourself.
+ *
+ * First call on a device.  The first call for a given desc.device looks up the device address
+ * of the array (with that device current) and remembers it; that lookup may load the library's
+ * device code.  Make this first call early, outside any stream capture; later calls on that
+ * device only launch kernels.
+ *
+ * Sharing.  Every call on a device uses the SAME array, whatever its stream, thread or bunch,
+ * and the array keeps what the previous call left there: each call clears the slots it is going
+ * to use before reducing into them, but two calls whose kernels can overlap on the GPU (different
+ * streams without an ordering event between them) overwrite each other's maxima and both results
+ * are then garbage.  Order such calls yourself, or use handles (mhd_bunch_cfl_dt), whose
+ * scratch is private.                                                                        */
+#define MHD_CFL_STATIC_MAX_PATCHES 32768
+int mhd_bunch_cfl_dt_static(const mhd_bunch_desc *desc, const void *state_dev, double courant, void *dt_dev,
+                            void *dt_per_patch_dev);
+
 const char *mhd_bunch_strerror(int code);
 const char *mhd_bunch_last_cuda_error(void);
 

@@ -25,7 +25,9 @@ ABI_SYMBOLS = [
     "mhd_bunch_host_schedule",
     "mhd_bunch_ring_plan", "mhd_bunch_ring_attach", "mhd_bunch_step_ring", "mhd_bunch_ring_detach",
     "mhd_bunch_local_begin", "mhd_bunch_step_local", "mhd_bunch_cfl_local", "mhd_bunch_local_state", "mhd_bunch_local_end",
+    "mhd_bunch_cfl_dt_static",
 ]
+CFL_STATIC_MAX_PATCHES = 32768   # MHD_CFL_STATIC_MAX_PATCHES of include/mhd_bunch.h
 
 
 class Desc(C.Structure):
@@ -95,6 +97,7 @@ def load_library(build_if_missing=True):
     lib.mhd_bunch_cfl_local.argtypes = [vp, dbl, vp]
     lib.mhd_bunch_local_state.argtypes = [vp, vp, vp, vp]
     lib.mhd_bunch_local_end.argtypes = [vp]
+    lib.mhd_bunch_cfl_dt_static.argtypes = [C.POINTER(Desc), vp, dbl, vp, vp]
     lib.mhd_bunch_strerror.argtypes = [C.c_int]
     lib.mhd_bunch_strerror.restype = C.c_char_p
     lib.mhd_bunch_last_cuda_error.restype = C.c_char_p
@@ -137,6 +140,21 @@ def measure_alu_peak(dtype="f32", device=0):
     _check(load_library().mhd_bunch_measure_alu_peak(MHD_F32 if dtype == "f32" else MHD_F64, device, scratch.data_ptr(),
                                                      scratch.numel(), C.byref(v)), "mhd_bunch_measure_alu_peak")
     return v.value
+
+
+def cfl_dt_static(desc, state, courant, dt_dev, dt_patch=None):
+    """mhd_bunch_cfl_dt_static: the CFL step of a state buffer for callers that own no handle and no
+    workspace and cannot allocate one where they stand (a framework's task hook running under other
+    streams' work, an application whose pool holds all of HBM).  The reduction's scratch is an array
+    inside libmhd_bunch.so, good for CFL_STATIC_MAX_PATCHES patches and shared by every call on the
+    device, so calls that may overlap on the GPU must be ordered by the caller.
+
+    desc: make_desc(...); state: torch CUDA tensor in the layout query(desc) gives, closing faces up to
+    date; dt_dev: torch CUDA float64[1]; dt_patch: torch CUDA float64[npatch] or None.  Only enqueues
+    on desc.stream.  Raises RuntimeError (MHD_ENOMEM) beyond the limit."""
+    _check(load_library().mhd_bunch_cfl_dt_static(C.byref(desc), state.data_ptr(), courant, dt_dev.data_ptr(),
+                                                   dt_patch.data_ptr() if dt_patch is not None else None),
+           "mhd_bunch_cfl_dt_static")
 
 
 def host_schedule(nbr, chunk_patches=0, nz=32, guard=3, bands=0):

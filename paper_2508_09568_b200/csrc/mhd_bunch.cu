@@ -20,6 +20,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <mutex>
 #include <new>
 #include <vector>
 #include <algorithm>
@@ -2023,3 +2024,88 @@ int mhd_bunch_destroy(mhd_bunch* b) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------ CFL step without handle or workspace ----
+// mhd_bunch_cfl_dt_static (include/mhd_bunch.h): for callers that have nowhere to get scratch from --
+// a framework's task-update hook running while other streams are busy (cudaMalloc / cudaFree would
+// serialise the device under them), an application whose pool already owns all of HBM, a module that is
+// only handed a state pointer.  The per-patch rate maxima between k_cfl and k_cfl_final (what a handle
+// keeps in b->d_rate, carved from the caller's workspace) sit in this array instead.  It is part of the
+// library image: 8 * MHD_CFL_STATIC_MAX_PATCHES bytes (256 KiB) on every device that loads the library,
+// until the process exits.
+//
+// In HOST code the name g_cfl_static_rate is only a handle for the runtime's symbol calls, not a device
+// address: a kernel given `g_cfl_static_rate` from host code would fault (or scribble over host memory
+// where the GPU can reach it).  The address a kernel may use comes from cudaGetSymbolAddress, asked for
+// once per device with that device current, and is kept in g_cfl_static_ptr.
+static __device__ __align__(256) unsigned long long g_cfl_static_rate[MHD_CFL_STATIC_MAX_PATCHES];
+
+namespace {
+constexpr int kStaticMaxDev = 64;
+unsigned long long* g_cfl_static_ptr[kStaticMaxDev];   // device address of g_cfl_static_rate per ordinal (null: not asked yet)
+std::mutex g_cfl_static_mu;
+
+// Device address of the array on `device`, which must be the current device.  No allocation: the array
+// came with the module; the lookup may make the runtime load the module, which is why the header asks for
+// the first call on a device to come before any stream capture.
+int cfl_static_address(int device, unsigned long long** out) {
+  std::lock_guard<std::mutex> lock(g_cfl_static_mu);
+  if (device < kStaticMaxDev && g_cfl_static_ptr[device]) { *out = g_cfl_static_ptr[device]; return MHD_OK; }
+  void* p = nullptr;
+  CUDA_TRY(cudaGetSymbolAddress(&p, g_cfl_static_rate));
+  if (!p) return fail_cuda(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_cfl_static_rate) returned null");
+  if (device < kStaticMaxDev) g_cfl_static_ptr[device] = (unsigned long long*)p;   // ordinals past the table: looked up every call
+  *out = (unsigned long long*)p;
+  return MHD_OK;
+}
+
+template <typename T>
+int launch_cfl_static(const mhd_bunch_desc* desc, const Geom& G, const void* state, unsigned long long* rate, double courant,
+                      double* dt_dev, double* dt_patch) {
+  cudaStream_t st = (cudaStream_t)desc->stream;
+  Params<T> P;
+  memset(&P, 0, sizeof(P));
+  P.G = G;
+  P.U = (const T*)state;
+  P.npl = G.np;
+  P.gamma = (T)desc->gamma;
+  for (int a = 0; a < 3; ++a) {
+    P.dx[a] = (T)desc->dx[a];
+    P.idx[a] = (T)(1.0 / desc->dx[a]);
+  }
+  // the array still holds the previous call's maxima: the slots of this bunch start from zero
+  k_zero_u64<<<blocks_for(G.np, 256), 256, 0, st>>>(rate, G.np);
+  const long long per = (long long)G.n[0] * G.n[1] * G.n[2];
+  int bx = (int)((per + 256 * CFL_CPT - 1) / (256 * CFL_CPT));   // launch shape of launch_cfl
+  if (bx < 1) bx = 1;
+  k_cfl<T><<<dim3((unsigned)bx, (unsigned)G.np), 256, 0, st>>>(P, rate);
+  k_cfl_final<<<1, 256, 0, st>>>(rate, G.np, courant, dt_dev, nullptr, dt_patch);
+  CUDA_TRY(cudaGetLastError());
+  return MHD_OK;
+}
+}  // namespace
+
+extern "C" int mhd_bunch_cfl_dt_static(const mhd_bunch_desc* desc, const void* state_dev, double courant, void* dt_dev,
+                                       void* dt_per_patch_dev) {
+  if (!desc || !state_dev || !dt_dev) return MHD_EINVAL;
+  if (((uintptr_t)state_dev & 15) || ((uintptr_t)dt_dev & 7) || ((uintptr_t)dt_per_patch_dev & 7)) return MHD_EINVAL;
+  if (!(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
+  Geom G;
+  const int rc = build_geom(desc, &G);
+  if (rc != MHD_OK) return rc;
+  if (desc->npatch > MHD_CFL_STATIC_MAX_PATCHES) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "mhd_bunch_cfl_dt_static: %d patches, the built-in scratch holds %d (MHD_CFL_STATIC_MAX_PATCHES)",
+             (int)desc->npatch, (int)MHD_CFL_STATIC_MAX_PATCHES);
+    return MHD_ENOMEM;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= desc->device || desc->device < 0)
+    return fail_cuda(cudaErrorNoDevice, "no CUDA device: this library has no CPU fallback");
+  CUDA_TRY(cudaSetDevice(desc->device));
+  unsigned long long* rate = nullptr;
+  const int ra = cfl_static_address(desc->device, &rate);
+  if (ra != MHD_OK) return ra;
+  return desc->dtype == MHD_F64
+             ? launch_cfl_static<double>(desc, G, state_dev, rate, courant, (double*)dt_dev, (double*)dt_per_patch_dev)
+             : launch_cfl_static<float>(desc, G, state_dev, rate, courant, (double*)dt_dev, (double*)dt_per_patch_dev);
+}
