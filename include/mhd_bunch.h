@@ -226,7 +226,12 @@ int mhd_bunch_host_schedule(const int32_t *nbr, int32_t npatch, int32_t nz, int3
  *                          of the WHOLE bunch; dt > 0; HOST out, nullable: *dt_next = CFL step of the
  *                          new level (from the step's own epilogue).  Synchronises.  Results are bit
  *                          for bit those of the resident step.
- *   mhd_bunch_ring_detach  releases the streams; the handle is a plain window-sized bunch again.   */
+ *   mhd_bunch_ring_detach  releases the streams; the handle is a plain window-sized bunch again.
+ * While a ring is attached the device copy of the neighbour table belongs to it, so the calls that
+ * would read it as the window's own table -- mhd_bunch_fill_guards, sync_guards, cfl_dt, step, step_dev,
+ * host_attach, step_host, local_begin -- return MHD_ESTATE until mhd_bunch_ring_detach; ring_attach
+ * ends an attached host-streaming mode itself, and neither ring call is accepted in local-time-step
+ * mode.                                                                                           */
 int mhd_bunch_ring_plan(const int32_t *nbr, int32_t npatch, int32_t chunk_patches, int32_t ring_chunks, int32_t *nchunk,
                         int32_t *nupload, int32_t *up_chunk, int32_t *up_slot, int32_t *up_step, int32_t *step_slot, int32_t cap);
 int mhd_bunch_ring_attach(mhd_bunch *b, const int32_t *nbr, int32_t npatch, int32_t chunk_patches, void *staging_dev,
@@ -324,7 +329,14 @@ int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
  *                          two (0 = automatic; clipped to bands of at least eight planes; only
  *                          the one-pass path steps plane ranges).  Read by host_query / attach;
  *                          results do not depend on it, bit for bit.
+ *   MHD_TUNE_HOST_MAX_PITCH  largest host pitch in bytes that one strided host<->device copy of
+ *                          mhd_bunch_step_host / mhd_bunch_step_ring may name (0 = the device's
+ *                          cudaDevAttrMaxPitch, 2^31 - 1).  Host bunches whose fields are further
+ *                          apart than this are moved field by field (eight copies per transfer
+ *                          instead of one); tests set it to 1 to run that route on small bunches.
+ *                          Results do not depend on it, bit for bit.
  * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
+#define MHD_TUNE_HOST_MAX_PITCH 5
 #define MHD_TUNE_HOST_BANDS   4
 #define MHD_TUNE_ONEPASS_ZSEG 1
 #define MHD_TUNE_PREDICT_TY   2

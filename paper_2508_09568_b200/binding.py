@@ -13,7 +13,7 @@ from . import build as _build
 
 MHD_F32, MHD_F64 = 0, 1
 PATHS = {"auto": 0, "staged": 1, "two_kernel": 2, "onepass": 3, "tile2d": 4}
-TUNE = {"onepass_zseg": 1, "predict_ty": 2, "fused_cfl": 3, "host_bands": 4}
+TUNE = {"onepass_zseg": 1, "predict_ty": 2, "fused_cfl": 3, "host_bands": 4, "host_max_pitch": 5}
 _ERR = {0: "ok", -1: "MHD_EINVAL", -2: "MHD_ENOMEM", -3: "MHD_ECUDA", -4: "MHD_ESTATE"}
 
 ABI_SYMBOLS = [
@@ -388,7 +388,7 @@ class MhdBunch:
         return {k: n for n, k in PATHS.items()}[v.value]
 
     def set_tuning(self, key, value):
-        """key: 'onepass_zseg' | 'predict_ty' | 'fused_cfl' | 'host_bands' (include/mhd_bunch.h, MHD_TUNE_*)."""
+        """key: 'onepass_zseg' | 'predict_ty' | 'fused_cfl' | 'host_bands' | 'host_max_pitch' (include/mhd_bunch.h, MHD_TUNE_*)."""
         _check(self.lib.mhd_bunch_set_tuning(self.h, TUNE[key], int(value)), "mhd_bunch_set_tuning")
 
     def set_timing(self, on):

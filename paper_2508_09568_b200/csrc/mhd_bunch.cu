@@ -139,6 +139,8 @@ struct mhd_bunch {
   bool nbr_consistent; // the table composes like translations (see table_is_consistent)
   int tune_zseg;       // MHD_TUNE_ONEPASS_ZSEG: 0 = automatic
   int tune_bands;      // MHD_TUNE_HOST_BANDS: 0 = automatic
+  int tune_max_pitch;  // MHD_TUNE_HOST_MAX_PITCH: 0 = the device's limit (max_pitch)
+  size_t max_pitch;    // cudaDevAttrMaxPitch of the handle's device: largest pitch a strided copy may name
   bool fused_cfl;      // MHD_TUNE_FUSED_CFL: the one-pass step reduces the new level's CFL rates in its epilogue
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
@@ -426,6 +428,11 @@ template <> struct OnePassLaunch<float> {
       }
     }
     if (b->tune_zseg >= 1) zseg = b->tune_zseg < zhi - zlo ? b->tune_zseg : zhi - zlo;   // mhd_bunch_set_tuning
+    {  // no empty segments: the kernel cuts [zlo, zhi) into pieces of ceil(planes / zseg), so e.g. 32 planes in
+       // 31 segments would be 16 pieces of two planes and 15 CTAs that start past zhi; ask for the 16
+      const int nzr = zhi - zlo, zlen = (nzr + zseg - 1) / zseg;
+      zseg = (nzr + zlen - 1) / zlen;
+    }
     dim3 grid((unsigned)(xt * yt), (unsigned)npl, (unsigned)zseg);
     {
       LaunchScope ls(b, KC_ONEPASS);
@@ -576,6 +583,14 @@ bool table_is_consistent(const int32_t* nb, int np) {
 #define NOT_LOCAL(b)                                               \
   do {                                                             \
     if ((b)->loc && (b)->loc->active) return MHD_ESTATE;           \
+  } while (0)
+
+// ... and while a ring is attached: the device copy of the neighbour table then holds rows of the BIG
+// host bunch in slot numbers (mhd_bunch_step_ring rewrites them chunk by chunk), which the resident,
+// host-streaming and local-time-step calls would silently take for the window's own table
+#define NOT_RING(b)                                                \
+  do {                                                             \
+    if ((b)->ring) return MHD_ESTATE;                              \
   } while (0)
 
 // every launching entry point runs on the handle's device, whatever the caller's current one is
@@ -867,6 +882,12 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
   b->gather_t_ok = b->tile2d_ok && b->nbr_consistent;
   b->tune_zseg = 0;
   b->tune_bands = 0;
+  b->tune_max_pitch = 0;
+  {
+    int mp = 0;
+    b->max_pitch = (cudaDeviceGetAttribute(&mp, cudaDevAttrMaxPitch, desc->device) == cudaSuccess && mp > 0) ? (size_t)mp
+                                                                                                             : (size_t)0x7fffffff;
+  }
   b->fused_cfl = false;
   b->hs = nullptr;
   b->ring = nullptr;
@@ -892,6 +913,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
 int mhd_bunch_fill_guards(mhd_bunch* b) {
   ENTER(b);
   NOT_LOCAL(b);
+  NOT_RING(b);
   if (step_gathers(b)) {
     // deferred: the one-pass step reads halos from the neighbours' interiors, so only the
     // closing faces are brought up to date now; the rest of the shell is written if and when
@@ -908,12 +930,14 @@ int mhd_bunch_fill_guards(mhd_bunch* b) {
 
 int mhd_bunch_sync_guards(mhd_bunch* b) {
   ENTER(b);
+  NOT_RING(b);
   return materialise_guards(b);
 }
 
 int mhd_bunch_cfl_dt(mhd_bunch* b, double courant, double* dt_host, void* dt_dev, void* dt_per_patch_dev) {
   ENTER(b);
   NOT_LOCAL(b);
+  NOT_RING(b);
   if (!(courant > 0.0) || !isfinite(courant)) return MHD_EINVAL;
   const int rc = b->desc.dtype == MHD_F64 ? launch_cfl<double>(b, courant, dt_dev, dt_per_patch_dev)
                                            : launch_cfl<float>(b, courant, dt_dev, dt_per_patch_dev);
@@ -932,6 +956,7 @@ static int step_common(mhd_bunch* b) {
 int mhd_bunch_step(mhd_bunch* b, double dt) {
   ENTER(b);
   NOT_LOCAL(b);
+  NOT_RING(b);
   if (!(dt > 0.0) || !isfinite(dt)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, nullptr, dt, 0.0, b->d_rate_next, b->G.np); }
   return step_common(b);
@@ -940,6 +965,7 @@ int mhd_bunch_step(mhd_bunch* b, double dt) {
 int mhd_bunch_step_dev(mhd_bunch* b, const void* dt_dev, double dt_max) {
   ENTER(b);
   NOT_LOCAL(b);
+  NOT_RING(b);
   if (!dt_dev || !(dt_max >= 0.0)) return MHD_EINVAL;
   { LaunchScope ls(b, KC_MISC); k_set_dt<<<1, 256, 0, b->stream>>>(b->d_dt + 1, (const double*)dt_dev, 0.0, dt_max, b->d_rate_next, b->G.np); }
   return step_common(b);
@@ -993,6 +1019,10 @@ int mhd_bunch_set_tuning(mhd_bunch* b, int32_t key, int32_t value) {
   }
   if (key == MHD_TUNE_HOST_BANDS) {
     b->tune_bands = value;
+    return MHD_OK;
+  }
+  if (key == MHD_TUNE_HOST_MAX_PITCH) {
+    b->tune_max_pitch = value;
     return MHD_OK;
   }
   if (key == MHD_TUNE_FUSED_CFL) {
@@ -1158,33 +1188,57 @@ int launch_pack(mhd_bunch* b, cudaStream_t st, void* state, char* stage, int p0,
   return MHD_OK;
 }
 
-// One strided copy per transfer: host[f][p0 .. p0+npl)[k0 .. k0+nk) <-> stage[f][0 .. npl)[0 .. nk).
-// Whole patches are eight contiguous rows (the eight fields: a 2D copy); a z-range of every patch
-// is a 3D copy (row = the planes of one patch and field, rows per slice = patches, slices = fields).
+// host[f][p0 .. p0+npl)[k0 .. k0+nk) <-> stage[f][0 .. npl)[0 .. nk).  Normally ONE strided copy per
+// transfer: whole patches are eight contiguous rows (the eight fields: a 2D copy), a z-range of every
+// patch is a 3D copy (row = the planes of one patch and field, rows per slice = patches, slices =
+// fields).  The host stride between fields is that of the WHOLE host bunch, and CUDA refuses a pitch
+// above cudaDevAttrMaxPitch (2^31 - 1 bytes: cudaErrorInvalidPitchValue) -- reached by 4096 patches of
+// 64^3 in fp32 and by every bunch that really exceeds HBM, which is what ring mode is for.  From there
+// on the transfer is eight copies, one per field, none of which names the field stride: a contiguous
+// copy for whole patches, a 2D copy whose pitch is one patch for a z-range.
 int hs_copy(mhd_bunch* b, cudaStream_t st, char* stage, char* host, int p0, int npl, bool to_device, int host_np = -1,
             int k0 = 0, int nk = -1) {
   const int nz = b->G.n[2];
   if (nk < 0) nk = nz;
   const size_t plane = (size_t)b->G.n[0] * b->G.n[1] * b->esz, per = plane * nz;
   const size_t hnp = (size_t)(host_np < 0 ? b->G.np : host_np);
+  const size_t field = hnp * per;                                   // host bytes between two fields
+  const size_t maxp = b->tune_max_pitch > 0 ? (size_t)b->tune_max_pitch : b->max_pitch;
+  const cudaMemcpyKind kind = to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
   if (k0 == 0 && nk == nz) {
     char* h = host + (size_t)p0 * per;
-    const size_t hp = hnp * per, dp = (size_t)npl * per;
-    if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, hp, dp, 8, cudaMemcpyHostToDevice, st));
-    else CUDA_TRY(cudaMemcpy2DAsync(h, hp, stage, dp, dp, 8, cudaMemcpyDeviceToHost, st));
+    const size_t dp = (size_t)npl * per;
+    if (field <= maxp) {
+      if (to_device) CUDA_TRY(cudaMemcpy2DAsync(stage, dp, h, field, dp, 8, kind, st));
+      else CUDA_TRY(cudaMemcpy2DAsync(h, field, stage, dp, dp, 8, kind, st));
+      return MHD_OK;
+    }
+    for (int f = 0; f < 8; ++f) {
+      if (to_device) CUDA_TRY(cudaMemcpyAsync(stage + f * dp, h + f * field, dp, kind, st));
+      else CUDA_TRY(cudaMemcpyAsync(h + f * field, stage + f * dp, dp, kind, st));
+    }
     return MHD_OK;
   }
   const size_t w = plane * nk;
-  cudaMemcpy3DParms q;
-  memset(&q, 0, sizeof q);
-  const cudaPitchedPtr hptr = make_cudaPitchedPtr(host, per, per, hnp);
-  const cudaPitchedPtr dptr = make_cudaPitchedPtr(stage, w, w, (size_t)npl);
-  const cudaPos hpos = make_cudaPos(plane * k0, (size_t)p0, 0), dpos = make_cudaPos(0, 0, 0);
-  q.srcPtr = to_device ? hptr : dptr; q.srcPos = to_device ? hpos : dpos;
-  q.dstPtr = to_device ? dptr : hptr; q.dstPos = to_device ? dpos : hpos;
-  q.extent = make_cudaExtent(w, (size_t)npl, 8);
-  q.kind = to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
-  CUDA_TRY(cudaMemcpy3DAsync(&q, st));
+  if (field <= maxp) {
+    cudaMemcpy3DParms q;
+    memset(&q, 0, sizeof q);
+    const cudaPitchedPtr hptr = make_cudaPitchedPtr(host, per, per, hnp);
+    const cudaPitchedPtr dptr = make_cudaPitchedPtr(stage, w, w, (size_t)npl);
+    const cudaPos hpos = make_cudaPos(plane * k0, (size_t)p0, 0), dpos = make_cudaPos(0, 0, 0);
+    q.srcPtr = to_device ? hptr : dptr; q.srcPos = to_device ? hpos : dpos;
+    q.dstPtr = to_device ? dptr : hptr; q.dstPos = to_device ? dpos : hpos;
+    q.extent = make_cudaExtent(w, (size_t)npl, 8);
+    q.kind = kind;
+    CUDA_TRY(cudaMemcpy3DAsync(&q, st));
+    return MHD_OK;
+  }
+  for (int f = 0; f < 8; ++f) {
+    char* h = host + f * field + (size_t)p0 * per + plane * k0;
+    char* d = stage + f * (size_t)npl * w;
+    if (to_device) CUDA_TRY(cudaMemcpy2DAsync(d, w, h, per, w, (size_t)npl, kind, st));
+    else CUDA_TRY(cudaMemcpy2DAsync(h, per, d, w, w, (size_t)npl, kind, st));
+  }
   return MHD_OK;
 }
 
@@ -1370,6 +1424,7 @@ int mhd_bunch_host_schedule(const int32_t* nbr, int32_t npatch, int32_t nz, int3
 
 int mhd_bunch_host_attach(mhd_bunch* b, void* staging_dev, size_t staging_bytes, int32_t chunk_patches) {
   ENTER(b);
+  NOT_RING(b);
   if (!staging_dev || ((uintptr_t)staging_dev & 15)) return MHD_EINVAL;
   if (!b->all_nbr) return MHD_EINVAL;   // the compact host layout has no room for evolved closing faces
   mhd_bunch_host_layout lay;
@@ -1425,6 +1480,7 @@ int mhd_bunch_step_host(mhd_bunch* b, const void* host_in, void* host_out, doubl
                         double* dt_used, double* dt_next) {
   ENTER(b);
   NOT_LOCAL(b);
+  NOT_RING(b);
   const int rc = step_host_impl(b, host_in, host_out, dt, courant, dt_used, dt_next);
   if (rc != MHD_OK && b->hs) {
     // copies into / out of the caller's host buffers may still be in flight: drain them before
@@ -1791,6 +1847,7 @@ static int step_ring_body(mhd_bunch* b, const void* host_in, void* host_out, dou
 
 int mhd_bunch_step_ring(mhd_bunch* b, const void* host_in, void* host_out, double dt, double courant, double* dt_next) {
   ENTER(b);
+  NOT_LOCAL(b);
   mhd_bunch::Ring* r = b->ring;
   if (!r) return MHD_ESTATE;
   if (!host_in || !host_out || host_in == host_out) return MHD_EINVAL;
@@ -1851,6 +1908,7 @@ extern "C" {
 
 int mhd_bunch_local_begin(mhd_bunch* b, double t0) {
   ENTER(b);
+  NOT_RING(b);
   if (!isfinite(t0)) return MHD_EINVAL;
   int rc = materialise_guards(b);
   if (rc != MHD_OK) return rc;

@@ -187,6 +187,7 @@ k_step_onepass(Params<T> P, const int* __restrict__ nbr, int gather, const doubl
   // its patches (the whole column unless the host-streaming path steps a chunk band by band).
   const int zlen = (zhi - zlo + zseg - 1) / zseg;
   const int za = zlo + (int)blockIdx.z * zlen, zb = min(zhi, za + zlen);
+  if (za >= zb) return;   // an empty segment (the host asks for none): the whole CTA leaves before any barrier
   const int pl = blockIdx.y;
   const int xt = blockIdx.x % xtiles, yt = blockIdx.x / xtiles;
   const int x0 = xt * TX, y0 = yt * TY;

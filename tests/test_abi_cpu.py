@@ -123,8 +123,16 @@ def test_no_named_barrier_inside_a_convergence_region():
     (named barrier) may lie inside a BSSY ... BSYNC region that holds a lane-predicated forward
     branch before it."""
     import re
+    import shutil
     import subprocess
-    txt = subprocess.run(["cuobjdump", "-sass", B._build.TARGET], capture_output=True, text=True, check=True).stdout
+    # a toolchain test: it needs the CUDA toolkit's disassembler and a built library; boxes without
+    # either skip it instead of failing the CPU tier
+    exe = shutil.which("cuobjdump") or ("/usr/local/cuda/bin/cuobjdump" if os.path.exists("/usr/local/cuda/bin/cuobjdump") else None)
+    if exe is None:
+        pytest.skip("cuobjdump is not installed")
+    if not os.path.exists(B._build.TARGET):
+        pytest.skip("libmhd_bunch.so is not built")
+    txt = subprocess.run([exe, "-sass", B._build.TARGET], capture_output=True, text=True, check=True).stdout
     checked = 0
     for f in re.split(r"\n\s*Function : ", txt)[1:]:
         name = f.split("\n", 1)[0].strip()
@@ -135,6 +143,8 @@ def test_no_named_barrier_inside_a_convergence_region():
         regions = [(a, int(m.group(1), 16)) for a, x in ins
                    for m in [re.match(r"(?:@!?U?P\d+\s+)?BSSY(?:\.\w+)*\s+B\d+,\s*0x([0-9a-f]+)", x)] if m]
         bars = [(a, x) for a, x in ins if re.search(r"\bBAR\.(SYNC|ARV)", x) and not re.search(r"BAR\.SYNC(\.\w+)*\s+0x0\s*$", x)]
+        # a change of the disassembly format must fail here, not pass with nothing parsed
+        assert len(ins) > 1000 and regions, (name, len(ins), len(regions))
         assert len(bars) >= 10, name
         for a, x in bars:
             for s, e in regions:
