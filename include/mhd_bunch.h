@@ -252,7 +252,10 @@ int mhd_bunch_ring_detach(mhd_bunch *b);
  *                          a neighbour at the patch's own time contributes its newer slice bit for
  *                          bit; -1 neighbours: zero gradient as in mhd_bunch_fill_guards), then the
  *                          patch is advanced by its own dt into its older slice, which becomes the
- *                          newer one.  One set of launches covers the whole list whatever its size.
+ *                          newer one.  The number of launches does not depend on the list's size: one
+ *                          guard fill, then one set of step launches per buffer that holds newer slices
+ *                          of listed patches (so up to two sets).  Synchronises the stream once (the
+ *                          lists are staged through pageable memory).
  *                          MHD_ESTATE unless every neighbour q of every listed p satisfies
  *                          t_old[q] <= t_new[p] <= t_new[q] (values are interpolated, never
  *                          extrapolated -- the rule under which DISPATCH updates a task); nothing is
@@ -271,15 +274,6 @@ int mhd_bunch_cfl_local(mhd_bunch *b, double courant, double *dt_patch);
 int mhd_bunch_local_state(mhd_bunch *b, double *t_old, double *t_new, int32_t *slot);
 int mhd_bunch_local_end(mhd_bunch *b);
 
-/* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
- * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
- * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to
- * `cap` entries (name: HOST const char* owned by the library; ms: total device time;
- * count: launches) accumulated since timing was enabled, and returns the number of
- * classes through *n.                                                                    */
-int mhd_bunch_set_timing(mhd_bunch *b, int32_t enable);
-int mhd_bunch_kernel_times(mhd_bunch *b, int32_t cap, const char **names, double *ms, int64_t *count, int32_t *n);
-
 /* HOST out: which of state_a/state_b holds the current level.  This is the call through
  * which a caller gets at the state between library calls: a deferred guard fill is written
  * out first, and the library assumes the caller may then modify the buffer (so the next
@@ -290,9 +284,6 @@ int mhd_bunch_current(mhd_bunch *b, void **state);
 /* Synchronises.  *bad_cells = number of interior cells met so far whose density or
  * pressure was not positive and finite (the scheme has no floors: DESIGN.md Q19).       */
 int mhd_bunch_status(mhd_bunch *b, int64_t *bad_cells);
-
-/* Number of kernel launches issued so far through this handle (for bench.py).           */
-int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 
 /* The step has four CUDA implementations, all on the GPU:
  *   MHD_PATH_ONEPASS     the whole step in one kernel, nothing intermediate in HBM (three
@@ -314,44 +305,6 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
 #define MHD_PATH_TILE2D      4
 int mhd_bunch_set_path(mhd_bunch *b, int32_t path);
 int mhd_bunch_get_path(mhd_bunch *b, int32_t *path);
-
-/* Launch-shape knobs (tests and tuning runs; the library reads no environment variables).
- *   MHD_TUNE_ONEPASS_ZSEG  z segments per tile column of the one-pass kernel (0 = automatic:
- *                          1 unless the bunch has fewer tiles than the device has SMs);
- *                          results do not depend on it, bit for bit.
- *   MHD_TUNE_PREDICT_TY    y-tile of the two-kernel path's predictor: 16, 8 or 4.
- *   MHD_TUNE_FUSED_CFL     1: the one-pass step also reduces the CFL rates of the level it writes
- *                          (in its epilogue, from registers), so that the next mhd_bunch_cfl_dt
- *                          only runs the bunch-wide reduction instead of re-reading the state;
- *                          0 (default): mhd_bunch_cfl_dt makes its own pass.  Same dt, bit for
- *                          bit, either way (both evaluate one explicitly rounded function).
- *   MHD_TUNE_HOST_BANDS    z-bands in which mhd_bunch_step_host steps the first chunk and the last
- *                          two (0 = automatic; clipped to bands of at least eight planes; only
- *                          the one-pass path steps plane ranges).  Read by host_query / attach;
- *                          results do not depend on it, bit for bit.
- *   MHD_TUNE_HOST_MAX_PITCH  largest host pitch in bytes that one strided host<->device copy of
- *                          mhd_bunch_step_host / mhd_bunch_step_ring may name (0 = the device's
- *                          cudaDevAttrMaxPitch, 2^31 - 1).  Host bunches whose fields are further
- *                          apart than this are moved field by field (eight copies per transfer
- *                          instead of one); tests set it to 1 to run that route on small bunches.
- *                          Results do not depend on it, bit for bit.
- * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
-#define MHD_TUNE_HOST_MAX_PITCH 5
-#define MHD_TUNE_HOST_BANDS   4
-#define MHD_TUNE_ONEPASS_ZSEG 1
-#define MHD_TUNE_PREDICT_TY   2
-#define MHD_TUNE_FUSED_CFL    3
-int mhd_bunch_set_tuning(mhd_bunch *b, int32_t key, int32_t value);
-
-/* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted
- * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous.
- *   scratch_dev  DEVICE, caller-owned, >= 8 * 256 * 8 * (number of SMs) bytes (4 MiB is
- *                always enough; MHD_ENOMEM otherwise): the library allocates nothing.     */
-int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, void *scratch_dev, size_t scratch_bytes, double *tflops);
-
-/* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
- * patches) the workspace allows.                                                        */
-int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);
 
 int mhd_bunch_destroy(mhd_bunch *b);
 
@@ -403,6 +356,63 @@ int mhd_bunch_cfl_dt_static(const mhd_bunch_desc *desc, const void *state_dev, d
 
 const char *mhd_bunch_strerror(int code);
 const char *mhd_bunch_last_cuda_error(void);
+
+/* ------------------------------------------------------------------------------------------
+ * Diagnostics and tuning -- NOT part of the method.  A caller of the paper's problem statement
+ * (create / fill_guards / cfl_dt / step and the host, ring and local variants above) never needs
+ * these six calls; bench.py and the tests use them to time kernel classes, count launches, force
+ * launch shapes and measure the ALU peak the roofline is quoted against.
+ * ------------------------------------------------------------------------------------------ */
+
+/* Per-kernel-class device timing for roofline reports.  While enabled, every launch is
+ * bracketed by CUDA events on the stream (a few microseconds of overhead per launch, so
+ * leave it off in throughput runs).  mhd_bunch_kernel_times synchronises, fills up to
+ * `cap` entries (name: HOST const char* owned by the library; ms: total device time;
+ * count: launches) accumulated since timing was enabled, and returns the number of
+ * classes through *n.                                                                    */
+int mhd_bunch_set_timing(mhd_bunch *b, int32_t enable);
+int mhd_bunch_kernel_times(mhd_bunch *b, int32_t cap, const char **names, double *ms, int64_t *count, int32_t *n);
+
+/* Number of kernel launches issued so far through this handle (for bench.py).           */
+int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
+
+/* Launch-shape knobs (tests and tuning runs; the library reads no environment variables).
+ *   MHD_TUNE_ONEPASS_ZSEG  z segments per tile column of the one-pass kernel (0 = automatic:
+ *                          1 unless the bunch has fewer tiles than the device has SMs);
+ *                          results do not depend on it, bit for bit.
+ *   MHD_TUNE_PREDICT_TY    y-tile of the two-kernel path's predictor: 16, 8 or 4.
+ *   MHD_TUNE_FUSED_CFL     1: the one-pass step also reduces the CFL rates of the level it writes
+ *                          (in its epilogue, from registers), so that the next mhd_bunch_cfl_dt
+ *                          only runs the bunch-wide reduction instead of re-reading the state;
+ *                          0 (default): mhd_bunch_cfl_dt makes its own pass.  Same dt, bit for
+ *                          bit, either way (both evaluate one explicitly rounded function).
+ *   MHD_TUNE_HOST_BANDS    z-bands in which mhd_bunch_step_host steps the first chunk and the last
+ *                          two (0 = automatic; clipped to bands of at least eight planes; only
+ *                          the one-pass path steps plane ranges).  Read by host_query / attach;
+ *                          results do not depend on it, bit for bit.
+ *   MHD_TUNE_HOST_MAX_PITCH  largest host pitch in bytes that one strided host<->device copy of
+ *                          mhd_bunch_step_host / mhd_bunch_step_ring may name (0 = the device's
+ *                          cudaDevAttrMaxPitch, 2^31 - 1).  Host bunches whose fields are further
+ *                          apart than this are moved field by field (eight copies per transfer
+ *                          instead of one); tests set it to 1 to run that route on small bunches.
+ *                          Results do not depend on it, bit for bit.
+ * MHD_EINVAL for an unknown key or a value the bunch cannot run.                           */
+#define MHD_TUNE_HOST_MAX_PITCH 5
+#define MHD_TUNE_HOST_BANDS   4
+#define MHD_TUNE_ONEPASS_ZSEG 1
+#define MHD_TUNE_PREDICT_TY   2
+#define MHD_TUNE_FUSED_CFL    3
+int mhd_bunch_set_tuning(mhd_bunch *b, int32_t key, int32_t value);
+
+/* Measures the plain-ALU peak of the device with an FMA-chain microbenchmark (FMA counted
+ * as 2 flops), for the roofline bench.py reports: HOST out *tflops.  Synchronous.
+ *   scratch_dev  DEVICE, caller-owned, >= 8 * 256 * 8 * (number of SMs) bytes (4 MiB is
+ *                always enough; MHD_ENOMEM otherwise): the library allocates nothing.     */
+int mhd_bunch_measure_alu_peak(int32_t dtype, int32_t device, void *scratch_dev, size_t scratch_bytes, double *tflops);
+
+/* Names and device times are not part of the ABI; this reports the sub-bunch chunk (in
+ * patches) the workspace allows.                                                        */
+int mhd_bunch_chunk(mhd_bunch *b, int32_t *chunk_patches);
 
 #ifdef __cplusplus
 }

@@ -2050,12 +2050,19 @@ int mhd_bunch_local_end(mhd_bunch* b) {
   mhd_bunch::Local& L = *b->loc;
   for (int p = 1; p < b->G.np; ++p)
     if (!times_equal(L.t_new[p], L.t_new[0])) return MHD_ESTATE;      // the bunch is not at one time
-  // bring every newer slice into the current buffer (per patch and field: a strided device copy)
-  const size_t pb = (size_t)b->G.ps * b->esz, fb = (size_t)b->G.fs * b->esz;
-  for (int p = 0; p < b->G.np; ++p) {
-    if (L.slot[p] == b->cur) continue;
-    CUDA_TRY(cudaMemcpy2DAsync((char*)b->state[b->cur] + (size_t)p * pb, fb, (char*)b->state[1 - b->cur] + (size_t)p * pb, fb, pb, 8,
-                               cudaMemcpyDeviceToDevice, b->stream));
+  // bring every newer slice into the current buffer: one launch over (patch, field), whatever the bunch size
+  const size_t pb = (size_t)b->G.ps * b->esz, fb = (size_t)b->G.fs * b->esz;     // multiples of 16 bytes
+  bool any = false;
+  for (int p = 0; p < b->G.np && !any; ++p) any = L.slot[p] != b->cur;
+  if (any) {
+    CUDA_TRY(cudaMemcpyAsync(b->d_slot, L.slot.data(), sizeof(int) * b->G.np, cudaMemcpyHostToDevice, b->stream));
+    const long long pv = (long long)(pb / 16);
+    unsigned bx = blocks_for(pv, 256);
+    if (bx > 64) bx = 64;
+    LaunchScope ls(b, KC_MISC);
+    k_gather_slices<<<dim3(bx, (unsigned)b->G.np, 8), 256, 0, b->stream>>>((uint4*)b->state[b->cur], (const uint4*)b->state[1 - b->cur],
+                                                                          b->d_slot, b->cur, pv, (long long)(fb / 16));
+    CUDA_TRY(cudaGetLastError());
   }
   L.active = false;
   b->guards_stale = false;

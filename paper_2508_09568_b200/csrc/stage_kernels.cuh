@@ -319,6 +319,18 @@ __global__ void k_zero_u64(unsigned long long* p, int n) {
   if (t < n) p[t] = 0ull;
 }
 
+// mhd_bunch_local_end: the newer time slice of every patch whose slot is not `cur` moves into buffer
+// `cur` -- all eight fields of all such patches in ONE launch (blockIdx.y = patch, blockIdx.z = field),
+// 16 bytes per thread; a patch and a field start on 16-byte boundaries (ps is a multiple of four elements).
+__global__ void __launch_bounds__(256) k_gather_slices(uint4* __restrict__ dst, const uint4* __restrict__ src,
+                                                       const int* __restrict__ slot, int cur, long long patch_v, long long field_v) {
+  const int p = blockIdx.y;
+  if (slot[p] == cur) return;
+  const long long base = (long long)blockIdx.z * field_v + (long long)p * patch_v;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < patch_v; t += (long long)gridDim.x * blockDim.x)
+    dst[base + t] = src[base + t];
+}
+
 // FMA-chain microbenchmark: 16 independent chains per thread, used to MEASURE the fp32/fp64
 // pipe peak that the ALU roofline of the step kernels is reported against
 template <typename T>

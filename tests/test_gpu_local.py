@@ -81,6 +81,11 @@ def test_two_distinct_time_steps_against_the_oracle(name, path, fine, dtype):
     _, ref_dts = o.cfl_dt(ref, 0.4, per_patch=True)
     assert np.all(np.abs(dts - ref_dts) <= (1e-13 if dtype == "f64" else 2e-6) * ref_dts)
     assert b.status() == 0
+    # the coarse patches flipped buffers three times, the fine ones six: local_end gathers the newer slices
+    # from both buffers into the current level (one launch over patches and fields)
+    assert len(set(slot.tolist())) == 2
+    b.local_end()
+    assert np.array_equal(masked(b.download(), w.n), masked(got, w.n))
     b.close()
 
 
