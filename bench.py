@@ -198,8 +198,8 @@ def measure(name, args, local, world, rank, field_cache, headline):
     b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype=dtype, device=local)
     b.load(w.U if dtype == "f64" else w.U.astype(np.float32))
     b.set_path(args.path)
-    if args.fused_cfl and b.path == "onepass":
-        b.set_tuning("fused_cfl", 1)
+    if args.fused_cfl != 2 and b.path == "onepass":
+        b.set_tuning("fused_cfl", args.fused_cfl)
     stream = b.stream
     courant = 0.4
     steps = args.steps if headline else max(3, min(args.steps, args.sub_steps))
@@ -399,7 +399,7 @@ def measure_small(name, args, local):
 ARRANGE = {1: (1, 1, 1), 8: (2, 2, 2), 64: (4, 4, 4), 300: (5, 6, 10), 512: (8, 8, 8), 4096: (16, 16, 16)}
 
 
-def replicated_bunch(n, P, dtype, device, max_side=256):
+def replicated_bunch(n, P, dtype, device, max_side=256, stream=None):
     """A periodic bunch of P patches whose global field would be too large to build on the host:
     the seeded field is built on a block of at most max_side cells per side and repeated
     periodically ON THE DEVICE (patch (px,py,pz) holds block patch (px mod Bx, ...)), which is again
@@ -411,7 +411,7 @@ def replicated_bunch(n, P, dtype, device, max_side=256):
     nbr = W.neighbour_table(P, (True, True, True))
     npatch = P[0] * P[1] * P[2]
     dx = tuple(1.0 / (n * max(P)) for _ in range(3))
-    b = MhdBunch(wb.n, npatch, nbr, wb.gamma, dx, dtype=dtype, device=device, workspace_bytes=1 << 30)
+    b = MhdBunch(wb.n, npatch, nbr, wb.gamma, dx, dtype=dtype, device=device, workspace_bytes=1 << 30, stream=stream)
     src = torch.from_numpy(wb.U).to(b.device)                 # [8, block patches, mz, my, mx]
     v = b.view()
     ids = np.arange(npatch)
@@ -421,14 +421,43 @@ def replicated_bunch(n, P, dtype, device, max_side=256):
         sel = torch.from_numpy(ids[img == q]).to(b.device)
         for f in range(8):                                    # field by field: no large temporaries
             v[f].index_copy_(0, sel, src[f, q].unsqueeze(0).expand(len(sel), -1, -1, -1))
-    b.stream.synchronize()
+    torch.cuda.synchronize(b.device)       # the copies ran on torch's current stream, which need not be the bunch's
     return b, wb, B
+
+
+def replay_us_per_step(b, one, steps):
+    """Device time per step of `steps` back-to-back steps captured in ONE CUDA graph and replayed:
+    the kernels of the loop with no per-call launch cost between them.  The capture holds kernel launches only
+    (the loop neither copies nor synchronises).  None if the capture is refused."""
+    import torch
+    try:
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=b.stream):
+            for _ in range(steps):
+                one()
+        b.stream.synchronize()
+        best = None
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(b.stream):
+                e0.record()
+                g.replay()
+                e1.record()
+            e1.synchronize()
+            t = e0.elapsed_time(e1) * 1e3 / steps
+            best = t if best is None else min(best, t)
+        del g
+        return best
+    except Exception as e:                      # a capture that failed leaves nothing half-done on the stream
+        print("graph capture refused: %s" % str(e).splitlines()[0][:120], file=sys.stderr)
+        return None
 
 
 def sweep(args, local):
     """BASELINE.json config 4: patch sizes x bunch sizes, fp32, config-2 field construction; per
-    point the resident loop's rate, device-busy time (events around every launch) and the
-    launch-overhead share 1 - busy/wall."""
+    point the resident loop's rate with per-call launches (wall clock), the same steps replayed from
+    one CUDA graph (device time, no launch cost between kernels) and the launch-overhead share
+    1 - graph/wall that the paper's bunching study is about (Fig. 5)."""
     import torch
     from paper_2508_09568_b200.binding import MhdBunch
     sizes = [int(x) for x in args.sizes.split(",")]
@@ -440,13 +469,16 @@ def sweep(args, local):
         N = tuple(n * p for p in P)
         rec = {"patch": n, "bunch": k, "cells": k * n ** 3}
         try:
+            side = torch.cuda.Stream(device=local)     # a stream of its own: the default stream cannot be captured
             if max(N) > 512:
-                b, wb, B = replicated_bunch(n, P, "f32", local)
+                b, wb, B = replicated_bunch(n, P, "f32", local, stream=side)
                 rec["field"] = "block of %dx%dx%d patches repeated periodically on the device" % B
             else:
                 w = W.turbulence(N=N, n=n, dtype=np.float32, config=2, patches=P)
-                b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype="f32", device=local)
+                b = MhdBunch(w.n, w.npatch, w.nbr, w.gamma, w.dx, dtype="f32", device=local, stream=side)
                 b.load(w.U)
+            if args.fused_cfl != 2 and b.path == "onepass":
+                b.set_tuning("fused_cfl", args.fused_cfl)
         except Exception as e:
             rec["skipped"] = str(e).splitlines()[0][:100]
             out.append(rec)
@@ -465,14 +497,20 @@ def sweep(args, local):
         torch.cuda.synchronize()
         wall = (time.perf_counter() - t0) / steps
         launches = (b.launches - l0) / steps
+        graph_us = replay_us_per_step(b, one, steps)
         b.set_timing(True)
         for _ in range(steps):
             one()
         kt = b.kernel_times()
         b.set_timing(False)
         busy = sum(v[0] for v in kt.values()) * 1e-3 / steps
-        rec.update({"step_path": b.path, "launches_per_step": launches, "wall_us": wall * 1e6, "busy_us": busy * 1e6,
-                    "value": rec["cells"] / wall, "launch_overhead_share": max(0.0, 1.0 - busy / wall), "bad_cells": b.status()})
+        share = None if graph_us is None else max(0.0, 1.0 - graph_us / (wall * 1e6))
+        rec.update({"step_path": b.path, "launches_per_step": launches, "wall_us": wall * 1e6, "graph_us": graph_us,
+                    "busy_us": busy * 1e6, "value": rec["cells"] / wall,
+                    "value_graph": None if graph_us is None else rec["cells"] / (graph_us * 1e-6),
+                    "launch_overhead_share": share,
+                    "share_is": "1 - (device time per step of the timed steps replayed from one CUDA graph) / (wall time per step with per-call launches)",
+                    "bad_cells": b.status()})
         b.close()
         del b
         torch.cuda.empty_cache()
@@ -499,8 +537,9 @@ def main():
                     help="which CUDA implementation of the step runs (include/mhd_bunch.h, MHD_PATH_*)")
     ap.add_argument("--explicit-fill", action="store_true",
                     help="materialise the guard shell in HBM every step (the fill is otherwise folded into the step's halo loads)")
-    ap.add_argument("--fused-cfl", type=int, default=0, choices=[0, 1],
-                    help="one-pass step: reduce the new level's CFL rates in the step's epilogue (MHD_TUNE_FUSED_CFL)")
+    ap.add_argument("--fused-cfl", type=int, default=2, choices=[0, 1, 2],
+                    help="one-pass step: reduce the new level's CFL rates in the step's epilogue (MHD_TUNE_FUSED_CFL; "
+                         "2 = the library's choice: on bunches of at most one wave of tiles)")
     ap.add_argument("--sizes", default="16,24,32,64", help="c4: patch sizes")
     ap.add_argument("--bunches", default="1,8,64,512,4096", help="c4: bunch sizes")
     args = ap.parse_args()
@@ -592,6 +631,19 @@ def main():
                 "bad_cells": head["bad_cells"], "conservation": head["conservation"], "roofline": head["roofline"],
                 "step_roofline": head["step_roofline"], "kernel_classes": head["kernel_classes"],
                 "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "sub_records": subs}
+        # Compact digest LAST on the line (a record that keeps only the tail of the output still holds it): the
+        # metric is "(fp32/fp64)", so the fp64 half and the other configurations, one short entry each, no blobs.
+        def brief(r):
+            rf = r.get("roofline") or {}
+            e = r.get("e2e") or {}
+            return {"dtype": r.get("dtype"), "value": r.get("value"), "ms_per_step": r.get("ms_per_step"),
+                    "kernel": rf.get("kernel"), "bound": rf.get("bound"), "frac": rf.get("frac"), "e2e_value": e.get("value")}
+        digest = {"c2": brief({**head, "dtype": head["dtype"]})}
+        for r in subs:
+            digest[r.get("workload", "?")] = brief(r) if "error" not in r else {"error": r["error"]}
+        line["value_f64"] = (digest.get("c2f64") or {}).get("value")
+        line["roofline_f64"] = {k: (digest.get("c2f64") or {}).get(k) for k in ("kernel", "bound", "frac")}
+        line["digest"] = digest
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

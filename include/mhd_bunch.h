@@ -383,9 +383,13 @@ int mhd_bunch_launch_count(mhd_bunch *b, int64_t *launches);
  *   MHD_TUNE_PREDICT_TY    y-tile of the two-kernel path's predictor: 16, 8 or 4.
  *   MHD_TUNE_FUSED_CFL     1: the one-pass step also reduces the CFL rates of the level it writes
  *                          (in its epilogue, from registers), so that the next mhd_bunch_cfl_dt
- *                          only runs the bunch-wide reduction instead of re-reading the state;
- *                          0 (default): mhd_bunch_cfl_dt makes its own pass.  Same dt, bit for
- *                          bit, either way (both evaluate one explicitly rounded function).
+ *                          only runs the bunch-wide reduction instead of re-reading the state
+ *                          (three launches per step instead of five); 0: mhd_bunch_cfl_dt always
+ *                          makes its own pass; 2 (default): the library chooses -- the epilogue
+ *                          on bunches of at most one wave of tiles, which are bound by launch
+ *                          latency, the pass on larger ones, where it is cheaper.  Same dt, bit
+ *                          for bit, either way (both evaluate one explicitly rounded function);
+ *                          the stepped state of the two kernel variants agrees to rounding.
  *   MHD_TUNE_HOST_BANDS    z-bands in which mhd_bunch_step_host steps the first chunk and the last
  *                          two (0 = automatic; clipped to bands of at least eight planes; only
  *                          the one-pass path steps plane ranges).  Read by host_query / attach;

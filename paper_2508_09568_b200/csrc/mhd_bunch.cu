@@ -141,7 +141,8 @@ struct mhd_bunch {
   int tune_bands;      // MHD_TUNE_HOST_BANDS: 0 = automatic
   int tune_max_pitch;  // MHD_TUNE_HOST_MAX_PITCH: 0 = the device's limit (max_pitch)
   size_t max_pitch;    // cudaDevAttrMaxPitch of the handle's device: largest pitch a strided copy may name
-  bool fused_cfl;      // MHD_TUNE_FUSED_CFL: the one-pass step reduces the new level's CFL rates in its epilogue
+  bool fused_cfl;      // MHD_TUNE_FUSED_CFL = 1: the one-pass step reduces the new level's CFL rates in its epilogue
+  bool fused_cfl_auto; // MHD_TUNE_FUSED_CFL = 2 (default): it does so on small bunches (onepass_cfle)
   bool timing;
   struct Ev { int cls; cudaEvent_t a, b; };
   std::vector<Ev>* events;
@@ -384,6 +385,24 @@ bool step_gathers(const mhd_bunch* b) {
          (path == MHD_PATH_TILE2D && b->gather_t_ok);
 }
 
+// Does the one-pass step reduce the CFL rates of the level it writes in its epilogue?  Asked for
+// (MHD_TUNE_FUSED_CFL = 1), or by itself on bunches of at most ONEPASS_CFLE_WAVES waves of tiles: those are bound
+// by launch latency, and the epilogue replaces two of the five launches of a step (the rate
+// pass and its clear).  Measured (profiles/r3_c4_sweep.md): one 32^3 patch 59 -> 51 us per step, 8 x 32^3 86 -> 79,
+// 64 x 16^3 91 -> 85; break-even at one to two waves (64 x 32^3: 465 either way; 64 x 24^3, 1.3 waves: 282 -> 292);
+// on bunches that fill the GPU the stand-alone pass is cheaper (config 2: 3.03 against 3.15 ms per step).  The
+// choice is made for the WHOLE bunch, so every launch of a step (chunks, bands, patch lists) runs the same variant.
+#ifndef ONEPASS_CFLE_WAVES
+#define ONEPASS_CFLE_WAVES 1
+#endif
+bool onepass_cfle(const mhd_bunch* b) {
+  if (b->fused_cfl) return true;
+  if (!b->fused_cfl_auto) return false;
+  const int tx = b->G.n[0] <= 16 ? 16 : OneTile::TX, ty = b->G.n[0] <= 16 ? 16 : OneTile::TY;
+  const long long tiles = (long long)((b->G.n[0] + tx - 1) / tx) * ((b->G.n[1] + ty - 1) / ty) * b->G.np;
+  return tiles <= (long long)ONEPASS_CFLE_WAVES * b->nsm;
+}
+
 template <typename T> struct OnePassLaunch {
   static int prepare(mhd_bunch*) { return MHD_OK; }
   static int run(mhd_bunch*, const double*, int = 0, int = -1, bool = true, int = 0, int = -1) { return MHD_EINVAL; }
@@ -403,11 +422,12 @@ template <> struct OnePassLaunch<float> {
       return MHD_OK;
     }
     // the limiter and the CFL epilogue are compile-time parameters of the kernel
-    auto kern = b->fused_cfl
+    const bool cfle = onepass_cfle(b);
+    auto kern = cfle
                     ? (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, true> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, true>)
                     : (G.limiter == 1 ? k_step_onepass<float, TX, TY, OneTile::NPW, 1, false> : k_step_onepass<float, TX, TY, OneTile::NPW, 2, false>);
     // the default scheme (minmod, HLLD, HLLD-2D) has an instantiation with the solvers fixed at compile time
-    if (!b->fused_cfl && G.limiter == 1 && G.emf_solver == 0 && G.flux_solver == 0)
+    if (!cfle && G.limiter == 1 && G.emf_solver == 0 && G.flux_solver == 0)
       kern = k_step_onepass<float, TX, TY, OneTile::NPW, 1, false, true>;
     Params<float> P = make_params<float>(b, p0, npl);
     if (zhi < 0) zhi = G.n[2];
@@ -454,7 +474,7 @@ template <> struct OnePassLaunch<float> {
     if (last) {
       b->cur = 1 - b->cur;
       b->guards_stale = false;   // the new level's guards are undefined until the next fill_guards
-      b->rate_valid = b->fused_cfl;   // every patch went through the epilogue since the last k_set_dt
+      b->rate_valid = onepass_cfle(b);   // every patch went through the epilogue since the last k_set_dt
     }
     return MHD_OK;
   }
@@ -889,6 +909,7 @@ int mhd_bunch_create(const mhd_bunch_desc* desc, const int32_t* nbr, void* state
                                                                                                              : (size_t)0x7fffffff;
   }
   b->fused_cfl = false;
+  b->fused_cfl_auto = true;
   b->hs = nullptr;
   b->ring = nullptr;
   b->h_nbr = new (std::nothrow) std::vector<int>(nbr, nbr + 27 * (size_t)desc->npatch);
@@ -1026,8 +1047,9 @@ int mhd_bunch_set_tuning(mhd_bunch* b, int32_t key, int32_t value) {
     return MHD_OK;
   }
   if (key == MHD_TUNE_FUSED_CFL) {
-    if (value > 1 || !b->onepass_ok) return MHD_EINVAL;
+    if (value > 2 || !b->onepass_ok) return MHD_EINVAL;
     b->fused_cfl = value == 1;
+    b->fused_cfl_auto = value == 2;
     b->rate_valid = false;
     return MHD_OK;
   }
@@ -1594,7 +1616,7 @@ static int step_host_impl(mhd_bunch* b, const void* host_in, void* host_out, dou
     b->cur = 1 - b->cur;
     b->guards_stale = true;   // the new level's shell is owed (deferred fill), its closing faces are current
     b->closing_ok = true;
-    b->rate_valid = onepass && b->fused_cfl;  // every unit went through the one-pass epilogue since k_set_dt
+    b->rate_valid = onepass && onepass_cfle(b);  // every unit went through the one-pass epilogue since k_set_dt
   } else {
     if ((rc = step_common(b)) != MHD_OK) return rc;
     CUDA_TRY(cudaEventRecord(h->ev_all_steps, b->stream));

@@ -707,7 +707,23 @@ def test_fused_cfl_epilogue_is_bitwise_the_standalone_reduction(name):
     # the state does not depend on the epilogue beyond round-off: the kernel without it is a separate
     # compilation of the same source (a handful of values in a million differ by one ulp)
     c = make_gpu(w, "f32")
+    c.set_tuning("fused_cfl", 0)
+    dts_c = []
     for _ in range(3):
-        c.fill_guards(); dt = c.cfl_dt(0.4, sync=True); c.step(dt)
+        c.fill_guards(); dt = c.cfl_dt(0.4, sync=True); c.step(dt); dts_c.append(dt)
     assert rel_err(masked(c.download(), w.n), masked(U, w.n)) <= 2e-7
-    b.close(); c.close()
+    # the library's own choice (MHD_TUNE_FUSED_CFL = 2, the default): these bunches are far below one wave of
+    # tiles, so the epilogue runs -- three launches per step (cfl_final, set_dt, step) after the first, the state
+    # bit for bit that of the handle with the epilogue forced on
+    d = make_gpu(w, "f32")
+    e = make_gpu(w, "f32")
+    e.set_tuning("fused_cfl", 1)
+    for s in range(3):
+        l0 = d.launches
+        d.fill_guards(); dt_d = d.cfl_dt(0.4, sync=True); d.step(dt_d)
+        e.fill_guards(); dt_e = e.cfl_dt(0.4, sync=True); e.step(dt_e)
+        assert dt_d == dt_e
+        if s > 0:                                  # rows of whole 16-byte chunks: the fill is folded into the step too
+            assert d.launches - l0 == (3 if w.n[0] % 4 == 0 else 4), d.launches - l0
+    assert np.array_equal(d.download(), e.download())
+    b.close(); c.close(); d.close(); e.close()
