@@ -53,6 +53,25 @@ def rel_err_pure(g, o, floor=PURE_FLOOR):
     return worst
 
 
+# Where the secondary metric can be asserted, and with which floor (Q21; measured in round 3).
+# Its worst cell always sits just above the floor, in a transverse field component that nearly cancels (By, Bz of the
+# turbulence field at 1.0-1.4e-3 of the group scale): the absolute error there is the fp32 rounding of the update's
+# terms, 1-4e-8 of the SCALE, so the metric is (1-4e-8) / floor and grows with the number of cells over which the
+# maximum is taken and with the steps taken: 1.0e-5 (8 x 16^3 or 8 x 32^3, one step), 2.1e-5 (8 x 64^3, one step),
+# 3.6e-5 (8 x 32^3, three steps).  With the floor 1e-3 it is held to 2e-5 on the small one-step cases only
+# (assert_step_parity); full-size bunches and multi-step runs use the floor 1e-2 below, where the same absolute
+# errors give (1-4)e-6 -- still a statement the primary metric does not make (a cell at a hundredth of the scale
+# that is wrong by a tenth of a percent fails it).
+PURE_FLOOR_LARGE = 1e-2
+
+
+def assert_pure_large(g, o, dtype, what=()):
+    """Secondary metric of Q21 on full-size bunches and after several steps: floor 1e-2, north_star tolerance."""
+    e = rel_err_pure(g, o, floor=PURE_FLOOR_LARGE)
+    assert e <= TOL_PURE[dtype], (what, dtype, "pure relative (floor 1e-2)", e)
+    return e
+
+
 def assert_step_parity(g, o, dtype, what=(), tight=True):
     """Both Q21 metrics of a stepped state against the oracle's, at the north_star tolerance and
     (tight) at the regression bound; returns (primary, secondary)."""

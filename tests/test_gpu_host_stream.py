@@ -6,7 +6,7 @@ path of the same library."""
 import numpy as np
 import pytest
 
-from parity_util import TOL_STEP, make_gpu, make_oracle, rel_err
+from parity_util import TOL_STEP, assert_pure_large, make_gpu, make_oracle, rel_err
 from paper_2508_09568_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -54,6 +54,7 @@ def test_step_host_on_the_other_step_paths(dtype, path):
     hout = torch.zeros_like(hin).pin_memory()
     used, nxt = b.step_host(hin, hout, dt=dt_ref, courant=0.4)
     assert rel_err(hout.numpy().astype(np.float64), W.to_compact(ref, w.n)) <= TOL_STEP[dtype]
+    assert_pure_large(hout.numpy().astype(np.float64), W.to_compact(ref, w.n), dtype, path)
     assert abs(nxt - dt_next_ref) <= 10 * TOL_STEP[dtype] * dt_next_ref
     b.close()
 
@@ -79,6 +80,7 @@ def test_step_host_matches_oracle(name, given_dt, chunk, dtype):
     got = hout.numpy().astype(np.float64)
     err = rel_err(got, W.to_compact(ref, w.n))
     assert err <= TOL_STEP[dtype], err
+    assert_pure_large(got, W.to_compact(ref, w.n), dtype, name)
     assert np.array_equal(hin.numpy(), W.to_compact(w.U, w.n))     # the input is read-only
     assert b.status() == 0
     b.close()

@@ -3,7 +3,7 @@ the extended oracle, on every implementation of the step."""
 import numpy as np
 import pytest
 
-from parity_util import TOL_STEP, assert_nstep_parity, make_gpu, make_oracle, masked, rel_err
+from parity_util import TOL_STEP, assert_nstep_parity, assert_pure_large, make_gpu, make_oracle, masked, rel_err
 from paper_2508_09568_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -75,6 +75,7 @@ def test_two_distinct_time_steps_against_the_oracle(name, path, fine, dtype):
     assert np.allclose(t1, st["t_new"], rtol=0, atol=1e-15) and np.array_equal(slot, st["cur"])
     got, ref = b.local_newest(), o.local_newest(st)
     assert rel_err(masked(got, w.n), masked(ref, w.n)) <= TOL_STEP[dtype], (name, path, dtype)
+    assert_pure_large(masked(got, w.n), masked(ref, w.n), dtype, (name, path))
     assert_nstep_parity(W.gather(got, w.n, w.P), W.gather(ref, w.n, w.P), dtype, name)
     # per-patch CFL steps of the newer slices
     dts = b.cfl_local(0.4)

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import exact_riemann
-from parity_util import (TOL_L1_F32, TOL_STEP, TOL_TOTALS_F64, assert_nstep_parity, assert_step_parity, make_gpu,
+from parity_util import (TOL_L1_F32, TOL_STEP, TOL_TOTALS_F64, assert_nstep_parity, assert_pure_large, assert_step_parity, make_gpu,
                          make_oracle, masked, rel_err)
 from paper_2508_09568_b200 import workloads as W
 
@@ -545,6 +545,7 @@ def test_config2_full_size_sampled_patches_and_invariants():
     ref = o.step(np.ascontiguousarray(ref_fill[:, sample]), dt_ref)
     err = rel_err(masked(got[:, sample], w.n), masked(ref, w.n))
     assert err <= TOL_STEP["f32"], err
+    assert_pure_large(masked(got[:, sample], w.n), masked(ref, w.n), "f32", "config 2, sampled patches")
     g0, g1 = W.gather(w.U, w.n, w.P).astype(np.float64), W.gather(got, w.n, w.P).astype(np.float64)
     t0, t1 = g0[:5].sum(axis=(1, 2, 3)), g1[:5].sum(axis=(1, 2, 3))
     assert abs(t1[0] - t0[0]) <= 2e-6 * t0[0] and abs(t1[4] - t0[4]) <= 2e-6 * t0[4]
@@ -612,6 +613,7 @@ def test_config3_full_size_sampled_patches_and_invariants(dtype):
     got = b.download()
     err = rel_err(masked(got[:, sample], w.n), masked(ref, w.n))
     assert err <= TOL_STEP[dtype], err
+    assert_pure_large(masked(got[:, sample], w.n), masked(ref, w.n), dtype, "config 3, sampled patches")
     g1 = W.gather(got, w.n, w.P)
     del got
     tol = 1e-12 if dtype == "f64" else 2e-6
