@@ -43,7 +43,7 @@ WORKLOADS = {
 # the CPU oracle's bounded samples: the same seeded field construction on a cut of the cube
 SAMPLE_1 = (64, 64, 64)          # 8 patches of 32^3, single thread
 SAMPLE_ALL = (128, 128, 64)      # 32 patches of 32^3, OpenMP over patches on all host cores
-TRAFFIC_FILE = os.path.join("profiles", "r2_ncu_traffic.txt")
+TRAFFIC_FILE = os.path.join("profiles", "r3_ncu_traffic.txt")
 
 
 def peaks():
